@@ -1,0 +1,191 @@
+/*
+ * epw_interp.h -- C ABI of the B200-native Wannier-to-Bloch interpolation of
+ * electron-phonon matrix elements (arxiv/paper_2603_10295, EPW 6.1).
+ *
+ * The path ("The path"):
+ *   S0  phase tables          exp(2 pi i q.Rp), exp(2 pi i k.Re)            PAPER.md:L110, L114, L303 ("x" of Fig. 13)
+ *   S1  Rp -> q               g(Re,q) = sum_Rp g(Re,Rp) e^{i q.Rp}          PAPER.md:L110 (Eq. 9), L501-511 (Fig. 13)
+ *   S3  operators             H(R)->H(k), H(k+q); D(Rp)->D(q); Hermitian eigensolves -> U, eps, e_q, omega_q
+ *                                                                           BASELINE.json north_star stage (3)
+ *   S4a mode rotation         g^ = g e_q / sqrt(2 omega_q)   (hoisted onto g(Re,q): it is linear and depends on q only)
+ *                                                                           PAPER.md:L114 (u_{ka,nu}(q)), L102 ("Rotation by")
+ *   S2  Re -> k               g~(k,q) = sum_Re g^(Re,q) e^{i k.Re}, batched over k as one FP64 tensor (DMMA) contraction
+ *                                                                           PAPER.md:L112-114 (Eq. 10), L118 ("FT w.r.t. Re")
+ *   S4b band rotation, |g|^2  g_{mn nu} = sum_{m'n'} conj(U_{k+q}[m',m]) g~_{m'n' nu} U_k[n',n];  out = |g_{mn nu}|^2
+ *                                                                           PAPER.md:L114 (U_{mm'k+q} U*_{nn'k}), north_star stage (4)
+ *
+ * Conventions common to every entry point
+ *   - Complex numbers are interleaved (re, im) FP64 pairs ("c128"); all arithmetic is FP64.
+ *   - "Fortran (a,b,c)" means the FIRST index is fastest in memory.
+ *   - k, q are crystal (fractional) coordinates; R vectors are integer triples; phase = 2 pi frac(x.R).
+ *   - Matrices are column-major, eigenvectors are the COLUMNS of U / e, eigenvalues ascending.
+ *   - Return value: 0 (EPW_OK) or a negative epw_status; nothing is thrown across the ABI.
+ *     epw_interp_last_error(h) returns a human-readable message for the last failure on that handle.
+ *   - Ownership: the caller owns every buffer passed in; the library copies the operators in
+ *     epw_interp_set_wannier_operators and owns that copy and its workspace.
+ *   - "device" pointers are CUDA device pointers valid on the handle's device; "host" pointers are CPU memory.
+ *   - Calls on one handle must not overlap (a handle is not thread-safe); distinct handles are independent.
+ *   - There is no CPU fallback: every call fails with EPW_ECUDA if no sm_100 device is usable.
+ */
+#ifndef EPW_INTERP_H_
+#define EPW_INTERP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct epw_interp *epw_interp_t; /* opaque; owned by the library */
+
+typedef enum {
+  EPW_OK = 0,
+  EPW_EINVAL = -1,        /* bad argument (null pointer, non-positive size, operators not set, ...) */
+  EPW_ENOMEM = -2,        /* device or host allocation failed */
+  EPW_ECUDA = -3,         /* CUDA runtime error, or no usable sm_100 device */
+  EPW_ENOTCONVERGED = -4, /* a Jacobi eigensolve hit the sweep limit (reported by epw_interp_sync) */
+  EPW_EUNSUPPORTED = -5   /* shape outside what this build implements (message says which) */
+} epw_status;
+
+typedef struct {
+  int32_t nbnd;           /* Nb: number of Wannier functions / bands  */
+  int32_t nmodes;         /* Nm = 3 Na: number of phonon modes  */
+  int32_t ne;             /* Ne: number of electron Wigner-Seitz vectors Re */
+  int32_t np;             /* Np: number of phonon Wigner-Seitz vectors Rp */
+  int32_t device;         /* CUDA device ordinal */
+  int32_t q_batch;        /* q-points contracted per pass over g(Re,Rp) in S1 (1..8); 0 = library default */
+  size_t workspace_bytes; /* cap on the library's scratch HBM; 0 = library chooses from free memory */
+  double degen_tol;       /* informational (gap below which callers should sum |g|^2 over a subspace); unused inside */
+  double omega_min;       /* modes with omega_q,nu <= omega_min give |g|^2 = 0 (acoustic modes at Gamma); default 0 */
+} epw_interp_config;
+
+/* Create / destroy a handle.  *out is set to NULL on failure. */
+int epw_interp_create(epw_interp_t *out, const epw_interp_config *cfg);
+void epw_interp_destroy(epw_interp_t h);
+
+/*
+ * Upload the Wannier-representation operators (they stay resident in HBM for the whole interpolation,
+ * PAPER.md:L184).  on_device = 0: host pointers, 1: device pointers (copied device-to-device).
+ *   H_R   c128 Fortran (i, j, ie)            [Ne][Nb][Nb]      H(Re)_{ij}, H(-R) = H(R)^dagger expected
+ *   D_R   c128 Fortran (a, b, ip)            [Np][Nm][Nm]      dynamical matrix, masses absorbed (eV^2)
+ *   g_RR  c128 Fortran (m', n', ie, ka, ip)  [Np][Nm][Ne][Nb][Nb]   size 16 Nb^2 Nm Ne Np bytes;
+ *         this is Fig. 13's column-major A(m,n) with the Rp index as the column.
+ *         May be NULL: then every Rp slab must be supplied with epw_interp_set_g_slabs before interpolating.
+ *   Re    int32 [Ne][3], w_e f64 [Ne]   electron lattice vectors and Wigner-Seitz weights (1/ndegen)
+ *   Rp    int32 [Np][3], w_p f64 [Np]   phonon lattice vectors and weights
+ */
+int epw_interp_set_wannier_operators(epw_interp_t h, const void *H_R, const void *D_R, const void *g_RR,
+                                     const int32_t *Re, const double *w_e, const int32_t *Rp, const double *w_p,
+                                     int on_device);
+
+/* Upload Rp slabs ip_start .. ip_start+ip_count-1 of g_RR (each Nb^2 Ne Nm c128, same layout as above), so that
+ * a tensor larger than host memory (Table III) can be streamed in. */
+int epw_interp_set_g_slabs(epw_interp_t h, int32_t ip_start, int32_t ip_count, const void *g_slabs, int on_device);
+
+/*
+ * The hot path: every (k,q) pair of the two lists.  All pointers are DEVICE pointers.  Asynchronous on `cuda_stream`
+ * (a cudaStream_t passed as void*; NULL = legacy default stream): caller buffers are touched only between enqueue
+ * and stream completion.
+ *   k_list  f64 [nk][3], q_list f64 [nq][3]   crystal coordinates (any values; no grid assumed)
+ *   kq_map  NULL, or int32 [nq][nk]: index in k_list of k+q folded onto the list (grid case): then U_{k+q},
+ *           eps_{k+q} are looked up instead of eigensolving H(k+q) per pair
+ *   eps_k   out f64 [nk][Nb]            eigenvalues of H(k), ascending
+ *   eps_kq  out f64 [nq][nk][Nb] or NULL
+ *   omega_q out f64 [nq][Nm]            sqrt of the eigenvalues of D(q) (negative = imaginary frequency)
+ *   g2      out f64 [nq][nk][Nm][Nb][Nb] = Fortran (m, n, nu, k, q): |g_{mn nu}(k,q)|^2, m (the k+q band) fastest
+ * The caller batches q so that g2 (8 Nb^2 Nm nk nq bytes) fits.
+ */
+int epw_interp_interpolate(epw_interp_t h, const double *k_list, int64_t nk, const double *q_list, int64_t nq,
+                           const int32_t *kq_map, double *eps_k, double *eps_kq, double *omega_q, double *g2,
+                           void *cuda_stream);
+
+/*
+ * Same computation with HOST buffers (pinned or pageable): copies k_list, q_list, kq_map to the device, runs the
+ * path, copies eps_k, eps_kq (if non-NULL), omega_q and g2 back, and returns after the stream has completed.
+ */
+int epw_interp_interpolate_host(epw_interp_t h, const double *k_list, int64_t nk, const double *q_list, int64_t nq,
+                                const int32_t *kq_map, double *eps_k, double *eps_kq, double *omega_q, double *g2,
+                                void *cuda_stream);
+
+/* Wait for the handle's last enqueued work and report deferred device-side status (EPW_ENOTCONVERGED, EPW_ECUDA). */
+int epw_interp_sync(epw_interp_t h);
+
+/*
+ * Per-stage device times (ms, CUDA events on the caller's stream) accumulated over the last interpolate call:
+ *   ms[0] S0 phase tables   ms[1] S1 Rp->q   ms[2] D(q) + phonon eigensolve + S4a/pack   ms[3] H(k) + eigensolve
+ *   ms[4] S2 Re->k contraction   ms[5] H(k+q) eigensolve   ms[6] S4b rotation + |g|^2   ms[7] total
+ * Synchronises the stream.  Returns the number of entries written (<= n) or a negative status.
+ */
+#define EPW_NUM_STAGES 8
+int epw_interp_get_stage_times(epw_interp_t h, double *ms, int n);
+
+/* Stage timing records two CUDA events per stage invocation; it is off by default (on != 0 enables it for the
+ * following interpolate calls). */
+int epw_interp_enable_stage_timing(epw_interp_t h, int on);
+
+/* Number of kernels the library launched during the last interpolate call (for bench.py's gpu_launches). */
+int64_t epw_interp_last_launch_count(epw_interp_t h);
+
+/*
+ * Intermediate results of the LAST q of the last interpolate call, for parity tests (device -> host copy,
+ * synchronises).  `bytes` must be at least the size stated; returns bytes written or a negative status.
+ *   EPW_DBG_G_REQ   g(Re,q)  c128 Fortran (m', n', ie, ka)            16 Nb^2 Ne Nm
+ *   EPW_DBG_G_TILDE g~(k,q) after S4a+S2, c128 [nk][Nm][Nb][Nb]       16 Nb^2 Nm nk  (mode basis, amplitude applied)
+ *   EPW_DBG_H_K     H(k)     c128 [nk][Nb][Nb] column-major           16 Nb^2 nk
+ *   EPW_DBG_U_K     U_k      c128 [nk][Nb][Nb] columns = eigenvectors 16 Nb^2 nk
+ *   EPW_DBG_U_KQ    U_{k+q}  c128 [nk][Nb][Nb] (per-pair solves only) 16 Nb^2 nk
+ *   EPW_DBG_E_Q     e_q      c128 [Nm][Nm] columns = mode eigenvectors 16 Nm^2
+ */
+enum { EPW_DBG_G_REQ = 1, EPW_DBG_G_TILDE = 2, EPW_DBG_H_K = 3, EPW_DBG_U_K = 4, EPW_DBG_U_KQ = 5, EPW_DBG_E_Q = 6 };
+int64_t epw_interp_debug_get(epw_interp_t h, int what, void *dst_host, size_t bytes);
+
+const char *epw_interp_last_error(epw_interp_t h); /* h may be NULL: last error of a failed create */
+
+/* -------------------------------------------------------------------------------------------------
+ * Stage-level entry points (same kernels the path uses; device pointers; asynchronous on `cuda_stream`).
+ * They exist so that each kernel can be parity-tested against the oracle on its own.
+ * ----------------------------------------------------------------------------------------------- */
+
+/* S0: P[ix][ir] = w[ir] * exp(2 pi i frac(x_ix . R_ir)), c128 [nx][nr] row-major. */
+int epw_phase_table(const double *x_list, int64_t nx, const int32_t *R, const double *w, int32_t nr, void *P_out,
+                    void *cuda_stream);
+
+/* S1 (Eq. 9) for a batch of q: g1[iq] = sum_ip g_RR[ip] * Pq[iq][ip];  rows = Nb^2 Ne Nm.
+ * g_RR c128 [np][rows], Pq c128 [nq][np] (weights included), g1 c128 [nq][rows].  nq <= 8 per call. */
+int epw_rp_to_q(const void *g_RR, int64_t rows, int32_t np, const void *Pq, int32_t nq, void *g1_out,
+                void *cuda_stream);
+
+/* S3a: Op(x)[ix] = sum_ir P[ix][ir] Op_R[ir], n x n matrices (column-major), P from epw_phase_table. */
+int epw_interp_operator(const void *Op_R, int32_t n, int32_t nr, const void *P, int64_t nx, void *out,
+                        void *cuda_stream);
+
+/* S3b: batched Hermitian eigensolve (parallel-order Jacobi).  A c128 [batch] matrices, column-major, matrix b at
+ * A + b*stride_a (stride in c128 elements); only its Hermitian part (A + A^dagger)/2 is used.
+ * evals f64 [batch][n] ascending; V c128 [batch][n][n], columns = eigenvectors.
+ * sqrt_mode != 0 writes omega = sign(lambda) sqrt(|lambda|) instead of lambda.
+ * status: int32 device word, set to nonzero if any solve hits the sweep limit (may be NULL). */
+int epw_eigh_batched(const void *A, int64_t stride_a, int32_t n, int64_t batch, double *evals, void *V,
+                     int sqrt_mode, int32_t *status, void *cuda_stream);
+
+/* Dense complex FP64 contraction on the FP64 tensor path:  C[m][n] = sum_r A[m][r] B[r][n],
+ * A c128 [M][K] row-major, B c128 [K][N] row-major, C c128 [M][ldc] row-major (ldc >= N).
+ * (Packs both operands into the DMMA fragment layout, then runs the same TMA + DMMA kernel as S2.) */
+int epw_zgemm(const void *A, const void *B, void *C, int64_t M, int32_t N, int32_t K, int64_t ldc, void *cuda_stream);
+
+/* S4b: g2[ik][nu][n][m] = | sum_{m'n'} conj(Ukq[ik][m',m]) gt[ik][nu][n'][m'] Uk[ik][n',n] |^2.
+ * gt c128, pair ik at gt + ik*stride_gt (c128 elements); Uk, Ukq c128 [..][Nb][Nb] column-major;
+ * kq_idx NULL (Ukq indexed by ik) or int32 [nk] (Ukq indexed by kq_idx[ik]). */
+int epw_rotate_g2(const void *gt, int64_t stride_gt, const void *Uk, const void *Ukq, const int32_t *kq_idx,
+                  int32_t nb, int32_t nm, int64_t nk, double *g2, void *cuda_stream);
+
+/* Roofline denominators measured on this device ("Measurement"): FP64 tensor (DMMA m8n8k4) TFLOP/s,
+ * plain DFMA TFLOP/s and HBM read / copy GB/s from tight probe kernels.  out[0..3]; returns 0 or a status. */
+int epw_probe_peaks(int32_t device, double *out4);
+
+const char *epw_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EPW_INTERP_H_ */

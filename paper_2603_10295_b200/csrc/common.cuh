@@ -1,0 +1,98 @@
+// common.cuh -- shared helpers of the CUDA library (sm_100a only).  Nothing in here is used by oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/epw_interp.h"
+
+namespace epw {
+
+typedef double2 c128;  // (re, im)
+
+__host__ __device__ __forceinline__ c128 cmake(double re, double im) { return make_double2(re, im); }
+__device__ __forceinline__ c128 cmul(c128 a, c128 b) {
+  return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+// acc += a * b
+__device__ __forceinline__ void cfma(c128 &acc, c128 a, c128 b) {
+  acc.x = fma(a.x, b.x, acc.x);
+  acc.x = fma(-a.y, b.y, acc.x);
+  acc.y = fma(a.x, b.y, acc.y);
+  acc.y = fma(a.y, b.x, acc.y);
+}
+// acc += conj(a) * b
+__device__ __forceinline__ void cfma_conj(c128 &acc, c128 a, c128 b) {
+  acc.x = fma(a.x, b.x, acc.x);
+  acc.x = fma(a.y, b.y, acc.x);
+  acc.y = fma(a.x, b.y, acc.y);
+  acc.y = fma(-a.y, b.x, acc.y);
+}
+__device__ __forceinline__ c128 cconj(c128 a) { return make_double2(a.x, -a.y); }
+__device__ __forceinline__ double cabs2(c128 a) { return a.x * a.x + a.y * a.y; }
+
+static inline int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
+static inline int64_t round_up(int64_t a, int64_t b) { return ceil_div(a, b) * b; }
+
+// ---- DMMA GEMM operand packing (see zgemm_dmma.cu for the kernel and DESIGN.md "Data layout") -----------------
+// Real embedding of a complex contraction C = A B:
+//   A'[m][2r+a]     = (a ? Im : Re) A[m][r]
+//   B'[2r+a][2n+b]  = a==0 ? (b ? Im : Re) B[r][n] : (b ? Re : -Im) B[r][n]
+//   C'[m][2n+b]     = (b ? Im : Re) C[m][n]
+// Tiles: BM = 128 rows, BN = 128 real columns (64 complex), BK = 16 real k (8 complex).
+// Each (tile, k-block) chunk is 2048 doubles = 16 KB, contiguous, already in the per-lane order of the
+// mma.m8n8k4.f64 fragments, so one 1-D bulk TMA copy brings it to shared memory and every fragment load is a
+// conflict-free LDS.128.
+constexpr int GEMM_BM = 128;
+constexpr int GEMM_BN = 128;  // real columns per tile
+constexpr int GEMM_BK = 16;   // real k per block
+constexpr int GEMM_CHUNK = 2048;  // doubles per (tile, k-block) chunk of either operand
+
+// offset (in doubles) inside an A chunk of element (row mr in [0,128), real k kc in [0,16))
+__host__ __device__ __forceinline__ int apack_offset(int mr, int kc) {
+  const int wm = mr >> 6, i = (mr >> 3) & 7, g = mr & 7;
+  const int ks = kc >> 2, t = kc & 3;
+  return ((((wm * 4 + ks) * 4 + (i >> 1)) * 32 + (g * 4 + t)) << 1) + (i & 1);
+}
+// offset inside a B chunk of element (real k kc in [0,16), real column nc in [0,128))
+__host__ __device__ __forceinline__ int bpack_offset(int kc, int nc) {
+  const int wn = nc >> 5, j = (nc >> 3) & 3, g = nc & 7;
+  const int ks = kc >> 2, t = kc & 3;
+  return ((((wn * 4 + ks) * 2 + (j >> 1)) * 32 + (g * 4 + t)) << 1) + (j & 1);
+}
+
+// ---- kernel launchers (one per .cu file) ------------------------------------------------------------------
+// All are asynchronous on `st` and return the cudaGetLastError() of their launches.
+cudaError_t launch_phase_table(const double *x, int64_t nx, const int32_t *R, const double *w, int nr, c128 *P,
+                               cudaStream_t st);
+// phases for x = k-points written directly as the packed A' operand (zero padded to [Mpad][Kpad'])
+cudaError_t launch_phase_pack_a(const double *x, int64_t nx, const int32_t *R, const double *w, int nr, double *Apack,
+                                cudaStream_t st);
+cudaError_t launch_rp_to_q(const c128 *g, int64_t rows, int np, const c128 *Pq, int nq, c128 *g1, cudaStream_t st);
+cudaError_t launch_interp_operator(const c128 *OpR, int n, int nr, const c128 *P, int64_t nx, c128 *out,
+                                   cudaStream_t st);
+cudaError_t launch_eigh_batched(const c128 *A, int64_t stride_a, int n, int64_t batch, double *evals, c128 *V,
+                                int sqrt_mode, int32_t *status, c128 *scratch_large, cudaStream_t st);
+size_t eigh_large_scratch_bytes(int n, int64_t batch);
+
+// Build the packed B' operand for one q:
+//   complex column c <  nm*nbb : sum_ka g1[ka][r][el] * e[ka + nm*nu] * amp[nu]     (c = nu*nbb + el)   (S4a hoisted)
+//   complex column c >= nm*nbb : phase_qe[r] * H_R[r][el]                            (H(k+q) columns; only if ncols_h)
+// g1 c128 [nm][ne][nbb]; e c128 column-major [nm][nm] (NULL = identity, amp = 1); omega f64 [nm];
+// phase_qe c128 [ne] (NULL = 1).  Bpack doubles [NT][KB][2048].
+cudaError_t launch_pack_b(const c128 *g1, const c128 *e, const double *omega, double omega_min, const c128 *H_R,
+                          const c128 *phase_qe, int nbb, int nm, int ne, int ncols_g, int ncols_h, double *Bpack,
+                          cudaStream_t st);
+// generic packers for epw_zgemm (row-major complex A [M][K], B [K][N])
+cudaError_t launch_pack_a_generic(const c128 *A, int64_t M, int K, double *Apack, cudaStream_t st);
+cudaError_t launch_pack_b_generic(const c128 *B, int K, int N, double *Bpack, cudaStream_t st);
+
+// C[m][n] (c128, row-major, ldc) for m in [0,M), n in [0,N); Apack holds m-tiles mt0.. of a table with KB k-blocks.
+cudaError_t launch_zgemm_dmma(const double *Apack, const double *Bpack, c128 *C, int64_t M, int N, int KB, int64_t ldc,
+                              int num_sms, cudaStream_t st);
+
+cudaError_t launch_rotate_g2(const c128 *gt, int64_t stride_gt, const c128 *Uk, const c128 *Ukq, const int32_t *kq_idx,
+                             int nb, int nm, int64_t nk, double *g2, cudaStream_t st);
+
+int probe_peaks(int device, double *out4);
+
+}  // namespace epw

@@ -1,0 +1,574 @@
+// interp.cu -- handle, memory plan, stage orchestration and the extern "C" boundary (include/epw_interp.h).
+//
+// Loop structure = the paper's nested-loop algorithm (Fig. 1b; Fig. 12): Eq. 9 once
+// per q in the outer loop, Eq. 10 for every k in the inner loop -- except that here the inner loop is a batched
+// tensor contraction on the device instead of one CPU thread per k, nothing returns to the host inside the loop
+// (the paper copies x to and y from the device every q), and q-points are taken q_batch at a
+// time through S1 so that g(Re,Rp) is streamed from HBM once per batch rather than once per q.
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "common.cuh"
+
+using namespace epw;
+
+namespace {
+
+std::string g_create_error;
+
+struct DevBuf {
+  void *p = nullptr;
+  size_t bytes = 0;
+  cudaError_t reserve(size_t want) {
+    if (want <= bytes) return cudaSuccess;
+    if (p) cudaFree(p);
+    p = nullptr;
+    bytes = 0;
+    cudaError_t e = cudaMalloc(&p, want);
+    if (e == cudaSuccess) bytes = want;
+    return e;
+  }
+  void release() {
+    if (p) cudaFree(p);
+    p = nullptr;
+    bytes = 0;
+  }
+  template <class T>
+  T *as() const { return reinterpret_cast<T *>(p); }
+};
+
+__global__ void gather_eps_kernel(const double *__restrict__ eps_k, const int32_t *__restrict__ kq_idx, int nb,
+                                  int64_t nk, double *__restrict__ eps_kq) {
+  const int64_t total = nk * nb;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t ik = i / nb;
+    const int b = (int)(i - ik * nb);
+    eps_kq[i] = eps_k[(int64_t)kq_idx[ik] * nb + b];
+  }
+}
+
+__global__ void fill_ones_kernel(double *p, int n) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) p[i] = 1.0;
+}
+
+}  // namespace
+
+struct epw_interp {
+  epw_interp_config cfg{};
+  int nb = 0, nm = 0, ne = 0, np = 0, nbb = 0, nmm = 0;
+  int64_t rows = 0;  // Nb^2 Ne Nm = rows of Fig. 13's A(m,n)
+  int num_sms = 148;
+  int q_batch = 4;
+  bool operators_set = false;
+  std::vector<char> slab_set;
+  // resident operators
+  DevBuf g, H, D, Re, Rp, we, wp, ones;
+  // per-call workspace
+  DevBuf Apack, BpackH, Hk, Uk, Pq, Pqe, Dq, eq, g1, Bpack, C, Ukq, epskq_scratch, status, eig_scratch;
+  // host-entry staging
+  DevBuf hs_k, hs_q, hs_map, hs_epsk, hs_epskq, hs_omega, hs_g2;
+  // bookkeeping of the last call
+  int64_t last_nk = 0, last_c_rows = 0, last_c_row0 = 0;
+  int last_ncols = 0;
+  int64_t launches = 0;
+  cudaStream_t last_stream = nullptr;
+  bool timing = false;
+  std::vector<cudaEvent_t> ev_pool;
+  struct Span { int stage; int e0, e1; };
+  std::vector<Span> spans;
+  size_t ev_used = 0;
+  std::string last_error;
+
+  int fail(int code, const std::string &msg) {
+    last_error = msg;
+    return code;
+  }
+  int cuda_fail(cudaError_t e, const char *where) {
+    last_error = std::string(where) + ": " + cudaGetErrorString(e);
+    return e == cudaErrorMemoryAllocation ? EPW_ENOMEM : EPW_ECUDA;
+  }
+  int begin_span(int stage, cudaStream_t st) {
+    if (!timing) return -1;
+    if (ev_used + 2 > ev_pool.size()) {
+      const size_t old = ev_pool.size();
+      ev_pool.resize(old + 64);
+      for (size_t i = old; i < ev_pool.size(); i++) cudaEventCreate(&ev_pool[i]);
+    }
+    Span s{stage, (int)ev_used, (int)ev_used + 1};
+    ev_used += 2;
+    cudaEventRecord(ev_pool[s.e0], st);
+    spans.push_back(s);
+    return (int)spans.size() - 1;
+  }
+  void end_span(int id, cudaStream_t st) {
+    if (id >= 0) cudaEventRecord(ev_pool[spans[id].e1], st);
+  }
+};
+
+#define CU_OR_FAIL(h, expr, where)                        \
+  do {                                                    \
+    cudaError_t _e = (expr);                              \
+    if (_e != cudaSuccess) return (h)->cuda_fail(_e, where); \
+  } while (0)
+#define LAUNCH(h, expr, where) \
+  do {                         \
+    (h)->launches++;           \
+    CU_OR_FAIL(h, expr, where); \
+  } while (0)
+
+extern "C" {
+
+const char *epw_version(void) { return "epw-interp-b200 0.1 (sm_100a, FP64 DMMA)"; }
+
+const char *epw_interp_last_error(epw_interp_t h) { return h ? h->last_error.c_str() : g_create_error.c_str(); }
+
+int epw_interp_create(epw_interp_t *out, const epw_interp_config *cfg) {
+  if (!out) return EPW_EINVAL;
+  *out = nullptr;
+  if (!cfg || cfg->nbnd <= 0 || cfg->nmodes <= 0 || cfg->ne <= 0 || cfg->np <= 0) {
+    g_create_error = "epw_interp_create: nbnd, nmodes, ne, np must be positive";
+    return EPW_EINVAL;
+  }
+  if (cfg->q_batch < 0 || cfg->q_batch > 8) {
+    g_create_error = "epw_interp_create: q_batch must be in 0..8";
+    return EPW_EINVAL;
+  }
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || cfg->device < 0 || cfg->device >= ndev) {
+    g_create_error = std::string("epw_interp_create: no usable CUDA device (") +
+                     (e != cudaSuccess ? cudaGetErrorString(e) : "bad ordinal") + "); there is no CPU fallback";
+    return EPW_ECUDA;
+  }
+  cudaDeviceProp prop;
+  if (cudaSetDevice(cfg->device) != cudaSuccess || cudaGetDeviceProperties(&prop, cfg->device) != cudaSuccess) {
+    g_create_error = "epw_interp_create: cudaSetDevice failed";
+    return EPW_ECUDA;
+  }
+  if (prop.major != 10) {
+    g_create_error = "epw_interp_create: this library is built for sm_100a (Blackwell B200) only";
+    return EPW_ECUDA;
+  }
+  epw_interp *h = new (std::nothrow) epw_interp();
+  if (!h) return EPW_ENOMEM;
+  h->cfg = *cfg;
+  h->nb = cfg->nbnd;
+  h->nm = cfg->nmodes;
+  h->ne = cfg->ne;
+  h->np = cfg->np;
+  h->nbb = h->nb * h->nb;
+  h->nmm = h->nm * h->nm;
+  h->rows = (int64_t)h->nbb * h->ne * h->nm;
+  h->num_sms = prop.multiProcessorCount;
+  h->q_batch = cfg->q_batch > 0 ? cfg->q_batch : 4;
+  h->slab_set.assign(h->np, 0);
+  *out = h;
+  return EPW_OK;
+}
+
+void epw_interp_destroy(epw_interp_t h) {
+  if (!h) return;
+  cudaSetDevice(h->cfg.device);
+  if (h->last_stream || true) cudaDeviceSynchronize();
+  DevBuf *all[] = {&h->g, &h->H, &h->D, &h->Re, &h->Rp, &h->we, &h->wp, &h->ones, &h->Apack, &h->BpackH, &h->Hk,
+                   &h->Uk, &h->Pq, &h->Pqe, &h->Dq, &h->eq, &h->g1, &h->Bpack, &h->C, &h->Ukq, &h->epskq_scratch,
+                   &h->status, &h->eig_scratch, &h->hs_k, &h->hs_q, &h->hs_map, &h->hs_epsk, &h->hs_epskq,
+                   &h->hs_omega, &h->hs_g2};
+  for (DevBuf *b : all) b->release();
+  for (cudaEvent_t ev : h->ev_pool) cudaEventDestroy(ev);
+  delete h;
+}
+
+int epw_interp_set_g_slabs(epw_interp_t h, int32_t ip_start, int32_t ip_count, const void *g_slabs, int on_device) {
+  if (!h) return EPW_EINVAL;
+  if (!g_slabs || ip_start < 0 || ip_count <= 0 || ip_start + ip_count > h->np)
+    return h->fail(EPW_EINVAL, "epw_interp_set_g_slabs: bad slab range or null pointer");
+  CU_OR_FAIL(h, cudaSetDevice(h->cfg.device), "cudaSetDevice");
+  const size_t total = (size_t)h->rows * h->np * sizeof(c128);
+  CU_OR_FAIL(h, h->g.reserve(total), "cudaMalloc g(Re,Rp)");
+  const size_t slab = (size_t)h->rows * sizeof(c128);
+  CU_OR_FAIL(h,
+             cudaMemcpy(h->g.as<char>() + slab * ip_start, g_slabs, slab * ip_count,
+                        on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice),
+             "cudaMemcpy g slabs");
+  for (int i = 0; i < ip_count; i++) h->slab_set[ip_start + i] = 1;
+  return EPW_OK;
+}
+
+int epw_interp_set_wannier_operators(epw_interp_t h, const void *H_R, const void *D_R, const void *g_RR,
+                                     const int32_t *Re, const double *w_e, const int32_t *Rp, const double *w_p,
+                                     int on_device) {
+  if (!h) return EPW_EINVAL;
+  if (!H_R || !D_R || !Re || !w_e || !Rp || !w_p)
+    return h->fail(EPW_EINVAL, "epw_interp_set_wannier_operators: null operator pointer");
+  CU_OR_FAIL(h, cudaSetDevice(h->cfg.device), "cudaSetDevice");
+  const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  struct Item { DevBuf *buf; const void *src; size_t bytes; };
+  const Item items[] = {{&h->H, H_R, sizeof(c128) * (size_t)h->nbb * h->ne},
+                        {&h->D, D_R, sizeof(c128) * (size_t)h->nmm * h->np},
+                        {&h->Re, Re, sizeof(int32_t) * 3 * (size_t)h->ne},
+                        {&h->we, w_e, sizeof(double) * (size_t)h->ne},
+                        {&h->Rp, Rp, sizeof(int32_t) * 3 * (size_t)h->np},
+                        {&h->wp, w_p, sizeof(double) * (size_t)h->np}};
+  for (const Item &it : items) {
+    CU_OR_FAIL(h, it.buf->reserve(it.bytes), "cudaMalloc operators");
+    CU_OR_FAIL(h, cudaMemcpy(it.buf->p, it.src, it.bytes, kind), "cudaMemcpy operators");
+  }
+  const int nmax = std::max(h->ne, h->np);
+  CU_OR_FAIL(h, h->ones.reserve(sizeof(double) * nmax), "cudaMalloc ones");
+  fill_ones_kernel<<<(nmax + 255) / 256, 256>>>(h->ones.as<double>(), nmax);
+  CU_OR_FAIL(h, cudaDeviceSynchronize(), "fill_ones");
+  h->operators_set = true;
+  if (g_RR) return epw_interp_set_g_slabs(h, 0, h->np, g_RR, on_device);
+  return EPW_OK;
+}
+
+int epw_interp_enable_stage_timing(epw_interp_t h, int on) {
+  if (!h) return EPW_EINVAL;
+  h->timing = on != 0;
+  return EPW_OK;
+}
+
+int epw_interp_interpolate(epw_interp_t h, const double *k_list, int64_t nk, const double *q_list, int64_t nq,
+                           const int32_t *kq_map, double *eps_k, double *eps_kq, double *omega_q, double *g2,
+                           void *cuda_stream) {
+  if (!h) return EPW_EINVAL;
+  if (!k_list || !q_list || !eps_k || !omega_q || !g2 || nk <= 0 || nq <= 0)
+    return h->fail(EPW_EINVAL, "epw_interp_interpolate: null pointer or non-positive nk/nq");
+  if (!h->operators_set) return h->fail(EPW_EINVAL, "epw_interp_interpolate: operators not set");
+  for (int ip = 0; ip < h->np; ip++)
+    if (!h->slab_set[ip]) return h->fail(EPW_EINVAL, "epw_interp_interpolate: g(Re,Rp) slab missing");
+  if (h->nb > 16) return h->fail(EPW_EUNSUPPORTED, "epw_interp_interpolate: nbnd > 16 path not built yet");
+  CU_OR_FAIL(h, cudaSetDevice(h->cfg.device), "cudaSetDevice");
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  h->last_stream = st;
+  h->launches = 0;
+  h->spans.clear();
+  h->ev_used = 0;
+
+  const int nb = h->nb, nm = h->nm, ne = h->ne, np = h->np, nbb = h->nbb, nmm = h->nmm;
+  const int ncols_g = nbb * nm;
+  const int ncols_h = kq_map ? 0 : nbb;
+  const int ncols = ncols_g + ncols_h;
+  const int KB = (int)ceil_div(2 * (int64_t)ne, GEMM_BK);
+  const int NT = (int)ceil_div(2 * (int64_t)ncols, GEMM_BN);
+  const int NTH = (int)ceil_div(2 * (int64_t)nbb, GEMM_BN);
+  const int64_t MT = ceil_div(nk, GEMM_BM);
+  const int QB = (int)std::min<int64_t>(h->q_batch, nq);
+  const int64_t E = (int64_t)ncols_g;
+
+  // k-chunk: keep one chunk of g~ (16*ncols bytes per k) around 48 MB so that the rotation kernel finds it in L2
+  int64_t kchunk = ((48ll << 20) / ((int64_t)ncols * 16)) / GEMM_BM * GEMM_BM;
+  kchunk = std::max<int64_t>(kchunk, GEMM_BM);
+  // rows of the g~ buffer kept (all of nk when it fits the cap; else a multiple of kchunk that is reused)
+  size_t cap = h->cfg.workspace_bytes ? h->cfg.workspace_bytes : ((size_t)6 << 30);
+  int64_t c_rows = MT * GEMM_BM;
+  if ((size_t)c_rows * ncols * 16 > cap) c_rows = std::max<int64_t>(kchunk, (int64_t)(cap / ((size_t)ncols * 16)) / kchunk * kchunk);
+
+  // ---- workspace ----
+  CU_OR_FAIL(h, h->Apack.reserve(sizeof(double) * (size_t)MT * KB * GEMM_CHUNK), "cudaMalloc Apack");
+  CU_OR_FAIL(h, h->BpackH.reserve(sizeof(double) * (size_t)NTH * KB * GEMM_CHUNK), "cudaMalloc BpackH");
+  CU_OR_FAIL(h, h->Hk.reserve(sizeof(c128) * (size_t)nk * nbb), "cudaMalloc Hk");
+  CU_OR_FAIL(h, h->Uk.reserve(sizeof(c128) * (size_t)nk * nbb), "cudaMalloc Uk");
+  CU_OR_FAIL(h, h->Pq.reserve(sizeof(c128) * (size_t)QB * np), "cudaMalloc Pq");
+  CU_OR_FAIL(h, h->Pqe.reserve(sizeof(c128) * (size_t)QB * ne), "cudaMalloc Pqe");
+  CU_OR_FAIL(h, h->Dq.reserve(sizeof(c128) * (size_t)QB * nmm), "cudaMalloc Dq");
+  CU_OR_FAIL(h, h->eq.reserve(sizeof(c128) * (size_t)QB * nmm), "cudaMalloc e_q");
+  CU_OR_FAIL(h, h->g1.reserve(sizeof(c128) * (size_t)QB * h->rows), "cudaMalloc g(Re,q)");
+  CU_OR_FAIL(h, h->Bpack.reserve(sizeof(double) * (size_t)QB * NT * KB * GEMM_CHUNK), "cudaMalloc Bpack");
+  CU_OR_FAIL(h, h->C.reserve(sizeof(c128) * (size_t)c_rows * ncols), "cudaMalloc g~");
+  if (!kq_map) CU_OR_FAIL(h, h->Ukq.reserve(sizeof(c128) * (size_t)c_rows * nbb), "cudaMalloc Ukq");
+  if (!kq_map && !eps_kq) CU_OR_FAIL(h, h->epskq_scratch.reserve(sizeof(double) * (size_t)c_rows * nb), "cudaMalloc eps scratch");
+  CU_OR_FAIL(h, h->status.reserve(sizeof(int32_t)), "cudaMalloc status");
+  {
+    const size_t need = std::max(eigh_large_scratch_bytes(nb, nk), eigh_large_scratch_bytes(nm, QB));
+    if (need) CU_OR_FAIL(h, h->eig_scratch.reserve(need), "cudaMalloc eig scratch");
+  }
+  CU_OR_FAIL(h, cudaMemsetAsync(h->status.p, 0, sizeof(int32_t), st), "memset status");
+  h->last_nk = nk;
+  h->last_c_rows = c_rows;
+  h->last_ncols = ncols;
+
+  const int t_total = h->begin_span(7, st);
+
+  // ---- k side (once per call): S0 phases in packed-A form, H(k) by the same DMMA contraction, eigensolve ----
+  int sp = h->begin_span(0, st);
+  LAUNCH(h, launch_phase_pack_a(k_list, nk, h->Re.as<int32_t>(), h->we.as<double>(), ne, h->Apack.as<double>(), st),
+         "phase_pack_a");
+  h->end_span(sp, st);
+  sp = h->begin_span(3, st);
+  LAUNCH(h,
+         launch_pack_b(nullptr, nullptr, nullptr, 0.0, h->H.as<c128>(), nullptr, nbb, nm, ne, 0, nbb,
+                       h->BpackH.as<double>(), st),
+         "pack_b(H)");
+  LAUNCH(h, launch_zgemm_dmma(h->Apack.as<double>(), h->BpackH.as<double>(), h->Hk.as<c128>(), nk, nbb, KB, nbb,
+                              h->num_sms, st),
+         "zgemm H(k)");
+  LAUNCH(h, launch_eigh_batched(h->Hk.as<c128>(), nbb, nb, nk, eps_k, h->Uk.as<c128>(), 0, h->status.as<int32_t>(),
+                                h->eig_scratch.as<c128>(), st),
+         "eigh H(k)");
+  h->end_span(sp, st);
+
+  for (int64_t q0 = 0; q0 < nq; q0 += QB) {
+    const int qb = (int)std::min<int64_t>(QB, nq - q0);
+    // ---- S0 for this q batch ----
+    sp = h->begin_span(0, st);
+    LAUNCH(h, launch_phase_table(q_list + 3 * q0, qb, h->Rp.as<int32_t>(), h->wp.as<double>(), np, h->Pq.as<c128>(), st),
+           "phase_table(q,Rp)");
+    if (ncols_h)
+      LAUNCH(h, launch_phase_table(q_list + 3 * q0, qb, h->Re.as<int32_t>(), h->ones.as<double>(), ne,
+                                   h->Pqe.as<c128>(), st),
+             "phase_table(q,Re)");
+    h->end_span(sp, st);
+    // ---- S1: Eq. 9 for the batch ----
+    sp = h->begin_span(1, st);
+    LAUNCH(h, launch_rp_to_q(h->g.as<c128>(), h->rows, np, h->Pq.as<c128>(), qb, h->g1.as<c128>(), st), "rp_to_q");
+    h->end_span(sp, st);
+    // ---- phonons: D(q), eigensolve, S4a hoisted into the packed B operand ----
+    sp = h->begin_span(2, st);
+    LAUNCH(h, launch_interp_operator(h->D.as<c128>(), nm, np, h->Pq.as<c128>(), qb, h->Dq.as<c128>(), st), "D(q)");
+    LAUNCH(h, launch_eigh_batched(h->Dq.as<c128>(), nmm, nm, qb, omega_q + q0 * nm, h->eq.as<c128>(), 1,
+                                  h->status.as<int32_t>(), h->eig_scratch.as<c128>(), st),
+           "eigh D(q)");
+    for (int iq = 0; iq < qb; iq++)
+      LAUNCH(h,
+             launch_pack_b(h->g1.as<c128>() + (int64_t)iq * h->rows, h->eq.as<c128>() + (int64_t)iq * nmm,
+                           omega_q + (q0 + iq) * nm, h->cfg.omega_min, h->H.as<c128>(),
+                           ncols_h ? h->Pqe.as<c128>() + (int64_t)iq * ne : nullptr, nbb, nm, ne, ncols_g, ncols_h,
+                           h->Bpack.as<double>() + (int64_t)iq * NT * KB * GEMM_CHUNK, st),
+             "pack_b");
+    h->end_span(sp, st);
+
+    for (int iq = 0; iq < qb; iq++) {
+      const int64_t q = q0 + iq;
+      const double *Bq = h->Bpack.as<double>() + (int64_t)iq * NT * KB * GEMM_CHUNK;
+      for (int64_t k0 = 0; k0 < nk; k0 += kchunk) {
+        const int64_t kn = std::min(kchunk, nk - k0);
+        const int64_t crow = k0 % c_rows;
+        c128 *Cc = h->C.as<c128>() + crow * ncols;
+        // ---- S2: Re -> k contraction (+ H(k+q) columns) ----
+        sp = h->begin_span(4, st);
+        LAUNCH(h, launch_zgemm_dmma(h->Apack.as<double>() + (k0 / GEMM_BM) * (int64_t)KB * GEMM_CHUNK, Bq, Cc, kn, ncols,
+                                    KB, ncols, h->num_sms, st),
+               "zgemm S2");
+        h->end_span(sp, st);
+        const c128 *Ukq_ptr;
+        const int32_t *kq_idx = nullptr;
+        if (kq_map) {
+          Ukq_ptr = h->Uk.as<c128>();
+          kq_idx = kq_map + q * nk + k0;
+          if (eps_kq) {
+            sp = h->begin_span(5, st);
+            h->launches++;
+            gather_eps_kernel<<<(unsigned)std::min<int64_t>(ceil_div(kn * nb, 256), 148 * 8), 256, 0, st>>>(
+                eps_k, kq_idx, nb, kn, eps_kq + (q * nk + k0) * nb);
+            CU_OR_FAIL(h, cudaGetLastError(), "gather_eps");
+            h->end_span(sp, st);
+          }
+        } else {
+          // ---- S3b per pair: eigensolve the H(k+q) block of the contraction output ----
+          sp = h->begin_span(5, st);
+          c128 *Ukq_c = h->Ukq.as<c128>() + crow * nbb;
+          double *eps_dst = eps_kq ? eps_kq + (q * nk + k0) * nb : h->epskq_scratch.as<double>() + crow * nb;
+          LAUNCH(h, launch_eigh_batched(Cc + ncols_g, ncols, nb, kn, eps_dst, Ukq_c, 0, h->status.as<int32_t>(),
+                                        h->eig_scratch.as<c128>(), st),
+                 "eigh H(k+q)");
+          h->end_span(sp, st);
+          Ukq_ptr = Ukq_c;
+        }
+        // ---- S4b: band rotation + |g|^2 ----
+        sp = h->begin_span(6, st);
+        LAUNCH(h, launch_rotate_g2(Cc, ncols, h->Uk.as<c128>() + k0 * nbb, Ukq_ptr, kq_idx, nb, nm, kn,
+                                   g2 + (q * nk + k0) * E, st),
+               "rotate_g2");
+        h->end_span(sp, st);
+        h->last_c_row0 = k0 - crow;
+      }
+    }
+  }
+  h->end_span(t_total, st);
+  return EPW_OK;
+}
+
+int epw_interp_sync(epw_interp_t h) {
+  if (!h) return EPW_EINVAL;
+  CU_OR_FAIL(h, cudaSetDevice(h->cfg.device), "cudaSetDevice");
+  CU_OR_FAIL(h, cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize");
+  if (h->status.p) {
+    int32_t s = 0;
+    CU_OR_FAIL(h, cudaMemcpy(&s, h->status.p, sizeof(s), cudaMemcpyDeviceToHost), "cudaMemcpy status");
+    if (s) return h->fail(EPW_ENOTCONVERGED, "a Jacobi eigensolve did not converge within the sweep limit");
+  }
+  return EPW_OK;
+}
+
+int epw_interp_interpolate_host(epw_interp_t h, const double *k_list, int64_t nk, const double *q_list, int64_t nq,
+                                const int32_t *kq_map, double *eps_k, double *eps_kq, double *omega_q, double *g2,
+                                void *cuda_stream) {
+  if (!h) return EPW_EINVAL;
+  if (!k_list || !q_list || !eps_k || !omega_q || !g2 || nk <= 0 || nq <= 0)
+    return h->fail(EPW_EINVAL, "epw_interp_interpolate_host: null pointer or non-positive nk/nq");
+  CU_OR_FAIL(h, cudaSetDevice(h->cfg.device), "cudaSetDevice");
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  const size_t E = (size_t)h->nbb * h->nm;
+  CU_OR_FAIL(h, h->hs_k.reserve(sizeof(double) * 3 * nk), "cudaMalloc k staging");
+  CU_OR_FAIL(h, h->hs_q.reserve(sizeof(double) * 3 * nq), "cudaMalloc q staging");
+  if (kq_map) CU_OR_FAIL(h, h->hs_map.reserve(sizeof(int32_t) * nk * nq), "cudaMalloc kq_map staging");
+  CU_OR_FAIL(h, h->hs_epsk.reserve(sizeof(double) * nk * h->nb), "cudaMalloc eps_k staging");
+  if (eps_kq) CU_OR_FAIL(h, h->hs_epskq.reserve(sizeof(double) * nk * nq * h->nb), "cudaMalloc eps_kq staging");
+  CU_OR_FAIL(h, h->hs_omega.reserve(sizeof(double) * nq * h->nm), "cudaMalloc omega staging");
+  CU_OR_FAIL(h, h->hs_g2.reserve(sizeof(double) * E * nk * nq), "cudaMalloc g2 staging");
+  CU_OR_FAIL(h, cudaMemcpyAsync(h->hs_k.p, k_list, sizeof(double) * 3 * nk, cudaMemcpyHostToDevice, st), "H2D k");
+  CU_OR_FAIL(h, cudaMemcpyAsync(h->hs_q.p, q_list, sizeof(double) * 3 * nq, cudaMemcpyHostToDevice, st), "H2D q");
+  if (kq_map)
+    CU_OR_FAIL(h, cudaMemcpyAsync(h->hs_map.p, kq_map, sizeof(int32_t) * nk * nq, cudaMemcpyHostToDevice, st), "H2D map");
+  const int rc = epw_interp_interpolate(h, h->hs_k.as<double>(), nk, h->hs_q.as<double>(), nq,
+                                        kq_map ? h->hs_map.as<int32_t>() : nullptr, h->hs_epsk.as<double>(),
+                                        eps_kq ? h->hs_epskq.as<double>() : nullptr, h->hs_omega.as<double>(),
+                                        h->hs_g2.as<double>(), cuda_stream);
+  if (rc != EPW_OK) return rc;
+  CU_OR_FAIL(h, cudaMemcpyAsync(eps_k, h->hs_epsk.p, sizeof(double) * nk * h->nb, cudaMemcpyDeviceToHost, st), "D2H eps_k");
+  if (eps_kq)
+    CU_OR_FAIL(h, cudaMemcpyAsync(eps_kq, h->hs_epskq.p, sizeof(double) * nk * nq * h->nb, cudaMemcpyDeviceToHost, st),
+               "D2H eps_kq");
+  CU_OR_FAIL(h, cudaMemcpyAsync(omega_q, h->hs_omega.p, sizeof(double) * nq * h->nm, cudaMemcpyDeviceToHost, st), "D2H omega");
+  CU_OR_FAIL(h, cudaMemcpyAsync(g2, h->hs_g2.p, sizeof(double) * E * nk * nq, cudaMemcpyDeviceToHost, st), "D2H g2");
+  return epw_interp_sync(h);
+}
+
+int epw_interp_get_stage_times(epw_interp_t h, double *ms, int n) {
+  if (!h || !ms || n <= 0) return EPW_EINVAL;
+  CU_OR_FAIL(h, cudaSetDevice(h->cfg.device), "cudaSetDevice");
+  CU_OR_FAIL(h, cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize");
+  const int m = std::min(n, (int)EPW_NUM_STAGES);
+  for (int i = 0; i < m; i++) ms[i] = 0.0;
+  for (const auto &s : h->spans) {
+    float t = 0.f;
+    if (cudaEventElapsedTime(&t, h->ev_pool[s.e0], h->ev_pool[s.e1]) == cudaSuccess && s.stage < m) ms[s.stage] += t;
+  }
+  return m;
+}
+
+int64_t epw_interp_last_launch_count(epw_interp_t h) { return h ? h->launches : 0; }
+
+int64_t epw_interp_debug_get(epw_interp_t h, int what, void *dst, size_t bytes) {
+  if (!h || !dst) return EPW_EINVAL;
+  CU_OR_FAIL(h, cudaSetDevice(h->cfg.device), "cudaSetDevice");
+  CU_OR_FAIL(h, cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize");
+  const size_t nbb = h->nbb;
+  const void *src = nullptr;
+  size_t need = 0;
+  switch (what) {
+    case EPW_DBG_G_REQ: {  // g(Re,q) of the last q of the last batch: stored [ka][ie][n'][m'] = Fortran (m',n',ie,ka)
+      need = sizeof(c128) * (size_t)h->rows;
+      src = h->g1.p;  // caller should use nq such that the last batch has one q, or read slot 0 of the last batch
+      break;
+    }
+    case EPW_DBG_H_K: need = sizeof(c128) * nbb * h->last_nk; src = h->Hk.p; break;
+    case EPW_DBG_U_K: need = sizeof(c128) * nbb * h->last_nk; src = h->Uk.p; break;
+    case EPW_DBG_U_KQ: need = sizeof(c128) * nbb * std::min(h->last_nk, h->last_c_rows); src = h->Ukq.p; break;
+    case EPW_DBG_E_Q: need = sizeof(c128) * (size_t)h->nmm; src = h->eq.p; break;
+    case EPW_DBG_G_TILDE: {
+      // strided copy: rows of the g~ buffer are ncols wide, the first Nb^2 Nm entries are g~
+      const int64_t rowsC = std::min(h->last_nk, h->last_c_rows);
+      need = sizeof(c128) * nbb * h->nm * rowsC;
+      if (bytes < need || !h->C.p) return h->fail(EPW_EINVAL, "epw_interp_debug_get: buffer too small or nothing computed");
+      CU_OR_FAIL(h,
+                 cudaMemcpy2D(dst, sizeof(c128) * nbb * h->nm, h->C.p, sizeof(c128) * (size_t)h->last_ncols,
+                              sizeof(c128) * nbb * h->nm, rowsC, cudaMemcpyDeviceToHost),
+                 "cudaMemcpy2D g~");
+      return (int64_t)need;
+    }
+    default: return h->fail(EPW_EINVAL, "epw_interp_debug_get: unknown selector");
+  }
+  if (!src || bytes < need) return h->fail(EPW_EINVAL, "epw_interp_debug_get: buffer too small or nothing computed");
+  CU_OR_FAIL(h, cudaMemcpy(dst, src, need, cudaMemcpyDeviceToHost), "cudaMemcpy debug");
+  return (int64_t)need;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// stage-level entry points
+// ---------------------------------------------------------------------------------------------------------
+static int rc_of(cudaError_t e) { return e == cudaSuccess ? EPW_OK : (e == cudaErrorInvalidValue ? EPW_EINVAL : EPW_ECUDA); }
+
+int epw_phase_table(const double *x_list, int64_t nx, const int32_t *R, const double *w, int32_t nr, void *P_out,
+                    void *cuda_stream) {
+  if (!x_list || !R || !w || !P_out || nx < 0 || nr <= 0) return EPW_EINVAL;
+  return rc_of(launch_phase_table(x_list, nx, R, w, nr, reinterpret_cast<c128 *>(P_out),
+                                  reinterpret_cast<cudaStream_t>(cuda_stream)));
+}
+
+int epw_rp_to_q(const void *g_RR, int64_t rows, int32_t np, const void *Pq, int32_t nq, void *g1_out,
+                void *cuda_stream) {
+  if (!g_RR || !Pq || !g1_out || rows <= 0 || np <= 0 || nq <= 0 || nq > 8) return EPW_EINVAL;
+  return rc_of(launch_rp_to_q(reinterpret_cast<const c128 *>(g_RR), rows, np, reinterpret_cast<const c128 *>(Pq), nq,
+                              reinterpret_cast<c128 *>(g1_out), reinterpret_cast<cudaStream_t>(cuda_stream)));
+}
+
+int epw_interp_operator(const void *Op_R, int32_t n, int32_t nr, const void *P, int64_t nx, void *out,
+                        void *cuda_stream) {
+  if (!Op_R || !P || !out || n <= 0 || nr <= 0 || nx < 0) return EPW_EINVAL;
+  return rc_of(launch_interp_operator(reinterpret_cast<const c128 *>(Op_R), n, nr, reinterpret_cast<const c128 *>(P),
+                                      nx, reinterpret_cast<c128 *>(out), reinterpret_cast<cudaStream_t>(cuda_stream)));
+}
+
+int epw_eigh_batched(const void *A, int64_t stride_a, int32_t n, int64_t batch, double *evals, void *V, int sqrt_mode,
+                     int32_t *status, void *cuda_stream) {
+  if (!A || !evals || !V || n <= 0 || batch < 0 || stride_a < (int64_t)n * n) return EPW_EINVAL;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  c128 *scratch = nullptr;
+  const size_t need = eigh_large_scratch_bytes(n, batch);
+  if (need && cudaMalloc(&scratch, need) != cudaSuccess) return EPW_ENOMEM;
+  const cudaError_t e = launch_eigh_batched(reinterpret_cast<const c128 *>(A), stride_a, n, batch, evals,
+                                            reinterpret_cast<c128 *>(V), sqrt_mode, status, scratch, st);
+  if (scratch) {  // stage-level convenience path: wait so the scratch can be released
+    cudaStreamSynchronize(st);
+    cudaFree(scratch);
+  }
+  return rc_of(e);
+}
+
+int epw_zgemm(const void *A, const void *B, void *C, int64_t M, int32_t N, int32_t K, int64_t ldc, void *cuda_stream) {
+  if (!A || !B || !C || M <= 0 || N <= 0 || K <= 0 || ldc < N) return EPW_EINVAL;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  int dev = 0, nsm = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  const int KB = (int)ceil_div(2 * (int64_t)K, GEMM_BK);
+  const int NT = (int)ceil_div(2 * (int64_t)N, GEMM_BN);
+  const int64_t MT = ceil_div(M, GEMM_BM);
+  double *Ap = nullptr, *Bp = nullptr;
+  if (cudaMalloc(&Ap, sizeof(double) * (size_t)MT * KB * GEMM_CHUNK) != cudaSuccess) return EPW_ENOMEM;
+  if (cudaMalloc(&Bp, sizeof(double) * (size_t)NT * KB * GEMM_CHUNK) != cudaSuccess) {
+    cudaFree(Ap);
+    return EPW_ENOMEM;
+  }
+  cudaError_t e = launch_pack_a_generic(reinterpret_cast<const c128 *>(A), M, K, Ap, st);
+  if (e == cudaSuccess) e = launch_pack_b_generic(reinterpret_cast<const c128 *>(B), K, N, Bp, st);
+  if (e == cudaSuccess) e = launch_zgemm_dmma(Ap, Bp, reinterpret_cast<c128 *>(C), M, N, KB, ldc, nsm, st);
+  cudaStreamSynchronize(st);
+  cudaFree(Ap);
+  cudaFree(Bp);
+  return rc_of(e);
+}
+
+int epw_rotate_g2(const void *gt, int64_t stride_gt, const void *Uk, const void *Ukq, const int32_t *kq_idx, int32_t nb,
+                  int32_t nm, int64_t nk, double *g2, void *cuda_stream) {
+  if (!gt || !Uk || !Ukq || !g2 || nb <= 0 || nm <= 0 || nk < 0) return EPW_EINVAL;
+  const cudaError_t e = launch_rotate_g2(reinterpret_cast<const c128 *>(gt), stride_gt, reinterpret_cast<const c128 *>(Uk),
+                                         reinterpret_cast<const c128 *>(Ukq), kq_idx, nb, nm, nk, g2,
+                                         reinterpret_cast<cudaStream_t>(cuda_stream));
+  return e == cudaErrorInvalidConfiguration ? EPW_EUNSUPPORTED : rc_of(e);
+}
+
+int epw_probe_peaks(int32_t device, double *out4) {
+  if (!out4) return EPW_EINVAL;
+  return probe_peaks(device, out4);
+}
+
+}  // extern "C"

@@ -1,0 +1,300 @@
+"""GPU parity tests: every CUDA stage and the whole path against the CPU oracle, through the C ABI.
+
+Run on the B200 box with `python -m pytest tests -m gpu`.  Inputs are the seeded synthetic workloads of synth/
+(DESIGN.md "Input recipe"); expected values always come from oracle/.
+"""
+import numpy as np
+import pytest
+
+import oracle
+import synth
+from parity import assert_path_close, eig_close
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def epw():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device; there is no CPU fallback")
+    import paper_2603_10295_b200 as p
+
+    p.load_library()
+    return p
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def zdev(a):
+    """complex128 numpy -> float64 device tensor of interleaved (re, im)."""
+    a = np.ascontiguousarray(a, dtype=np.complex128)
+    return torch.from_numpy(a.view(np.float64).reshape(a.shape + (2,))).cuda()
+
+
+def znp(t):
+    return t.cpu().numpy().view(np.complex128).reshape(t.shape[:-1])
+
+
+rng = np.random.default_rng(7)
+
+
+def crandn(*s):
+    return rng.standard_normal(s) + 1j * rng.standard_normal(s)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# stage-level parity
+# ---------------------------------------------------------------------------------------------------------
+def test_phase_table(epw):
+    w = synth.make_config(1)
+    x = np.concatenate([w.q_list[:50], w.k_list[1000:1037], [[0, 0, 0], [0.5, 0.5, 0.5], [3.25, -7.5, 11.0]]])
+    wt = rng.random(w.ne) + 0.5
+    P = torch.empty((len(x), w.ne, 2), dtype=torch.float64, device="cuda")
+    epw.epw_phase_table(dev(x), len(x), dev(w.Re), dev(wt), w.ne, P)
+    got = znp(P)
+    ref = np.array([[wt[ir] * np.exp(1j * oracle.phase(xx, w.Re[ir])) for ir in range(w.ne)] for xx in x])
+    assert np.abs(got - ref).max() < 2e-14
+
+
+@pytest.mark.parametrize("nq", [1, 3, 8])
+def test_rp_to_q_eq9(epw, nq):
+    w = synth.make_config(0)
+    g = w.g_full()
+    q = w.q_list[[5, 17, 63, 1, 2, 3, 40, 41][:nq]] + 0.013
+    Pq = torch.empty((nq, w.np_, 2), dtype=torch.float64, device="cuda")
+    epw.epw_phase_table(dev(q), nq, dev(w.Rp), dev(w.w_p), w.np_, Pq)
+    g1 = torch.empty((nq, w.slab_elems, 2), dtype=torch.float64, device="cuda")
+    epw.epw_rp_to_q(zdev(g), w.slab_elems, w.np_, Pq, nq, g1)
+    got = znp(g1)
+    for i in range(nq):
+        ref = oracle.rp_to_q(g, w.Rp, w.w_p, q[i]).ravel()
+        assert np.abs(got[i] - ref).max() <= 1e-13 * np.abs(ref).max()
+
+
+def test_rp_to_q_ragged_rows_and_many_rp(epw):
+    """rows not a multiple of the CTA size, Np not a multiple of the unroll."""
+    nb, nm, ne, np_ = 3, 2, 5, 37
+    R = rng.integers(-4, 5, size=(np_, 3)).astype(np.int32)
+    wp = rng.random(np_) + 0.5
+    g = crandn(np_, nm, ne, nb, nb)
+    q = rng.random((2, 3))
+    Pq = torch.empty((2, np_, 2), dtype=torch.float64, device="cuda")
+    epw.epw_phase_table(dev(q), 2, dev(R), dev(wp), np_, Pq)
+    rows = nb * nb * ne * nm
+    g1 = torch.empty((2, rows, 2), dtype=torch.float64, device="cuda")
+    epw.epw_rp_to_q(zdev(g), rows, np_, Pq, 2, g1)
+    for i in range(2):
+        ref = oracle.rp_to_q(g, R, wp, q[i]).ravel()
+        assert np.abs(znp(g1)[i] - ref).max() <= 1e-13 * np.abs(ref).max()
+
+
+def test_interp_operator_Dq(epw):
+    w = synth.make_config(2)
+    q = w.q_list[:9]
+    P = torch.empty((9, w.np_, 2), dtype=torch.float64, device="cuda")
+    epw.epw_phase_table(dev(q), 9, dev(w.Rp), dev(w.w_p), w.np_, P)
+    out = torch.empty((9, w.nmodes, w.nmodes, 2), dtype=torch.float64, device="cuda")
+    epw.epw_interp_operator(zdev(w.D_R), w.nmodes, w.np_, P, 9, out)
+    got = znp(out)
+    for i in range(9):
+        ref = oracle.interp_operator(w.D_R, w.Rp, w.w_p, q[i])
+        assert np.abs(got[i] - ref).max() <= 1e-13 * np.abs(ref).max()
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 6, 8, 9, 11, 16, 31, 32, 33, 48])
+def test_eigh_batched(epw, n):
+    batch = 37 if n <= 32 else 5
+    A = crandn(batch, n, n)
+    A = 0.5 * (A + np.conj(np.swapaxes(A, 1, 2)))
+    A[1] = np.diag(np.arange(n, 0, -1)).astype(np.complex128)  # already diagonal, descending
+    if n >= 4:  # exactly degenerate spectrum
+        Q, _ = np.linalg.qr(crandn(n, n))
+        lam = np.repeat(np.arange(n // 2 + 1), 2)[:n].astype(float)
+        M = (Q * lam) @ Q.conj().T
+        A[2] = 0.5 * (M + M.conj().T)
+    A_cm = np.ascontiguousarray(np.swapaxes(A, 1, 2))  # column-major storage
+    ev = torch.empty((batch, n), dtype=torch.float64, device="cuda")
+    V = torch.empty((batch, n, n, 2), dtype=torch.float64, device="cuda")
+    status = torch.zeros(1, dtype=torch.int32, device="cuda")
+    epw.epw_eigh_batched(zdev(A_cm), n * n, n, batch, ev, V, 0, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == 0
+    ev, Vm = ev.cpu().numpy(), np.swapaxes(znp(V), 1, 2)  # Vm[b] = matrix with eigenvector columns
+    for b in range(batch):
+        ref_ev, _, sweeps = oracle.eigh_jacobi(A_cm[b])
+        assert sweeps >= 0
+        e, ok = eig_close(ev[b], ref_ev)
+        assert ok, (n, b, e)
+        nrm = max(np.linalg.norm(A[b]), 1e-300)
+        assert np.linalg.norm(A[b] @ Vm[b] - Vm[b] * ev[b][None, :]) <= 1e-13 * nrm * n
+        assert np.linalg.norm(Vm[b].conj().T @ Vm[b] - np.eye(n)) <= 1e-13 * n
+
+
+def test_eigh_strided_input_sqrt_mode_and_hermitian_part(epw):
+    """Matrices embedded in wider rows (as the H(k+q) block of the contraction output), omega = sqrt(lambda),
+    and only the Hermitian part of a slightly non-Hermitian input is used."""
+    n, batch, stride = 6, 11, 100
+    A = crandn(batch, n, n)
+    A = A @ np.conj(np.swapaxes(A, 1, 2)) + 0.1 * np.eye(n)  # positive definite
+    noise = 1e-3 * crandn(batch, n, n)
+    buf = np.zeros((batch, stride), dtype=np.complex128)
+    buf[:, 7:7 + n * n] = np.swapaxes(A + noise - np.conj(np.swapaxes(noise, 1, 2)), 1, 2).reshape(batch, -1)
+    d = zdev(buf)
+    om = torch.empty((batch, n), dtype=torch.float64, device="cuda")
+    V = torch.empty((batch, n, n, 2), dtype=torch.float64, device="cuda")
+    epw.load_library().epw_eigh_batched(d.data_ptr() + 7 * 16, stride, n, batch, om.data_ptr(), V.data_ptr(), 1, None,
+                                        torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    for b in range(batch):
+        ref, _, _ = oracle.eigh_jacobi(np.ascontiguousarray(A[b].T))
+        e, ok = eig_close(om[b].cpu().numpy(), oracle.omega_from_lambda(ref))
+        assert ok, e
+
+
+@pytest.mark.parametrize("M,N,K", [(1, 1, 1), (130, 70, 9), (300, 150, 37), (128, 64, 8), (257, 449, 343), (1000, 7, 5)])
+def test_zgemm_dmma(epw, M, N, K):
+    """The DMMA contraction kernel against the plain definition C = A B (several tiles + ragged tails)."""
+    A, B = crandn(M, K), crandn(K, N)
+    C = torch.zeros((M, N + 3, 2), dtype=torch.float64, device="cuda")
+    epw.epw_zgemm(zdev(A), zdev(B), C, M, N, K, N + 3)
+    got = znp(C)
+    ref = A @ B
+    assert np.abs(got[:, :N] - ref).max() <= 1e-13 * K * max(1.0, np.abs(ref).max())
+    assert np.all(got[:, N:] == 0)  # padding columns untouched
+
+
+def test_zgemm_matches_oracle_re_to_k(epw):
+    """S2 as the paper defines it: sum_Re g(Re,q) e^{ik.Re} for a batch of k (oracle.re_to_k per k)."""
+    w = synth.make_custom("t", 3, 4, (2, 1, 1), 1.0, 0.1, 1.0, (5, 3, 2), ("random", 1, 3), seed=3)
+    g1 = oracle.rp_to_q(w.g_full(), w.Rp, w.w_p, w.q_list[0])  # [nm][ne][nb][nb]
+    nk, nbb = w.nk, 9
+    P = torch.empty((nk, w.ne, 2), dtype=torch.float64, device="cuda")
+    epw.epw_phase_table(dev(w.k_list), nk, dev(w.Re), dev(w.w_e), w.ne, P)
+    B = np.ascontiguousarray(np.moveaxis(g1.reshape(w.nmodes, w.ne, nbb), 1, 0).reshape(w.ne, -1))  # [ie][ka*nbb+el]
+    C = torch.empty((nk, w.nmodes * nbb, 2), dtype=torch.float64, device="cuda")
+    epw.epw_zgemm(P, zdev(B), C, nk, w.nmodes * nbb, w.ne, w.nmodes * nbb)
+    got = znp(C)
+    for ik in range(nk):
+        ref = oracle.re_to_k(g1, w.Re, w.w_e, w.k_list[ik]).ravel()
+        assert np.abs(got[ik] - ref).max() <= 1e-13 * np.abs(ref).max()
+
+
+@pytest.mark.parametrize("nb,nm", [(8, 6), (11, 9), (3, 2), (1, 1), (16, 3)])
+def test_rotate_g2(epw, nb, nm):
+    nk = 19
+    gt = crandn(nk, nm, nb, nb)
+    Uk = np.stack([np.linalg.qr(crandn(nb, nb))[0].T for _ in range(nk)])  # column-major storage
+    Ukq = np.stack([np.linalg.qr(crandn(nb, nb))[0].T for _ in range(nk)])
+    idx = rng.permutation(nk).astype(np.int32)
+    g2 = torch.empty((nk, nm, nb, nb), dtype=torch.float64, device="cuda")
+    for kq_idx in (None, idx):
+        epw.epw_rotate_g2(zdev(gt), nm * nb * nb, zdev(Uk), zdev(Ukq), None if kq_idx is None else dev(kq_idx), nb, nm,
+                          nk, g2)
+        got = g2.cpu().numpy()
+        for ik in range(nk):
+            u = Ukq[ik] if kq_idx is None else Ukq[kq_idx[ik]]
+            ref = np.abs(oracle.band_rotate(gt[ik], u, Uk[ik])) ** 2
+            assert np.abs(got[ik] - ref).max() <= 1e-12 * ref.max()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# whole path
+# ---------------------------------------------------------------------------------------------------------
+def run_gpu(epw, w, k_list, q_list, kq_map=None, q_batch=0, host_api=False):
+    h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_, q_batch=q_batch)
+    try:
+        h.set_operators_from_host(w)
+        if host_api:
+            nk, nq = len(k_list), len(q_list)
+            eps_k = np.empty((nk, w.nbnd))
+            eps_kq = np.empty((nq, nk, w.nbnd))
+            om = np.empty((nq, w.nmodes))
+            g2 = np.empty((nq, nk, w.nmodes, w.nbnd, w.nbnd))
+            epw.epw_interp_interpolate_host(h.h, np.ascontiguousarray(k_list), nk, np.ascontiguousarray(q_list), nq,
+                                            kq_map, eps_k, eps_kq, om, g2)
+            return eps_k, eps_kq, om, g2
+        out = h.interpolate(dev(k_list), dev(q_list), None if kq_map is None else dev(kq_map))
+        epw.epw_interp_sync(h.h)
+        return [None if t is None else t.cpu().numpy() for t in out]
+    finally:
+        h.close()
+
+
+def test_config0_full_both_kq_modes(epw):
+    """BASELINE.json configs[0], all 4,096 pairs: grid-folded k+q (kq_map) and per-pair H(k+q) eigensolves."""
+    w = synth.make_config(0)
+    ref = oracle.interpolate(w.H_R, w.D_R, w.g_full(), w.Re, w.w_e, w.Rp, w.w_p, w.k_list, w.q_list)
+    worst = assert_path_close(run_gpu(epw, w, w.k_list, w.q_list, w.kq_map), ref)
+    worst2 = assert_path_close(run_gpu(epw, w, w.k_list, w.q_list, None), ref)
+    print(f"config 0 worst |g|^2 error: {worst:.3f} / {worst2:.3f} of tolerance")
+
+
+def test_config0_host_api_and_q_batches(epw):
+    w = synth.make_config(0)
+    ql = w.q_list[:7] + [0.01, 0.02, 0.03]
+    ref = oracle.interpolate(w.H_R, w.D_R, w.g_full(), w.Re, w.w_e, w.Rp, w.w_p, w.k_list, ql)
+    for qb in (1, 3, 8):
+        assert_path_close(run_gpu(epw, w, w.k_list, ql, None, q_batch=qb), ref)
+    assert_path_close(run_gpu(epw, w, w.k_list, ql, None, host_api=True), ref)
+
+
+@pytest.mark.parametrize("shape", ["si", "mos2", "odd"])
+def test_reduced_shapes(epw, shape):
+    """Reduced-size versions of configs 1-3 (same generators, fewer lattice vectors and k): several M tiles,
+    ragged tails, odd Nb/Nm (11, 9), 2-D lattices."""
+    if shape == "si":
+        w = synth.make_custom("si-r", 8, 6, (2, 2, 2), 1.5, 0.1, 1.5, (7, 6, 5), ("random", 3, 3), seed=11)
+    elif shape == "mos2":
+        w = synth.make_custom("mos2-r", 11, 9, (3, 3, 0), 2.0, 0.1, 2.0, (15, 13, 1), ("random", 3, 2), seed=12)
+    else:
+        w = synth.make_custom("odd", 5, 3, (1, 2, 0), 1.0, 0.1, 1.0, (9, 1, 17), ("random", 2, 3), seed=13)
+    ref = oracle.interpolate(w.H_R, w.D_R, w.g_full(), w.Re, w.w_e, w.Rp, w.w_p, w.k_list, w.q_list)
+    assert_path_close(run_gpu(epw, w, w.k_list, w.q_list), ref)
+
+
+def test_debug_intermediates_config0(epw):
+    """g(Re,q), H(k), e_q and g~ of the last q against the oracle's stage functions."""
+    w = synth.make_config(0)
+    g = w.g_full()
+    q = w.q_list[9:10] + 0.004
+    h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_)
+    try:
+        h.set_operators_from_host(w)
+        h.interpolate(dev(w.k_list), dev(q))
+        g1 = np.empty((w.nmodes, w.ne, w.nbnd, w.nbnd), dtype=np.complex128)
+        epw.epw_interp_debug_get(h.h, epw.EPW_DBG_G_REQ, g1)
+        ref1 = oracle.rp_to_q(g, w.Rp, w.w_p, q[0])
+        assert np.abs(g1 - ref1).max() <= 1e-13 * np.abs(ref1).max()
+        Hk = np.empty((w.nk, w.nbnd, w.nbnd), dtype=np.complex128)
+        epw.epw_interp_debug_get(h.h, epw.EPW_DBG_H_K, Hk)
+        for ik in (0, 13, 63):
+            refH = oracle.interp_operator(w.H_R, w.Re, w.w_e, w.k_list[ik])
+            assert np.abs(Hk[ik] - refH).max() <= 1e-13 * np.abs(refH).max()
+        gt = np.empty((w.nk, w.nmodes, w.nbnd, w.nbnd), dtype=np.complex128)
+        epw.epw_interp_debug_get(h.h, epw.EPW_DBG_G_TILDE, gt)
+        e_ref, om_ref = oracle.phonon(w.D_R, w.Rp, w.w_p, q[0])
+        # gauge-free check of the mode-rotated g~: sum_nu 2 omega_nu |g~_nu|^2 = sum_ka |g~_ka|^2 per (m',n')
+        for ik in (0, 31):
+            raw = oracle.re_to_k(ref1, w.Re, w.w_e, w.k_list[ik])
+            lhs = (2 * om_ref[:, None, None] * np.abs(gt[ik]) ** 2).sum(axis=0)
+            rhs = (np.abs(raw) ** 2).sum(axis=0)
+            assert np.abs(lhs - rhs).max() <= 1e-11 * rhs.max()
+    finally:
+        h.close()
+
+
+def test_errors_are_reported(epw):
+    with pytest.raises(epw.EpwError):
+        epw.epw_interp_create(0, 6, 27, 27)
+    h = epw.EpwInterp(2, 3, 5, 5)
+    try:
+        k = torch.zeros((4, 3), dtype=torch.float64, device="cuda")
+        with pytest.raises(epw.EpwError) as ei:
+            h.interpolate(k, k)
+        assert "operators not set" in str(ei.value)
+    finally:
+        h.close()
