@@ -1,0 +1,367 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the Wannier-to-Bloch e-ph interpolation path on B200.
+
+Metric (BASELINE.json): interpolated |g(k,q)|^2 elements/s in FP64, elements = Nk * Nq * Nb^2 * Nm.
+Workload at N = 1: BASELINE.json configs[1] ("Si-like production": Nb=8, Nm=6, Ne=Np=343, 40^3 k grid, random q).
+A step = one epw_interp_interpolate call over ALL 64,000 k and a batch of `--nq-step` q-points: every stage of the
+path (S0 phase tables, S1 Rp->q, D(q)/H(k)/H(k+q) + eigensolves, S4a, S2 Re->k on the FP64 tensor path, S4b + |g|^2).
+With N > 1 the q-points are sharded over ranks (the paper's image level: no communication inside
+the loop) -> weak scaling, no data-path collective.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--nq-step Q] [--impl reference]
+
+`--impl reference` times the CPU oracle (oracle/, plain C) on the host cores on a bounded sample of the same
+workload; it is a deliberately slow baseline, not a target.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "interpolated |g(k,q)|^2 elements/s (FP64)"
+UNIT = "elements/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=6)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (default 1 = Si-like production)")
+    ap.add_argument("--nq-step", type=int, default=8, help="q-points per step (per GPU)")
+    ap.add_argument("--q-batch", type=int, default=0, help="library q_batch for S1 (0 = default)")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--stages", action="store_true", help="also print per-stage device times to stderr")
+    return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------------------------------------
+# clocks: sample nvidia-smi during the timed region (B200_PROFILING.md "clocks DURING the timed region")
+# ------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.samples = []
+        self.proc = None
+        self.gpu_index = gpu_index
+        self.thread = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.gpu_index), f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.samples.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for s in self.samples:
+            f = [x.strip() for x in s.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1])); power.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)), "power_w_max": float(max(power)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------------------
+# CPU oracle legs
+# ------------------------------------------------------------------------------------------------------------
+def oracle_sample(w, n_q: int, n_k: int, seed: int = 1234):
+    """Time the oracle, as it stands, on n_q sampled q x n_k sampled k of workload w (g must fit host memory).
+    Returns (elements/s amortising Eq. 9 over the full Nk, seconds spent, threads, description, raw results)."""
+    import oracle
+
+    rng = np.random.default_rng(seed)
+    iq = np.sort(rng.choice(w.nq, size=min(n_q, w.nq), replace=False))
+    ik = np.sort(rng.choice(w.nk, size=min(n_k, w.nk), replace=False))
+    ks = np.ascontiguousarray(w.k_list[ik])
+    qs = np.ascontiguousarray(w.q_list[iq])
+    g = w.g_full()
+    t0 = time.perf_counter()
+    g1 = oracle.rp_to_q(g, w.Rp, w.w_p, qs[0])  # Eq. 9 for one q (single thread, as written)
+    t_eq9 = time.perf_counter() - t0
+    del g1
+    t0 = time.perf_counter()
+    res = oracle.interpolate(w.H_R, w.D_R, g, w.Re, w.w_e, w.Rp, w.w_p, ks, qs)
+    t_all = time.perf_counter() - t0
+    pairs = len(iq) * len(ik)
+    E = w.elements_per_pair
+    t_pair = max(t_all - len(iq) * t_eq9, 1e-9) / pairs
+    per_elem = (t_pair + t_eq9 / w.nk) / E
+    threads = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    desc = (f"{len(iq)} random q x {len(ik)} random k of config {w.index} ({pairs} pairs); Eq. 9 per q "
+            f"({t_eq9:.3f} s, 1 thread) amortised over the full Nk={w.nk}")
+    return 1.0 / per_elem, t_all + t_eq9, threads, desc, (iq, ik, res)
+
+
+def run_reference(args):
+    """`--impl reference`: the oracle on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import synth
+
+    w = synth.make_config(args.config)
+    if w.g_bytes > (8 << 30):
+        print(json.dumps({"impl": "reference", "unavailable": "config too large for the host-side oracle sample"}))
+        return
+    n_k = 1024 if w.elements_per_pair < 2000 else 256
+    vals, secs = [], []
+    threads, desc = 1, ""
+    for step in range(args.warmup + args.steps):
+        v, s, threads, desc, _ = oracle_sample(w, 2, n_k, seed=100 + step)
+        if step >= args.warmup:
+            vals.append(v); secs.append(s)
+    value = float(np.mean(vals))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(secs)), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{w.index}] {w.name}", "sample": desc},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------------------
+# B200 arm
+# ------------------------------------------------------------------------------------------------------------
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+
+    import torch
+    import torch.distributed as dist
+
+    import paper_2603_10295_b200 as epw
+    import synth
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the interpolation path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    epw.load_library()
+
+    w = synth.make_config(args.config)
+    nq_step = min(args.nq_step, w.nq)
+    nk, E = w.nk, w.elements_per_pair
+    h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_, device=local_rank, q_batch=args.q_batch)
+    t0 = time.perf_counter()
+    h.set_operators_from_host(w)  # upload once; resident for the whole run
+    torch.cuda.synchronize()
+    t_upload = time.perf_counter() - t0
+
+    k_dev = torch.from_numpy(w.k_list).cuda()
+    kq_map = w.kq_map
+    total_steps = args.warmup + args.steps
+
+    def q_block(step):
+        """q-points of this rank for this step (ranks own disjoint q: the image level of the paper)."""
+        start = ((step * world + rank) * nq_step) % w.nq
+        idx = (start + np.arange(nq_step)) % w.nq
+        return idx
+
+    q_blocks = [q_block(s) for s in range(total_steps)]
+    q_dev = [torch.from_numpy(np.ascontiguousarray(w.q_list[i])).cuda() for i in q_blocks]
+    map_dev = None
+    if kq_map is not None:
+        map_dev = [torch.from_numpy(np.ascontiguousarray(kq_map[i])).cuda() for i in q_blocks]
+    eps_k = torch.empty((nk, w.nbnd), dtype=torch.float64, device="cuda")
+    eps_kq = torch.empty((nq_step, nk, w.nbnd), dtype=torch.float64, device="cuda")
+    omega = torch.empty((nq_step, w.nmodes), dtype=torch.float64, device="cuda")
+    g2 = torch.empty((nq_step, nk, w.nmodes, w.nbnd, w.nbnd), dtype=torch.float64, device="cuda")  # reused every step
+
+    def step(s):
+        epw.epw_interp_interpolate(h.h, k_dev, nk, q_dev[s], nq_step, None if map_dev is None else map_dev[s], eps_k,
+                                   eps_kq, omega, g2)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for s in range(args.warmup):
+        step(s)
+    epw.epw_interp_sync(h.h)
+
+    # ---- timed region: K steps, device time from CUDA events on the launching stream, max over ranks ----
+    epw.epw_interp_enable_stage_timing(h.h, True)
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches = 0
+    barrier()
+    ev0.record()
+    for s in range(args.warmup, total_steps):
+        step(s)
+        launches += epw.epw_interp_last_launch_count(h.h)
+    ev1.record()
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    clocks = sampler.stop() if rank == 0 else None
+    epw.epw_interp_sync(h.h)  # raises if an eigensolve did not converge
+    stage_ms = epw.epw_interp_get_stage_times(h.h)
+    epw.epw_interp_enable_stage_timing(h.h, False)
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    elements_per_step = nk * nq_step * E
+    value = world * elements_per_step * args.steps / (ms * 1e-3)
+
+    # ---- roofline of the dominant kernel (S2: the DMMA contraction) ----
+    ncols = E + (0 if kq_map is not None else w.nbnd * w.nbnd)
+    flops_s2 = 8.0 * nk * ncols * w.ne * nq_step * args.steps  # 8 real flops per complex MAC, algorithmic (unpadded)
+    kchunk = max(128, ((48 << 20) // (ncols * 16)) // 128 * 128)
+    launches_s2 = -(-nk // kchunk) * nq_step * args.steps
+    s2_ms = stage_ms["S2_re_to_k_dmma"]
+    roofline = None
+    if rank == 0:
+        peaks = epw.epw_probe_peaks(local_rank)
+        achieved = flops_s2 / (s2_ms * 1e-3) / 1e12
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+        if os.path.exists(tpath):
+            traffic = json.load(open(tpath)).get("zgemm_dmma_kernel_dram_bytes_per_launch")
+        mp = {}
+        if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")):
+            mp = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        roofline = {
+            "bound": "tensor", "kernel": "zgemm_dmma_kernel (S2 Re->k, FP64 DMMA)", "achieved": achieved,
+            "peak": peaks["fp64_dmma_tflops"], "unit": "TFLOP/s", "frac": achieved / peaks["fp64_dmma_tflops"],
+            "traffic": traffic,
+            "peak_source": "FP64 DMMA m8n8k4 issue-loop probe run live on this GPU (epw_probe_peaks); "
+                           "MEASURED_PEAKS.json has no FP64 entry",
+            "peak_from_measured_bf16_x_nominal_ratio": (mp.get("bf16_tflops_sustained", 0.0) * 45.0 / 2250.0) or None,
+            "flops_per_launch": flops_s2 / launches_s2, "launches": launches_s2,
+            "avg_launch_ms": s2_ms / launches_s2, "share_of_step": s2_ms / stage_ms["total"],
+            "hbm_read_gbs_probe": peaks["hbm_read_gbs"], "fp64_dfma_tflops_probe": peaks["fp64_dfma_tflops"],
+            "stage_ms_per_step": {k: v / args.steps for k, v in stage_ms.items()},
+        }
+        # S1 is the HBM-bound stage: report it too
+        s1_bytes = (16.0 * w.slab_elems * w.np_ * -(-nq_step // (args.q_batch or 4)) + 16.0 * w.slab_elems * nq_step) * args.steps
+        roofline["s1_rp_to_q"] = {"bound": "hbm", "achieved": s1_bytes / (stage_ms["S1_rp_to_q"] * 1e-3) / 1e9,
+                                  "peak": mp.get("hbm_gbs"), "unit": "GB/s"}
+        if roofline["s1_rp_to_q"]["peak"]:
+            roofline["s1_rp_to_q"]["frac"] = roofline["s1_rp_to_q"]["achieved"] / roofline["s1_rp_to_q"]["peak"]
+    if args.stages and rank == 0:
+        print(json.dumps({k: round(v / args.steps, 4) for k, v in stage_ms.items()}), file=sys.stderr)
+
+    # ---- e2e: the same steps through the host-buffer entry point (H2D of k/q lists, D2H of all outputs) ----
+    e2e = None
+    if not args.no_e2e:
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        k_host = pin(w.k_list)
+        q_host = [pin(w.q_list[i]) for i in q_blocks]
+        map_host = None if kq_map is None else [pin(kq_map[i]) for i in q_blocks]
+        o_eps_k = torch.empty((nk, w.nbnd), dtype=torch.float64).pin_memory()
+        o_eps_kq = torch.empty((nq_step, nk, w.nbnd), dtype=torch.float64).pin_memory()
+        o_omega = torch.empty((nq_step, w.nmodes), dtype=torch.float64).pin_memory()
+        o_g2 = torch.empty((nq_step, nk, w.nmodes, w.nbnd, w.nbnd), dtype=torch.float64).pin_memory()
+
+        def step_host(s):
+            epw.epw_interp_interpolate_host(h.h, k_host, nk, q_host[s], nq_step, None if map_host is None else map_host[s],
+                                            o_eps_k, o_eps_kq, o_omega, o_g2)
+
+        n_e2e_warm = min(args.warmup, 2)
+        for s in range(n_e2e_warm):
+            step_host(s)
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for s in range(args.warmup, total_steps):
+            step_host(s)
+        e1.record()
+        barrier()
+        ms_e2e = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms_e2e], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms_e2e = float(t.item())
+        h2d = k_host.numel() * 8 + q_host[0].numel() * 8 + (0 if map_host is None else map_host[0].numel() * 4)
+        d2h = (o_eps_k.numel() + o_eps_kq.numel() + o_omega.numel() + o_g2.numel()) * 8
+        e2e = {"value": world * elements_per_step * args.steps / (ms_e2e * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "ms_per_step": ms_e2e / args.steps,
+               "api": "epw_interp_interpolate_host (pinned host buffers in and out)"}
+
+    # ---- CPU oracle beside it (rank 0, N = 1 only) ----
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and w.g_bytes <= (8 << 30):
+        n_k = 4096 if E < 2000 else 512
+        v, secs, threads, desc, _ = oracle_sample(w, 4, n_k)
+        cpu_baseline = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc,
+                        "seconds": secs}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {
+                "workload": f"BASELINE.json configs[{w.index}] {w.name}: Nb={w.nbnd} Nm={w.nmodes} Ne={w.ne} Np={w.np_} "
+                            f"Nk={nk} ({'x'.join(map(str, w.k_grid))}), {nq_step} q per step per GPU ({w.q_desc})",
+                "global_batch_pairs": world * nk * nq_step, "parallelism": f"q-sharded x{world}",
+                "l2": "inputs larger than L2: g(Re,Rp) %.0f MB streamed per q-batch, phase table %.0f MB, |g|^2 output %.0f MB "
+                      "per step" % (w.g_bytes / 1e6, 16.0 * nk * w.ne / 1e6, 8.0 * elements_per_step / 1e6),
+                "operator_upload_s": t_upload,
+            },
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+            "cpu_baseline": cpu_baseline,
+        }
+        print(json.dumps(line))
+    h.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

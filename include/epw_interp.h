@@ -112,7 +112,8 @@ int epw_interp_interpolate_host(epw_interp_t h, const double *k_list, int64_t nk
 int epw_interp_sync(epw_interp_t h);
 
 /*
- * Per-stage device times (ms, CUDA events on the caller's stream) accumulated over the last interpolate call:
+ * Per-stage device times (ms, CUDA events on the caller's stream) accumulated over every interpolate call since
+ * stage timing was last enabled:
  *   ms[0] S0 phase tables   ms[1] S1 Rp->q   ms[2] D(q) + phonon eigensolve + S4a/pack   ms[3] H(k) + eigensolve
  *   ms[4] S2 Re->k contraction   ms[5] H(k+q) eigensolve   ms[6] S4b rotation + |g|^2   ms[7] total
  * Synchronises the stream.  Returns the number of entries written (<= n) or a negative status.
@@ -120,8 +121,8 @@ int epw_interp_sync(epw_interp_t h);
 #define EPW_NUM_STAGES 8
 int epw_interp_get_stage_times(epw_interp_t h, double *ms, int n);
 
-/* Stage timing records two CUDA events per stage invocation; it is off by default (on != 0 enables it for the
- * following interpolate calls). */
+/* Stage timing records two CUDA events per stage invocation; it is off by default.  on != 0 enables it for the
+ * following interpolate calls and clears the accumulated times; on == 0 disables it. */
 int epw_interp_enable_stage_timing(epw_interp_t h, int on);
 
 /* Number of kernels the library launched during the last interpolate call (for bench.py's gpu_launches). */

@@ -73,7 +73,7 @@ struct epw_interp {
   // host-entry staging
   DevBuf hs_k, hs_q, hs_map, hs_epsk, hs_epskq, hs_omega, hs_g2;
   // bookkeeping of the last call
-  int64_t last_nk = 0, last_c_rows = 0, last_c_row0 = 0;
+  int64_t last_nk = 0, last_c_rows = 0;
   int last_ncols = 0;
   int64_t launches = 0;
   cudaStream_t last_stream = nullptr;
@@ -231,6 +231,8 @@ int epw_interp_set_wannier_operators(epw_interp_t h, const void *H_R, const void
 int epw_interp_enable_stage_timing(epw_interp_t h, int on) {
   if (!h) return EPW_EINVAL;
   h->timing = on != 0;
+  h->spans.clear();  // (re)enabling starts a fresh accumulation
+  h->ev_used = 0;
   return EPW_OK;
 }
 
@@ -248,8 +250,6 @@ int epw_interp_interpolate(epw_interp_t h, const double *k_list, int64_t nk, con
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
   h->last_stream = st;
   h->launches = 0;
-  h->spans.clear();
-  h->ev_used = 0;
 
   const int nb = h->nb, nm = h->nm, ne = h->ne, np = h->np, nbb = h->nbb, nmm = h->nmm;
   const int ncols_g = nbb * nm;
@@ -387,7 +387,6 @@ int epw_interp_interpolate(epw_interp_t h, const double *k_list, int64_t nk, con
                                    g2 + (q * nk + k0) * E, st),
                "rotate_g2");
         h->end_span(sp, st);
-        h->last_c_row0 = k0 - crow;
       }
     }
   }
