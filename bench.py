@@ -250,6 +250,7 @@ def main():
     clocks = sampler.stop() if rank == 0 else None
     epw.epw_interp_sync(h.h)  # raises if an eigensolve did not converge
     stage_ms = epw.epw_interp_get_stage_times(h.h)
+    stage_launches = epw.epw_interp_get_stage_launches(h.h)
     epw.epw_interp_enable_stage_timing(h.h, False)
     if world > 1:
         t = torch.tensor([ms], dtype=torch.float64, device="cuda")
@@ -261,8 +262,7 @@ def main():
     # ---- roofline of the dominant kernel (S2: the DMMA contraction) ----
     ncols = E + (0 if kq_map is not None else w.nbnd * w.nbnd)
     flops_s2 = 8.0 * nk * ncols * w.ne * nq_step * args.steps  # 8 real flops per complex MAC, algorithmic (unpadded)
-    kchunk = max(128, ((48 << 20) // (ncols * 16)) // 128 * 128)
-    launches_s2 = -(-nk // kchunk) * nq_step * args.steps
+    launches_s2 = max(1, stage_launches["S2_re_to_k_dmma"])
     s2_ms = stage_ms["S2_re_to_k_dmma"]
     roofline = None
     if rank == 0:

@@ -121,6 +121,10 @@ int epw_interp_sync(epw_interp_t h);
 #define EPW_NUM_STAGES 8
 int epw_interp_get_stage_times(epw_interp_t h, double *ms, int n);
 
+/* Kernel launches per stage over the same accumulation period as epw_interp_get_stage_times (same indices;
+ * counts[7] = all launches).  Returns the number of entries written or a negative status. */
+int epw_interp_get_stage_launches(epw_interp_t h, int64_t *counts, int n);
+
 /* Stage timing records two CUDA events per stage invocation; it is off by default.  on != 0 enables it for the
  * following interpolate calls and clears the accumulated times; on == 0 disables it. */
 int epw_interp_enable_stage_timing(epw_interp_t h, int on);

@@ -29,7 +29,7 @@ EPW_DBG_G_REQ, EPW_DBG_G_TILDE, EPW_DBG_H_K, EPW_DBG_U_K, EPW_DBG_U_KQ, EPW_DBG_
 EXPORTED_SYMBOLS = [
     "epw_interp_create", "epw_interp_destroy", "epw_interp_set_wannier_operators", "epw_interp_set_g_slabs",
     "epw_interp_interpolate", "epw_interp_interpolate_host", "epw_interp_sync", "epw_interp_get_stage_times",
-    "epw_interp_enable_stage_timing", "epw_interp_last_launch_count", "epw_interp_debug_get", "epw_interp_last_error",
+    "epw_interp_enable_stage_timing", "epw_interp_get_stage_launches", "epw_interp_last_launch_count", "epw_interp_debug_get", "epw_interp_last_error",
     "epw_phase_table", "epw_rp_to_q", "epw_interp_operator", "epw_eigh_batched", "epw_zgemm", "epw_rotate_g2",
     "epw_probe_peaks", "epw_version",
 ]
@@ -69,6 +69,7 @@ def load_library() -> ctypes.CDLL:
         L.epw_interp_sync.argtypes = [vp]
         L.epw_interp_get_stage_times.argtypes = [vp, POINTER(c_double), c_int]
         L.epw_interp_enable_stage_timing.argtypes = [vp, c_int]
+        L.epw_interp_get_stage_launches.argtypes = [vp, POINTER(c_int64), c_int]
         L.epw_interp_last_launch_count.argtypes = [vp]
         L.epw_interp_last_launch_count.restype = c_int64
         L.epw_interp_debug_get.argtypes = [vp, c_int, vp, c_size_t]
@@ -158,6 +159,12 @@ def epw_interp_get_stage_times(h) -> dict:
     buf = (c_double * EPW_NUM_STAGES)()
     n = _check(load_library().epw_interp_get_stage_times(h, buf, EPW_NUM_STAGES), h)
     return {STAGE_NAMES[i]: buf[i] for i in range(n)}
+
+
+def epw_interp_get_stage_launches(h) -> dict:
+    buf = (c_int64 * EPW_NUM_STAGES)()
+    n = _check(load_library().epw_interp_get_stage_launches(h, buf, EPW_NUM_STAGES), h)
+    return {STAGE_NAMES[i]: int(buf[i]) for i in range(n)}
 
 
 def epw_interp_last_launch_count(h) -> int:

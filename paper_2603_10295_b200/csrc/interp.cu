@@ -51,6 +51,24 @@ __global__ void gather_eps_kernel(const double *__restrict__ eps_k, const int32_
   }
 }
 
+// Number of 128-row m-tiles per k-chunk of the S2 contraction.  The chunk of C must stay within `l2_budget` bytes;
+// among the admissible sizes pick the largest one whose tile count (mtiles * NT) wastes at most 3 % of its last
+// wave on the `sms` persistent CTAs (wave quantisation), else the one with the best wave efficiency.
+int64_t choose_mtiles_per_chunk(int NT, int sms, size_t bytes_per_mtile, int64_t MT) {
+  const size_t l2_budget = (size_t)64 << 20;
+  int64_t max_mt = std::max<int64_t>(1, (int64_t)(l2_budget / bytes_per_mtile));
+  if (max_mt >= MT) return MT;
+  int64_t best = 1;
+  double best_eff = 0.0;
+  for (int64_t mt = max_mt; mt >= 1; mt--) {
+    const int64_t tiles = mt * NT;
+    const double eff = (double)tiles / (double)(ceil_div(tiles, sms) * sms);
+    if (eff >= 0.97) return mt;
+    if (eff > best_eff) { best_eff = eff; best = mt; }
+  }
+  return best;
+}
+
 __global__ void fill_ones_kernel(double *p, int n) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) p[i] = 1.0;
@@ -79,7 +97,7 @@ struct epw_interp {
   cudaStream_t last_stream = nullptr;
   bool timing = false;
   std::vector<cudaEvent_t> ev_pool;
-  struct Span { int stage; int e0, e1; };
+  struct Span { int stage; int e0, e1; int64_t launch0; int64_t nlaunch; };
   std::vector<Span> spans;
   size_t ev_used = 0;
   std::string last_error;
@@ -99,14 +117,16 @@ struct epw_interp {
       ev_pool.resize(old + 64);
       for (size_t i = old; i < ev_pool.size(); i++) cudaEventCreate(&ev_pool[i]);
     }
-    Span s{stage, (int)ev_used, (int)ev_used + 1};
+    Span s{stage, (int)ev_used, (int)ev_used + 1, launches, 0};
     ev_used += 2;
     cudaEventRecord(ev_pool[s.e0], st);
     spans.push_back(s);
     return (int)spans.size() - 1;
   }
   void end_span(int id, cudaStream_t st) {
-    if (id >= 0) cudaEventRecord(ev_pool[spans[id].e1], st);
+    if (id < 0) return;
+    cudaEventRecord(ev_pool[spans[id].e1], st);
+    spans[id].nlaunch = launches - spans[id].launch0;
   }
 };
 
@@ -262,9 +282,9 @@ int epw_interp_interpolate(epw_interp_t h, const double *k_list, int64_t nk, con
   const int QB = (int)std::min<int64_t>(h->q_batch, nq);
   const int64_t E = (int64_t)ncols_g;
 
-  // k-chunk: keep one chunk of g~ (16*ncols bytes per k) around 48 MB so that the rotation kernel finds it in L2
-  int64_t kchunk = ((48ll << 20) / ((int64_t)ncols * 16)) / GEMM_BM * GEMM_BM;
-  kchunk = std::max<int64_t>(kchunk, GEMM_BM);
+  // k-chunk: one chunk of [g~ | H(k+q)] (16*ncols bytes per k) must stay L2-resident for the eigensolve and the
+  // rotation that follow it, and its tile count should fill whole waves of the persistent contraction kernel
+  const int64_t kchunk = choose_mtiles_per_chunk(NT, h->num_sms, (size_t)GEMM_BM * ncols * 16, MT) * GEMM_BM;
   // rows of the g~ buffer kept (all of nk when it fits the cap; else a multiple of kchunk that is reused)
   size_t cap = h->cfg.workspace_bytes ? h->cfg.workspace_bytes : ((size_t)6 << 30);
   int64_t c_rows = MT * GEMM_BM;
@@ -450,6 +470,15 @@ int epw_interp_get_stage_times(epw_interp_t h, double *ms, int n) {
     float t = 0.f;
     if (cudaEventElapsedTime(&t, h->ev_pool[s.e0], h->ev_pool[s.e1]) == cudaSuccess && s.stage < m) ms[s.stage] += t;
   }
+  return m;
+}
+
+int epw_interp_get_stage_launches(epw_interp_t h, int64_t *counts, int n) {
+  if (!h || !counts || n <= 0) return EPW_EINVAL;
+  const int m = std::min(n, (int)EPW_NUM_STAGES);
+  for (int i = 0; i < m; i++) counts[i] = 0;
+  for (const auto &s : h->spans)
+    if (s.stage < m) counts[s.stage] += s.nlaunch;
   return m;
 }
 

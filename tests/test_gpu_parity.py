@@ -298,3 +298,62 @@ def test_errors_are_reported(epw):
         assert "operators not set" in str(ei.value)
     finally:
         h.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# full-size configurations, in the launch configuration bench.py times: sampled pairs against the oracle
+# ---------------------------------------------------------------------------------------------------------
+def check_sampled_pairs(epw, w, q_idx, k_idx, q_batch=0):
+    """Run the library on ALL k of workload w and the q-points q_idx (one interpolate call, as bench.py does), then
+    compare eps_k, omega_q, eps_kq and |g|^2 on the sampled (q, k) pairs with the oracle computed pair by pair."""
+    g = w.g_full()
+    ql = np.ascontiguousarray(w.q_list[q_idx])
+    kq_map = None if w.kq_map is None else np.ascontiguousarray(w.kq_map[q_idx])
+    eps_k, eps_kq, om, g2 = run_gpu(epw, w, w.k_list, ql, kq_map, q_batch=q_batch)
+    worst = 0.0
+    for jq in range(len(q_idx)):
+        e_ref, om_ref = oracle.phonon(w.D_R, w.Rp, w.w_p, ql[jq])
+        err, ok = eig_close(om[jq], om_ref)
+        assert ok, f"omega mismatch at q {q_idx[jq]}: {err:.3e}"
+        g1 = oracle.rp_to_q(g, w.Rp, w.w_p, ql[jq])
+        for ik in k_idx:
+            r_g2, r_ek, r_ekq = oracle.pair(g1, w.H_R, w.Re, w.w_e, e_ref, om_ref, w.k_list[ik], ql[jq])
+            err, ok = eig_close(eps_k[ik], r_ek)
+            assert ok, f"eps_k mismatch at k {ik}: {err:.3e}"
+            err, ok = eig_close(eps_kq[jq, ik], r_ekq)
+            assert ok, f"eps_kq mismatch at (q {q_idx[jq]}, k {ik}): {err:.3e}"
+            from parity import g2_pair_close
+
+            wst, ok = g2_pair_close(g2[jq, ik], r_g2, r_ekq, r_ek, om_ref)
+            assert ok, f"|g|^2 mismatch at (q {q_idx[jq]}, k {ik}): {wst:.3f} x tolerance"
+            worst = max(worst, wst)
+    return worst
+
+
+def sample_k(nk, n=24, seed=5):
+    """first / last rows, the rows around the 128-row tile edges and a few random ones"""
+    r = np.random.default_rng(seed)
+    fixed = [0, 1, 127, 128, nk // 2, nk - 129, nk - 128, nk - 1]
+    return sorted(set(int(x) for x in fixed if 0 <= x < nk) | set(int(x) for x in r.integers(0, nk, size=n)))
+
+
+def test_config1_full_size_sampled(epw):
+    """BASELINE.json configs[1] exactly as bench.py runs it: all 64,000 k, 8 q per call (two S1 batches of 4)."""
+    w = synth.make_config(1)
+    q_idx = [0, 1, 2, 3, 500, 501, 998, 999]
+    worst = check_sampled_pairs(epw, w, q_idx, sample_k(w.nk))
+    print(f"config 1 full size: worst |g|^2 deviation {worst:.3f} x tolerance")
+
+
+def test_config2_full_size_sampled(epw):
+    """BASELINE.json configs[2] (MoS2-like, Nb=11, Nm=9, 2-D): all 14,400 k, 3 q."""
+    w = synth.make_config(2)
+    worst = check_sampled_pairs(epw, w, [0, 1000, 1999], sample_k(w.nk, 16))
+    print(f"config 2 full size: worst |g|^2 deviation {worst:.3f} x tolerance")
+
+
+def test_config3_full_size_sampled(epw):
+    """BASELINE.json configs[3] (10^6 k streamed through a reused g~ buffer, Ne=Np=729): 2 q, sampled k."""
+    w = synth.make_config(3)
+    worst = check_sampled_pairs(epw, w, [0, 255], sample_k(w.nk, 16))
+    print(f"config 3 full size: worst |g|^2 deviation {worst:.3f} x tolerance")
