@@ -55,10 +55,16 @@ typedef struct {
   int32_t np;             /* Np: number of phonon Wigner-Seitz vectors Rp */
   int32_t device;         /* CUDA device ordinal */
   int32_t q_batch;        /* q-points contracted per pass over g(Re,Rp) in S1 (1..8); 0 = library default */
+  int32_t path;           /* EPW_PATH_AUTO (0): chosen from Nb, Nm; EPW_PATH_SMALL / EPW_PATH_LARGE force one (tests) */
   size_t workspace_bytes; /* cap on the library's scratch HBM; 0 = library chooses from free memory */
   double degen_tol;       /* informational (gap below which callers should sum |g|^2 over a subspace); unused inside */
   double omega_min;       /* modes with omega_q,nu <= omega_min give |g|^2 = 0 (acoustic modes at Gamma); default 0 */
 } epw_interp_config;
+
+/* Kernel families of the path.  SMALL: a whole (k,q) pair lives in shared memory (Nb <= 16, configs[0..3]).
+ * LARGE: S4a, S2 and both halves of S4b are FP64 tensor-path contractions that read their operand in place
+ * (any Nb; configs[4], Nb = 192, Nm = 288).  Same results; AUTO picks by size. */
+enum { EPW_PATH_AUTO = 0, EPW_PATH_SMALL = 1, EPW_PATH_LARGE = 2 };
 
 /* Create / destroy a handle.  *out is set to NULL on failure. */
 int epw_interp_create(epw_interp_t *out, const epw_interp_config *cfg);
@@ -114,11 +120,12 @@ int epw_interp_sync(epw_interp_t h);
 /*
  * Per-stage device times (ms, CUDA events on the caller's stream) accumulated over every interpolate call since
  * stage timing was last enabled:
- *   ms[0] S0 phase tables   ms[1] S1 Rp->q   ms[2] D(q) + phonon eigensolve + S4a/pack   ms[3] H(k) + eigensolve
+ *   ms[0] S0 phase tables   ms[1] S1 Rp->q   ms[2] D(q) + phonon eigensolve   ms[3] H(k) + eigensolve
  *   ms[4] S2 Re->k contraction   ms[5] H(k+q) eigensolve   ms[6] S4b rotation + |g|^2   ms[7] total
+ *   ms[8] S4a mode rotation (hoisted onto g(Re,q)) incl. building the packed operand of S2
  * Synchronises the stream.  Returns the number of entries written (<= n) or a negative status.
  */
-#define EPW_NUM_STAGES 8
+#define EPW_NUM_STAGES 9
 int epw_interp_get_stage_times(epw_interp_t h, double *ms, int n);
 
 /* Kernel launches per stage over the same accumulation period as epw_interp_get_stage_times (same indices;
@@ -178,9 +185,24 @@ int epw_eigh_batched(const void *A, int64_t stride_a, int32_t n, int64_t batch, 
  * (Packs both operands into the DMMA fragment layout, then runs the same TMA + DMMA kernel as S2.) */
 int epw_zgemm(const void *A, const void *B, void *C, int64_t M, int32_t N, int32_t K, int64_t ldc, void *cuda_stream);
 
+/* The contraction kernel of the large-Nb path (zgemm_strided.cu): `batch` problems C_b = A_b B_b on the FP64 tensor
+ * path with the big operand A read in place:
+ *   A_b[row][r] at A + b*a_batch + (row / a_rb)*a_bs + (row % a_rb) + r*a_ks      (c128 elements; rows contiguous)
+ *   B_b[r][col] at B + bb*b_batch + r*b_sr + col*b_sn, conjugated if b_conj, bb = b_gather ? b_gather[b] : b,
+ *               nb_mats matrices are packed (b_gather values must be < nb_mats; nb_mats = batch when b_gather is NULL)
+ *   C_b[row][col] at C + b*c_batch + (row / c_rb)*c_bs + (row % c_rb)*c_rs + col*c_cs   as c128, or, if abs2 != 0,
+ *               |C_b[row][col]|^2 as f64 (strides then count f64 elements).
+ * All device pointers.  Synchronises the stream before returning (temporary packed B). */
+int epw_zgemm_strided(const void *A, int64_t a_rb, int64_t a_bs, int64_t a_ks, int64_t a_batch, const void *B,
+                      int64_t b_sr, int64_t b_sn, int64_t b_batch, int b_conj, const int32_t *b_gather, int64_t nb_mats,
+                      void *C, int64_t c_rb, int64_t c_bs, int64_t c_rs, int64_t c_cs, int64_t c_batch, int abs2,
+                      int64_t M, int32_t N, int32_t K, int64_t batch, void *cuda_stream);
+
 /* S4b: g2[ik][nu][n][m] = | sum_{m'n'} conj(Ukq[ik][m',m]) gt[ik][nu][n'][m'] Uk[ik][n',n] |^2.
  * gt c128, pair ik at gt + ik*stride_gt (c128 elements); Uk, Ukq c128 [..][Nb][Nb] column-major;
- * kq_idx NULL (Ukq indexed by ik) or int32 [nk] (Ukq indexed by kq_idx[ik]). */
+ * kq_idx NULL (Ukq indexed by ik) or int32 [nk] (Ukq indexed by kq_idx[ik]).
+ * Small (Nb, Nm): one CTA per pair in shared memory; otherwise two epw_zgemm_strided contractions (needs
+ * stride_gt == Nb^2 Nm there; allocates and frees a temporary of the size of gt, synchronising the stream). */
 int epw_rotate_g2(const void *gt, int64_t stride_gt, const void *Uk, const void *Ukq, const int32_t *kq_idx,
                   int32_t nb, int32_t nm, int64_t nk, double *g2, void *cuda_stream);
 

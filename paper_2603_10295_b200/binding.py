@@ -20,9 +20,10 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(PKG, "libepw_interp.so")
 
 EPW_OK, EPW_EINVAL, EPW_ENOMEM, EPW_ECUDA, EPW_ENOTCONVERGED, EPW_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
-EPW_NUM_STAGES = 8
+EPW_PATH_AUTO, EPW_PATH_SMALL, EPW_PATH_LARGE = 0, 1, 2
+EPW_NUM_STAGES = 9
 STAGE_NAMES = ["S0_phase_tables", "S1_rp_to_q", "phonon_Dq_eig_S4a_pack", "Hk_eig", "S2_re_to_k_dmma", "Hkq_eig",
-               "S4b_rotate_g2", "total"]
+               "S4b_rotate_g2", "total", "S4a_mode_rotation"]
 EPW_DBG_G_REQ, EPW_DBG_G_TILDE, EPW_DBG_H_K, EPW_DBG_U_K, EPW_DBG_U_KQ, EPW_DBG_E_Q = 1, 2, 3, 4, 5, 6
 
 # every symbol include/epw_interp.h declares (tests check that the library exports each of them)
@@ -30,7 +31,8 @@ EXPORTED_SYMBOLS = [
     "epw_interp_create", "epw_interp_destroy", "epw_interp_set_wannier_operators", "epw_interp_set_g_slabs",
     "epw_interp_interpolate", "epw_interp_interpolate_host", "epw_interp_sync", "epw_interp_get_stage_times",
     "epw_interp_enable_stage_timing", "epw_interp_get_stage_launches", "epw_interp_last_launch_count", "epw_interp_debug_get", "epw_interp_last_error",
-    "epw_phase_table", "epw_rp_to_q", "epw_interp_operator", "epw_eigh_batched", "epw_zgemm", "epw_rotate_g2",
+    "epw_phase_table", "epw_rp_to_q", "epw_interp_operator", "epw_eigh_batched", "epw_zgemm", "epw_zgemm_strided",
+    "epw_rotate_g2",
     "epw_probe_peaks", "epw_version",
 ]
 
@@ -43,7 +45,7 @@ class EpwError(RuntimeError):
 
 class epw_interp_config(ctypes.Structure):
     _fields_ = [("nbnd", c_int32), ("nmodes", c_int32), ("ne", c_int32), ("np", c_int32), ("device", c_int32),
-                ("q_batch", c_int32), ("workspace_bytes", c_size_t), ("degen_tol", c_double), ("omega_min", c_double)]
+                ("q_batch", c_int32), ("path", c_int32), ("workspace_bytes", c_size_t), ("degen_tol", c_double), ("omega_min", c_double)]
 
 
 _lib = None
@@ -81,6 +83,9 @@ def load_library() -> ctypes.CDLL:
         L.epw_interp_operator.argtypes = [vp, c_int32, c_int32, vp, c_int64, vp, vp]
         L.epw_eigh_batched.argtypes = [vp, c_int64, c_int32, c_int64, vp, vp, c_int, vp, vp]
         L.epw_zgemm.argtypes = [vp, vp, vp, c_int64, c_int32, c_int32, c_int64, vp]
+        L.epw_zgemm_strided.argtypes = [vp, c_int64, c_int64, c_int64, c_int64, vp, c_int64, c_int64, c_int64, c_int, vp,
+                                        c_int64, vp, c_int64, c_int64, c_int64, c_int64, c_int64, c_int, c_int64,
+                                        c_int32, c_int32, c_int64, vp]
         L.epw_rotate_g2.argtypes = [vp, c_int64, vp, vp, vp, c_int32, c_int32, c_int64, vp, vp]
         L.epw_probe_peaks.argtypes = [c_int32, POINTER(c_double)]
         L.epw_version.restype = c_char_p
@@ -115,8 +120,9 @@ def epw_version() -> str:
     return load_library().epw_version().decode()
 
 
-def epw_interp_create(nbnd, nmodes, ne, np_, device=0, q_batch=0, workspace_bytes=0, degen_tol=1e-6, omega_min=0.0):
-    cfg = epw_interp_config(nbnd, nmodes, ne, np_, device, q_batch, workspace_bytes, degen_tol, omega_min)
+def epw_interp_create(nbnd, nmodes, ne, np_, device=0, q_batch=0, workspace_bytes=0, degen_tol=1e-6, omega_min=0.0,
+                      path=EPW_PATH_AUTO):
+    cfg = epw_interp_config(nbnd, nmodes, ne, np_, device, q_batch, path, workspace_bytes, degen_tol, omega_min)
     h = c_void_p()
     _check(load_library().epw_interp_create(byref(h), byref(cfg)))
     return h
@@ -199,6 +205,14 @@ def epw_zgemm(A, B, C, M, N, K, ldc, stream=None):
     _check(load_library().epw_zgemm(_ptr(A), _ptr(B), _ptr(C), M, N, K, ldc, _stream() if stream is None else stream))
 
 
+def epw_zgemm_strided(A, a_rb, a_bs, a_ks, a_batch, B, b_sr, b_sn, b_batch, b_conj, b_gather, nb_mats, C, c_rb, c_bs,
+                      c_rs, c_cs, c_batch, abs2, M, N, K, batch, stream=None):
+    _check(load_library().epw_zgemm_strided(_ptr(A), a_rb, a_bs, a_ks, a_batch, _ptr(B), b_sr, b_sn, b_batch,
+                                            int(b_conj), _ptr(b_gather), nb_mats, _ptr(C), c_rb, c_bs, c_rs, c_cs,
+                                            c_batch, int(abs2), M, N, K, batch,
+                                            _stream() if stream is None else stream))
+
+
 def epw_rotate_g2(gt, stride_gt, Uk, Ukq, kq_idx, nb, nm, nk, g2, stream=None):
     _check(load_library().epw_rotate_g2(_ptr(gt), stride_gt, _ptr(Uk), _ptr(Ukq), _ptr(kq_idx), nb, nm, nk, _ptr(g2),
                                         _stream() if stream is None else stream))
@@ -213,10 +227,11 @@ def epw_probe_peaks(device=0) -> dict:
 class EpwInterp:
     """Owns one library handle.  `workload` is a synth.Workload-like object (numpy operators on the host)."""
 
-    def __init__(self, nbnd, nmodes, ne, np_, device=0, q_batch=0, workspace_bytes=0, omega_min=0.0):
+    def __init__(self, nbnd, nmodes, ne, np_, device=0, q_batch=0, workspace_bytes=0, omega_min=0.0,
+                 path=EPW_PATH_AUTO):
         self.nbnd, self.nmodes, self.ne, self.np = nbnd, nmodes, ne, np_
         self.device = device
-        self.h = epw_interp_create(nbnd, nmodes, ne, np_, device, q_batch, workspace_bytes, 1e-6, omega_min)
+        self.h = epw_interp_create(nbnd, nmodes, ne, np_, device, q_batch, workspace_bytes, 1e-6, omega_min, path)
 
     def close(self):
         if self.h is not None:

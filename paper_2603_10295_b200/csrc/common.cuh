@@ -90,6 +90,19 @@ cudaError_t launch_pack_b_generic(const c128 *B, int K, int N, double *Bpack, cu
 cudaError_t launch_zgemm_dmma(const double *Apack, const double *Bpack, c128 *C, int64_t M, int N, int KB, int64_t ldc,
                               int num_sms, cudaStream_t st);
 
+// Large-Nb path (zgemm_strided.cu): C[row][col] = sum_r A[row][r] B[r][col] with A read in place,
+//   A[row][r] at A + b*a_batch + (row / a_rb)*a_bs + (row % a_rb) + r*a_ks,
+//   C[row][col] at C + b*c_batch + (row / c_rb)*c_bs + (row % c_rb)*c_rs + col*c_cs   (c128, or |.|^2 as f64 when abs2),
+//   packed B' of problem b at Bpack + (b_gather ? b_gather[b] : b) * NT*KB*2048.
+cudaError_t launch_zgemm_strided(const c128 *A, int64_t a_rb, int64_t a_bs, int64_t a_ks, int64_t a_batch,
+                                 const double *Bpack, const int32_t *b_gather, void *C, int64_t c_rb, int64_t c_bs,
+                                 int64_t c_rs, int64_t c_cs, int64_t c_batch, int abs2, int64_t M, int N, int K,
+                                 int64_t batch, int num_sms, cudaStream_t st);
+// packed B' from a strided complex operand: B[r][n] at B + b*batch_stride + r*sr + n*sn (conj optional; columns scaled
+// by 1/sqrt(2 omega[n]) when omega != NULL).  Bpack doubles [batch][NT][KB][2048].
+cudaError_t launch_pack_b_strided(const c128 *B, int64_t sr, int64_t sn, int64_t batch_stride, int64_t batch, int conj,
+                                  const double *omega, double omega_min, int K, int N, double *Bpack, cudaStream_t st);
+
 cudaError_t launch_rotate_g2(const c128 *gt, int64_t stride_gt, const c128 *Uk, const c128 *Ukq, const int32_t *kq_idx,
                              int nb, int nm, int64_t nk, double *g2, cudaStream_t st);
 

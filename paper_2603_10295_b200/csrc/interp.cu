@@ -88,6 +88,8 @@ struct epw_interp {
   DevBuf g, H, D, Re, Rp, we, wp, ones;
   // per-call workspace
   DevBuf Apack, BpackH, Hk, Uk, Pq, Pqe, Dq, eq, g1, Bpack, C, Ukq, epskq_scratch, status, eig_scratch;
+  // large-Nb path only
+  DevBuf Pk, BpackPk, UpackK, UpackKH, BpackE, ghat, T, Hkq;
   // host-entry staging
   DevBuf hs_k, hs_q, hs_map, hs_epsk, hs_epskq, hs_omega, hs_g2;
   // bookkeeping of the last call
@@ -141,6 +143,198 @@ struct epw_interp {
     CU_OR_FAIL(h, expr, where); \
   } while (0)
 
+
+// The small-Nb kernels (pack_b_kernel, rotate_g2_small_kernel) keep a whole (k,q) pair in shared memory; beyond that
+// (or when the caller asks for it) the large-Nb path of zgemm_strided.cu runs.
+static bool use_large_path(const epw_interp *h) {
+  if (h->cfg.path == EPW_PATH_SMALL) return false;
+  if (h->cfg.path == EPW_PATH_LARGE) return true;
+  const size_t rot_smem = sizeof(c128) * ((size_t)2 * h->nbb * h->nm + 2 * (size_t)h->nbb);
+  return h->nb > 16 || rot_smem > (size_t)200 * 1024;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Large-Nb path (BASELINE.json configs[4]: Nb = 192, Nm = 288, g(Re,Rp) = 49 GB; Table III).
+// Same stages, same order of the nested-loop algorithm, but S4a, S2 and both halves of S4b are
+// FP64 tensor-path contractions that read their big operand in place (zgemm_strided.cu):
+//   S4a  g^(Re,q) = g(Re,q) . e_q/sqrt(2 omega)       [Ne Nb^2 x Nm] . [Nm x Nm]            once per q
+//   S2   g~(k,q)  = g^(Re,q)^T-contracted with P_k     [Nb^2 Nm x Ne] . [Ne x k-chunk]        per k-chunk
+//   S4b  T = g~ U_k ;  |g|^2 = |T conj(U_{k+q})|^2      [Nm Nb x Nb] . [Nb x Nb], batched over the k of the chunk
+// ---------------------------------------------------------------------------------------------------------
+static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, const double *q_list, int64_t nq,
+                             const int32_t *kq_map, double *eps_k, double *eps_kq, double *omega_q, double *g2,
+                             cudaStream_t st) {
+  const int nb = h->nb, nm = h->nm, ne = h->ne, np = h->np, nbb = h->nbb, nmm = h->nmm;
+  const int64_t E = (int64_t)nbb * nm;        // elements per (k,q) pair
+  const int64_t xrows = (int64_t)ne * nbb;    // rows of the S4a contraction
+  const int64_t MR = (int64_t)nm * nb;        // rows of the two S4b contractions
+  const int KBe = (int)ceil_div(2 * (int64_t)ne, GEMM_BK), KBb = (int)ceil_div(2 * (int64_t)nb, GEMM_BK);
+  const int KBm = (int)ceil_div(2 * (int64_t)nm, GEMM_BK);
+  const int NTb = (int)ceil_div(2 * (int64_t)nb, GEMM_BN), NTm = (int)ceil_div(2 * (int64_t)nm, GEMM_BN);
+  const int NTH = (int)ceil_div(2 * (int64_t)nbb, GEMM_BN);
+  const int64_t NTk = ceil_div(nk, 64);
+  const int64_t MTk = ceil_div(nk, GEMM_BM);
+  const int64_t upack = (int64_t)NTb * KBb * GEMM_CHUNK;  // doubles of one packed Nb x Nb operand
+
+  // q per pass over g(Re,Rp): g(Re,q) is 16 Nb^2 Nm Ne bytes per q here (2.9 GB for configs[4]); keep the batch <= 8 GB
+  int QB = (int)std::min<int64_t>(h->q_batch, nq);
+  {
+    const size_t per_q = sizeof(c128) * (size_t)h->rows;
+    QB = (int)std::max<int64_t>(1, std::min<int64_t>(QB, (int64_t)(((size_t)8 << 30) / per_q)));
+  }
+  // k per chunk: g~ and T are 16 E bytes per k each; whole 64-column tiles of the S2 contraction
+  const size_t cap = h->cfg.workspace_bytes ? h->cfg.workspace_bytes : ((size_t)24 << 30);
+  int64_t kc = (int64_t)(cap / (2 * sizeof(c128) * (size_t)E));
+  if (kc >= nk) kc = nk;
+  else if (kc >= 64) kc = kc / 64 * 64;
+  else return h->fail(EPW_ENOMEM, "epw_interp_interpolate: workspace_bytes too small for one 64-k chunk of g~ and T");
+
+  CU_OR_FAIL(h, h->Apack.reserve(sizeof(double) * (size_t)MTk * KBe * GEMM_CHUNK), "cudaMalloc Apack");
+  CU_OR_FAIL(h, h->BpackH.reserve(sizeof(double) * (size_t)NTH * KBe * GEMM_CHUNK), "cudaMalloc BpackH");
+  CU_OR_FAIL(h, h->Hk.reserve(sizeof(c128) * (size_t)nk * nbb), "cudaMalloc Hk");
+  CU_OR_FAIL(h, h->Uk.reserve(sizeof(c128) * (size_t)nk * nbb), "cudaMalloc Uk");
+  CU_OR_FAIL(h, h->Pk.reserve(sizeof(c128) * (size_t)nk * ne), "cudaMalloc Pk");
+  CU_OR_FAIL(h, h->BpackPk.reserve(sizeof(double) * (size_t)NTk * KBe * GEMM_CHUNK), "cudaMalloc BpackPk");
+  CU_OR_FAIL(h, h->UpackK.reserve(sizeof(double) * (size_t)nk * upack), "cudaMalloc UpackK");
+  CU_OR_FAIL(h, h->UpackKH.reserve(sizeof(double) * (size_t)nk * upack), "cudaMalloc UpackKH");
+  CU_OR_FAIL(h, h->Pq.reserve(sizeof(c128) * (size_t)QB * np), "cudaMalloc Pq");
+  CU_OR_FAIL(h, h->Dq.reserve(sizeof(c128) * (size_t)QB * nmm), "cudaMalloc Dq");
+  CU_OR_FAIL(h, h->eq.reserve(sizeof(c128) * (size_t)QB * nmm), "cudaMalloc e_q");
+  CU_OR_FAIL(h, h->g1.reserve(sizeof(c128) * (size_t)QB * h->rows), "cudaMalloc g(Re,q)");
+  CU_OR_FAIL(h, h->BpackE.reserve(sizeof(double) * (size_t)NTm * KBm * GEMM_CHUNK), "cudaMalloc BpackE");
+  CU_OR_FAIL(h, h->ghat.reserve(sizeof(c128) * (size_t)ne * E), "cudaMalloc g^(Re,q)");
+  CU_OR_FAIL(h, h->C.reserve(sizeof(c128) * (size_t)kc * E), "cudaMalloc g~");
+  CU_OR_FAIL(h, h->T.reserve(sizeof(c128) * (size_t)kc * E), "cudaMalloc T");
+  if (!kq_map) {
+    CU_OR_FAIL(h, h->Pqe.reserve(sizeof(c128) * (size_t)QB * ne), "cudaMalloc Pqe");
+    CU_OR_FAIL(h, h->Hkq.reserve(sizeof(c128) * (size_t)nk * nbb), "cudaMalloc Hkq");
+    CU_OR_FAIL(h, h->Ukq.reserve(sizeof(c128) * (size_t)nk * nbb), "cudaMalloc Ukq");
+    if (!eps_kq) CU_OR_FAIL(h, h->epskq_scratch.reserve(sizeof(double) * (size_t)nk * nb), "cudaMalloc eps scratch");
+  }
+  CU_OR_FAIL(h, h->status.reserve(sizeof(int32_t)), "cudaMalloc status");
+  {
+    const size_t need = std::max(eigh_large_scratch_bytes(nb, nk), eigh_large_scratch_bytes(nm, QB));
+    if (need) CU_OR_FAIL(h, h->eig_scratch.reserve(need), "cudaMalloc eig scratch");
+  }
+  CU_OR_FAIL(h, cudaMemsetAsync(h->status.p, 0, sizeof(int32_t), st), "memset status");
+  h->last_nk = nk;
+  h->last_c_rows = kc;
+  h->last_ncols = (int)E;
+
+  const int t_total = h->begin_span(7, st);
+
+  // ---- k side, once per call: phases, H(k) (same DMMA contraction as the small path), eigensolve, packed U_k ----
+  int sp = h->begin_span(0, st);
+  LAUNCH(h, launch_phase_pack_a(k_list, nk, h->Re.as<int32_t>(), h->we.as<double>(), ne, h->Apack.as<double>(), st),
+         "phase_pack_a");
+  LAUNCH(h, launch_phase_table(k_list, nk, h->Re.as<int32_t>(), h->we.as<double>(), ne, h->Pk.as<c128>(), st),
+         "phase_table(k,Re)");
+  LAUNCH(h, launch_pack_b_strided(h->Pk.as<c128>(), 1, ne, 0, 1, 0, nullptr, 0.0, ne, (int)nk, h->BpackPk.as<double>(), st),
+         "pack P_k");
+  h->end_span(sp, st);
+  sp = h->begin_span(3, st);
+  LAUNCH(h,
+         launch_pack_b(nullptr, nullptr, nullptr, 0.0, h->H.as<c128>(), nullptr, nbb, nm, ne, 0, nbb,
+                       h->BpackH.as<double>(), st),
+         "pack_b(H)");
+  LAUNCH(h, launch_zgemm_dmma(h->Apack.as<double>(), h->BpackH.as<double>(), h->Hk.as<c128>(), nk, nbb, KBe, nbb,
+                              h->num_sms, st),
+         "zgemm H(k)");
+  LAUNCH(h, launch_eigh_batched(h->Hk.as<c128>(), nbb, nb, nk, eps_k, h->Uk.as<c128>(), 0, h->status.as<int32_t>(),
+                                h->eig_scratch.as<c128>(), st),
+         "eigh H(k)");
+  LAUNCH(h, launch_pack_b_strided(h->Uk.as<c128>(), 1, nb, nbb, nk, 0, nullptr, 0.0, nb, nb, h->UpackK.as<double>(), st),
+         "pack U_k");
+  if (kq_map)
+    LAUNCH(h, launch_pack_b_strided(h->Uk.as<c128>(), 1, nb, nbb, nk, 1, nullptr, 0.0, nb, nb, h->UpackKH.as<double>(), st),
+           "pack conj U_k");
+  h->end_span(sp, st);
+
+  for (int64_t q0 = 0; q0 < nq; q0 += QB) {
+    const int qb = (int)std::min<int64_t>(QB, nq - q0);
+    sp = h->begin_span(0, st);
+    LAUNCH(h, launch_phase_table(q_list + 3 * q0, qb, h->Rp.as<int32_t>(), h->wp.as<double>(), np, h->Pq.as<c128>(), st),
+           "phase_table(q,Rp)");
+    if (!kq_map)
+      LAUNCH(h, launch_phase_table(q_list + 3 * q0, qb, h->Re.as<int32_t>(), h->ones.as<double>(), ne,
+                                   h->Pqe.as<c128>(), st),
+             "phase_table(q,Re)");
+    h->end_span(sp, st);
+    sp = h->begin_span(1, st);
+    LAUNCH(h, launch_rp_to_q(h->g.as<c128>(), h->rows, np, h->Pq.as<c128>(), qb, h->g1.as<c128>(), st), "rp_to_q");
+    h->end_span(sp, st);
+    sp = h->begin_span(2, st);
+    LAUNCH(h, launch_interp_operator(h->D.as<c128>(), nm, np, h->Pq.as<c128>(), qb, h->Dq.as<c128>(), st), "D(q)");
+    LAUNCH(h, launch_eigh_batched(h->Dq.as<c128>(), nmm, nm, qb, omega_q + q0 * nm, h->eq.as<c128>(), 1,
+                                  h->status.as<int32_t>(), h->eig_scratch.as<c128>(), st),
+           "eigh D(q)");
+    h->end_span(sp, st);
+
+    for (int iq = 0; iq < qb; iq++) {
+      const int64_t q = q0 + iq;
+      // ---- S4a (hoisted): g^(Re,q)[Re][nu][n'][m'] = sum_ka g(Re,q)[ka][Re][n'][m'] e_q[ka][nu] / sqrt(2 omega_nu) ----
+      sp = h->begin_span(8, st);
+      LAUNCH(h, launch_pack_b_strided(h->eq.as<c128>() + (int64_t)iq * nmm, 1, nm, 0, 1, 0, omega_q + q * nm,
+                                      h->cfg.omega_min, nm, nm, h->BpackE.as<double>(), st),
+             "pack e_q");
+      LAUNCH(h, launch_zgemm_strided(h->g1.as<c128>() + (int64_t)iq * h->rows, xrows, 0, xrows, 0,
+                                     h->BpackE.as<double>(), nullptr, h->ghat.p, nbb, E, 1, nbb, 0, 0, xrows, nm, nm, 1,
+                                     h->num_sms, st),
+             "zgemm S4a");
+      h->end_span(sp, st);
+      const double *Bconj = h->UpackKH.as<double>();
+      if (!kq_map) {
+        // ---- off-grid q: H(k+q) for every k, eigensolve, packed conj(U_{k+q}) ----
+        sp = h->begin_span(5, st);
+        LAUNCH(h,
+               launch_pack_b(nullptr, nullptr, nullptr, 0.0, h->H.as<c128>(), h->Pqe.as<c128>() + (int64_t)iq * ne, nbb,
+                             nm, ne, 0, nbb, h->BpackH.as<double>(), st),
+               "pack_b(H e^{iqR})");
+        LAUNCH(h, launch_zgemm_dmma(h->Apack.as<double>(), h->BpackH.as<double>(), h->Hkq.as<c128>(), nk, nbb, KBe, nbb,
+                                    h->num_sms, st),
+               "zgemm H(k+q)");
+        double *eps_dst = eps_kq ? eps_kq + q * nk * nb : h->epskq_scratch.as<double>();
+        LAUNCH(h, launch_eigh_batched(h->Hkq.as<c128>(), nbb, nb, nk, eps_dst, h->Ukq.as<c128>(), 0,
+                                      h->status.as<int32_t>(), h->eig_scratch.as<c128>(), st),
+               "eigh H(k+q)");
+        LAUNCH(h, launch_pack_b_strided(h->Ukq.as<c128>(), 1, nb, nbb, nk, 1, nullptr, 0.0, nb, nb,
+                                        h->UpackKH.as<double>(), st),
+               "pack conj U_{k+q}");
+        h->end_span(sp, st);
+      } else if (eps_kq) {
+        sp = h->begin_span(5, st);
+        h->launches++;
+        gather_eps_kernel<<<(unsigned)std::min<int64_t>(ceil_div(nk * nb, 256), 148 * 8), 256, 0, st>>>(
+            eps_k, kq_map + q * nk, nb, nk, eps_kq + q * nk * nb);
+        CU_OR_FAIL(h, cudaGetLastError(), "gather_eps");
+        h->end_span(sp, st);
+      }
+      for (int64_t k0 = 0; k0 < nk; k0 += kc) {
+        const int64_t kn = std::min(kc, nk - k0);
+        // ---- S2: g~[k][nu][n'][m'] = sum_Re g^[Re][nu][n'][m'] P_k[k][Re] ----
+        sp = h->begin_span(4, st);
+        LAUNCH(h, launch_zgemm_strided(h->ghat.as<c128>(), E, 0, E, 0,
+                                       h->BpackPk.as<double>() + (k0 / 64) * (int64_t)KBe * GEMM_CHUNK, nullptr, h->C.p, E, 0,
+                                       1, E, 0, 0, E, (int)kn, ne, 1, h->num_sms, st),
+               "zgemm S2");
+        h->end_span(sp, st);
+        // ---- S4b: T[k][nu][m'][n] = sum_n' g~[k][nu][n'][m'] U_k[n'][n];  |g|^2[k][nu][n][m] = |sum_m' T conj(U_{k+q}[m'][m])|^2 ----
+        sp = h->begin_span(6, st);
+        LAUNCH(h, launch_zgemm_strided(h->C.as<c128>(), nb, nbb, nb, E, h->UpackK.as<double>() + k0 * upack, nullptr,
+                                       h->T.p, MR, 0, nb, 1, E, 0, MR, nb, nb, kn, h->num_sms, st),
+               "zgemm S4b (U_k)");
+        LAUNCH(h, launch_zgemm_strided(h->T.as<c128>(), nb, nbb, nb, E, kq_map ? Bconj : Bconj + k0 * upack,
+                                       kq_map ? kq_map + q * nk + k0 : nullptr, g2 + (q * nk + k0) * E, MR, 0, nb, 1, E,
+                                       1, MR, nb, nb, kn, h->num_sms, st),
+               "zgemm S4b (U_{k+q}) + |g|^2");
+        h->end_span(sp, st);
+      }
+    }
+  }
+  h->end_span(t_total, st);
+  return EPW_OK;
+}
+
 extern "C" {
 
 const char *epw_version(void) { return "epw-interp-b200 0.1 (sm_100a, FP64 DMMA)"; }
@@ -152,6 +346,10 @@ int epw_interp_create(epw_interp_t *out, const epw_interp_config *cfg) {
   *out = nullptr;
   if (!cfg || cfg->nbnd <= 0 || cfg->nmodes <= 0 || cfg->ne <= 0 || cfg->np <= 0) {
     g_create_error = "epw_interp_create: nbnd, nmodes, ne, np must be positive";
+    return EPW_EINVAL;
+  }
+  if (cfg->path < EPW_PATH_AUTO || cfg->path > EPW_PATH_LARGE) {
+    g_create_error = "epw_interp_create: path must be EPW_PATH_AUTO, EPW_PATH_SMALL or EPW_PATH_LARGE";
     return EPW_EINVAL;
   }
   if (cfg->q_batch < 0 || cfg->q_batch > 8) {
@@ -198,7 +396,8 @@ void epw_interp_destroy(epw_interp_t h) {
   DevBuf *all[] = {&h->g, &h->H, &h->D, &h->Re, &h->Rp, &h->we, &h->wp, &h->ones, &h->Apack, &h->BpackH, &h->Hk,
                    &h->Uk, &h->Pq, &h->Pqe, &h->Dq, &h->eq, &h->g1, &h->Bpack, &h->C, &h->Ukq, &h->epskq_scratch,
                    &h->status, &h->eig_scratch, &h->hs_k, &h->hs_q, &h->hs_map, &h->hs_epsk, &h->hs_epskq,
-                   &h->hs_omega, &h->hs_g2};
+                   &h->hs_omega, &h->hs_g2, &h->Pk, &h->BpackPk, &h->UpackK, &h->UpackKH, &h->BpackE,
+                   &h->ghat, &h->T, &h->Hkq};
   for (DevBuf *b : all) b->release();
   for (cudaEvent_t ev : h->ev_pool) cudaEventDestroy(ev);
   delete h;
@@ -265,11 +464,12 @@ int epw_interp_interpolate(epw_interp_t h, const double *k_list, int64_t nk, con
   if (!h->operators_set) return h->fail(EPW_EINVAL, "epw_interp_interpolate: operators not set");
   for (int ip = 0; ip < h->np; ip++)
     if (!h->slab_set[ip]) return h->fail(EPW_EINVAL, "epw_interp_interpolate: g(Re,Rp) slab missing");
-  if (h->nb > 16) return h->fail(EPW_EUNSUPPORTED, "epw_interp_interpolate: nbnd > 16 path not built yet");
   CU_OR_FAIL(h, cudaSetDevice(h->cfg.device), "cudaSetDevice");
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
   h->last_stream = st;
   h->launches = 0;
+  if (use_large_path(h))
+    return interpolate_large(h, k_list, nk, q_list, nq, kq_map, eps_k, eps_kq, omega_q, g2, st);
 
   const int nb = h->nb, nm = h->nm, ne = h->ne, np = h->np, nbb = h->nbb, nmm = h->nmm;
   const int ncols_g = nbb * nm;
@@ -355,6 +555,8 @@ int epw_interp_interpolate(epw_interp_t h, const double *k_list, int64_t nk, con
     LAUNCH(h, launch_eigh_batched(h->Dq.as<c128>(), nmm, nm, qb, omega_q + q0 * nm, h->eq.as<c128>(), 1,
                                   h->status.as<int32_t>(), h->eig_scratch.as<c128>(), st),
            "eigh D(q)");
+    h->end_span(sp, st);
+    sp = h->begin_span(8, st);
     for (int iq = 0; iq < qb; iq++)
       LAUNCH(h,
              launch_pack_b(h->g1.as<c128>() + (int64_t)iq * h->rows, h->eq.as<c128>() + (int64_t)iq * nmm,
@@ -585,13 +787,52 @@ int epw_zgemm(const void *A, const void *B, void *C, int64_t M, int32_t N, int32
   return rc_of(e);
 }
 
+int epw_zgemm_strided(const void *A, int64_t a_rb, int64_t a_bs, int64_t a_ks, int64_t a_batch, const void *B,
+                      int64_t b_sr, int64_t b_sn, int64_t b_batch, int b_conj, const int32_t *b_gather, int64_t nb_mats,
+                      void *C, int64_t c_rb, int64_t c_bs, int64_t c_rs, int64_t c_cs, int64_t c_batch, int abs2,
+                      int64_t M, int32_t N, int32_t K, int64_t batch, void *cuda_stream) {
+  if (!A || !B || !C || M <= 0 || N <= 0 || K <= 0 || batch <= 0 || a_rb <= 0 || c_rb <= 0 || nb_mats <= 0)
+    return EPW_EINVAL;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  int dev = 0, nsm = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  const int KB = (int)ceil_div(2 * (int64_t)K, GEMM_BK);
+  const int NT = (int)ceil_div(2 * (int64_t)N, GEMM_BN);
+  double *Bp = nullptr;
+  if (cudaMalloc(&Bp, sizeof(double) * (size_t)nb_mats * NT * KB * GEMM_CHUNK) != cudaSuccess) return EPW_ENOMEM;
+  cudaError_t e = launch_pack_b_strided(reinterpret_cast<const c128 *>(B), b_sr, b_sn, b_batch, nb_mats, b_conj, nullptr,
+                                        0.0, K, N, Bp, st);
+  if (e == cudaSuccess)
+    e = launch_zgemm_strided(reinterpret_cast<const c128 *>(A), a_rb, a_bs, a_ks, a_batch, Bp, b_gather, C, c_rb, c_bs,
+                             c_rs, c_cs, c_batch, abs2, M, N, K, batch, nsm, st);
+  cudaStreamSynchronize(st);
+  cudaFree(Bp);
+  return rc_of(e);
+}
+
 int epw_rotate_g2(const void *gt, int64_t stride_gt, const void *Uk, const void *Ukq, const int32_t *kq_idx, int32_t nb,
                   int32_t nm, int64_t nk, double *g2, void *cuda_stream) {
   if (!gt || !Uk || !Ukq || !g2 || nb <= 0 || nm <= 0 || nk < 0) return EPW_EINVAL;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
   const cudaError_t e = launch_rotate_g2(reinterpret_cast<const c128 *>(gt), stride_gt, reinterpret_cast<const c128 *>(Uk),
-                                         reinterpret_cast<const c128 *>(Ukq), kq_idx, nb, nm, nk, g2,
-                                         reinterpret_cast<cudaStream_t>(cuda_stream));
-  return e == cudaErrorInvalidConfiguration ? EPW_EUNSUPPORTED : rc_of(e);
+                                         reinterpret_cast<const c128 *>(Ukq), kq_idx, nb, nm, nk, g2, st);
+  if (e != cudaErrorInvalidConfiguration) return rc_of(e);
+  // large (Nb, Nm): T[(nu,m')][n] = sum_n' g~[(nu,m')][n'] U_k[n'][n];  |g|^2[(nu,n)][m] = |sum_m' T[(nu,n)][m'] conj(Ukq[m'][m])|^2
+  cudaGetLastError();
+  const int64_t E = (int64_t)nb * nb * nm, MR = (int64_t)nm * nb, nbb = (int64_t)nb * nb;
+  if (stride_gt != E) return EPW_EUNSUPPORTED;
+  if (nk == 0) return EPW_OK;
+  // Ukq may be indexed through kq_idx by values up to the size of the caller's U table: the caller guarantees nk entries
+  c128 *T = nullptr;
+  if (cudaMalloc(&T, sizeof(c128) * (size_t)nk * E) != cudaSuccess) return EPW_ENOMEM;
+  int rc = epw_zgemm_strided(gt, nb, nbb, nb, E, Uk, 1, nb, nbb, 0, nullptr, nk, T, MR, 0, nb, 1, E, 0, MR, nb, nb, nk,
+                             cuda_stream);
+  if (rc == EPW_OK)
+    rc = epw_zgemm_strided(T, nb, nbb, nb, E, Ukq, 1, nb, nbb, 1, kq_idx, nk, g2, MR, 0, nb, 1, E, 1, MR, nb, nb, nk,
+                           cuda_stream);
+  cudaFree(T);
+  return rc;
 }
 
 int epw_probe_peaks(int32_t device, double *out4) {

@@ -133,6 +133,53 @@ __global__ void __launch_bounds__(256) pack_b_generic_kernel(const c128 *__restr
   for (int i = threadIdx.x; i < GEMM_CHUNK / 2; i += blockDim.x) dst[i] = src[i];
 }
 
+// Strided / batched B' builder of the large-Nb path: complex B[r][n] read at  B + b*batch_stride + r*sr + n*sn,
+// optionally conjugated, optionally scaled per column n by the zero-point amplitude 1/sqrt(2 omega[n]) (0 when
+// omega[n] <= omega_min: BASELINE.json north_star stage 4; reading G12).  One CTA per 16 KB chunk.
+__global__ void __launch_bounds__(256) pack_b_strided_kernel(const c128 *__restrict__ B, int64_t sr, int64_t sn,
+                                                             int64_t batch_stride, int conj,
+                                                             const double *__restrict__ omega, double omega_min, int K,
+                                                             int N, int KB, int NT, double *__restrict__ Bpack) {
+  __shared__ double chunk[GEMM_CHUNK];
+  const int64_t b = blockIdx.x / (NT * KB);
+  const int rem = (int)(blockIdx.x - b * (NT * KB));
+  const int nt = rem / KB;
+  const int kb = rem - nt * KB;
+  const c128 *src = B + b * batch_stride;
+  for (int el = threadIdx.x; el < 8 * 64; el += blockDim.x) {
+    // r fastest when the operand is r-contiguous (sr == 1), n fastest otherwise: coalesced either way
+    const int rc = sr == 1 ? (el & 7) : (el >> 6);
+    const int cc = sr == 1 ? (el >> 3) : (el & 63);
+    const int c = nt * 64 + cc, r = kb * 8 + rc;
+    c128 v = cmake(0.0, 0.0);
+    if (r < K && c < N) {
+      v = src[(int64_t)r * sr + (int64_t)c * sn];
+      if (conj) v.y = -v.y;
+      if (omega != nullptr) {
+        const double om = omega[c];
+        const double amp = om > omega_min ? 1.0 / sqrt(2.0 * om) : 0.0;
+        v.x *= amp;
+        v.y *= amp;
+      }
+    }
+    put_b(chunk, rc, cc, v);
+  }
+  __syncthreads();
+  double2 *dst = reinterpret_cast<double2 *>(Bpack + (int64_t)blockIdx.x * GEMM_CHUNK);
+  const double2 *s2 = reinterpret_cast<const double2 *>(chunk);
+  for (int i = threadIdx.x; i < GEMM_CHUNK / 2; i += blockDim.x) dst[i] = s2[i];
+}
+
+cudaError_t launch_pack_b_strided(const c128 *B, int64_t sr, int64_t sn, int64_t batch_stride, int64_t batch, int conj,
+                                  const double *omega, double omega_min, int K, int N, double *Bpack, cudaStream_t st) {
+  if (batch <= 0) return cudaSuccess;
+  const int KB = (int)ceil_div(2 * (int64_t)K, GEMM_BK);
+  const int NT = (int)ceil_div(2 * (int64_t)N, GEMM_BN);
+  pack_b_strided_kernel<<<(unsigned)(batch * NT * KB), 256, 0, st>>>(B, sr, sn, batch_stride, conj, omega, omega_min, K,
+                                                                    N, KB, NT, Bpack);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_pack_a_generic(const c128 *A, int64_t M, int K, double *Apack, cudaStream_t st) {
   const int KB = (int)ceil_div(2 * (int64_t)K, GEMM_BK);
   pack_a_generic_kernel<<<(unsigned)(ceil_div(M, GEMM_BM) * KB), 256, 0, st>>>(A, M, K, KB, Apack);

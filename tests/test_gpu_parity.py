@@ -201,11 +201,73 @@ def test_rotate_g2(epw, nb, nm):
             assert np.abs(got[ik] - ref).max() <= 1e-12 * ref.max()
 
 
+
+@pytest.mark.parametrize("case", ["plain", "blocked", "blocked_ragged", "colmajor_c", "batched_gather_conj_abs2"])
+def test_zgemm_strided(epw, case):
+    """The in-place-A DMMA contraction of the large-Nb path against the plain definition, in every addressing mode the
+    path uses: blocked rows (a_rb < tile), several row blocks per tile, ragged M / N / K, transposed store, batches with
+    gathered conjugated B and the |.|^2 epilogue."""
+    if case == "plain":            # S4a-like: A[row][r] at r*M + row ; C row-major
+        M, N, K, batch = 300, 70, 21, 1
+        A = crandn(K, M); B = crandn(K, N)
+        ref = np.einsum("rm,rn->mn", A, B)
+        C = torch.zeros((M, N, 2), dtype=torch.float64, device="cuda")
+        epw.epw_zgemm_strided(zdev(A), M, 0, M, 0, zdev(B), N, 1, 0, 0, None, 1, C, M, 0, N, 1, 0, 0, M, N, K, 1)
+        got = znp(C)
+    elif case in ("blocked", "blocked_ragged"):   # S4b-like: row = (nu, x), A at nu*nbb + r*nb + x
+        nb, nm = (192, 3) if case == "blocked" else (13, 37)
+        M, N, K = nm * nb, nb, nb
+        G = crandn(nm, nb, nb)      # [nu][r][x]
+        U = crandn(nb, nb)          # column-major storage: U[n][r] <-> B[r][n]
+        ref = np.einsum("vrx,nr->vxn", G, U).reshape(M, N)
+        C = torch.zeros((M, N, 2), dtype=torch.float64, device="cuda")
+        epw.epw_zgemm_strided(zdev(G), nb, nb * nb, nb, 0, zdev(U), 1, nb, 0, 0, None, 1, C, M, 0, N, 1, 0, 0, M, N, K, 1)
+        got = znp(C)
+    elif case == "colmajor_c":     # S2-like: C[c][k] stored at k*M + c, N not a multiple of the tile
+        M, N, K = 1000, 70, 17
+        A = crandn(K, M); P = crandn(N, K)     # B[r][n] = P[n][r]
+        ref = np.einsum("rm,nr->mn", A, P)
+        C = torch.zeros((N, M, 2), dtype=torch.float64, device="cuda")
+        epw.epw_zgemm_strided(zdev(A), M, 0, M, 0, zdev(P), 1, K, 0, 0, None, 1, C, M, 0, 1, M, 0, 0, M, N, K, 1)
+        got = znp(C).T
+    else:
+        nb, nm, batch = 20, 9, 5
+        M, N, K = nm * nb, nb, nb
+        T = crandn(batch, nm, nb, nb)   # [b][nu][r][x]
+        U = crandn(7, nb, nb)           # 7 matrices, column-major: U[i][m][r]
+        idx = np.array([6, 0, 3, 3, 1], dtype=np.int32)
+        ref = np.abs(np.einsum("bvrx,bmr->bvxm", T, U[idx].conj())) ** 2
+        C = torch.zeros((batch, M, N), dtype=torch.float64, device="cuda")
+        epw.epw_zgemm_strided(zdev(T), nb, nb * nb, nb, nm * nb * nb, zdev(U), 1, nb, nb * nb, 1, dev(idx), 7, C, M, 0, N,
+                              1, M * N, 1, M, N, K, batch)
+        got = C.cpu().numpy().reshape(ref.shape)
+    torch.cuda.synchronize()
+    assert np.abs(got.reshape(ref.shape) - ref).max() <= 1e-13 * K * max(1.0, np.abs(ref).max())
+
+
+def test_rotate_g2_large(epw):
+    """S4b beyond the shared-memory kernel (Nb = 48): two in-place DMMA contractions, against oracle.band_rotate."""
+    nb, nm, nk = 48, 7, 5
+    gt = crandn(nk, nm, nb, nb)
+    Uk = np.stack([np.linalg.qr(crandn(nb, nb))[0].T for _ in range(nk)])
+    Ukq = np.stack([np.linalg.qr(crandn(nb, nb))[0].T for _ in range(nk)])
+    idx = rng.permutation(nk).astype(np.int32)
+    g2 = torch.empty((nk, nm, nb, nb), dtype=torch.float64, device="cuda")
+    for kq_idx in (None, idx):
+        epw.epw_rotate_g2(zdev(gt), nm * nb * nb, zdev(Uk), zdev(Ukq), None if kq_idx is None else dev(kq_idx), nb, nm,
+                          nk, g2)
+        got = g2.cpu().numpy()
+        for ik in range(nk):
+            u = Ukq[ik] if kq_idx is None else Ukq[kq_idx[ik]]
+            ref = np.abs(oracle.band_rotate(gt[ik], u, Uk[ik])) ** 2
+            assert np.abs(got[ik] - ref).max() <= 1e-12 * ref.max()
+
+
 # ---------------------------------------------------------------------------------------------------------
 # whole path
 # ---------------------------------------------------------------------------------------------------------
-def run_gpu(epw, w, k_list, q_list, kq_map=None, q_batch=0, host_api=False):
-    h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_, q_batch=q_batch)
+def run_gpu(epw, w, k_list, q_list, kq_map=None, q_batch=0, host_api=False, path=0, workspace_bytes=0):
+    h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_, q_batch=q_batch, path=path, workspace_bytes=workspace_bytes)
     try:
         h.set_operators_from_host(w)
         if host_api:
@@ -254,6 +316,40 @@ def test_reduced_shapes(epw, shape):
         w = synth.make_custom("odd", 5, 3, (1, 2, 0), 1.0, 0.1, 1.0, (9, 1, 17), ("random", 2, 3), seed=13)
     ref = oracle.interpolate(w.H_R, w.D_R, w.g_full(), w.Re, w.w_e, w.Rp, w.w_p, w.k_list, w.q_list)
     assert_path_close(run_gpu(epw, w, w.k_list, w.q_list), ref)
+
+
+def test_large_path_forced_on_config0(epw):
+    """The large-Nb kernels (S4a, S2, S4b as in-place DMMA contractions) on configs[0], where the small-Nb path and the
+    oracle are both available: grid-folded k+q and per-pair H(k+q)."""
+    w = synth.make_config(0)
+    ref = oracle.interpolate(w.H_R, w.D_R, w.g_full(), w.Re, w.w_e, w.Rp, w.w_p, w.k_list, w.q_list[:9])
+    assert_path_close(run_gpu(epw, w, w.k_list, w.q_list[:9], w.kq_map[:9], path=2), ref)
+    assert_path_close(run_gpu(epw, w, w.k_list, w.q_list[:9], None, path=2, q_batch=3), ref)
+
+
+@pytest.mark.parametrize("shape", ["zsnr-r", "zsnr-r-offgrid", "mos2-r-large"])
+def test_large_path_reduced_shapes(epw, shape):
+    """Reduced configs[4]-like ribbon (1-D lattice, Nb > 16 so the large path is chosen, Nb > 32 so the CTA-per-matrix
+    eigensolver runs, ragged tiles everywhere), with k+q on the grid and off it; and an odd 2-D shape forced large."""
+    if shape == "zsnr-r":
+        w = synth.make_custom("zsnr-r", 36, 15, (3, 0, 0), 1.0, 0.05, 2.0, (70, 1, 1), ("grid", (10, 1, 1)), seed=21)
+        kq, path = w.kq_map, 0
+    elif shape == "zsnr-r-offgrid":
+        w = synth.make_custom("zsnr-o", 20, 12, (2, 0, 0), 1.0, 0.05, 2.0, (9, 1, 1), ("random", 3, 1), seed=22)
+        kq, path = None, 0
+    else:
+        w = synth.make_custom("mos2-l", 11, 9, (2, 2, 0), 2.0, 0.1, 2.0, (13, 11, 1), ("random", 2, 2), seed=23)
+        kq, path = None, 2
+    ref = oracle.interpolate(w.H_R, w.D_R, w.g_full(), w.Re, w.w_e, w.Rp, w.w_p, w.k_list, w.q_list)
+    assert_path_close(run_gpu(epw, w, w.k_list, w.q_list, kq, path=path), ref)
+
+
+def test_large_path_k_chunks(epw):
+    """A workspace cap that forces several 64-k chunks (and a ragged last one) through S2 / S4b of the large path."""
+    w = synth.make_custom("zsnr-c", 18, 6, (2, 0, 0), 1.0, 0.05, 2.0, (150, 1, 1), ("grid", (3, 1, 1)), seed=24)
+    E = w.nbnd * w.nbnd * w.nmodes
+    ref = oracle.interpolate(w.H_R, w.D_R, w.g_full(), w.Re, w.w_e, w.Rp, w.w_p, w.k_list, w.q_list)
+    assert_path_close(run_gpu(epw, w, w.k_list, w.q_list, w.kq_map, workspace_bytes=2 * 16 * E * 64 + 1000), ref)
 
 
 def test_debug_intermediates_config0(epw):
