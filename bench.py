@@ -38,7 +38,8 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=6)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (default 1 = Si-like production)")
-    ap.add_argument("--nq-step", type=int, default=8, help="q-points per step (per GPU)")
+    ap.add_argument("--nq-step", type=int, default=0,
+                    help="q-points per step (per GPU); 0 = 8, reduced so that the |g|^2 buffer of a step stays below 20 GB")
     ap.add_argument("--q-batch", type=int, default=0, help="library q_batch for S1 (0 = default)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -108,7 +109,8 @@ class ClockSampler:
 # CPU oracle legs
 # ------------------------------------------------------------------------------------------------------------
 def oracle_sample(w, n_q: int, n_k: int, seed: int = 1234):
-    """Time the oracle, as it stands, on n_q sampled q x n_k sampled k of workload w (g must fit host memory).
+    """Time the oracle, as it stands, on n_q sampled q x n_k sampled k of workload w.  g(Re,Rp) is taken whole when it
+    fits the host, else Eq. 9 is accumulated one Rp slab at a time (it is a sum over Rp; slab generation is not timed).
     Returns (elements/s amortising Eq. 9 over the full Nk, seconds spent, threads, description, raw results)."""
     import oracle
 
@@ -117,22 +119,49 @@ def oracle_sample(w, n_q: int, n_k: int, seed: int = 1234):
     ik = np.sort(rng.choice(w.nk, size=min(n_k, w.nk), replace=False))
     ks = np.ascontiguousarray(w.k_list[ik])
     qs = np.ascontiguousarray(w.q_list[iq])
-    g = w.g_full()
-    t0 = time.perf_counter()
-    g1 = oracle.rp_to_q(g, w.Rp, w.w_p, qs[0])  # Eq. 9 for one q (single thread, as written)
-    t_eq9 = time.perf_counter() - t0
-    del g1
-    t0 = time.perf_counter()
-    res = oracle.interpolate(w.H_R, w.D_R, g, w.Re, w.w_e, w.Rp, w.w_p, ks, qs)
-    t_all = time.perf_counter() - t0
-    pairs = len(iq) * len(ik)
     E = w.elements_per_pair
-    t_pair = max(t_all - len(iq) * t_eq9, 1e-9) / pairs
-    per_elem = (t_pair + t_eq9 / w.nk) / E
     threads = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    pairs = len(iq) * len(ik)
+    if w.g_bytes <= (8 << 30):
+        g = w.g_full()
+        t0 = time.perf_counter()
+        g1 = oracle.rp_to_q(g, w.Rp, w.w_p, qs[0])  # Eq. 9 for one q (single thread, as written)
+        t_eq9 = time.perf_counter() - t0
+        del g1
+        t0 = time.perf_counter()
+        res = oracle.interpolate(w.H_R, w.D_R, g, w.Re, w.w_e, w.Rp, w.w_p, ks, qs)
+        t_all = time.perf_counter() - t0
+        t_pair = max(t_all - len(iq) * t_eq9, 1e-9) / pairs
+    else:
+        t_eq9, t_pairs, res = 0.0, 0.0, []
+        for q in qs:
+            g1 = np.zeros((w.nmodes, w.ne, w.nbnd, w.nbnd), dtype=np.complex128)
+            for ip in range(w.np_):
+                slab = w.g_slabs(ip, 1)
+                t0 = time.perf_counter()
+                g1 += oracle.rp_to_q(slab, w.Rp[ip:ip + 1], w.w_p[ip:ip + 1], q)
+                t_eq9 += time.perf_counter() - t0
+                del slab
+            t0 = time.perf_counter()
+            e_cm, om = oracle.phonon(w.D_R, w.Rp, w.w_p, q)
+            for k in ks:
+                res.append(oracle.pair(g1, w.H_R, w.Re, w.w_e, e_cm, om, k, q))
+            t_pairs += time.perf_counter() - t0
+        t_eq9 /= len(qs)
+        t_all = t_pairs + len(qs) * t_eq9
+        t_pair = t_pairs / pairs
+    per_elem = (t_pair + t_eq9 / w.nk) / E
     desc = (f"{len(iq)} random q x {len(ik)} random k of config {w.index} ({pairs} pairs); Eq. 9 per q "
             f"({t_eq9:.3f} s, 1 thread) amortised over the full Nk={w.nk}")
     return 1.0 / per_elem, t_all + t_eq9, threads, desc, (iq, ik, res)
+
+
+def sample_size(w):
+    """(n_q, n_k) of the bounded oracle sample: about 10-30 s of CPU work."""
+    E = w.elements_per_pair
+    if E > 1_000_000:
+        return 1, 2     # configs[4]: ~50 s per pair in the oracle's plain loops
+    return (4, 4096) if E < 2000 else (4, 512)
 
 
 def run_reference(args):
@@ -142,14 +171,12 @@ def run_reference(args):
     import synth
 
     w = synth.make_config(args.config)
-    if w.g_bytes > (8 << 30):
-        print(json.dumps({"impl": "reference", "unavailable": "config too large for the host-side oracle sample"}))
-        return
-    n_k = 1024 if w.elements_per_pair < 2000 else 256
+    n_q, n_k = sample_size(w)
+    n_q, n_k = max(1, n_q // 2), max(1, n_k // 4)
     vals, secs = [], []
     threads, desc = 1, ""
     for step in range(args.warmup + args.steps):
-        v, s, threads, desc, _ = oracle_sample(w, 2, n_k, seed=100 + step)
+        v, s, threads, desc, _ = oracle_sample(w, n_q, n_k, seed=100 + step)
         if step >= args.warmup:
             vals.append(v); secs.append(s)
     value = float(np.mean(vals))
@@ -191,8 +218,9 @@ def main():
     epw.load_library()
 
     w = synth.make_config(args.config)
-    nq_step = min(args.nq_step, w.nq)
     nk, E = w.nk, w.elements_per_pair
+    nq_step = args.nq_step or max(1, min(8, int((20 << 30) // (8 * nk * E))))
+    nq_step = min(nq_step, w.nq)
     h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_, device=local_rank, q_batch=args.q_batch)
     t0 = time.perf_counter()
     h.set_operators_from_host(w)  # upload once; resident for the whole run
@@ -259,40 +287,61 @@ def main():
     elements_per_step = nk * nq_step * E
     value = world * elements_per_step * args.steps / (ms * 1e-3)
 
-    # ---- roofline of the dominant kernel (S2: the DMMA contraction) ----
-    ncols = E + (0 if kq_map is not None else w.nbnd * w.nbnd)
-    flops_s2 = 8.0 * nk * ncols * w.ne * nq_step * args.steps  # 8 real flops per complex MAC, algorithmic (unpadded)
-    launches_s2 = max(1, stage_launches["S2_re_to_k_dmma"])
-    s2_ms = stage_ms["S2_re_to_k_dmma"]
+    # ---- rooflines: every contraction stage, the dominant one (largest share of the step) at top level ----
     roofline = None
     if rank == 0:
+        plan = epw.epw_interp_last_plan(h.h)
+        large = plan["path"] == "large"
         peaks = epw.epw_probe_peaks(local_rank)
-        achieved = flops_s2 / (s2_ms * 1e-3) / 1e12
-        traffic = None
-        tpath = os.path.join(ROOT, "profiles", "roofline_traffic.json")
-        if os.path.exists(tpath):
-            traffic = json.load(open(tpath)).get("zgemm_dmma_kernel_dram_bytes_per_launch")
         mp = {}
         if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")):
             mp = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
-        roofline = {
-            "bound": "tensor", "kernel": "zgemm_dmma_kernel (S2 Re->k, FP64 DMMA)", "achieved": achieved,
-            "peak": peaks["fp64_dmma_tflops"], "unit": "TFLOP/s", "frac": achieved / peaks["fp64_dmma_tflops"],
-            "traffic": traffic,
-            "peak_source": "FP64 DMMA m8n8k4 issue-loop probe run live on this GPU (epw_probe_peaks); "
-                           "MEASURED_PEAKS.json has no FP64 entry",
-            "peak_from_measured_bf16_x_nominal_ratio": (mp.get("bf16_tflops_sustained", 0.0) * 45.0 / 2250.0) or None,
-            "flops_per_launch": flops_s2 / launches_s2, "launches": launches_s2,
-            "avg_launch_ms": s2_ms / launches_s2, "share_of_step": s2_ms / stage_ms["total"],
-            "hbm_read_gbs_probe": peaks["hbm_read_gbs"], "fp64_dfma_tflops_probe": peaks["fp64_dfma_tflops"],
-            "stage_ms_per_step": {k: v / args.steps for k, v in stage_ms.items()},
+        traffic = {}
+        tpath = os.path.join(ROOT, "profiles", "roofline_traffic.txt")
+        if os.path.exists(tpath):
+            traffic = json.load(open(tpath))
+        nb, nm, ne = w.nbnd, w.nmodes, w.ne
+        pairs = float(nk) * nq_step * args.steps
+        # algorithmic (unpadded) flops, 8 real flops per complex multiply-add
+        ncols = E + (0 if (kq_map is not None or large) else nb * nb)  # small path: H(k+q) rides on S2 as Nb^2 extra columns
+        dmma, dfma = peaks["fp64_dmma_tflops"], peaks["fp64_dfma_tflops"]
+        spec = {
+            "S2_re_to_k_dmma": ("tensor", "zgemm_strided_kernel" if large else "zgemm_dmma_kernel", 8.0 * ncols * ne * pairs, dmma),
+            "S4b_rotate_g2": ("tensor" if large else "alu", "zgemm_strided_kernel" if large else "rotate_g2_small_kernel",
+                              16.0 * nb ** 3 * nm * pairs, dmma if large else dfma),
+            "S4a_mode_rotation": ("tensor" if large else "alu", "zgemm_strided_kernel" if large else "pack_b_kernel",
+                                  8.0 * nb * nb * nm * nm * ne * nq_step * args.steps, dmma if large else dfma),
         }
-        # S1 is the HBM-bound stage: report it too
-        s1_bytes = (16.0 * w.slab_elems * w.np_ * -(-nq_step // (args.q_batch or 4)) + 16.0 * w.slab_elems * nq_step) * args.steps
-        roofline["s1_rp_to_q"] = {"bound": "hbm", "achieved": s1_bytes / (stage_ms["S1_rp_to_q"] * 1e-3) / 1e9,
-                                  "peak": mp.get("hbm_gbs"), "unit": "GB/s"}
-        if roofline["s1_rp_to_q"]["peak"]:
-            roofline["s1_rp_to_q"]["frac"] = roofline["s1_rp_to_q"]["achieved"] / roofline["s1_rp_to_q"]["peak"]
+        stages = {}
+        for name, (bound, kernel, flops, peak) in spec.items():
+            t_ms, nl = stage_ms[name], max(1, stage_launches[name])
+            if t_ms <= 0:
+                continue
+            ach = flops / (t_ms * 1e-3) / 1e12
+            stages[name] = {"bound": bound, "kernel": kernel, "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+                            "frac": ach / peak, "flops_per_launch": flops / nl, "launches": nl,
+                            "avg_launch_ms": t_ms / nl, "share_of_step": t_ms / stage_ms["total"]}
+        n_s1 = -(-nq_step // plan["q_batch"])
+        s1_bytes = (16.0 * w.slab_elems * w.np_ * n_s1 + 16.0 * w.slab_elems * nq_step) * args.steps
+        s1 = {"bound": "hbm", "kernel": "rp_to_q_kernel", "achieved": s1_bytes / (stage_ms["S1_rp_to_q"] * 1e-3) / 1e9,
+              "peak": mp.get("hbm_gbs"), "unit": "GB/s", "bytes_per_launch": s1_bytes / (n_s1 * args.steps),
+              "launches": n_s1 * args.steps, "share_of_step": stage_ms["S1_rp_to_q"] / stage_ms["total"]}
+        if s1["peak"]:
+            s1["frac"] = s1["achieved"] / s1["peak"]
+        dom = max(("S2_re_to_k_dmma", "S4b_rotate_g2"), key=lambda n: stages[n]["share_of_step"] if n in stages else 0.0)
+        roofline = dict(stages[dom])
+        roofline["stage"] = dom
+        roofline["traffic"] = traffic.get(f"{stages[dom]['kernel']}:{dom}:config{w.index}")
+        roofline["peak_source"] = ("FP64 DMMA m8n8k4 issue-loop probe (tensor) / dependent-free DFMA loop probe (alu) run live on "
+                                   "this GPU by epw_probe_peaks; MEASURED_PEAKS.json has no FP64 entry")
+        roofline["peak_from_measured_bf16_x_nominal_ratio"] = (mp.get("bf16_tflops_sustained", 0.0) * 45.0 / 2250.0) or None
+        roofline["hbm_read_gbs_probe"] = peaks["hbm_read_gbs"]
+        roofline["fp64_dfma_tflops_probe"] = dfma
+        roofline["fp64_dmma_tflops_probe"] = dmma
+        roofline["plan"] = plan
+        roofline["stages"] = stages
+        roofline["s1_rp_to_q"] = s1
+        roofline["stage_ms_per_step"] = {k: v / args.steps for k, v in stage_ms.items()}
     if args.stages and rank == 0:
         print(json.dumps({k: round(v / args.steps, 4) for k, v in stage_ms.items()}), file=sys.stderr)
 
@@ -335,9 +384,9 @@ def main():
 
     # ---- CPU oracle beside it (rank 0, N = 1 only) ----
     cpu_baseline = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline and w.g_bytes <= (8 << 30):
-        n_k = 4096 if E < 2000 else 512
-        v, secs, threads, desc, _ = oracle_sample(w, 4, n_k)
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        n_q, n_k = sample_size(w)
+        v, secs, threads, desc, _ = oracle_sample(w, n_q, n_k)
         cpu_baseline = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc,
                         "seconds": secs}
 

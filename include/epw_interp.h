@@ -139,6 +139,10 @@ int epw_interp_enable_stage_timing(epw_interp_t h, int on);
 /* Number of kernels the library launched during the last interpolate call (for bench.py's gpu_launches). */
 int64_t epw_interp_last_launch_count(epw_interp_t h);
 
+/* How the last interpolate call was executed: plan[0] = EPW_PATH_SMALL or EPW_PATH_LARGE, plan[1] = q-points per pass
+ * over g(Re,Rp) in S1, plan[2] = k-points per chunk of S2 / S3b / S4b.  Returns the number of entries written. */
+int epw_interp_last_plan(epw_interp_t h, int64_t *plan, int n);
+
 /*
  * Intermediate results of the LAST q of the last interpolate call, for parity tests (device -> host copy,
  * synchronises).  `bytes` must be at least the size stated; returns bytes written or a negative status.

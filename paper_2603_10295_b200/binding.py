@@ -30,7 +30,7 @@ EPW_DBG_G_REQ, EPW_DBG_G_TILDE, EPW_DBG_H_K, EPW_DBG_U_K, EPW_DBG_U_KQ, EPW_DBG_
 EXPORTED_SYMBOLS = [
     "epw_interp_create", "epw_interp_destroy", "epw_interp_set_wannier_operators", "epw_interp_set_g_slabs",
     "epw_interp_interpolate", "epw_interp_interpolate_host", "epw_interp_sync", "epw_interp_get_stage_times",
-    "epw_interp_enable_stage_timing", "epw_interp_get_stage_launches", "epw_interp_last_launch_count", "epw_interp_debug_get", "epw_interp_last_error",
+    "epw_interp_enable_stage_timing", "epw_interp_get_stage_launches", "epw_interp_last_launch_count", "epw_interp_last_plan", "epw_interp_debug_get", "epw_interp_last_error",
     "epw_phase_table", "epw_rp_to_q", "epw_interp_operator", "epw_eigh_batched", "epw_zgemm", "epw_zgemm_strided",
     "epw_rotate_g2",
     "epw_probe_peaks", "epw_version",
@@ -74,6 +74,7 @@ def load_library() -> ctypes.CDLL:
         L.epw_interp_get_stage_launches.argtypes = [vp, POINTER(c_int64), c_int]
         L.epw_interp_last_launch_count.argtypes = [vp]
         L.epw_interp_last_launch_count.restype = c_int64
+        L.epw_interp_last_plan.argtypes = [vp, POINTER(c_int64), c_int]
         L.epw_interp_debug_get.argtypes = [vp, c_int, vp, c_size_t]
         L.epw_interp_debug_get.restype = c_int64
         L.epw_interp_last_error.argtypes = [vp]
@@ -175,6 +176,12 @@ def epw_interp_get_stage_launches(h) -> dict:
 
 def epw_interp_last_launch_count(h) -> int:
     return int(load_library().epw_interp_last_launch_count(h))
+
+
+def epw_interp_last_plan(h) -> dict:
+    buf = (c_int64 * 3)()
+    _check(load_library().epw_interp_last_plan(h, buf, 3), h)
+    return {"path": "large" if buf[0] == EPW_PATH_LARGE else "small", "q_batch": int(buf[1]), "k_chunk": int(buf[2])}
 
 
 def epw_interp_debug_get(h, what, dst_host):

@@ -93,7 +93,8 @@ struct epw_interp {
   // host-entry staging
   DevBuf hs_k, hs_q, hs_map, hs_epsk, hs_epskq, hs_omega, hs_g2;
   // bookkeeping of the last call
-  int64_t last_nk = 0, last_c_rows = 0;
+  int64_t last_nk = 0, last_c_rows = 0, last_kchunk = 0;
+  int last_path = 0, last_qb = 0;
   int last_ncols = 0;
   int64_t launches = 0;
   cudaStream_t last_stream = nullptr;
@@ -220,6 +221,9 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
   h->last_nk = nk;
   h->last_c_rows = kc;
   h->last_ncols = (int)E;
+  h->last_path = EPW_PATH_LARGE;
+  h->last_qb = QB;
+  h->last_kchunk = kc;
 
   const int t_total = h->begin_span(7, st);
 
@@ -513,6 +517,9 @@ int epw_interp_interpolate(epw_interp_t h, const double *k_list, int64_t nk, con
   h->last_nk = nk;
   h->last_c_rows = c_rows;
   h->last_ncols = ncols;
+  h->last_path = EPW_PATH_SMALL;
+  h->last_qb = QB;
+  h->last_kchunk = kchunk;
 
   const int t_total = h->begin_span(7, st);
 
@@ -685,6 +692,14 @@ int epw_interp_get_stage_launches(epw_interp_t h, int64_t *counts, int n) {
 }
 
 int64_t epw_interp_last_launch_count(epw_interp_t h) { return h ? h->launches : 0; }
+
+int epw_interp_last_plan(epw_interp_t h, int64_t *plan, int n) {
+  if (!h || !plan || n <= 0) return EPW_EINVAL;
+  const int64_t v[3] = {h->last_path, h->last_qb, h->last_kchunk};
+  const int m = std::min(n, 3);
+  for (int i = 0; i < m; i++) plan[i] = v[i];
+  return m;
+}
 
 int64_t epw_interp_debug_get(epw_interp_t h, int what, void *dst, size_t bytes) {
   if (!h || !dst) return EPW_EINVAL;

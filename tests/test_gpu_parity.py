@@ -453,3 +453,42 @@ def test_config3_full_size_sampled(epw):
     w = synth.make_config(3)
     worst = check_sampled_pairs(epw, w, [0, 255], sample_k(w.nk, 16))
     print(f"config 3 full size: worst |g|^2 deviation {worst:.3f} x tolerance")
+
+
+def test_config4_full_size_sampled(epw):
+    """BASELINE.json configs[4] (stanene-nanoribbon-like: Nb=192, Nm=288, Ne=Np=17, g(Re,Rp) = 49 GB streamed to the GPU
+    in Rp slabs) in the launch configuration bench.py times: all 200 k, one q of the grid (k+q folded through kq_map).
+    The oracle gets g(Re,q) from the same slabs, one Rp at a time (Eq. 9 is a sum over Rp), and two sampled pairs."""
+    from parity import g2_pair_close
+
+    w = synth.make_config(4)
+    iq = 37
+    q = w.q_list[iq]
+    k_idx = [0, 133]
+    h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_)
+    try:
+        epw.epw_interp_set_wannier_operators(h.h, w.H_R, w.D_R, None, w.Re, w.w_e, w.Rp, w.w_p, 0)
+        g1_ref = np.zeros((w.nmodes, w.ne, w.nbnd, w.nbnd), dtype=np.complex128)
+        for ip in range(w.np_):
+            slab = w.g_slabs(ip, 1)
+            epw.epw_interp_set_g_slabs(h.h, ip, 1, slab, 0)
+            g1_ref += oracle.rp_to_q(slab, w.Rp[ip:ip + 1], w.w_p[ip:ip + 1], q)
+            del slab
+        kq_map = np.ascontiguousarray(w.kq_map[iq:iq + 1])
+        eps_k, eps_kq, om, g2 = h.interpolate(dev(w.k_list), dev(q[None, :]), dev(kq_map))
+        epw.epw_interp_sync(h.h)
+        eps_k, eps_kq, om = eps_k.cpu().numpy(), eps_kq.cpu().numpy(), om.cpu().numpy()
+        e_ref, om_ref = oracle.phonon(w.D_R, w.Rp, w.w_p, q)
+        err, ok = eig_close(om[0], om_ref)
+        assert ok, f"omega mismatch: {err:.3e}"
+        for ik in k_idx:
+            r_g2, r_ek, r_ekq = oracle.pair(g1_ref, w.H_R, w.Re, w.w_e, e_ref, om_ref, w.k_list[ik], q)
+            err, ok = eig_close(eps_k[ik], r_ek)
+            assert ok, f"eps_k mismatch at k {ik}: {err:.3e}"
+            err, ok = eig_close(eps_kq[0, ik], r_ekq)
+            assert ok, f"eps_kq mismatch at k {ik}: {err:.3e}"
+            wst, ok = g2_pair_close(g2[0, ik].cpu().numpy(), r_g2, r_ekq, r_ek, om_ref)
+            assert ok, f"|g|^2 mismatch at k {ik}: {wst:.3f} x tolerance"
+            print(f"config 4 full size, k {ik}: worst |g|^2 deviation {wst:.3f} x tolerance")
+    finally:
+        h.close()
