@@ -105,9 +105,9 @@ def test_interp_operator_Dq(epw):
         assert np.abs(got[i] - ref).max() <= 1e-13 * np.abs(ref).max()
 
 
-@pytest.mark.parametrize("n", [1, 2, 3, 6, 8, 9, 11, 16, 31, 32, 33, 48])
+@pytest.mark.parametrize("n", [1, 2, 3, 6, 8, 9, 11, 16, 31, 32, 33, 48, 97, 192, 288])
 def test_eigh_batched(epw, n):
-    batch = 37 if n <= 32 else 5
+    batch = 37 if n <= 32 else (5 if n < 100 else 3)
     A = crandn(batch, n, n)
     A = 0.5 * (A + np.conj(np.swapaxes(A, 1, 2)))
     A[1] = np.diag(np.arange(n, 0, -1)).astype(np.complex128)  # already diagonal, descending
@@ -132,6 +132,39 @@ def test_eigh_batched(epw, n):
         nrm = max(np.linalg.norm(A[b]), 1e-300)
         assert np.linalg.norm(A[b] @ Vm[b] - Vm[b] * ev[b][None, :]) <= 1e-13 * nrm * n
         assert np.linalg.norm(Vm[b].conj().T @ Vm[b] - np.eye(n)) <= 1e-13 * n
+
+
+@pytest.mark.parametrize("n,batch", [(192, 150), (40, 300), (288, 9)])
+def test_eigh_cluster_many_matrices(epw, n, batch):
+    """The cluster eigensolver in its throughput configuration (more matrices than clusters: smallest cluster that holds
+    the matrix, several matrices per cluster): a few matrices against the oracle's Jacobi, all of them against the
+    defining invariants (residual, unitarity, ascending order)."""
+    A = crandn(batch, n, n)
+    A = 0.5 * (A + np.conj(np.swapaxes(A, 1, 2)))
+    A_cm = np.ascontiguousarray(np.swapaxes(A, 1, 2))
+    ev = torch.empty((batch, n), dtype=torch.float64, device="cuda")
+    V = torch.empty((batch, n, n, 2), dtype=torch.float64, device="cuda")
+    status = torch.zeros(1, dtype=torch.int32, device="cuda")
+    dA = zdev(A_cm)
+    epw.epw_eigh_batched(dA, n * n, n, batch, ev, V, 0, status)
+    torch.cuda.synchronize()
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0.record()
+    epw.epw_eigh_batched(dA, n * n, n, batch, ev, V, 0, status)
+    t1.record()
+    torch.cuda.synchronize()
+    print(f"eigh n={n} batch={batch}: {t0.elapsed_time(t1):.2f} ms")
+    assert int(status.item()) == 0
+    ev, Vm = ev.cpu().numpy(), np.swapaxes(znp(V), 1, 2)
+    for b in range(batch):
+        nrm = np.linalg.norm(A[b])
+        assert np.all(np.diff(ev[b]) >= 0)
+        assert np.linalg.norm(A[b] @ Vm[b] - Vm[b] * ev[b][None, :]) <= 1e-13 * nrm * n
+        assert np.linalg.norm(Vm[b].conj().T @ Vm[b] - np.eye(n)) <= 1e-13 * n
+    for b in (0, batch // 2, batch - 1):
+        ref_ev, _, _ = oracle.eigh_jacobi(A_cm[b])
+        e, ok = eig_close(ev[b], ref_ev)
+        assert ok, (n, b, e)
 
 
 def test_eigh_strided_input_sqrt_mode_and_hermitian_part(epw):
