@@ -341,7 +341,7 @@ __global__ void __launch_bounds__(EIGH_LARGE_THREADS)
 // The two-sided kernel above needs the whole matrix twice per round (column pass and row pass) and the accumulated
 // eigenvectors once; at n = 192..288 (configs[4]: H(k) 192 x 192, D(q) 288 x 288; 0.6 / 1.3 MB) that lives in L2 and
 // every one of the (n-1) x sweeps rounds pays L2 latency.  Here the matrix is made positive definite by a shift,
-// G = A + sigma I with sigma = ||A||_F >= rho(A), and its COLUMNS are orthogonalised by plane rotations from the right:
+// G = A + sigma I with sigma = ||A - mu I||_F - mu, mu = tr(A)/n, and its COLUMNS are orthogonalised by plane rotations from the right:
 //   round:  alpha = ||g_p||^2, beta = ||g_q||^2, gamma = g_p^dagger g_q  for the N/2 disjoint pairs of the round
 //           J_pq = the rotation that diagonalises [[alpha, gamma], [conj gamma, beta]]   (same formula as make_rot)
 //           (g_p, g_q) <- (g_p, g_q) J_pq
@@ -387,12 +387,23 @@ __global__ void __launch_bounds__(EC_THREADS, 1)
 
   for (int64_t b = cluster_id; b < batch; b += num_clusters) {
     const c128 *src = Ain + b * stride_a;
-    // ---- sigma = ||(A + A^dagger)/2||_F, computed identically by every CTA ----
+    // ---- centre the spectrum, mu = tr(A)/n, then sigma = ||A_h - mu I||_F >= rho(A_h - mu I)  (A_h = Hermitian part);
+    //      without the centring a nearly scalar matrix (D(q) = big diagonal + small couplings) would get a shift
+    //      sqrt(n) times its own size and lose that factor in eigenvector accuracy.  Computed identically by every CTA.
+    double tr = 0.0;
+    for (int i = tid; i < n; i += EC_THREADS) tr += src[i + (int64_t)n * i].x;
+    tr = warp_sum(tr);
+    __syncthreads();
+    if (lane == 0) red[warp] = tr;
+    __syncthreads();
+    tr = 0.0;
+    for (int w2 = 0; w2 < EC_THREADS / 32; w2++) tr += red[w2];
+    const double mu = tr / n;
     double fro2 = 0.0;
     for (int e = tid; e < n * n; e += EC_THREADS) {
       const int i = e % n, j = e / n;
       const c128 x = src[i + (int64_t)n * j], y = src[j + (int64_t)n * i];
-      const double re = 0.5 * (x.x + y.x), im = i == j ? 0.0 : 0.5 * (x.y - y.y);
+      const double re = 0.5 * (x.x + y.x) - (i == j ? mu : 0.0), im = i == j ? 0.0 : 0.5 * (x.y - y.y);
       fro2 += re * re + im * im;
     }
     fro2 = warp_sum(fro2);
@@ -401,8 +412,8 @@ __global__ void __launch_bounds__(EC_THREADS, 1)
     __syncthreads();
     fro2 = 0.0;
     for (int w2 = 0; w2 < EC_THREADS / 32; w2++) fro2 += red[w2];
-    const double sigma = fro2 > 0.0 ? sqrt(fro2) : 1.0;
-    // ---- local rows of G = Hermitian part + sigma I ----
+    const double sigma = (fro2 > 0.0 ? sqrt(fro2) : 1.0) - mu;   // G = A_h + sigma I = (A_h - mu I) + ||.||_F I
+    // ---- local rows of G ----
     for (int e = tid; e < n * nloc; e += EC_THREADS) {
       const int il = e % nloc, j = e / nloc;
       const int i = r0 + il;
