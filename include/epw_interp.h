@@ -183,6 +183,14 @@ int epw_interp_operator(const void *Op_R, int32_t n, int32_t nr, const void *P, 
  * status: int32 device word, set to nonzero if any solve hits the sweep limit (may be NULL). */
 int epw_eigh_batched(const void *A, int64_t stride_a, int32_t n, int64_t batch, double *evals, void *V,
                      int sqrt_mode, int32_t *status, void *cuda_stream);
+/* The same solve with an explicit kernel choice (parity tests exercise every kernel at every size it supports):
+ *   EPW_EIGH_AUTO    what epw_eigh_batched and the path use: THREAD for 2 <= n <= 8 and batch >= 2048, else WARP
+ *   EPW_EIGH_WARP    n <= 32: one warp per matrix in shared memory; n > 32: thread-block cluster / CTA per matrix
+ *   EPW_EIGH_THREAD  2 <= n <= 8 only (EPW_EINVAL otherwise): one thread per matrix, matrix and eigenvectors in
+ *                    registers, rotation schedule unrolled at compile time */
+enum { EPW_EIGH_AUTO = 0, EPW_EIGH_WARP = 1, EPW_EIGH_THREAD = 2 };
+int epw_eigh_batched_algo(const void *A, int64_t stride_a, int32_t n, int64_t batch, double *evals, void *V,
+                          int sqrt_mode, int32_t *status, int algo, void *cuda_stream);
 
 /* Dense complex FP64 contraction on the FP64 tensor path:  C[m][n] = sum_r A[m][r] B[r][n],
  * A c128 [M][K] row-major, B c128 [K][N] row-major, C c128 [M][ldc] row-major (ldc >= N).

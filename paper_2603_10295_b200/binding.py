@@ -31,7 +31,7 @@ EXPORTED_SYMBOLS = [
     "epw_interp_create", "epw_interp_destroy", "epw_interp_set_wannier_operators", "epw_interp_set_g_slabs",
     "epw_interp_interpolate", "epw_interp_interpolate_host", "epw_interp_sync", "epw_interp_get_stage_times",
     "epw_interp_enable_stage_timing", "epw_interp_get_stage_launches", "epw_interp_last_launch_count", "epw_interp_last_plan", "epw_interp_debug_get", "epw_interp_last_error",
-    "epw_phase_table", "epw_rp_to_q", "epw_interp_operator", "epw_eigh_batched", "epw_zgemm", "epw_zgemm_strided",
+    "epw_phase_table", "epw_rp_to_q", "epw_interp_operator", "epw_eigh_batched", "epw_eigh_batched_algo", "epw_zgemm", "epw_zgemm_strided",
     "epw_rotate_g2",
     "epw_probe_peaks", "epw_version",
 ]
@@ -83,6 +83,7 @@ def load_library() -> ctypes.CDLL:
         L.epw_rp_to_q.argtypes = [vp, c_int64, c_int32, vp, c_int32, vp, vp]
         L.epw_interp_operator.argtypes = [vp, c_int32, c_int32, vp, c_int64, vp, vp]
         L.epw_eigh_batched.argtypes = [vp, c_int64, c_int32, c_int64, vp, vp, c_int, vp, vp]
+        L.epw_eigh_batched_algo.argtypes = [vp, c_int64, c_int32, c_int64, vp, vp, c_int, vp, c_int, vp]
         L.epw_zgemm.argtypes = [vp, vp, vp, c_int64, c_int32, c_int32, c_int64, vp]
         L.epw_zgemm_strided.argtypes = [vp, c_int64, c_int64, c_int64, c_int64, vp, c_int64, c_int64, c_int64, c_int, vp,
                                         c_int64, vp, c_int64, c_int64, c_int64, c_int64, c_int64, c_int, c_int64,
@@ -206,6 +207,14 @@ def epw_interp_operator(Op_R, n, nr, P, nx, out, stream=None):
 def epw_eigh_batched(A, stride_a, n, batch, evals, V, sqrt_mode=0, status=None, stream=None):
     _check(load_library().epw_eigh_batched(_ptr(A), stride_a, n, batch, _ptr(evals), _ptr(V), int(sqrt_mode),
                                            _ptr(status), _stream() if stream is None else stream))
+
+
+EPW_EIGH_AUTO, EPW_EIGH_WARP, EPW_EIGH_THREAD = 0, 1, 2
+
+
+def epw_eigh_batched_algo(A, stride_a, n, batch, evals, V, sqrt_mode=0, status=None, algo=EPW_EIGH_AUTO, stream=None):
+    _check(load_library().epw_eigh_batched_algo(_ptr(A), stride_a, n, batch, _ptr(evals), _ptr(V), int(sqrt_mode),
+                                                _ptr(status), int(algo), _stream() if stream is None else stream))
 
 
 def epw_zgemm(A, B, C, M, N, K, ldc, stream=None):

@@ -764,13 +764,19 @@ int epw_interp_operator(const void *Op_R, int32_t n, int32_t nr, const void *P, 
 
 int epw_eigh_batched(const void *A, int64_t stride_a, int32_t n, int64_t batch, double *evals, void *V, int sqrt_mode,
                      int32_t *status, void *cuda_stream) {
+  return epw_eigh_batched_algo(A, stride_a, n, batch, evals, V, sqrt_mode, status, EPW_EIGH_AUTO, cuda_stream);
+}
+
+int epw_eigh_batched_algo(const void *A, int64_t stride_a, int32_t n, int64_t batch, double *evals, void *V,
+                          int sqrt_mode, int32_t *status, int algo, void *cuda_stream) {
   if (!A || !evals || !V || n <= 0 || batch < 0 || stride_a < (int64_t)n * n) return EPW_EINVAL;
+  if (algo < EPW_EIGH_AUTO || algo > EPW_EIGH_THREAD) return EPW_EINVAL;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
   c128 *scratch = nullptr;
   const size_t need = eigh_large_scratch_bytes(n, batch);
   if (need && cudaMalloc(&scratch, need) != cudaSuccess) return EPW_ENOMEM;
-  const cudaError_t e = launch_eigh_batched(reinterpret_cast<const c128 *>(A), stride_a, n, batch, evals,
-                                            reinterpret_cast<c128 *>(V), sqrt_mode, status, scratch, st);
+  const cudaError_t e = launch_eigh_batched_algo(reinterpret_cast<const c128 *>(A), stride_a, n, batch, evals,
+                                                 reinterpret_cast<c128 *>(V), sqrt_mode, status, scratch, algo, st);
   if (scratch) {  // stage-level convenience path: wait so the scratch can be released
     cudaStreamSynchronize(st);
     cudaFree(scratch);

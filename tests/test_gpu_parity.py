@@ -134,6 +134,44 @@ def test_eigh_batched(epw, n):
         assert np.linalg.norm(Vm[b].conj().T @ Vm[b] - np.eye(n)) <= 1e-13 * n
 
 
+@pytest.mark.parametrize("n,batch", [(2, 70), (3, 33), (5, 64), (6, 100), (7, 31), (8, 37), (8, 4099)])
+def test_eigh_thread_per_matrix(epw, n, batch):
+    """The register-resident thread-per-matrix solver (EPW_EIGH_THREAD, the kernel of the per-pair H(k+q) solves):
+    ragged batches (not a multiple of the 32 matrices of a CTA), diagonal and exactly degenerate inputs, every
+    matrix against the defining invariants and a sample against the oracle's Jacobi; AUTO must agree with it."""
+    A = crandn(batch, n, n)
+    A = 0.5 * (A + np.conj(np.swapaxes(A, 1, 2)))
+    A[1] = np.diag(np.arange(n, 0, -1)).astype(np.complex128)
+    if n >= 4:
+        Q, _ = np.linalg.qr(crandn(n, n))
+        lam = np.repeat(np.arange(n // 2 + 1), 2)[:n].astype(float)
+        M = (Q * lam) @ Q.conj().T
+        A[2] = 0.5 * (M + M.conj().T)
+    A[3] = 0.0  # zero matrix
+    A_cm = np.ascontiguousarray(np.swapaxes(A, 1, 2))
+    ev = torch.empty((batch, n), dtype=torch.float64, device="cuda")
+    V = torch.empty((batch, n, n, 2), dtype=torch.float64, device="cuda")
+    status = torch.zeros(1, dtype=torch.int32, device="cuda")
+    epw.epw_eigh_batched_algo(zdev(A_cm), n * n, n, batch, ev, V, 0, status, epw.EPW_EIGH_THREAD)
+    torch.cuda.synchronize()
+    assert int(status.item()) == 0
+    ev, Vm = ev.cpu().numpy(), np.swapaxes(znp(V), 1, 2)
+    for b in range(batch):
+        nrm = max(np.linalg.norm(A[b]), 1e-300)
+        assert np.all(np.diff(ev[b]) >= 0)
+        assert np.linalg.norm(A[b] @ Vm[b] - Vm[b] * ev[b][None, :]) <= 1e-13 * nrm * n
+        assert np.linalg.norm(Vm[b].conj().T @ Vm[b] - np.eye(n)) <= 1e-13 * n
+    assert np.all(ev[3] == 0.0)
+    for b in [0, 1, 2, 4, 5, 6, 7, batch // 2, batch - 1]:
+        ref_ev, _, _ = oracle.eigh_jacobi(A_cm[b])
+        e, ok = eig_close(ev[b], ref_ev)
+        assert ok, (n, b, e)
+    with pytest.raises(epw.EpwError):
+        epw.epw_eigh_batched_algo(zdev(A_cm), n * n, 9, 1, torch.empty((1, 9), dtype=torch.float64, device="cuda"),
+                                  torch.empty((1, 9, 9, 2), dtype=torch.float64, device="cuda"), 0, status,
+                                  epw.EPW_EIGH_THREAD)
+
+
 @pytest.mark.parametrize("n,batch", [(192, 150), (40, 300), (288, 9)])
 def test_eigh_cluster_many_matrices(epw, n, batch):
     """The cluster eigensolver in its throughput configuration (more matrices than clusters: smallest cluster that holds
