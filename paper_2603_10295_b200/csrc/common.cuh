@@ -113,6 +113,8 @@ cudaError_t launch_pack_b_strided(const c128 *B, int64_t sr, int64_t sn, int64_t
 cudaError_t launch_rotate_g2(const c128 *gt, int64_t stride_gt, const c128 *Uk, const c128 *Ukq, const int32_t *kq_idx,
                              int nb, int nm, int64_t nk, double *g2, cudaStream_t st);
 
+bool rotate_g2_small_supported(int nb, int nm);  // Nb <= 16 and the T staging buffer of one pair fits shared memory
+
 int probe_peaks(int device, double *out4);
 
 }  // namespace epw

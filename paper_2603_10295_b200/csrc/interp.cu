@@ -54,8 +54,7 @@ __global__ void gather_eps_kernel(const double *__restrict__ eps_k, const int32_
 // Number of 128-row m-tiles per k-chunk of the S2 contraction.  The chunk of C must stay within `l2_budget` bytes;
 // among the admissible sizes pick the largest one whose tile count (mtiles * NT) wastes at most 3 % of its last
 // wave on the `sms` persistent CTAs (wave quantisation), else the one with the best wave efficiency.
-int64_t choose_mtiles_per_chunk(int NT, int sms, size_t bytes_per_mtile, int64_t MT) {
-  const size_t l2_budget = (size_t)64 << 20;
+int64_t choose_mtiles_per_chunk(int NT, int sms, size_t bytes_per_mtile, int64_t MT, size_t l2_budget) {
   int64_t max_mt = std::max<int64_t>(1, (int64_t)(l2_budget / bytes_per_mtile));
   if (max_mt >= MT) return MT;
   int64_t best = 1;
@@ -150,8 +149,7 @@ struct epw_interp {
 static bool use_large_path(const epw_interp *h) {
   if (h->cfg.path == EPW_PATH_SMALL) return false;
   if (h->cfg.path == EPW_PATH_LARGE) return true;
-  const size_t rot_smem = sizeof(c128) * ((size_t)2 * h->nbb * h->nm + 2 * (size_t)h->nbb);
-  return h->nb > 16 || rot_smem > (size_t)200 * 1024;
+  return !rotate_g2_small_supported(h->nb, h->nm);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -488,7 +486,12 @@ int epw_interp_interpolate(epw_interp_t h, const double *k_list, int64_t nk, con
 
   // k-chunk: one chunk of [g~ | H(k+q)] (16*ncols bytes per k) must stay L2-resident for the eigensolve and the
   // rotation that follow it, and its tile count should fill whole waves of the persistent contraction kernel
-  const int64_t kchunk = choose_mtiles_per_chunk(NT, h->num_sms, (size_t)GEMM_BM * ncols * 16, MT) * GEMM_BM;
+  // (the thread-per-matrix eigensolver of the per-pair H(k+q) solves needs tens of thousands of matrices per launch to
+  // fill the GPU; it is worth more than L2 residency of the chunk: 16*ncols bytes per k written and read once more
+  // from HBM is a few per cent of the S2 time)
+  const size_t chunk_budget = (!kq_map && eigh_thread_supported(nb)) ? ((size_t)512 << 20) : ((size_t)64 << 20);
+  const int64_t kchunk =
+      choose_mtiles_per_chunk(NT, h->num_sms, (size_t)GEMM_BM * ncols * 16, MT, chunk_budget) * GEMM_BM;
   // rows of the g~ buffer kept (all of nk when it fits the cap; else a multiple of kchunk that is reused)
   size_t cap = h->cfg.workspace_bytes ? h->cfg.workspace_bytes : ((size_t)6 << 30);
   int64_t c_rows = MT * GEMM_BM;

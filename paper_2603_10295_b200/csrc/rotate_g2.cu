@@ -3,70 +3,181 @@
 //     g_{mn nu}(k,q) = sum_{m'n'} conj(Ukq[m',m]) g~_{m'n' nu}(k,q) Uk[n',n],     out = |g_{mn nu}|^2.
 // The mode rotation and the 1/sqrt(2 omega) amplitude were already applied to g(Re,q) (pack.cu), so g~ arrives in
 // the mode basis.  Two successive small matrix products per mode ("successive multiplication"):
-//     T[nu][n][m'] = sum_n' g~[nu][n'][m'] Uk[n'][n]          then      g[nu][n][m] = sum_m' conj(Ukq[m'][m]) T[nu][n][m'].
-// Small-Nb kernel: one CTA per (k,q) pair, everything staged in shared memory; 2 Nb^3 Nm complex MACs per pair on
-// the plain FP64 pipe; reads 16 (Nb^2 Nm + 2 Nb^2) bytes and writes 8 Nb^2 Nm bytes per pair.
+//     T[nu][n][m'] = sum_n' g~[nu][n'][m'] Uk[n'][n]          then      g[nu][n][m] = sum_m' T[nu][n][m'] conj(Ukq[m'][m]).
+//
+// Small-Nb kernel (Nb <= 16): both products run on the FP64 tensor path (mma.sync.m8n8k4.f64, SASS DMMA) -- the same
+// FP64 pipe as plain DFMA, but one fragment register feeds 8 FMAs per lane, which removes the shared-memory operand
+// traffic that bound the scalar version (short_scoreboard stalls, profiles/r01b_full_summary.md).
+//   product 1:  rows (nu,m') [Nm*Nb, tiles of 8]  x  K = n' (2 Nb real)  x  columns n (2 Nb real)
+//               A' fragments = re/im of g~ straight from global memory (8 consecutive m' = 128 contiguous bytes),
+//               B' fragments = 2x2 real embedding of Uk, built once per pair in registers;
+//   T goes through shared memory [nu][n][m'] (row pitch = 2 mod 4 complex: conflict-free STS.128 and LDS.64);
+//   product 2:  rows (nu,n)  x  K = m'  x  columns m,  B'' = embedding of conj(Ukq);  epilogue re^2 + im^2 -> g2.
+// WPP warps share one pair (its row tiles are dealt round-robin); a CTA of 4 warps works on 4 / WPP pairs at a time.
+// Work: 16 Nb^3 Nm flops per pair; reads 16 (Nb^2 Nm + 2 Nb^2) bytes (L2 / HBM), writes 8 Nb^2 Nm bytes per pair.
 #include "common.cuh"
+#include "dmma_pipe.cuh"
 
 namespace epw {
 
-constexpr int ROT_THREADS = 128;
+constexpr int ROT_WARPS = 4;
+constexpr int ROT_THREADS = ROT_WARPS * 32;
 
+// shared-memory row pitch of T in complex elements: >= NB and = 2 (mod 4)
+__host__ __device__ constexpr int rot_pitch(int nb) { return nb + ((6 - (nb & 3)) & 3); }
+
+template <int NB, int WPP>
 __global__ void __launch_bounds__(ROT_THREADS)
-    rotate_g2_small_kernel(const c128 *__restrict__ gt, int64_t stride_gt, const c128 *__restrict__ Uk,
-                           const c128 *__restrict__ Ukq, const int32_t *__restrict__ kq_idx, int nb, int nm,
-                           int64_t nk, double *__restrict__ g2) {
+    rotate_g2_dmma_kernel(const c128 *__restrict__ gt, int64_t stride_gt, const c128 *__restrict__ Uk,
+                          const c128 *__restrict__ Ukq, const int32_t *__restrict__ kq_idx, int nm, int64_t nk,
+                          double *__restrict__ g2) {
+  constexpr int KS = (2 * NB + 3) / 4;  // k-steps of 4 real
+  constexpr int NT = (2 * NB + 7) / 8;  // column tiles of 8 real
+  constexpr int SP = rot_pitch(NB);
+  constexpr int PPC = ROT_WARPS / WPP;  // pairs in flight per CTA
+  static_assert(2 * KS <= SP, "T pitch must cover the padded K range");
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int nbb = nb * nb, E = nbb * nm;
-  c128 *sG = reinterpret_cast<c128 *>(smem_raw);  // [nu][n'][m']
-  c128 *sT = sG + E;                              // [nu][n][m']
-  c128 *sUk = sT + E;                             // [n][n'] column-major: Uk[n' + nb*n]
-  c128 *sUkqH = sUk + nbb;                        // conj(Ukq[m'][m]) stored at [m'][m] (m fastest)
-  for (int64_t ik = blockIdx.x; ik < nk; ik += gridDim.x) {
-    const c128 *src = gt + ik * stride_gt;
-    for (int e = threadIdx.x; e < E; e += ROT_THREADS) sG[e] = src[e];
-    const c128 *uk = Uk + ik * nbb;
-    const c128 *ukq = Ukq + (kq_idx ? (int64_t)kq_idx[ik] : ik) * nbb;
-    for (int e = threadIdx.x; e < nbb; e += ROT_THREADS) {
-      sUk[e] = uk[e];
-      const int mp = e % nb, m = e / nb;  // ukq[e] = Ukq[m' + nb*m]
-      sUkqH[m + nb * mp] = cconj(ukq[e]);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int g = lane >> 2, t = lane & 3;
+  const int slot = warp / WPP, sub = warp - slot * WPP;
+  const int rows = nm * NB;               // rows of either product
+  const int MT = (rows + 7) >> 3;
+  double *sT = reinterpret_cast<double *>(smem_raw) + (size_t)slot * MT * 8 * SP * 2;  // [MT*8 rows][SP] complex
+
+  // zero the staging buffers once: padded K columns and padded rows must stay finite (they meet zero B'' entries)
+  for (int i = threadIdx.x; i < PPC * MT * 8 * SP * 2; i += ROT_THREADS) reinterpret_cast<double *>(smem_raw)[i] = 0.0;
+  __syncthreads();
+
+  const int64_t npass = (nk + (int64_t)gridDim.x * PPC - 1) / ((int64_t)gridDim.x * PPC);
+  for (int64_t pass = 0; pass < npass; pass++) {
+    const int64_t ik = (pass * gridDim.x + blockIdx.x) * PPC + slot;
+    const bool have = ik < nk;
+    const int64_t ikc = have ? ik : 0;
+    // ---- B' = embedding of Uk, B'' = embedding of conj(Ukq); fragment (ks, nt): k-row 4 ks + t, column 8 nt + g ----
+    double b1[KS][NT], b2[KS][NT];
+    {
+      const c128 *uk = Uk + ikc * (NB * NB);
+      const c128 *ukq = Ukq + (kq_idx ? (int64_t)kq_idx[ikc] : ikc) * (NB * NB);
+#pragma unroll
+      for (int ks = 0; ks < KS; ks++)
+#pragma unroll
+        for (int nt = 0; nt < NT; nt++) {
+          const int r = 2 * ks + (t >> 1), a = t & 1;   // complex row (n' or m'), real sub-row
+          const int c = 4 * nt + (g >> 1), b = g & 1;   // complex column (n or m), real sub-column
+          c128 x = make_double2(0.0, 0.0), y = make_double2(0.0, 0.0);
+          if (r < NB && c < NB) {
+            x = uk[r + NB * c];
+            y = ukq[r + NB * c];
+          }
+          y.y = -y.y;  // conj(Ukq)
+          b1[ks][nt] = a == 0 ? (b ? x.y : x.x) : (b ? x.x : -x.y);
+          b2[ks][nt] = a == 0 ? (b ? y.y : y.x) : (b ? y.x : -y.y);
+        }
     }
-    __syncthreads();
-    for (int e = threadIdx.x; e < E; e += ROT_THREADS) {
-      const int mp = e % nb, n = (e / nb) % nb, nu = e / nbb;
-      c128 acc = cmake(0.0, 0.0);
-      const c128 *gcol = sG + nu * nbb + mp;
-      const c128 *ucol = sUk + nb * n;
-      for (int np_ = 0; np_ < nb; np_++) cfma(acc, gcol[nb * np_], ucol[np_]);
-      sT[e] = acc;
+    // ---- product 1: T[(nu,m')][n] ----
+    const double *gsrc = reinterpret_cast<const double *>(gt + ikc * stride_gt);
+    for (int mt = sub; mt < MT; mt += WPP) {
+      const int row = 8 * mt + g;
+      const bool rv = row < rows;
+      const int nu = row / NB, mp = row - nu * NB;
+      double a[KS];
+#pragma unroll
+      for (int ks = 0; ks < KS; ks++) {
+        const int np_ = 2 * ks + (t >> 1);
+        a[ks] = (rv && np_ < NB) ? gsrc[(((int64_t)nu * NB + np_) * NB + mp) * 2 + (t & 1)] : 0.0;
+      }
+      double acc[NT][2];
+#pragma unroll
+      for (int nt = 0; nt < NT; nt++) acc[nt][0] = acc[nt][1] = 0.0;
+#pragma unroll
+      for (int ks = 0; ks < KS; ks++)
+#pragma unroll
+        for (int nt = 0; nt < NT; nt++) dmma884(acc[nt][0], acc[nt][1], a[ks], b1[ks][nt]);
+      // thread owns T_nu[m' = mp][n = 4 nt + t]  ->  sT[(nu, n)][m']
+      if (rv) {
+#pragma unroll
+        for (int nt = 0; nt < NT; nt++) {
+          const int n = 4 * nt + t;
+          if (n < NB)
+            *reinterpret_cast<double2 *>(sT + ((size_t)(nu * NB + n) * SP + mp) * 2) = make_double2(acc[nt][0], acc[nt][1]);
+        }
+      }
     }
-    __syncthreads();
-    double *dst = g2 + ik * (int64_t)E;
-    for (int e = threadIdx.x; e < E; e += ROT_THREADS) {
-      const int m = e % nb, rest = e / nb;  // rest = n + nb*nu
-      c128 acc = cmake(0.0, 0.0);
-      const c128 *trow = sT + rest * nb;
-      for (int mp = 0; mp < nb; mp++) cfma(acc, sUkqH[m + nb * mp], trow[mp]);
-      dst[e] = acc.x * acc.x + acc.y * acc.y;
+    if (WPP == 1) __syncwarp();
+    else __syncthreads();
+    // ---- product 2: |sum_m' T[(nu,n)][m'] conj(Ukq[m'][m])|^2 ----
+    double *dst = g2 + ikc * (int64_t)rows * NB;
+    for (int mt = sub; mt < MT; mt += WPP) {
+      const int row = 8 * mt + g;
+      const double *arow = sT + (size_t)row * SP * 2 + t;
+      double acc[NT][2];
+#pragma unroll
+      for (int nt = 0; nt < NT; nt++) acc[nt][0] = acc[nt][1] = 0.0;
+#pragma unroll
+      for (int ks = 0; ks < KS; ks++) {
+        const double a = arow[4 * ks];
+#pragma unroll
+        for (int nt = 0; nt < NT; nt++) dmma884(acc[nt][0], acc[nt][1], a, b2[ks][nt]);
+      }
+      if (have && row < rows) {
+#pragma unroll
+        for (int nt = 0; nt < NT; nt++) {
+          const int m = 4 * nt + t;
+          if (m < NB) dst[(int64_t)row * NB + m] = acc[nt][0] * acc[nt][0] + acc[nt][1] * acc[nt][1];
+        }
+      }
     }
-    __syncthreads();
+    if (WPP == 1) __syncwarp();
+    else __syncthreads();
   }
+}
+
+template <int NB, int WPP>
+static cudaError_t launch_rot(const c128 *gt, int64_t stride_gt, const c128 *Uk, const c128 *Ukq, const int32_t *kq_idx,
+                              int nm, int64_t nk, double *g2, size_t smem_per_pair, cudaStream_t st) {
+  constexpr int PPC = ROT_WARPS / WPP;
+  const size_t smem = smem_per_pair * PPC;
+  if (smem > 48 * 1024) {
+    cudaError_t e = cudaFuncSetAttribute(rotate_g2_dmma_kernel<NB, WPP>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)smem);
+    if (e != cudaSuccess) return e;
+  }
+  const int64_t want = ceil_div(nk, PPC);
+  const int64_t grid = want < 148 * 16 ? want : 148 * 16;
+  rotate_g2_dmma_kernel<NB, WPP><<<(unsigned)grid, ROT_THREADS, smem, st>>>(gt, stride_gt, Uk, Ukq, kq_idx, nm, nk, g2);
+  return cudaGetLastError();
+}
+
+template <int NB>
+static cudaError_t launch_rot_nb(const c128 *gt, int64_t stride_gt, const c128 *Uk, const c128 *Ukq,
+                                 const int32_t *kq_idx, int nm, int64_t nk, double *g2, cudaStream_t st) {
+  const int MT = (nm * NB + 7) / 8;
+  const size_t per_pair = sizeof(c128) * (size_t)MT * 8 * rot_pitch(NB);
+  if (per_pair > (size_t)200 * 1024) return cudaErrorInvalidConfiguration;
+  // one warp per pair while four staging buffers fit comfortably; otherwise 2 or 4 warps share a pair
+  if (per_pair <= (size_t)12 * 1024) return launch_rot<NB, 1>(gt, stride_gt, Uk, Ukq, kq_idx, nm, nk, g2, per_pair, st);
+  if (per_pair <= (size_t)24 * 1024) return launch_rot<NB, 2>(gt, stride_gt, Uk, Ukq, kq_idx, nm, nk, g2, per_pair, st);
+  return launch_rot<NB, 4>(gt, stride_gt, Uk, Ukq, kq_idx, nm, nk, g2, per_pair, st);
+}
+
+bool rotate_g2_small_supported(int nb, int nm) {
+  if (nb < 1 || nb > 16) return false;
+  const int MT = (nm * nb + 7) / 8;
+  return sizeof(c128) * (size_t)MT * 8 * rot_pitch(nb) <= (size_t)200 * 1024;
 }
 
 cudaError_t launch_rotate_g2(const c128 *gt, int64_t stride_gt, const c128 *Uk, const c128 *Ukq, const int32_t *kq_idx,
                              int nb, int nm, int64_t nk, double *g2, cudaStream_t st) {
   if (nk <= 0) return cudaSuccess;
-  const size_t smem = sizeof(c128) * (size_t)(2 * nb * nb * nm + 2 * nb * nb);
-  if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;  // large-Nb path not built yet
-  if (smem > 48 * 1024) {
-    cudaError_t e =
-        cudaFuncSetAttribute(rotate_g2_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
+  switch (nb) {
+#define EPW_ROT_CASE(NB_) \
+  case NB_: return launch_rot_nb<NB_>(gt, stride_gt, Uk, Ukq, kq_idx, nm, nk, g2, st);
+    EPW_ROT_CASE(1) EPW_ROT_CASE(2) EPW_ROT_CASE(3) EPW_ROT_CASE(4) EPW_ROT_CASE(5) EPW_ROT_CASE(6) EPW_ROT_CASE(7)
+    EPW_ROT_CASE(8) EPW_ROT_CASE(9) EPW_ROT_CASE(10) EPW_ROT_CASE(11) EPW_ROT_CASE(12) EPW_ROT_CASE(13)
+    EPW_ROT_CASE(14) EPW_ROT_CASE(15) EPW_ROT_CASE(16)
+#undef EPW_ROT_CASE
+    default: return cudaErrorInvalidConfiguration;  // Nb > 16: the large-Nb path (zgemm_strided.cu) does S4b
   }
-  const int64_t grid = nk < 148 * 64 ? nk : 148 * 64;
-  rotate_g2_small_kernel<<<(unsigned)grid, ROT_THREADS, smem, st>>>(gt, stride_gt, Uk, Ukq, kq_idx, nb, nm, nk, g2);
-  return cudaGetLastError();
 }
 
 }  // namespace epw

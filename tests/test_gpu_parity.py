@@ -254,23 +254,29 @@ def test_zgemm_matches_oracle_re_to_k(epw):
         assert np.abs(got[ik] - ref).max() <= 1e-13 * np.abs(ref).max()
 
 
-@pytest.mark.parametrize("nb,nm", [(8, 6), (11, 9), (3, 2), (1, 1), (16, 3)])
-def test_rotate_g2(epw, nb, nm):
-    nk = 19
+@pytest.mark.parametrize("nb,nm,nk", [(8, 6, 19), (11, 9, 19), (3, 2, 19), (1, 1, 19), (16, 3, 19), (5, 7, 6), (7, 3, 33),
+                                      (13, 20, 9), (16, 48, 5), (8, 6, 9509), (11, 9, 4801)])
+def test_rotate_g2(epw, nb, nm, nk):
+    """S4b on the FP64 tensor path: every Nb tile shape (K and column padding, ragged row tiles), 1 / 2 / 4 warps per
+    pair (staging-buffer size), more pairs than one pass of the grid, with and without the k+q gather."""
     gt = crandn(nk, nm, nb, nb)
-    Uk = np.stack([np.linalg.qr(crandn(nb, nb))[0].T for _ in range(nk)])  # column-major storage
-    Ukq = np.stack([np.linalg.qr(crandn(nb, nb))[0].T for _ in range(nk)])
+    nu_ = min(nk, 64)  # distinct unitaries (QR on the host is slow); pairs reuse them cyclically
+    Ub = np.stack([np.linalg.qr(crandn(nb, nb))[0].T for _ in range(nu_)])  # column-major storage
+    Uk = np.ascontiguousarray(Ub[np.arange(nk) % nu_])
+    Ukq = np.ascontiguousarray(Ub[(np.arange(nk) * 7 + 3) % nu_])
     idx = rng.permutation(nk).astype(np.int32)
     g2 = torch.empty((nk, nm, nb, nb), dtype=torch.float64, device="cuda")
+    sample = range(nk) if nk <= 40 else sorted(set([0, 1, nk // 2, nk - 2, nk - 1]) | set(rng.integers(0, nk, 24).tolist()))
     for kq_idx in (None, idx):
+        g2.fill_(-1.0)
         epw.epw_rotate_g2(zdev(gt), nm * nb * nb, zdev(Uk), zdev(Ukq), None if kq_idx is None else dev(kq_idx), nb, nm,
                           nk, g2)
         got = g2.cpu().numpy()
-        for ik in range(nk):
+        assert got.min() >= 0.0  # every element written
+        for ik in sample:
             u = Ukq[ik] if kq_idx is None else Ukq[kq_idx[ik]]
             ref = np.abs(oracle.band_rotate(gt[ik], u, Uk[ik])) ** 2
             assert np.abs(got[ik] - ref).max() <= 1e-12 * ref.max()
-
 
 
 @pytest.mark.parametrize("case", ["plain", "blocked", "blocked_ragged", "colmajor_c", "batched_gather_conj_abs2"])
