@@ -307,8 +307,8 @@ def main():
         dmma, dfma = peaks["fp64_dmma_tflops"], peaks["fp64_dfma_tflops"]
         spec = {
             "S2_re_to_k_dmma": ("tensor", "zgemm_strided_kernel" if large else "zgemm_dmma_kernel", 8.0 * ncols * ne * pairs, dmma),
-            "S4b_rotate_g2": ("tensor" if large else "alu", "zgemm_strided_kernel" if large else "rotate_g2_small_kernel",
-                              16.0 * nb ** 3 * nm * pairs, dmma if large else dfma),
+            "S4b_rotate_g2": ("tensor", "zgemm_strided_kernel" if large else "rotate_g2_dmma_kernel",
+                              16.0 * nb ** 3 * nm * pairs, dmma),
             "S4a_mode_rotation": ("tensor" if large else "alu", "zgemm_strided_kernel" if large else "pack_b_kernel",
                                   8.0 * nb * nb * nm * nm * ne * nq_step * args.steps, dmma if large else dfma),
         }

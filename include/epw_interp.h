@@ -184,11 +184,14 @@ int epw_interp_operator(const void *Op_R, int32_t n, int32_t nr, const void *P, 
 int epw_eigh_batched(const void *A, int64_t stride_a, int32_t n, int64_t batch, double *evals, void *V,
                      int sqrt_mode, int32_t *status, void *cuda_stream);
 /* The same solve with an explicit kernel choice (parity tests exercise every kernel at every size it supports):
- *   EPW_EIGH_AUTO    what epw_eigh_batched and the path use: THREAD for 2 <= n <= 8 and batch >= 2048, else WARP
+ *   EPW_EIGH_AUTO    what epw_eigh_batched and the path use: for batch >= 2048 THREAD (2 <= n <= 8) or COLS
+ *                    (9 <= n <= 16), else WARP
  *   EPW_EIGH_WARP    n <= 32: one warp per matrix in shared memory; n > 32: thread-block cluster / CTA per matrix
  *   EPW_EIGH_THREAD  2 <= n <= 8 only (EPW_EINVAL otherwise): one thread per matrix, matrix and eigenvectors in
- *                    registers, rotation schedule unrolled at compile time */
-enum { EPW_EIGH_AUTO = 0, EPW_EIGH_WARP = 1, EPW_EIGH_THREAD = 2 };
+ *                    registers, rotation schedule unrolled at compile time
+ *   EPW_EIGH_COLS    9 <= n <= 16 only (EPW_EINVAL otherwise): one-sided Jacobi, the columns of 32 matrices spread
+ *                    over the warps of a CTA (lane = matrix), odd-even ordering */
+enum { EPW_EIGH_AUTO = 0, EPW_EIGH_WARP = 1, EPW_EIGH_THREAD = 2, EPW_EIGH_COLS = 3 };
 int epw_eigh_batched_algo(const void *A, int64_t stride_a, int32_t n, int64_t batch, double *evals, void *V,
                           int sqrt_mode, int32_t *status, int algo, void *cuda_stream);
 

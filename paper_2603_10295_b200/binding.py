@@ -209,7 +209,7 @@ def epw_eigh_batched(A, stride_a, n, batch, evals, V, sqrt_mode=0, status=None, 
                                            _ptr(status), _stream() if stream is None else stream))
 
 
-EPW_EIGH_AUTO, EPW_EIGH_WARP, EPW_EIGH_THREAD = 0, 1, 2
+EPW_EIGH_AUTO, EPW_EIGH_WARP, EPW_EIGH_THREAD, EPW_EIGH_COLS = 0, 1, 2, 3
 
 
 def epw_eigh_batched_algo(A, stride_a, n, batch, evals, V, sqrt_mode=0, status=None, algo=EPW_EIGH_AUTO, stream=None):

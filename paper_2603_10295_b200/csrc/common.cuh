@@ -73,9 +73,13 @@ cudaError_t launch_interp_operator(const c128 *OpR, int n, int nr, const c128 *P
 cudaError_t launch_eigh_batched(const c128 *A, int64_t stride_a, int n, int64_t batch, double *evals, c128 *V,
                                 int sqrt_mode, int32_t *status, c128 *scratch_large, cudaStream_t st);
 size_t eigh_large_scratch_bytes(int n, int64_t batch);
-// same with an explicit kernel choice (EPW_EIGH_AUTO / _WARP / _THREAD, include/epw_interp.h)
+// same with an explicit kernel choice (EPW_EIGH_AUTO / _WARP / _THREAD / _COLS, include/epw_interp.h)
 cudaError_t launch_eigh_batched_algo(const c128 *A, int64_t stride_a, int n, int64_t batch, double *evals, c128 *V,
                                      int sqrt_mode, int32_t *status, c128 *scratch_large, int algo, cudaStream_t st);
+// column-pair one-sided solver (eigh_cols.cu), n in 9..16
+bool eigh_cols_supported(int n);
+cudaError_t launch_eigh_cols(const c128 *A, int64_t stride_a, int n, int64_t batch, double *evals, c128 *V,
+                             int sqrt_mode, int32_t *status, cudaStream_t st);
 // thread-per-matrix register-resident solver (eigh_thread.cu), n in 2..8
 bool eigh_thread_supported(int n);
 cudaError_t launch_eigh_thread(const c128 *A, int64_t stride_a, int n, int64_t batch, double *evals, c128 *V,

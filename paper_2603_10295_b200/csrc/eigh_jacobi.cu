@@ -621,6 +621,9 @@ cudaError_t launch_eigh_batched_algo(const c128 *A, int64_t stride_a, int n, int
   if (algo == EPW_EIGH_THREAD && !eigh_thread_supported(n)) return cudaErrorInvalidValue;
   if (algo == EPW_EIGH_THREAD || (algo == EPW_EIGH_AUTO && eigh_thread_supported(n) && batch >= 2048))
     return launch_eigh_thread(A, stride_a, n, batch, evals, V, sqrt_mode, status, st);
+  if (algo == EPW_EIGH_COLS && !eigh_cols_supported(n)) return cudaErrorInvalidValue;
+  if (algo == EPW_EIGH_COLS || (algo == EPW_EIGH_AUTO && eigh_cols_supported(n) && batch >= 2048))
+    return launch_eigh_cols(A, stride_a, n, batch, evals, V, sqrt_mode, status, st);
   if (n <= EIGH_SMALL_MAX_N) {
     const int ld = n | 1, half = (n + (n & 1)) >> 1;
     size_t per_warp = (size_t)(2 * ld * n) * sizeof(c128) + (size_t)half * sizeof(Rot) + (size_t)n * sizeof(double);

@@ -489,7 +489,7 @@ int epw_interp_interpolate(epw_interp_t h, const double *k_list, int64_t nk, con
   // (the thread-per-matrix eigensolver of the per-pair H(k+q) solves needs tens of thousands of matrices per launch to
   // fill the GPU; it is worth more than L2 residency of the chunk: 16*ncols bytes per k written and read once more
   // from HBM is a few per cent of the S2 time)
-  const size_t chunk_budget = (!kq_map && eigh_thread_supported(nb)) ? ((size_t)512 << 20) : ((size_t)64 << 20);
+  const size_t chunk_budget = (!kq_map && (eigh_thread_supported(nb) || eigh_cols_supported(nb))) ? ((size_t)512 << 20) : ((size_t)64 << 20);
   const int64_t kchunk =
       choose_mtiles_per_chunk(NT, h->num_sms, (size_t)GEMM_BM * ncols * 16, MT, chunk_budget) * GEMM_BM;
   // rows of the g~ buffer kept (all of nk when it fits the cap; else a multiple of kchunk that is reused)
@@ -773,7 +773,7 @@ int epw_eigh_batched(const void *A, int64_t stride_a, int32_t n, int64_t batch, 
 int epw_eigh_batched_algo(const void *A, int64_t stride_a, int32_t n, int64_t batch, double *evals, void *V,
                           int sqrt_mode, int32_t *status, int algo, void *cuda_stream) {
   if (!A || !evals || !V || n <= 0 || batch < 0 || stride_a < (int64_t)n * n) return EPW_EINVAL;
-  if (algo < EPW_EIGH_AUTO || algo > EPW_EIGH_THREAD) return EPW_EINVAL;
+  if (algo < EPW_EIGH_AUTO || algo > EPW_EIGH_COLS) return EPW_EINVAL;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
   c128 *scratch = nullptr;
   const size_t need = eigh_large_scratch_bytes(n, batch);

@@ -134,11 +134,13 @@ def test_eigh_batched(epw, n):
         assert np.linalg.norm(Vm[b].conj().T @ Vm[b] - np.eye(n)) <= 1e-13 * n
 
 
-@pytest.mark.parametrize("n,batch", [(2, 70), (3, 33), (5, 64), (6, 100), (7, 31), (8, 37), (8, 4099)])
+@pytest.mark.parametrize("n,batch", [(2, 70), (3, 33), (5, 64), (6, 100), (7, 31), (8, 37), (8, 4099),
+                                     (9, 37), (10, 64), (11, 70), (11, 2100), (12, 33), (13, 31), (14, 40), (15, 65), (16, 37)])
 def test_eigh_thread_per_matrix(epw, n, batch):
-    """The register-resident thread-per-matrix solver (EPW_EIGH_THREAD, the kernel of the per-pair H(k+q) solves):
-    ragged batches (not a multiple of the 32 matrices of a CTA), diagonal and exactly degenerate inputs, every
-    matrix against the defining invariants and a sample against the oracle's Jacobi; AUTO must agree with it."""
+    """The register-resident solvers of the per-pair H(k+q) solves (EPW_EIGH_THREAD for n <= 8, EPW_EIGH_COLS for
+    9 <= n <= 16): ragged batches (not a multiple of the 32 matrices of a CTA), diagonal, zero and exactly degenerate
+    inputs, every matrix against the defining invariants and a sample against the oracle's Jacobi."""
+    algo = epw.EPW_EIGH_THREAD if n <= 8 else epw.EPW_EIGH_COLS
     A = crandn(batch, n, n)
     A = 0.5 * (A + np.conj(np.swapaxes(A, 1, 2)))
     A[1] = np.diag(np.arange(n, 0, -1)).astype(np.complex128)
@@ -152,7 +154,7 @@ def test_eigh_thread_per_matrix(epw, n, batch):
     ev = torch.empty((batch, n), dtype=torch.float64, device="cuda")
     V = torch.empty((batch, n, n, 2), dtype=torch.float64, device="cuda")
     status = torch.zeros(1, dtype=torch.int32, device="cuda")
-    epw.epw_eigh_batched_algo(zdev(A_cm), n * n, n, batch, ev, V, 0, status, epw.EPW_EIGH_THREAD)
+    epw.epw_eigh_batched_algo(zdev(A_cm), n * n, n, batch, ev, V, 0, status, algo)
     torch.cuda.synchronize()
     assert int(status.item()) == 0
     ev, Vm = ev.cpu().numpy(), np.swapaxes(znp(V), 1, 2)
@@ -166,10 +168,10 @@ def test_eigh_thread_per_matrix(epw, n, batch):
         ref_ev, _, _ = oracle.eigh_jacobi(A_cm[b])
         e, ok = eig_close(ev[b], ref_ev)
         assert ok, (n, b, e)
+    bad_n, bad_algo = (9, epw.EPW_EIGH_THREAD) if n <= 8 else (8, epw.EPW_EIGH_COLS)
     with pytest.raises(epw.EpwError):
-        epw.epw_eigh_batched_algo(zdev(A_cm), n * n, 9, 1, torch.empty((1, 9), dtype=torch.float64, device="cuda"),
-                                  torch.empty((1, 9, 9, 2), dtype=torch.float64, device="cuda"), 0, status,
-                                  epw.EPW_EIGH_THREAD)
+        epw.epw_eigh_batched_algo(zdev(A_cm), n * n, bad_n, 1, torch.empty((1, 16), dtype=torch.float64, device="cuda"),
+                                  torch.empty((1, 16, 16, 2), dtype=torch.float64, device="cuda"), 0, status, bad_algo)
 
 
 @pytest.mark.parametrize("n,batch", [(192, 150), (40, 300), (288, 9)])
