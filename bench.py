@@ -206,6 +206,7 @@ def main():
 
     import paper_2603_10295_b200 as epw
     import synth
+    from paper_2603_10295_b200 import shard
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -233,9 +234,7 @@ def main():
 
     def q_block(step):
         """q-points of this rank for this step (ranks own disjoint q: the image level of the paper)."""
-        start = ((step * world + rank) * nq_step) % w.nq
-        idx = (start + np.arange(nq_step)) % w.nq
-        return idx
+        return shard.q_block(step, world, rank, nq_step, w.nq)
 
     q_blocks = [q_block(s) for s in range(total_steps)]
     q_dev = [torch.from_numpy(np.ascontiguousarray(w.q_list[i])).cuda() for i in q_blocks]
@@ -280,10 +279,7 @@ def main():
     stage_ms = epw.epw_interp_get_stage_times(h.h)
     stage_launches = epw.epw_interp_get_stage_launches(h.h)
     epw.epw_interp_enable_stage_timing(h.h, False)
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = shard.max_over_ranks_ms(ms, dist if world > 1 else None, device="cuda")
     elements_per_step = nk * nq_step * E
     value = world * elements_per_step * args.steps / (ms * 1e-3)
 
@@ -372,10 +368,7 @@ def main():
         e1.record()
         barrier()
         ms_e2e = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms_e2e], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms_e2e = float(t.item())
+        ms_e2e = shard.max_over_ranks_ms(ms_e2e, dist if world > 1 else None, device="cuda")
         h2d = k_host.numel() * 8 + q_host[0].numel() * 8 + (0 if map_host is None else map_host[0].numel() * 4)
         d2h = (o_eps_k.numel() + o_eps_kq.numel() + o_omega.numel() + o_g2.numel()) * 8
         e2e = {"value": world * elements_per_step * args.steps / (ms_e2e * 1e-3), "unit": UNIT,
