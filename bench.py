@@ -41,9 +41,13 @@ def parse_args():
     ap.add_argument("--nq-step", type=int, default=0,
                     help="q-points per step (per GPU); 0 = 8, reduced so that the |g|^2 buffer of a step stays below 20 GB")
     ap.add_argument("--q-batch", type=int, default=0, help="library q_batch for S1 (0 = default)")
+    ap.add_argument("--k-mode", default="grid", choices=["grid", "list"],
+                    help="grid: epw_interp_interpolate_grid (the configs' k-points ARE uniform grids; factorised S2); "
+                         "list: epw_interp_interpolate on the same k-points as a plain list (dense DMMA S2)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-klist-arm", action="store_true", help="skip the extra list-mode measurement of --k-mode grid")
     ap.add_argument("--stages", action="store_true", help="also print per-stage device times to stderr")
     return ap.parse_args()
 
@@ -246,48 +250,61 @@ def main():
     omega = torch.empty((nq_step, w.nmodes), dtype=torch.float64, device="cuda")
     g2 = torch.empty((nq_step, nk, w.nmodes, w.nbnd, w.nbnd), dtype=torch.float64, device="cuda")  # reused every step
 
-    def step(s):
-        epw.epw_interp_interpolate(h.h, k_dev, nk, q_dev[s], nq_step, None if map_dev is None else map_dev[s], eps_k,
-                                   eps_kq, omega, g2)
+    use_grid = args.k_mode == "grid"
+
+    def step(s, grid=None):
+        if use_grid if grid is None else grid:
+            epw.epw_interp_interpolate_grid(h.h, w.k_grid, None, q_dev[s], nq_step,
+                                            None if map_dev is None else map_dev[s], eps_k, eps_kq, omega, g2)
+        else:
+            epw.epw_interp_interpolate(h.h, k_dev, nk, q_dev[s], nq_step, None if map_dev is None else map_dev[s],
+                                       eps_k, eps_kq, omega, g2)
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for s in range(args.warmup):
-        step(s)
-    epw.epw_interp_sync(h.h)
+    def measure(grid, with_clocks):
+        """W warm-up steps, then K timed steps (CUDA events on the launching stream, barrier + synchronize on both
+        sides, max over ranks).  Returns everything the JSON line needs about this arm."""
+        for s in range(args.warmup):
+            step(s, grid)
+        epw.epw_interp_sync(h.h)
+        epw.epw_interp_enable_stage_timing(h.h, True)
+        sampler = ClockSampler(local_rank)
+        if rank == 0 and with_clocks:
+            sampler.start()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        launches = 0
+        barrier()
+        ev0.record()
+        for s in range(args.warmup, total_steps):
+            step(s, grid)
+            launches += epw.epw_interp_last_launch_count(h.h)
+        ev1.record()
+        barrier()
+        ms = ev0.elapsed_time(ev1)
+        clocks = sampler.stop() if (rank == 0 and with_clocks) else None
+        epw.epw_interp_sync(h.h)  # raises if an eigensolve did not converge
+        out = {"stage_ms": epw.epw_interp_get_stage_times(h.h), "stage_launches": epw.epw_interp_get_stage_launches(h.h),
+               "rotations": epw.epw_interp_get_eigh_rotations(h.h), "plan": epw.epw_interp_last_plan(h.h),
+               "launches": launches, "clocks": clocks}
+        epw.epw_interp_enable_stage_timing(h.h, False)
+        out["ms"] = shard.max_over_ranks_ms(ms, dist if world > 1 else None, device="cuda")
+        return out
 
-    # ---- timed region: K steps, device time from CUDA events on the launching stream, max over ranks ----
-    epw.epw_interp_enable_stage_timing(h.h, True)
-    sampler = ClockSampler(local_rank)
-    if rank == 0:
-        sampler.start()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    launches = 0
-    barrier()
-    ev0.record()
-    for s in range(args.warmup, total_steps):
-        step(s)
-        launches += epw.epw_interp_last_launch_count(h.h)
-    ev1.record()
-    barrier()
-    ms = ev0.elapsed_time(ev1)
-    clocks = sampler.stop() if rank == 0 else None
-    epw.epw_interp_sync(h.h)  # raises if an eigensolve did not converge
-    stage_ms = epw.epw_interp_get_stage_times(h.h)
-    stage_launches = epw.epw_interp_get_stage_launches(h.h)
-    epw.epw_interp_enable_stage_timing(h.h, False)
-    ms = shard.max_over_ranks_ms(ms, dist if world > 1 else None, device="cuda")
+    m = measure(use_grid, True)
+    ms, clocks, launches = m["ms"], m["clocks"], m["launches"]
     elements_per_step = nk * nq_step * E
     value = world * elements_per_step * args.steps / (ms * 1e-3)
+    # the same k-points handed over as a plain list (dense FP64 tensor-path S2), reported beside the grid arm
+    m_list = measure(False, False) if (use_grid and not args.no_klist_arm) else None
 
-    # ---- rooflines: every contraction stage, the dominant one (largest share of the step) at top level ----
+    # ---- rooflines: every stage with a stated bound, the dominant one (largest share of the step) at top level ----
     roofline = None
+    klist_path = None
     if rank == 0:
-        plan = epw.epw_interp_last_plan(h.h)
-        large = plan["path"] == "large"
         peaks = epw.epw_probe_peaks(local_rank)
         mp = {}
         if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")):
@@ -297,49 +314,94 @@ def main():
         if os.path.exists(tpath):
             traffic = json.load(open(tpath))
         nb, nm, ne = w.nbnd, w.nmodes, w.ne
-        pairs = float(nk) * nq_step * args.steps
-        # algorithmic (unpadded) flops, 8 real flops per complex multiply-add
-        ncols = E + (0 if (kq_map is not None or large) else nb * nb)  # small path: H(k+q) rides on S2 as Nb^2 extra columns
-        dmma, dfma = peaks["fp64_dmma_tflops"], peaks["fp64_dfma_tflops"]
-        spec = {
-            "S2_re_to_k_dmma": ("tensor", "zgemm_strided_kernel" if large else "zgemm_dmma_kernel", 8.0 * ncols * ne * pairs, dmma),
-            "S4b_rotate_g2": ("tensor", "zgemm_strided_kernel" if large else "rotate_g2_dmma_kernel",
-                              16.0 * nb ** 3 * nm * pairs, dmma),
-            "S4a_mode_rotation": ("tensor" if large else "alu", "zgemm_strided_kernel" if large else "pack_b_kernel",
-                                  8.0 * nb * nb * nm * nm * ne * nq_step * args.steps, dmma if large else dfma),
-        }
-        stages = {}
-        for name, (bound, kernel, flops, peak) in spec.items():
-            t_ms, nl = stage_ms[name], max(1, stage_launches[name])
-            if t_ms <= 0:
-                continue
-            ach = flops / (t_ms * 1e-3) / 1e12
-            stages[name] = {"bound": bound, "kernel": kernel, "achieved": ach, "peak": peak, "unit": "TFLOP/s",
-                            "frac": ach / peak, "flops_per_launch": flops / nl, "launches": nl,
-                            "avg_launch_ms": t_ms / nl, "share_of_step": t_ms / stage_ms["total"]}
-        n_s1 = -(-nq_step // plan["q_batch"])
-        s1_bytes = (16.0 * w.slab_elems * w.np_ * n_s1 + 16.0 * w.slab_elems * nq_step) * args.steps
-        s1 = {"bound": "hbm", "kernel": "rp_to_q_kernel", "achieved": s1_bytes / (stage_ms["S1_rp_to_q"] * 1e-3) / 1e9,
-              "peak": mp.get("hbm_gbs"), "unit": "GB/s", "bytes_per_launch": s1_bytes / (n_s1 * args.steps),
-              "launches": n_s1 * args.steps, "share_of_step": stage_ms["S1_rp_to_q"] / stage_ms["total"]}
-        if s1["peak"]:
-            s1["frac"] = s1["achieved"] / s1["peak"]
-        dom = max(("S2_re_to_k_dmma", "S4b_rotate_g2"), key=lambda n: stages[n]["share_of_step"] if n in stages else 0.0)
+        dmma, dfma, hbm = peaks["fp64_dmma_tflops"], peaks["fp64_dfma_tflops"], mp.get("hbm_gbs")
+        Lbox = [int(w.Re[:, d].max() - w.Re[:, d].min() + 1) for d in range(3)]
+
+        def stage_table(mm):
+            """Algorithmic work of the algorithm actually executed / CUDA-event time of the stage."""
+            plan, stage_ms, stage_launches, rot = mm["plan"], mm["stage_ms"], mm["stage_launches"], mm["rotations"]
+            large, grid = plan["path"] == "large", plan["k_mode"] == "grid"
+            nsteps = args.steps
+            pairs = float(nk) * nq_step * nsteps
+            nq_tot = float(nq_step) * nsteps
+            # H(k+q) rides on S2 as Nb^2 extra columns in the small path when k+q is not folded onto the grid
+            ncols = E + (0 if (kq_map is not None or large) else nb * nb)
+            n_eig = "eigh_thread_kernel" if nb <= 8 else ("eigh_cols_kernel" if nb <= 16 else "eigh_cluster_kernel")
+            # FP64 flops of one plane rotation (DESIGN.md 6.2): thread kernel 20(2n-2)+25, column-pair kernel 36n+25
+            rot_flops = (20.0 * (2 * nb - 2) + 25.0) if nb <= 8 else (36.0 * nb + 25.0)
+            spec = {}
+            if grid:
+                N1, N2, N3 = w.k_grid
+                L1, L2, L3 = Lbox
+                mults = L1 * L2 * N3 * L3 + L1 * N2 * N3 * L2 + float(nk) * L1          # per column and q
+                byts = 16.0 * ncols * ((L1 * L2 * L3 + L1 * L2 * N3) + (L1 * L2 * N3 + L1 * N2 * N3) + (L1 * N2 * N3 + nk))
+                spec["S2_re_to_k"] = ("hbm", "zgemm_strided_kernel (3 axis passes)", byts * nq_tot, hbm, "GB/s",
+                                      {"flops": 8.0 * ncols * mults * nq_tot})
+            else:
+                spec["S2_re_to_k"] = ("tensor", "zgemm_strided_kernel" if large else "zgemm_dmma_kernel",
+                                      8.0 * ncols * ne * pairs, dmma, "TFLOP/s", {})
+            spec["S4b_rotate_g2"] = ("tensor", "zgemm_strided_kernel" if large else "rotate_g2_dmma_kernel",
+                                     16.0 * nb ** 3 * nm * pairs, dmma, "TFLOP/s",
+                                     {"hbm_bytes": (16.0 * (E + 2 * nb * nb) + 8.0 * E) * pairs})
+            spec["S4a_mode_rotation"] = ("tensor" if large else "alu",
+                                         "zgemm_strided_kernel" if large else ("box_scatter_kernel" if grid else "pack_b_kernel"),
+                                         8.0 * nb * nb * nm * nm * ne * nq_tot, dmma if large else dfma, "TFLOP/s", {})
+            if rot["Hkq"]:
+                spec["Hkq_eig"] = ("alu", n_eig, rot_flops * rot["Hkq"], dfma, "TFLOP/s",
+                                   {"rotations": rot["Hkq"], "solves": pairs, "rotations_per_solve": rot["Hkq"] / pairs})
+            if rot["Hk"]:
+                spec["Hk_eig"] = ("alu", n_eig + " (+ H(k) interpolation)", rot_flops * rot["Hk"], dfma, "TFLOP/s",
+                                  {"rotations": rot["Hk"]})
+            names = {"S2_re_to_k": "S2_re_to_k_dmma"}
+            stages = {}
+            for name, (bound, kernel, work, peak, unit, extra) in spec.items():
+                key = names.get(name, name)
+                t_ms, nl = stage_ms[key], max(1, stage_launches[key])
+                if t_ms <= 0 or not peak:
+                    continue
+                ach = work / (t_ms * 1e-3) / (1e9 if unit == "GB/s" else 1e12)
+                st = {"bound": bound, "kernel": kernel, "achieved": ach, "peak": peak, "unit": unit, "frac": ach / peak,
+                      ("bytes_per_launch" if unit == "GB/s" else "flops_per_launch"): work / nl, "launches": nl,
+                      "avg_launch_ms": t_ms / nl, "share_of_step": t_ms / stage_ms["total"]}
+                if "hbm_bytes" in extra and hbm:
+                    st["hbm_frac"] = extra["hbm_bytes"] / (t_ms * 1e-3) / 1e9 / hbm
+                st.update({k: v for k, v in extra.items() if k != "hbm_bytes"})
+                stages[name] = st
+            n_s1 = -(-nq_step // plan["q_batch"])
+            s1_bytes = (16.0 * w.slab_elems * w.np_ * n_s1 + 16.0 * w.slab_elems * nq_step) * nsteps
+            s1 = {"bound": "hbm", "kernel": "rp_to_q_kernel", "achieved": s1_bytes / (stage_ms["S1_rp_to_q"] * 1e-3) / 1e9,
+                  "peak": hbm, "unit": "GB/s", "bytes_per_launch": s1_bytes / (n_s1 * nsteps),
+                  "launches": n_s1 * nsteps, "avg_launch_ms": stage_ms["S1_rp_to_q"] / (n_s1 * nsteps),
+                  "share_of_step": stage_ms["S1_rp_to_q"] / stage_ms["total"]}
+            if hbm:
+                s1["frac"] = s1["achieved"] / hbm
+            stages["S1_rp_to_q"] = s1
+            return stages
+
+        stages = stage_table(m)
+        dom = max(stages, key=lambda n: stages[n]["share_of_step"])
         roofline = dict(stages[dom])
         roofline["stage"] = dom
-        roofline["traffic"] = traffic.get(f"{stages[dom]['kernel']}:{dom}:config{w.index}")
-        roofline["peak_source"] = ("FP64 DMMA m8n8k4 issue-loop probe (tensor) / dependent-free DFMA loop probe (alu) run live on "
-                                   "this GPU by epw_probe_peaks; MEASURED_PEAKS.json has no FP64 entry")
+        roofline["traffic"] = traffic.get(f"{stages[dom]['kernel'].split(' ')[0]}:{dom}:config{w.index}:{m['plan']['k_mode']}")
+        roofline["peak_source"] = ("tensor: FP64 DMMA m8n8k4 issue-loop probe, alu: dependent-free DFMA loop probe, both run live on "
+                                   "this GPU by epw_probe_peaks (MEASURED_PEAKS.json has no FP64 entry); hbm: MEASURED_PEAKS.json hbm_gbs")
         roofline["peak_from_measured_bf16_x_nominal_ratio"] = (mp.get("bf16_tflops_sustained", 0.0) * 45.0 / 2250.0) or None
         roofline["hbm_read_gbs_probe"] = peaks["hbm_read_gbs"]
         roofline["fp64_dfma_tflops_probe"] = dfma
         roofline["fp64_dmma_tflops_probe"] = dmma
-        roofline["plan"] = plan
+        roofline["plan"] = m["plan"]
         roofline["stages"] = stages
-        roofline["s1_rp_to_q"] = s1
-        roofline["stage_ms_per_step"] = {k: v / args.steps for k, v in stage_ms.items()}
+        roofline["stage_ms_per_step"] = {k: v / args.steps for k, v in m["stage_ms"].items()}
+        if m_list is not None:
+            st_l = stage_table(m_list)
+            klist_path = {"what": "the same k-points passed as a plain list to epw_interp_interpolate: dense S2 on the FP64 "
+                                  "tensor path (zgemm_dmma_kernel), everything else identical",
+                          "value": world * elements_per_step * args.steps / (m_list["ms"] * 1e-3), "unit": UNIT,
+                          "ms_per_step": m_list["ms"] / args.steps, "S2_re_to_k": st_l.get("S2_re_to_k"),
+                          "traffic": traffic.get(f"zgemm_dmma_kernel:S2_re_to_k_dmma:config{w.index}"),
+                          "stage_ms_per_step": {k: v / args.steps for k, v in m_list["stage_ms"].items()}}
     if args.stages and rank == 0:
-        print(json.dumps({k: round(v / args.steps, 4) for k, v in stage_ms.items()}), file=sys.stderr)
+        print(json.dumps({k: round(v / args.steps, 4) for k, v in m["stage_ms"].items()}), file=sys.stderr)
 
     # ---- e2e: the same steps through the host-buffer entry point (H2D of k/q lists, D2H of all outputs) ----
     e2e = None
@@ -354,8 +416,14 @@ def main():
         o_g2 = torch.empty((nq_step, nk, w.nmodes, w.nbnd, w.nbnd), dtype=torch.float64).pin_memory()
 
         def step_host(s):
-            epw.epw_interp_interpolate_host(h.h, k_host, nk, q_host[s], nq_step, None if map_host is None else map_host[s],
-                                            o_eps_k, o_eps_kq, o_omega, o_g2)
+            if use_grid:
+                epw.epw_interp_interpolate_grid_host(h.h, w.k_grid, None, q_host[s], nq_step,
+                                                     None if map_host is None else map_host[s], o_eps_k, o_eps_kq,
+                                                     o_omega, o_g2)
+            else:
+                epw.epw_interp_interpolate_host(h.h, k_host, nk, q_host[s], nq_step,
+                                                None if map_host is None else map_host[s], o_eps_k, o_eps_kq, o_omega,
+                                                o_g2)
 
         n_e2e_warm = min(args.warmup, 2)
         for s in range(n_e2e_warm):
@@ -369,11 +437,12 @@ def main():
         barrier()
         ms_e2e = e0.elapsed_time(e1)
         ms_e2e = shard.max_over_ranks_ms(ms_e2e, dist if world > 1 else None, device="cuda")
-        h2d = k_host.numel() * 8 + q_host[0].numel() * 8 + (0 if map_host is None else map_host[0].numel() * 4)
+        h2d = (0 if use_grid else k_host.numel() * 8) + q_host[0].numel() * 8 + (0 if map_host is None else map_host[0].numel() * 4)
         d2h = (o_eps_k.numel() + o_eps_kq.numel() + o_omega.numel() + o_g2.numel()) * 8
         e2e = {"value": world * elements_per_step * args.steps / (ms_e2e * 1e-3), "unit": UNIT,
                "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "ms_per_step": ms_e2e / args.steps,
-               "api": "epw_interp_interpolate_host (pinned host buffers in and out)"}
+               "api": ("epw_interp_interpolate_grid_host" if use_grid else "epw_interp_interpolate_host")
+                      + " (pinned host buffers in and out)"}
 
     # ---- CPU oracle beside it (rank 0, N = 1 only) ----
     cpu_baseline = None
@@ -392,12 +461,13 @@ def main():
                 "workload": f"BASELINE.json configs[{w.index}] {w.name}: Nb={w.nbnd} Nm={w.nmodes} Ne={w.ne} Np={w.np_} "
                             f"Nk={nk} ({'x'.join(map(str, w.k_grid))}), {nq_step} q per step per GPU ({w.q_desc})",
                 "global_batch_pairs": world * nk * nq_step, "parallelism": f"q-sharded x{world}",
+                "k_mode": ("uniform grid -> epw_interp_interpolate_grid" if use_grid else "k-list -> epw_interp_interpolate"),
                 "l2": "inputs larger than L2: g(Re,Rp) %.0f MB streamed per q-batch, phase table %.0f MB, |g|^2 output %.0f MB "
                       "per step" % (w.g_bytes / 1e6, 16.0 * nk * w.ne / 1e6, 8.0 * elements_per_step / 1e6),
                 "operator_upload_s": t_upload,
             },
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
-            "cpu_baseline": cpu_baseline,
+            "klist_path": klist_path, "cpu_baseline": cpu_baseline,
         }
         print(json.dumps(line))
     h.close()

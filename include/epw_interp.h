@@ -114,6 +114,25 @@ int epw_interp_interpolate_host(epw_interp_t h, const double *k_list, int64_t nk
                                 const int32_t *kq_map, double *eps_k, double *eps_kq, double *omega_q, double *g2,
                                 void *cuda_stream);
 
+/*
+ * The same hot path for k-points on a UNIFORM GRID, given by its three sizes instead of a list:
+ *     k[(i1*N2 + i2)*N3 + i3] = ((i1 + s1)/N1, (i2 + s2)/N2, (i3 + s3)/N3),   i3 fastest,   nk = N1 N2 N3
+ *   k_grid  int32 [3] HOST: N1, N2, N3 (all > 0);   k_shift f64 [3] HOST or NULL (= 0: Gamma-centred grid)
+ * Results, layouts and every other argument are those of epw_interp_interpolate called with that k-list (kq_map, if
+ * given, indexes the grid in the order above).  On a grid the phase of the Re -> k Fourier sum (PAPER.md:L112-118,
+ * Eq. 10) factorises over the crystal axes, so S2 and the H(k), H(k+q) part of S3a are taken one axis at a time
+ * (csrc/re_to_k_grid.cu): (L1 L2 N3 L3 + L1 N2 N3 L2 + N1 N2 N3 L1) instead of Nk Ne multiplications per column, with
+ * L_d the extents of the bounding box of the Re list -- the same sums re-associated, equal to the list form up to
+ * rounding order.  The large-Nb kernel family (one-dimensional grids) expands the grid to a list internally.
+ */
+int epw_interp_interpolate_grid(epw_interp_t h, const int32_t *k_grid, const double *k_shift, const double *q_list,
+                                int64_t nq, const int32_t *kq_map, double *eps_k, double *eps_kq, double *omega_q,
+                                double *g2, void *cuda_stream);
+/* Host-buffer form of epw_interp_interpolate_grid (cf. epw_interp_interpolate_host). */
+int epw_interp_interpolate_grid_host(epw_interp_t h, const int32_t *k_grid, const double *k_shift, const double *q_list,
+                                     int64_t nq, const int32_t *kq_map, double *eps_k, double *eps_kq, double *omega_q,
+                                     double *g2, void *cuda_stream);
+
 /* Wait for the handle's last enqueued work and report deferred device-side status (EPW_ENOTCONVERGED, EPW_ECUDA). */
 int epw_interp_sync(epw_interp_t h);
 
@@ -136,11 +155,18 @@ int epw_interp_get_stage_launches(epw_interp_t h, int64_t *counts, int n);
  * following interpolate calls and clears the accumulated times; on == 0 disables it. */
 int epw_interp_enable_stage_timing(epw_interp_t h, int on);
 
+/* Plane rotations (matrix-rotations) the register-resident Jacobi eigensolvers executed since stage timing was last
+ * enabled: counts[0] H(k), counts[1] H(k+q), counts[2] D(q).  The sweep count of Jacobi is data dependent, so this is
+ * what turns the eigensolve time into an FP64 rate (flops per rotation of each kernel).  Zero for the
+ * shared-memory / cluster kernels, which do not count.  Synchronises the stream.  Returns entries written. */
+int epw_interp_get_eigh_rotations(epw_interp_t h, uint64_t *counts, int n);
+
 /* Number of kernels the library launched during the last interpolate call (for bench.py's gpu_launches). */
 int64_t epw_interp_last_launch_count(epw_interp_t h);
 
 /* How the last interpolate call was executed: plan[0] = EPW_PATH_SMALL or EPW_PATH_LARGE, plan[1] = q-points per pass
- * over g(Re,Rp) in S1, plan[2] = k-points per chunk of S2 / S3b / S4b.  Returns the number of entries written. */
+ * over g(Re,Rp) in S1, plan[2] = k-points per chunk of S2 / S3b / S4b, plan[3] = 1 if S2 ran in its factorised
+ * uniform-grid form, 0 for the dense k-list contraction.  Returns the number of entries written. */
 int epw_interp_last_plan(epw_interp_t h, int64_t *plan, int n);
 
 /*

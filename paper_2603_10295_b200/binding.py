@@ -29,8 +29,9 @@ EPW_DBG_G_REQ, EPW_DBG_G_TILDE, EPW_DBG_H_K, EPW_DBG_U_K, EPW_DBG_U_KQ, EPW_DBG_
 # every symbol include/epw_interp.h declares (tests check that the library exports each of them)
 EXPORTED_SYMBOLS = [
     "epw_interp_create", "epw_interp_destroy", "epw_interp_set_wannier_operators", "epw_interp_set_g_slabs",
-    "epw_interp_interpolate", "epw_interp_interpolate_host", "epw_interp_sync", "epw_interp_get_stage_times",
-    "epw_interp_enable_stage_timing", "epw_interp_get_stage_launches", "epw_interp_last_launch_count", "epw_interp_last_plan", "epw_interp_debug_get", "epw_interp_last_error",
+    "epw_interp_interpolate", "epw_interp_interpolate_host", "epw_interp_interpolate_grid",
+    "epw_interp_interpolate_grid_host", "epw_interp_sync", "epw_interp_get_stage_times",
+    "epw_interp_enable_stage_timing", "epw_interp_get_stage_launches", "epw_interp_last_launch_count", "epw_interp_get_eigh_rotations", "epw_interp_last_plan", "epw_interp_debug_get", "epw_interp_last_error",
     "epw_phase_table", "epw_rp_to_q", "epw_interp_operator", "epw_eigh_batched", "epw_eigh_batched_algo", "epw_zgemm", "epw_zgemm_strided",
     "epw_rotate_g2",
     "epw_probe_peaks", "epw_version",
@@ -68,12 +69,15 @@ def load_library() -> ctypes.CDLL:
         L.epw_interp_set_g_slabs.argtypes = [vp, c_int32, c_int32, vp, c_int]
         L.epw_interp_interpolate.argtypes = [vp, vp, c_int64, vp, c_int64, vp, vp, vp, vp, vp, vp]
         L.epw_interp_interpolate_host.argtypes = [vp, vp, c_int64, vp, c_int64, vp, vp, vp, vp, vp, vp]
+        L.epw_interp_interpolate_grid.argtypes = [vp, vp, vp, vp, c_int64, vp, vp, vp, vp, vp, vp]
+        L.epw_interp_interpolate_grid_host.argtypes = [vp, vp, vp, vp, c_int64, vp, vp, vp, vp, vp, vp]
         L.epw_interp_sync.argtypes = [vp]
         L.epw_interp_get_stage_times.argtypes = [vp, POINTER(c_double), c_int]
         L.epw_interp_enable_stage_timing.argtypes = [vp, c_int]
         L.epw_interp_get_stage_launches.argtypes = [vp, POINTER(c_int64), c_int]
         L.epw_interp_last_launch_count.argtypes = [vp]
         L.epw_interp_last_launch_count.restype = c_int64
+        L.epw_interp_get_eigh_rotations.argtypes = [vp, POINTER(ctypes.c_uint64), c_int]
         L.epw_interp_last_plan.argtypes = [vp, POINTER(c_int64), c_int]
         L.epw_interp_debug_get.argtypes = [vp, c_int, vp, c_size_t]
         L.epw_interp_debug_get.restype = c_int64
@@ -155,6 +159,27 @@ def epw_interp_interpolate_host(h, k_list, nk, q_list, nq, kq_map, eps_k, eps_kq
                                                       _stream() if stream is None else stream), h)
 
 
+def _grid_args(k_grid, k_shift):
+    """k_grid / k_shift are HOST triples (the only host arguments of the grid entry points)."""
+    g = (c_int32 * 3)(*[int(x) for x in k_grid])
+    s = None if k_shift is None else (c_double * 3)(*[float(x) for x in k_shift])
+    return g, s
+
+
+def epw_interp_interpolate_grid(h, k_grid, k_shift, q_list, nq, kq_map, eps_k, eps_kq, omega_q, g2, stream=None):
+    g, s = _grid_args(k_grid, k_shift)
+    _check(load_library().epw_interp_interpolate_grid(h, g, s, _ptr(q_list), nq, _ptr(kq_map), _ptr(eps_k), _ptr(eps_kq),
+                                                      _ptr(omega_q), _ptr(g2),
+                                                      _stream() if stream is None else stream), h)
+
+
+def epw_interp_interpolate_grid_host(h, k_grid, k_shift, q_list, nq, kq_map, eps_k, eps_kq, omega_q, g2, stream=None):
+    g, s = _grid_args(k_grid, k_shift)
+    _check(load_library().epw_interp_interpolate_grid_host(h, g, s, _ptr(q_list), nq, _ptr(kq_map), _ptr(eps_k),
+                                                           _ptr(eps_kq), _ptr(omega_q), _ptr(g2),
+                                                           _stream() if stream is None else stream), h)
+
+
 def epw_interp_sync(h):
     _check(load_library().epw_interp_sync(h), h)
 
@@ -179,10 +204,17 @@ def epw_interp_last_launch_count(h) -> int:
     return int(load_library().epw_interp_last_launch_count(h))
 
 
+def epw_interp_get_eigh_rotations(h) -> dict:
+    buf = (ctypes.c_uint64 * 3)()
+    _check(load_library().epw_interp_get_eigh_rotations(h, buf, 3), h)
+    return {"Hk": int(buf[0]), "Hkq": int(buf[1]), "Dq": int(buf[2])}
+
+
 def epw_interp_last_plan(h) -> dict:
-    buf = (c_int64 * 3)()
-    _check(load_library().epw_interp_last_plan(h, buf, 3), h)
-    return {"path": "large" if buf[0] == EPW_PATH_LARGE else "small", "q_batch": int(buf[1]), "k_chunk": int(buf[2])}
+    buf = (c_int64 * 4)()
+    _check(load_library().epw_interp_last_plan(h, buf, 4), h)
+    return {"path": "large" if buf[0] == EPW_PATH_LARGE else "small", "q_batch": int(buf[1]), "k_chunk": int(buf[2]),
+            "k_mode": "grid" if buf[3] else "list"}
 
 
 def epw_interp_debug_get(h, what, dst_host):
@@ -280,4 +312,17 @@ class EpwInterp:
         omega_q = torch.empty((nq, self.nmodes), dtype=torch.float64, device=dev)
         g2 = torch.empty((nq, nk, self.nmodes, self.nbnd, self.nbnd), dtype=torch.float64, device=dev)
         epw_interp_interpolate(self.h, k_list, nk, q_list, nq, kq_map, eps_k, eps_kq, omega_q, g2)
+        return eps_k, eps_kq, omega_q, g2
+
+    def interpolate_grid(self, k_grid, q_list, k_shift=None, kq_map=None, want_eps_kq=True):
+        """Uniform k-grid (host triple of sizes, i3 fastest) and a device q-list in, device tensors out."""
+        import torch
+
+        nk, nq = int(k_grid[0]) * int(k_grid[1]) * int(k_grid[2]), q_list.shape[0]
+        dev = q_list.device
+        eps_k = torch.empty((nk, self.nbnd), dtype=torch.float64, device=dev)
+        eps_kq = torch.empty((nq, nk, self.nbnd), dtype=torch.float64, device=dev) if want_eps_kq else None
+        omega_q = torch.empty((nq, self.nmodes), dtype=torch.float64, device=dev)
+        g2 = torch.empty((nq, nk, self.nmodes, self.nbnd, self.nbnd), dtype=torch.float64, device=dev)
+        epw_interp_interpolate_grid(self.h, k_grid, k_shift, q_list, nq, kq_map, eps_k, eps_kq, omega_q, g2)
         return eps_k, eps_kq, omega_q, g2

@@ -76,6 +76,11 @@ size_t eigh_large_scratch_bytes(int n, int64_t batch);
 // same with an explicit kernel choice (EPW_EIGH_AUTO / _WARP / _THREAD / _COLS, include/epw_interp.h)
 cudaError_t launch_eigh_batched_algo(const c128 *A, int64_t stride_a, int n, int64_t batch, double *evals, c128 *V,
                                      int sqrt_mode, int32_t *status, c128 *scratch_large, int algo, cudaStream_t st);
+// Optional work counter of the two register-resident solvers: a device word that accumulates the number of plane
+// rotations executed (matrix-rotations), so that their FP64 work can be stated (the sweep count is data dependent).
+// NULL (default) = not counted.  Process-wide; set by the handle while stage timing is on.
+void eigh_set_work_counter(unsigned long long *dev_counter);
+unsigned long long *eigh_work_counter();
 // column-pair one-sided solver (eigh_cols.cu), n in 9..16
 bool eigh_cols_supported(int n);
 cudaError_t launch_eigh_cols(const c128 *A, int64_t stride_a, int n, int64_t batch, double *evals, c128 *V,
@@ -113,6 +118,15 @@ cudaError_t launch_zgemm_strided(const c128 *A, int64_t a_rb, int64_t a_bs, int6
 // by 1/sqrt(2 omega[n]) when omega != NULL).  Bpack doubles [batch][NT][KB][2048].
 cudaError_t launch_pack_b_strided(const c128 *B, int64_t sr, int64_t sn, int64_t batch_stride, int64_t batch, int conj,
                                   const double *omega, double omega_min, int K, int N, double *Bpack, cudaStream_t st);
+
+// Uniform-grid form of S2 / S3a (re_to_k_grid.cu): the B operand of the dense path scattered into the bounding box of
+// the Re list (X [box][ncols], zeros where the list has no vector), one axis of the factorised phase, and the k-list
+// a grid stands for.
+cudaError_t launch_box_scatter(const c128 *g1, const c128 *e, const double *omega, double omega_min, const c128 *H_R,
+                               const c128 *phase_qe, const double *w_e, const int32_t *box_idx, int64_t box_size, int nbb,
+                               int nm, int ne, int ncols_g, int ncols_h, c128 *X, cudaStream_t st);
+cudaError_t launch_grid_axis_phase(int N, int i0, int cnt, double shift, int lo, int L, c128 *P, cudaStream_t st);
+cudaError_t launch_grid_klist(const int32_t N[3], const double s[3], double *k_list, cudaStream_t st);
 
 cudaError_t launch_rotate_g2(const c128 *gt, int64_t stride_gt, const c128 *Uk, const c128 *Ukq, const int32_t *kq_idx,
                              int nb, int nm, int64_t nk, double *g2, cudaStream_t st);

@@ -52,14 +52,14 @@ __device__ __forceinline__ bool hestenes_rotate(c128 (&lo)[NN], c128 (&hi)[NN], 
   const double r2 = fma(gr, gr, gi * gi);
   const bool live = r2 > tol2 * al * be && r2 >= 1e-280;
   if (!__any_sync(0xffffffffu, live)) return false;
-  const double inv_r = rsqrt(live ? r2 : 1.0);
-  const double tau = 0.5 * (be - al) * inv_r;
-  const double w = sqrt(fma(tau, tau, 1.0));
-  const double t = copysign(1.0 / (fabs(tau) + w), tau);
-  const double c0 = rsqrt(fma(t, t, 1.0));
-  const double sor = t * c0 * inv_r;
+  // half-angle form (jacobi_packed.cuh): two dependent rsqrt, no subtraction
+  const double a = 0.5 * (be - al);
+  const double h = rsqrt(live ? fma(a, a, r2) : 1.0);
+  const double x = fma(0.5 * fabs(a), h, 0.5);
+  const double rc = rsqrt(x);
+  const double sor = copysign(0.5 * h * rc, a);
   PlaneRot R;
-  R.c = live ? c0 : 1.0;
+  R.c = live ? x * rc : 1.0;
   R.sr = live ? sor * gr : 0.0;
   R.si = live ? sor * gi : 0.0;
 #pragma unroll
@@ -70,7 +70,8 @@ __device__ __forceinline__ bool hestenes_rotate(c128 (&lo)[NN], c128 (&hi)[NN], 
 template <int NN>
 __global__ void __launch_bounds__(ColsCfg<NN>::THREADS, (NN <= 12 ? 2 : 1))
     eigh_cols_kernel(const c128 *__restrict__ Ain, int64_t stride_a, int64_t batch, double *__restrict__ evals,
-                     c128 *__restrict__ Vout, int sqrt_mode, int32_t *__restrict__ status) {
+                     c128 *__restrict__ Vout, int sqrt_mode, int32_t *__restrict__ status,
+                     unsigned long long *__restrict__ work) {
   typedef ColsCfg<NN> Cfg;
   constexpr int N = Cfg::N, L = Cfg::L;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -132,11 +133,12 @@ __global__ void __launch_bounds__(ColsCfg<NN>::THREADS, (NN <= 12 ? 2 : 1))
   const c128 *inB = bufB + ((size_t)(s + 1) * NN) * 32 + lane;                               // hi from warp s+1
   const c128 *inA = s > 0 ? bufA + ((size_t)(s - 1) * NN) * 32 + lane : bufB + lane;          // lo from warp s-1 / parked
   bool converged = false;
+  int nrot = 0;  // rotations this warp executed (for the optional work counter)
   for (int sweep = 0; sweep < EC2_MAX_SWEEPS && !converged; sweep++) {
     int any_act = 0;
     for (int step2 = 0; step2 < L; step2++) {
       // ---- first kind: pairs (2s, 2s+1) ----
-      any_act |= hestenes_rotate<NN>(lo, hi, tol2) ? 1 : 0;
+      { const bool a = hestenes_rotate<NN>(lo, hi, tol2); any_act |= a ? 1 : 0; nrot += a ? 1 : 0; }
 #pragma unroll
       for (int i = 0; i < NN; i++) outB[(size_t)i * 32] = hi[i];
       __syncthreads();
@@ -144,7 +146,7 @@ __global__ void __launch_bounds__(ColsCfg<NN>::THREADS, (NN <= 12 ? 2 : 1))
 #pragma unroll
         for (int i = 0; i < NN; i++) hi[i] = inB[(size_t)i * 32];
         // ---- second kind: pairs (2s+1, 2s+2); the last warp sits out ----
-        any_act |= hestenes_rotate<NN>(lo, hi, tol2) ? 1 : 0;
+        { const bool a = hestenes_rotate<NN>(lo, hi, tol2); any_act |= a ? 1 : 0; nrot += a ? 1 : 0; }
 #pragma unroll
         for (int i = 0; i < NN; i++) outA[(size_t)i * 32] = lo[i];
       } else {
@@ -158,6 +160,10 @@ __global__ void __launch_bounds__(ColsCfg<NN>::THREADS, (NN <= 12 ? 2 : 1))
     converged = __syncthreads_or(any_act) == 0;
   }
   if (!converged && status != nullptr && threadIdx.x == 0) atomicExch(status, 1);
+  if (work != nullptr) {
+    const unsigned m = __ballot_sync(0xffffffffu, have);
+    if (lane == 0) atomicAdd(work, (unsigned long long)nrot * __popc(m));
+  }
 
   // ---- eigenvectors = normalised columns; eigenvalues = Rayleigh quotients with the original Hermitian part ----
   double na = 0.0, nb2 = 0.0;
@@ -230,7 +236,7 @@ static cudaError_t launch_cols_n(const c128 *A, int64_t stride_a, int64_t batch,
   cudaError_t e = cudaFuncSetAttribute(eigh_cols_kernel<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
   if (e != cudaSuccess) return e;
   eigh_cols_kernel<NN><<<(unsigned)ceil_div(batch, 32), Cfg::THREADS, Cfg::SMEM, st>>>(A, stride_a, batch, evals, V,
-                                                                                      sqrt_mode, status);
+                                                                                      sqrt_mode, status, eigh_work_counter());
   return cudaGetLastError();
 }
 

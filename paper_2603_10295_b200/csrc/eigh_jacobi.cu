@@ -607,6 +607,10 @@ size_t eigh_large_scratch_bytes(int n, int64_t batch) {
   return (size_t)eigh_large_grid(batch) * 2 * (size_t)n * n * sizeof(c128);
 }
 
+static unsigned long long *g_work_counter = nullptr;
+void eigh_set_work_counter(unsigned long long *dev_counter) { g_work_counter = dev_counter; }
+unsigned long long *eigh_work_counter() { return g_work_counter; }
+
 cudaError_t launch_eigh_batched(const c128 *A, int64_t stride_a, int n, int64_t batch, double *evals, c128 *V,
                                 int sqrt_mode, int32_t *status, c128 *scratch_large, cudaStream_t st) {
   return launch_eigh_batched_algo(A, stride_a, n, batch, evals, V, sqrt_mode, status, scratch_large, EPW_EIGH_AUTO, st);

@@ -89,6 +89,16 @@ struct epw_interp {
   DevBuf Apack, BpackH, Hk, Uk, Pq, Pqe, Dq, eq, g1, Bpack, C, Ukq, epskq_scratch, status, eig_scratch;
   // large-Nb path only
   DevBuf Pk, BpackPk, UpackK, UpackKH, BpackE, ghat, T, Hkq;
+  // uniform-grid form of S2 (re_to_k_grid.cu): bounding box of the Re list, box-ordered operand and axis passes
+  int box_lo[3] = {0, 0, 0}, box_L[3] = {1, 1, 1};
+  int64_t box_size = 1;
+  DevBuf boxidx, X, T1, T2, Ptmp, P1pack, P2pack, P3pack, klist_gen;
+  DevBuf workctr;  // 3 x u64: plane rotations executed by the register-resident eigensolvers for H(k), H(k+q), D(q)
+  // route the eigensolver work counter to slot i (0 H(k), 1 H(k+q), 2 D(q)) while stage timing is on; -1 = off
+  void count_into(int slot) {
+    eigh_set_work_counter(timing && slot >= 0 && workctr.p ? workctr.as<unsigned long long>() + slot : nullptr);
+  }
+  int last_kmode = 0;
   // host-entry staging
   DevBuf hs_k, hs_q, hs_map, hs_epsk, hs_epskq, hs_omega, hs_g2;
   // bookkeeping of the last call
@@ -242,9 +252,11 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
   LAUNCH(h, launch_zgemm_dmma(h->Apack.as<double>(), h->BpackH.as<double>(), h->Hk.as<c128>(), nk, nbb, KBe, nbb,
                               h->num_sms, st),
          "zgemm H(k)");
+  h->count_into(0);
   LAUNCH(h, launch_eigh_batched(h->Hk.as<c128>(), nbb, nb, nk, eps_k, h->Uk.as<c128>(), 0, h->status.as<int32_t>(),
                                 h->eig_scratch.as<c128>(), st),
          "eigh H(k)");
+  h->count_into(-1);
   LAUNCH(h, launch_pack_b_strided(h->Uk.as<c128>(), 1, nb, nbb, nk, 0, nullptr, 0.0, nb, nb, h->UpackK.as<double>(), st),
          "pack U_k");
   if (kq_map)
@@ -267,9 +279,11 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
     h->end_span(sp, st);
     sp = h->begin_span(2, st);
     LAUNCH(h, launch_interp_operator(h->D.as<c128>(), nm, np, h->Pq.as<c128>(), qb, h->Dq.as<c128>(), st), "D(q)");
+    h->count_into(2);
     LAUNCH(h, launch_eigh_batched(h->Dq.as<c128>(), nmm, nm, qb, omega_q + q0 * nm, h->eq.as<c128>(), 1,
                                   h->status.as<int32_t>(), h->eig_scratch.as<c128>(), st),
            "eigh D(q)");
+    h->count_into(-1);
     h->end_span(sp, st);
 
     for (int iq = 0; iq < qb; iq++) {
@@ -296,9 +310,11 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
                                     h->num_sms, st),
                "zgemm H(k+q)");
         double *eps_dst = eps_kq ? eps_kq + q * nk * nb : h->epskq_scratch.as<double>();
+        h->count_into(1);
         LAUNCH(h, launch_eigh_batched(h->Hkq.as<c128>(), nbb, nb, nk, eps_dst, h->Ukq.as<c128>(), 0,
                                       h->status.as<int32_t>(), h->eig_scratch.as<c128>(), st),
                "eigh H(k+q)");
+        h->count_into(-1);
         LAUNCH(h, launch_pack_b_strided(h->Ukq.as<c128>(), 1, nb, nbb, nk, 1, nullptr, 0.0, nb, nb,
                                         h->UpackKH.as<double>(), st),
                "pack conj U_{k+q}");
@@ -336,6 +352,16 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
   h->end_span(t_total, st);
   return EPW_OK;
 }
+
+// Uniform k-grid handed to the small-Nb path instead of a k-list (epw_interp_interpolate_grid).
+struct GridSpec {
+  int32_t N[3];
+  double s[3];
+};
+
+static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec *grid, int64_t nk, const double *q_list,
+                             int64_t nq, const int32_t *kq_map, double *eps_k, double *eps_kq, double *omega_q,
+                             double *g2, cudaStream_t st);
 
 extern "C" {
 
@@ -399,7 +425,8 @@ void epw_interp_destroy(epw_interp_t h) {
                    &h->Uk, &h->Pq, &h->Pqe, &h->Dq, &h->eq, &h->g1, &h->Bpack, &h->C, &h->Ukq, &h->epskq_scratch,
                    &h->status, &h->eig_scratch, &h->hs_k, &h->hs_q, &h->hs_map, &h->hs_epsk, &h->hs_epskq,
                    &h->hs_omega, &h->hs_g2, &h->Pk, &h->BpackPk, &h->UpackK, &h->UpackKH, &h->BpackE,
-                   &h->ghat, &h->T, &h->Hkq};
+                   &h->ghat, &h->T, &h->Hkq, &h->boxidx, &h->X, &h->T1, &h->T2, &h->Ptmp, &h->P1pack, &h->P2pack,
+                   &h->P3pack, &h->klist_gen, &h->workctr};
   for (DevBuf *b : all) b->release();
   for (cudaEvent_t ev : h->ev_pool) cudaEventDestroy(ev);
   delete h;
@@ -440,6 +467,29 @@ int epw_interp_set_wannier_operators(epw_interp_t h, const void *H_R, const void
     CU_OR_FAIL(h, it.buf->reserve(it.bytes), "cudaMalloc operators");
     CU_OR_FAIL(h, cudaMemcpy(it.buf->p, it.src, it.bytes, kind), "cudaMemcpy operators");
   }
+  {
+    // bounding box of the Re list and the position of every vector inside it (uniform-grid form of S2)
+    std::vector<int32_t> re(3 * (size_t)h->ne), idx(h->ne);
+    CU_OR_FAIL(h, cudaMemcpy(re.data(), h->Re.p, sizeof(int32_t) * re.size(), cudaMemcpyDeviceToHost), "cudaMemcpy Re");
+    int hi[3];
+    for (int d = 0; d < 3; d++) h->box_lo[d] = hi[d] = re[d];
+    for (int i = 0; i < h->ne; i++)
+      for (int d = 0; d < 3; d++) {
+        h->box_lo[d] = std::min(h->box_lo[d], (int)re[3 * i + d]);
+        hi[d] = std::max(hi[d], (int)re[3 * i + d]);
+      }
+    h->box_size = 1;
+    for (int d = 0; d < 3; d++) {
+      h->box_L[d] = hi[d] - h->box_lo[d] + 1;
+      h->box_size *= h->box_L[d];
+    }
+    for (int i = 0; i < h->ne; i++)
+      idx[i] = ((re[3 * i] - h->box_lo[0]) * h->box_L[1] + (re[3 * i + 1] - h->box_lo[1])) * h->box_L[2] +
+               (re[3 * i + 2] - h->box_lo[2]);
+    CU_OR_FAIL(h, h->boxidx.reserve(sizeof(int32_t) * (size_t)h->ne), "cudaMalloc box index");
+    CU_OR_FAIL(h, cudaMemcpy(h->boxidx.p, idx.data(), sizeof(int32_t) * (size_t)h->ne, cudaMemcpyHostToDevice),
+               "cudaMemcpy box index");
+  }
   const int nmax = std::max(h->ne, h->np);
   CU_OR_FAIL(h, h->ones.reserve(sizeof(double) * nmax), "cudaMalloc ones");
   fill_ones_kernel<<<(nmax + 255) / 256, 256>>>(h->ones.as<double>(), nmax);
@@ -454,6 +504,21 @@ int epw_interp_enable_stage_timing(epw_interp_t h, int on) {
   h->timing = on != 0;
   h->spans.clear();  // (re)enabling starts a fresh accumulation
   h->ev_used = 0;
+  if (h->timing) {
+    CU_OR_FAIL(h, cudaSetDevice(h->cfg.device), "cudaSetDevice");
+    CU_OR_FAIL(h, h->workctr.reserve(3 * sizeof(unsigned long long)), "cudaMalloc work counters");
+    CU_OR_FAIL(h, cudaMemset(h->workctr.p, 0, 3 * sizeof(unsigned long long)), "memset work counters");
+  }
+  return EPW_OK;
+}
+
+static int check_interpolate_args(epw_interp *h, const void *k_src, int64_t nk, const double *q_list, int64_t nq,
+                                  const double *eps_k, const double *omega_q, const double *g2, const char *who) {
+  if (!k_src || !q_list || !eps_k || !omega_q || !g2 || nk <= 0 || nq <= 0)
+    return h->fail(EPW_EINVAL, std::string(who) + ": null pointer or non-positive nk/nq");
+  if (!h->operators_set) return h->fail(EPW_EINVAL, std::string(who) + ": operators not set");
+  for (int ip = 0; ip < h->np; ip++)
+    if (!h->slab_set[ip]) return h->fail(EPW_EINVAL, std::string(who) + ": g(Re,Rp) slab missing");
   return EPW_OK;
 }
 
@@ -461,18 +526,57 @@ int epw_interp_interpolate(epw_interp_t h, const double *k_list, int64_t nk, con
                            const int32_t *kq_map, double *eps_k, double *eps_kq, double *omega_q, double *g2,
                            void *cuda_stream) {
   if (!h) return EPW_EINVAL;
-  if (!k_list || !q_list || !eps_k || !omega_q || !g2 || nk <= 0 || nq <= 0)
-    return h->fail(EPW_EINVAL, "epw_interp_interpolate: null pointer or non-positive nk/nq");
-  if (!h->operators_set) return h->fail(EPW_EINVAL, "epw_interp_interpolate: operators not set");
-  for (int ip = 0; ip < h->np; ip++)
-    if (!h->slab_set[ip]) return h->fail(EPW_EINVAL, "epw_interp_interpolate: g(Re,Rp) slab missing");
+  const int rc = check_interpolate_args(h, k_list, nk, q_list, nq, eps_k, omega_q, g2, "epw_interp_interpolate");
+  if (rc != EPW_OK) return rc;
   CU_OR_FAIL(h, cudaSetDevice(h->cfg.device), "cudaSetDevice");
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
   h->last_stream = st;
   h->launches = 0;
+  h->last_kmode = 0;
   if (use_large_path(h))
     return interpolate_large(h, k_list, nk, q_list, nq, kq_map, eps_k, eps_kq, omega_q, g2, st);
+  return interpolate_small(h, k_list, nullptr, nk, q_list, nq, kq_map, eps_k, eps_kq, omega_q, g2, st);
+}
 
+int epw_interp_interpolate_grid(epw_interp_t h, const int32_t *k_grid, const double *k_shift, const double *q_list,
+                                int64_t nq, const int32_t *kq_map, double *eps_k, double *eps_kq, double *omega_q,
+                                double *g2, void *cuda_stream) {
+  if (!h) return EPW_EINVAL;
+  if (!k_grid || k_grid[0] <= 0 || k_grid[1] <= 0 || k_grid[2] <= 0)
+    return h->fail(EPW_EINVAL, "epw_interp_interpolate_grid: k_grid must hold three positive sizes");
+  GridSpec g;
+  for (int d = 0; d < 3; d++) {
+    g.N[d] = k_grid[d];
+    g.s[d] = k_shift ? k_shift[d] : 0.0;
+  }
+  const int64_t nk = (int64_t)g.N[0] * g.N[1] * g.N[2];
+  const int rc = check_interpolate_args(h, k_grid, nk, q_list, nq, eps_k, omega_q, g2, "epw_interp_interpolate_grid");
+  if (rc != EPW_OK) return rc;
+  CU_OR_FAIL(h, cudaSetDevice(h->cfg.device), "cudaSetDevice");
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  h->last_stream = st;
+  h->launches = 0;
+  if (use_large_path(h)) {
+    // the large-Nb kernels take a k-list (their grids are one-dimensional: nothing to factorise)
+    h->last_kmode = 0;
+    CU_OR_FAIL(h, h->klist_gen.reserve(sizeof(double) * 3 * (size_t)nk), "cudaMalloc k-list");
+    LAUNCH(h, launch_grid_klist(g.N, g.s, h->klist_gen.as<double>(), st), "grid k-list");
+    return interpolate_large(h, h->klist_gen.as<double>(), nk, q_list, nq, kq_map, eps_k, eps_kq, omega_q, g2, st);
+  }
+  h->last_kmode = 1;
+  return interpolate_small(h, nullptr, &g, nk, q_list, nq, kq_map, eps_k, eps_kq, omega_q, g2, st);
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------
+// Small-Nb path (Nb <= 16; BASELINE.json configs[0..3]).  k-points come either as a list (dense S2: one FP64
+// tensor-path contraction over all Re, zgemm_dmma.cu) or as a uniform grid (factorised S2: one contraction per
+// crystal axis, re_to_k_grid.cu); everything after S2 is shared.
+// ---------------------------------------------------------------------------------------------------------
+static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec *grid, int64_t nk, const double *q_list,
+                             int64_t nq, const int32_t *kq_map, double *eps_k, double *eps_kq, double *omega_q,
+                             double *g2, cudaStream_t st) {
   const int nb = h->nb, nm = h->nm, ne = h->ne, np = h->np, nbb = h->nbb, nmm = h->nmm;
   const int ncols_g = nbb * nm;
   const int ncols_h = kq_map ? 0 : nbb;
@@ -483,23 +587,64 @@ int epw_interp_interpolate(epw_interp_t h, const double *k_list, int64_t nk, con
   const int64_t MT = ceil_div(nk, GEMM_BM);
   const int QB = (int)std::min<int64_t>(h->q_batch, nq);
   const int64_t E = (int64_t)ncols_g;
+  const size_t cap = h->cfg.workspace_bytes ? h->cfg.workspace_bytes : ((size_t)6 << 30);
 
-  // k-chunk: one chunk of [g~ | H(k+q)] (16*ncols bytes per k) must stay L2-resident for the eigensolve and the
-  // rotation that follow it, and its tile count should fill whole waves of the persistent contraction kernel
-  // (the thread-per-matrix eigensolver of the per-pair H(k+q) solves needs tens of thousands of matrices per launch to
-  // fill the GPU; it is worth more than L2 residency of the chunk: 16*ncols bytes per k written and read once more
-  // from HBM is a few per cent of the S2 time)
-  const size_t chunk_budget = (!kq_map && (eigh_thread_supported(nb) || eigh_cols_supported(nb))) ? ((size_t)512 << 20) : ((size_t)64 << 20);
-  const int64_t kchunk =
-      choose_mtiles_per_chunk(NT, h->num_sms, (size_t)GEMM_BM * ncols * 16, MT, chunk_budget) * GEMM_BM;
-  // rows of the g~ buffer kept (all of nk when it fits the cap; else a multiple of kchunk that is reused)
-  size_t cap = h->cfg.workspace_bytes ? h->cfg.workspace_bytes : ((size_t)6 << 30);
-  int64_t c_rows = MT * GEMM_BM;
-  if ((size_t)c_rows * ncols * 16 > cap) c_rows = std::max<int64_t>(kchunk, (int64_t)(cap / ((size_t)ncols * 16)) / kchunk * kchunk);
+  int64_t kchunk, c_rows;
+  // grid mode: extents of the three axis passes (re_to_k_grid.cu)
+  const int *L = h->box_L;
+  int64_t slab = 0;          // k-points per i1 plane
+  int cs = 0, nchunks = 1;   // i1 planes per k-chunk
+  int KB1 = 0, NTc = 0;
+  if (!grid) {
+    // k-chunk: one chunk of [g~ | H(k+q)] (16*ncols bytes per k) must stay L2-resident for the eigensolve and the
+    // rotation that follow it, and its tile count should fill whole waves of the persistent contraction kernel
+    // (the thread-per-matrix eigensolver of the per-pair H(k+q) solves needs tens of thousands of matrices per launch
+    // to fill the GPU; it is worth more than L2 residency of the chunk: 16*ncols bytes per k written and read once
+    // more from HBM is a few per cent of the S2 time)
+    const size_t chunk_budget =
+        (!kq_map && (eigh_thread_supported(nb) || eigh_cols_supported(nb))) ? ((size_t)512 << 20) : ((size_t)64 << 20);
+    kchunk = choose_mtiles_per_chunk(NT, h->num_sms, (size_t)GEMM_BM * ncols * 16, MT, chunk_budget) * GEMM_BM;
+    // rows of the g~ buffer kept (all of nk when it fits the cap; else a multiple of kchunk that is reused)
+    c_rows = MT * GEMM_BM;
+    if ((size_t)c_rows * ncols * 16 > cap)
+      c_rows = std::max<int64_t>(kchunk, (int64_t)(cap / ((size_t)ncols * 16)) / kchunk * kchunk);
+  } else {
+    // k-chunk = whole i1 planes.  The last axis pass writes 64 complex columns (i1 values) per tile: prefer chunks of
+    // a multiple of 64 planes (or all of them); 512 MB of [g~ | H(k+q)] per chunk unless that gives fewer than 16 planes.
+    slab = (int64_t)grid->N[1] * grid->N[2];
+    const size_t plane_bytes = (size_t)slab * ncols * 16;
+    int64_t fit = (int64_t)(std::min(cap, (size_t)512 << 20) / plane_bytes);
+    if (fit < 16 && cap > ((size_t)512 << 20)) fit = std::min<int64_t>(64, (int64_t)(cap / plane_bytes));
+    if (fit < 1) return h->fail(EPW_ENOMEM, "epw_interp_interpolate_grid: workspace_bytes too small for one i1 plane of g~");
+    if (fit >= grid->N[0]) fit = grid->N[0];
+    else if (fit > 64) fit = fit / 64 * 64;
+    cs = (int)fit;
+    nchunks = (int)ceil_div(grid->N[0], cs);
+    kchunk = cs * slab;
+    c_rows = nchunks == 1 ? nk : kchunk;
+    KB1 = (int)ceil_div(2 * (int64_t)L[0], GEMM_BK);
+    NTc = (int)ceil_div(2 * (int64_t)cs, GEMM_BN);
+  }
 
   // ---- workspace ----
-  CU_OR_FAIL(h, h->Apack.reserve(sizeof(double) * (size_t)MT * KB * GEMM_CHUNK), "cudaMalloc Apack");
-  CU_OR_FAIL(h, h->BpackH.reserve(sizeof(double) * (size_t)NTH * KB * GEMM_CHUNK), "cudaMalloc BpackH");
+  if (!grid) {
+    CU_OR_FAIL(h, h->Apack.reserve(sizeof(double) * (size_t)MT * KB * GEMM_CHUNK), "cudaMalloc Apack");
+    CU_OR_FAIL(h, h->BpackH.reserve(sizeof(double) * (size_t)NTH * KB * GEMM_CHUNK), "cudaMalloc BpackH");
+    CU_OR_FAIL(h, h->Bpack.reserve(sizeof(double) * (size_t)QB * NT * KB * GEMM_CHUNK), "cudaMalloc Bpack");
+  } else {
+    const int nc = std::max(ncols, nbb);
+    const int maxN = std::max(std::max(grid->N[0], grid->N[1]), grid->N[2]);
+    const int maxL = std::max(std::max(L[0], L[1]), L[2]);
+    CU_OR_FAIL(h, h->X.reserve(sizeof(c128) * (size_t)h->box_size * nc), "cudaMalloc X");
+    CU_OR_FAIL(h, h->T1.reserve(sizeof(c128) * (size_t)L[0] * L[1] * grid->N[2] * nc), "cudaMalloc T1");
+    CU_OR_FAIL(h, h->T2.reserve(sizeof(c128) * (size_t)L[0] * slab * nc), "cudaMalloc T2");
+    CU_OR_FAIL(h, h->Ptmp.reserve(sizeof(c128) * (size_t)maxL * maxN), "cudaMalloc axis phases");
+    CU_OR_FAIL(h, h->P3pack.reserve(sizeof(double) * (size_t)ceil_div(2 * (int64_t)grid->N[2], GEMM_BN) *
+                                    ceil_div(2 * (int64_t)L[2], GEMM_BK) * GEMM_CHUNK), "cudaMalloc P3pack");
+    CU_OR_FAIL(h, h->P2pack.reserve(sizeof(double) * (size_t)ceil_div(2 * (int64_t)grid->N[1], GEMM_BN) *
+                                    ceil_div(2 * (int64_t)L[1], GEMM_BK) * GEMM_CHUNK), "cudaMalloc P2pack");
+    CU_OR_FAIL(h, h->P1pack.reserve(sizeof(double) * (size_t)nchunks * NTc * KB1 * GEMM_CHUNK), "cudaMalloc P1pack");
+  }
   CU_OR_FAIL(h, h->Hk.reserve(sizeof(c128) * (size_t)nk * nbb), "cudaMalloc Hk");
   CU_OR_FAIL(h, h->Uk.reserve(sizeof(c128) * (size_t)nk * nbb), "cudaMalloc Uk");
   CU_OR_FAIL(h, h->Pq.reserve(sizeof(c128) * (size_t)QB * np), "cudaMalloc Pq");
@@ -507,7 +652,6 @@ int epw_interp_interpolate(epw_interp_t h, const double *k_list, int64_t nk, con
   CU_OR_FAIL(h, h->Dq.reserve(sizeof(c128) * (size_t)QB * nmm), "cudaMalloc Dq");
   CU_OR_FAIL(h, h->eq.reserve(sizeof(c128) * (size_t)QB * nmm), "cudaMalloc e_q");
   CU_OR_FAIL(h, h->g1.reserve(sizeof(c128) * (size_t)QB * h->rows), "cudaMalloc g(Re,q)");
-  CU_OR_FAIL(h, h->Bpack.reserve(sizeof(double) * (size_t)QB * NT * KB * GEMM_CHUNK), "cudaMalloc Bpack");
   CU_OR_FAIL(h, h->C.reserve(sizeof(c128) * (size_t)c_rows * ncols), "cudaMalloc g~");
   if (!kq_map) CU_OR_FAIL(h, h->Ukq.reserve(sizeof(c128) * (size_t)c_rows * nbb), "cudaMalloc Ukq");
   if (!kq_map && !eps_kq) CU_OR_FAIL(h, h->epskq_scratch.reserve(sizeof(double) * (size_t)c_rows * nb), "cudaMalloc eps scratch");
@@ -524,24 +668,76 @@ int epw_interp_interpolate(epw_interp_t h, const double *k_list, int64_t nk, con
   h->last_qb = QB;
   h->last_kchunk = kchunk;
 
+  // the two leading axis passes of the factorised S2: X [L1][L2][L3][nc] -> T1 [L1][L2][N3][nc] -> T2 [L1][N2][N3][nc]
+  auto grid_pass_ab = [&](int nc) -> cudaError_t {
+    const int64_t N2 = grid->N[1], N3 = grid->N[2];
+    cudaError_t e = launch_zgemm_strided(h->X.as<c128>(), nc, (int64_t)L[2] * nc, nc, 0, h->P3pack.as<double>(), nullptr,
+                                         h->T1.p, nc, N3 * nc, 1, nc, 0, 0, (int64_t)L[0] * L[1] * nc, (int)N3, L[2], 1,
+                                         h->num_sms, st);
+    if (e != cudaSuccess) return e;
+    h->launches++;
+    return launch_zgemm_strided(h->T1.as<c128>(), N3 * nc, (int64_t)L[1] * N3 * nc, N3 * nc, 0, h->P2pack.as<double>(),
+                                nullptr, h->T2.p, N3 * nc, N2 * N3 * nc, 1, N3 * nc, 0, 0, (int64_t)L[0] * N3 * nc,
+                                (int)N2, L[1], 1, h->num_sms, st);
+  };
+  // the last axis pass for the i1 planes of chunk ci: T2 -> out [i1][i2][i3][nc]
+  auto grid_pass_c = [&](int nc, int ci, c128 *out) -> cudaError_t {
+    const int cnt = std::min(cs, grid->N[0] - ci * cs);
+    const int64_t Mrows = slab * nc;
+    return launch_zgemm_strided(h->T2.as<c128>(), Mrows, 0, Mrows, 0,
+                                h->P1pack.as<double>() + (int64_t)ci * NTc * KB1 * GEMM_CHUNK, nullptr, out, Mrows, 0, 1,
+                                Mrows, 0, 0, Mrows, cnt, L[0], 1, h->num_sms, st);
+  };
+
   const int t_total = h->begin_span(7, st);
 
-  // ---- k side (once per call): S0 phases in packed-A form, H(k) by the same DMMA contraction, eigensolve ----
+  // ---- k side (once per call): S0 phases, H(k) by the same contraction as S2, eigensolve ----
   int sp = h->begin_span(0, st);
-  LAUNCH(h, launch_phase_pack_a(k_list, nk, h->Re.as<int32_t>(), h->we.as<double>(), ne, h->Apack.as<double>(), st),
-         "phase_pack_a");
+  if (!grid) {
+    LAUNCH(h, launch_phase_pack_a(k_list, nk, h->Re.as<int32_t>(), h->we.as<double>(), ne, h->Apack.as<double>(), st),
+           "phase_pack_a");
+  } else {
+    // one small phase table per crystal axis, packed as the B operand of its pass
+    struct Axis { int d; DevBuf *pack; };
+    const Axis ax[2] = {{2, &h->P3pack}, {1, &h->P2pack}};
+    for (const Axis &a : ax) {
+      LAUNCH(h, launch_grid_axis_phase(grid->N[a.d], 0, grid->N[a.d], grid->s[a.d], h->box_lo[a.d], L[a.d],
+                                       h->Ptmp.as<c128>(), st), "axis phases");
+      LAUNCH(h, launch_pack_b_strided(h->Ptmp.as<c128>(), grid->N[a.d], 1, 0, 1, 0, nullptr, 0.0, L[a.d], grid->N[a.d],
+                                      a.pack->as<double>(), st), "pack axis phases");
+    }
+    for (int ci = 0; ci < nchunks; ci++) {
+      const int cnt = std::min(cs, grid->N[0] - ci * cs);
+      LAUNCH(h, launch_grid_axis_phase(grid->N[0], ci * cs, cnt, grid->s[0], h->box_lo[0], L[0], h->Ptmp.as<c128>(), st),
+             "axis phases");
+      LAUNCH(h, launch_pack_b_strided(h->Ptmp.as<c128>(), cnt, 1, 0, 1, 0, nullptr, 0.0, L[0], cnt,
+                                      h->P1pack.as<double>() + (int64_t)ci * NTc * KB1 * GEMM_CHUNK, st),
+             "pack axis phases");
+    }
+  }
   h->end_span(sp, st);
   sp = h->begin_span(3, st);
-  LAUNCH(h,
-         launch_pack_b(nullptr, nullptr, nullptr, 0.0, h->H.as<c128>(), nullptr, nbb, nm, ne, 0, nbb,
-                       h->BpackH.as<double>(), st),
-         "pack_b(H)");
-  LAUNCH(h, launch_zgemm_dmma(h->Apack.as<double>(), h->BpackH.as<double>(), h->Hk.as<c128>(), nk, nbb, KB, nbb,
-                              h->num_sms, st),
-         "zgemm H(k)");
+  if (!grid) {
+    LAUNCH(h,
+           launch_pack_b(nullptr, nullptr, nullptr, 0.0, h->H.as<c128>(), nullptr, nbb, nm, ne, 0, nbb,
+                         h->BpackH.as<double>(), st),
+           "pack_b(H)");
+    LAUNCH(h, launch_zgemm_dmma(h->Apack.as<double>(), h->BpackH.as<double>(), h->Hk.as<c128>(), nk, nbb, KB, nbb,
+                                h->num_sms, st),
+           "zgemm H(k)");
+  } else {
+    LAUNCH(h, launch_box_scatter(nullptr, nullptr, nullptr, 0.0, h->H.as<c128>(), nullptr, h->we.as<double>(),
+                                 h->boxidx.as<int32_t>(), h->box_size, nbb, nm, ne, 0, nbb, h->X.as<c128>(), st),
+           "box_scatter(H)");
+    LAUNCH(h, grid_pass_ab(nbb), "grid passes H(k)");
+    for (int ci = 0; ci < nchunks; ci++)
+      LAUNCH(h, grid_pass_c(nbb, ci, h->Hk.as<c128>() + (int64_t)ci * kchunk * nbb), "grid pass H(k)");
+  }
+  h->count_into(0);
   LAUNCH(h, launch_eigh_batched(h->Hk.as<c128>(), nbb, nb, nk, eps_k, h->Uk.as<c128>(), 0, h->status.as<int32_t>(),
                                 h->eig_scratch.as<c128>(), st),
          "eigh H(k)");
+  h->count_into(-1);
   h->end_span(sp, st);
 
   for (int64_t q0 = 0; q0 < nq; q0 += QB) {
@@ -559,35 +755,55 @@ int epw_interp_interpolate(epw_interp_t h, const double *k_list, int64_t nk, con
     sp = h->begin_span(1, st);
     LAUNCH(h, launch_rp_to_q(h->g.as<c128>(), h->rows, np, h->Pq.as<c128>(), qb, h->g1.as<c128>(), st), "rp_to_q");
     h->end_span(sp, st);
-    // ---- phonons: D(q), eigensolve, S4a hoisted into the packed B operand ----
+    // ---- phonons: D(q), eigensolve, S4a hoisted into the B operand of S2 ----
     sp = h->begin_span(2, st);
     LAUNCH(h, launch_interp_operator(h->D.as<c128>(), nm, np, h->Pq.as<c128>(), qb, h->Dq.as<c128>(), st), "D(q)");
+    h->count_into(2);
     LAUNCH(h, launch_eigh_batched(h->Dq.as<c128>(), nmm, nm, qb, omega_q + q0 * nm, h->eq.as<c128>(), 1,
                                   h->status.as<int32_t>(), h->eig_scratch.as<c128>(), st),
            "eigh D(q)");
+    h->count_into(-1);
     h->end_span(sp, st);
-    sp = h->begin_span(8, st);
-    for (int iq = 0; iq < qb; iq++)
-      LAUNCH(h,
-             launch_pack_b(h->g1.as<c128>() + (int64_t)iq * h->rows, h->eq.as<c128>() + (int64_t)iq * nmm,
-                           omega_q + (q0 + iq) * nm, h->cfg.omega_min, h->H.as<c128>(),
-                           ncols_h ? h->Pqe.as<c128>() + (int64_t)iq * ne : nullptr, nbb, nm, ne, ncols_g, ncols_h,
-                           h->Bpack.as<double>() + (int64_t)iq * NT * KB * GEMM_CHUNK, st),
-             "pack_b");
-    h->end_span(sp, st);
+    if (!grid) {
+      sp = h->begin_span(8, st);
+      for (int iq = 0; iq < qb; iq++)
+        LAUNCH(h,
+               launch_pack_b(h->g1.as<c128>() + (int64_t)iq * h->rows, h->eq.as<c128>() + (int64_t)iq * nmm,
+                             omega_q + (q0 + iq) * nm, h->cfg.omega_min, h->H.as<c128>(),
+                             ncols_h ? h->Pqe.as<c128>() + (int64_t)iq * ne : nullptr, nbb, nm, ne, ncols_g, ncols_h,
+                             h->Bpack.as<double>() + (int64_t)iq * NT * KB * GEMM_CHUNK, st),
+               "pack_b");
+      h->end_span(sp, st);
+    }
 
     for (int iq = 0; iq < qb; iq++) {
       const int64_t q = q0 + iq;
-      const double *Bq = h->Bpack.as<double>() + (int64_t)iq * NT * KB * GEMM_CHUNK;
+      const double *Bq = grid ? nullptr : h->Bpack.as<double>() + (int64_t)iq * NT * KB * GEMM_CHUNK;
+      if (grid) {
+        sp = h->begin_span(8, st);
+        LAUNCH(h, launch_box_scatter(h->g1.as<c128>() + (int64_t)iq * h->rows, h->eq.as<c128>() + (int64_t)iq * nmm,
+                                     omega_q + q * nm, h->cfg.omega_min, h->H.as<c128>(),
+                                     ncols_h ? h->Pqe.as<c128>() + (int64_t)iq * ne : nullptr, h->we.as<double>(),
+                                     h->boxidx.as<int32_t>(), h->box_size, nbb, nm, ne, ncols_g, ncols_h,
+                                     h->X.as<c128>(), st),
+               "box_scatter");
+        h->end_span(sp, st);
+        sp = h->begin_span(4, st);
+        LAUNCH(h, grid_pass_ab(ncols), "grid passes S2");
+        h->end_span(sp, st);
+      }
       for (int64_t k0 = 0; k0 < nk; k0 += kchunk) {
         const int64_t kn = std::min(kchunk, nk - k0);
         const int64_t crow = k0 % c_rows;
         c128 *Cc = h->C.as<c128>() + crow * ncols;
         // ---- S2: Re -> k contraction (+ H(k+q) columns) ----
         sp = h->begin_span(4, st);
-        LAUNCH(h, launch_zgemm_dmma(h->Apack.as<double>() + (k0 / GEMM_BM) * (int64_t)KB * GEMM_CHUNK, Bq, Cc, kn, ncols,
-                                    KB, ncols, h->num_sms, st),
-               "zgemm S2");
+        if (!grid)
+          LAUNCH(h, launch_zgemm_dmma(h->Apack.as<double>() + (k0 / GEMM_BM) * (int64_t)KB * GEMM_CHUNK, Bq, Cc, kn, ncols,
+                                      KB, ncols, h->num_sms, st),
+                 "zgemm S2");
+        else
+          LAUNCH(h, grid_pass_c(ncols, (int)(k0 / kchunk), Cc), "grid pass S2");
         h->end_span(sp, st);
         const c128 *Ukq_ptr;
         const int32_t *kq_idx = nullptr;
@@ -607,9 +823,11 @@ int epw_interp_interpolate(epw_interp_t h, const double *k_list, int64_t nk, con
           sp = h->begin_span(5, st);
           c128 *Ukq_c = h->Ukq.as<c128>() + crow * nbb;
           double *eps_dst = eps_kq ? eps_kq + (q * nk + k0) * nb : h->epskq_scratch.as<double>() + crow * nb;
+          h->count_into(1);
           LAUNCH(h, launch_eigh_batched(Cc + ncols_g, ncols, nb, kn, eps_dst, Ukq_c, 0, h->status.as<int32_t>(),
                                         h->eig_scratch.as<c128>(), st),
                  "eigh H(k+q)");
+          h->count_into(-1);
           h->end_span(sp, st);
           Ukq_ptr = Ukq_c;
         }
@@ -626,6 +844,8 @@ int epw_interp_interpolate(epw_interp_t h, const double *k_list, int64_t nk, con
   return EPW_OK;
 }
 
+extern "C" {
+
 int epw_interp_sync(epw_interp_t h) {
   if (!h) return EPW_EINVAL;
   CU_OR_FAIL(h, cudaSetDevice(h->cfg.device), "cudaSetDevice");
@@ -638,30 +858,35 @@ int epw_interp_sync(epw_interp_t h) {
   return EPW_OK;
 }
 
-int epw_interp_interpolate_host(epw_interp_t h, const double *k_list, int64_t nk, const double *q_list, int64_t nq,
-                                const int32_t *kq_map, double *eps_k, double *eps_kq, double *omega_q, double *g2,
-                                void *cuda_stream) {
+static int interpolate_host_impl(epw_interp_t h, const double *k_list, const int32_t *k_grid, const double *k_shift,
+                                 int64_t nk, const double *q_list, int64_t nq, const int32_t *kq_map, double *eps_k,
+                                 double *eps_kq, double *omega_q, double *g2, void *cuda_stream) {
   if (!h) return EPW_EINVAL;
-  if (!k_list || !q_list || !eps_k || !omega_q || !g2 || nk <= 0 || nq <= 0)
+  if ((!k_list && !k_grid) || !q_list || !eps_k || !omega_q || !g2 || nk <= 0 || nq <= 0)
     return h->fail(EPW_EINVAL, "epw_interp_interpolate_host: null pointer or non-positive nk/nq");
   CU_OR_FAIL(h, cudaSetDevice(h->cfg.device), "cudaSetDevice");
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
   const size_t E = (size_t)h->nbb * h->nm;
-  CU_OR_FAIL(h, h->hs_k.reserve(sizeof(double) * 3 * nk), "cudaMalloc k staging");
+  if (k_list) CU_OR_FAIL(h, h->hs_k.reserve(sizeof(double) * 3 * nk), "cudaMalloc k staging");
   CU_OR_FAIL(h, h->hs_q.reserve(sizeof(double) * 3 * nq), "cudaMalloc q staging");
   if (kq_map) CU_OR_FAIL(h, h->hs_map.reserve(sizeof(int32_t) * nk * nq), "cudaMalloc kq_map staging");
   CU_OR_FAIL(h, h->hs_epsk.reserve(sizeof(double) * nk * h->nb), "cudaMalloc eps_k staging");
   if (eps_kq) CU_OR_FAIL(h, h->hs_epskq.reserve(sizeof(double) * nk * nq * h->nb), "cudaMalloc eps_kq staging");
   CU_OR_FAIL(h, h->hs_omega.reserve(sizeof(double) * nq * h->nm), "cudaMalloc omega staging");
   CU_OR_FAIL(h, h->hs_g2.reserve(sizeof(double) * E * nk * nq), "cudaMalloc g2 staging");
-  CU_OR_FAIL(h, cudaMemcpyAsync(h->hs_k.p, k_list, sizeof(double) * 3 * nk, cudaMemcpyHostToDevice, st), "H2D k");
+  if (k_list)
+    CU_OR_FAIL(h, cudaMemcpyAsync(h->hs_k.p, k_list, sizeof(double) * 3 * nk, cudaMemcpyHostToDevice, st), "H2D k");
   CU_OR_FAIL(h, cudaMemcpyAsync(h->hs_q.p, q_list, sizeof(double) * 3 * nq, cudaMemcpyHostToDevice, st), "H2D q");
   if (kq_map)
     CU_OR_FAIL(h, cudaMemcpyAsync(h->hs_map.p, kq_map, sizeof(int32_t) * nk * nq, cudaMemcpyHostToDevice, st), "H2D map");
-  const int rc = epw_interp_interpolate(h, h->hs_k.as<double>(), nk, h->hs_q.as<double>(), nq,
-                                        kq_map ? h->hs_map.as<int32_t>() : nullptr, h->hs_epsk.as<double>(),
-                                        eps_kq ? h->hs_epskq.as<double>() : nullptr, h->hs_omega.as<double>(),
-                                        h->hs_g2.as<double>(), cuda_stream);
+  const int32_t *map_d = kq_map ? h->hs_map.as<int32_t>() : nullptr;
+  double *epskq_d = eps_kq ? h->hs_epskq.as<double>() : nullptr;
+  const int rc = k_list ? epw_interp_interpolate(h, h->hs_k.as<double>(), nk, h->hs_q.as<double>(), nq, map_d,
+                                                 h->hs_epsk.as<double>(), epskq_d, h->hs_omega.as<double>(),
+                                                 h->hs_g2.as<double>(), cuda_stream)
+                        : epw_interp_interpolate_grid(h, k_grid, k_shift, h->hs_q.as<double>(), nq, map_d,
+                                                      h->hs_epsk.as<double>(), epskq_d, h->hs_omega.as<double>(),
+                                                      h->hs_g2.as<double>(), cuda_stream);
   if (rc != EPW_OK) return rc;
   CU_OR_FAIL(h, cudaMemcpyAsync(eps_k, h->hs_epsk.p, sizeof(double) * nk * h->nb, cudaMemcpyDeviceToHost, st), "D2H eps_k");
   if (eps_kq)
@@ -670,6 +895,24 @@ int epw_interp_interpolate_host(epw_interp_t h, const double *k_list, int64_t nk
   CU_OR_FAIL(h, cudaMemcpyAsync(omega_q, h->hs_omega.p, sizeof(double) * nq * h->nm, cudaMemcpyDeviceToHost, st), "D2H omega");
   CU_OR_FAIL(h, cudaMemcpyAsync(g2, h->hs_g2.p, sizeof(double) * E * nk * nq, cudaMemcpyDeviceToHost, st), "D2H g2");
   return epw_interp_sync(h);
+}
+
+int epw_interp_interpolate_host(epw_interp_t h, const double *k_list, int64_t nk, const double *q_list, int64_t nq,
+                                const int32_t *kq_map, double *eps_k, double *eps_kq, double *omega_q, double *g2,
+                                void *cuda_stream) {
+  if (h && !k_list) return h->fail(EPW_EINVAL, "epw_interp_interpolate_host: null k_list");
+  return interpolate_host_impl(h, k_list, nullptr, nullptr, nk, q_list, nq, kq_map, eps_k, eps_kq, omega_q, g2,
+                               cuda_stream);
+}
+
+int epw_interp_interpolate_grid_host(epw_interp_t h, const int32_t *k_grid, const double *k_shift, const double *q_list,
+                                     int64_t nq, const int32_t *kq_map, double *eps_k, double *eps_kq, double *omega_q,
+                                     double *g2, void *cuda_stream) {
+  if (!h) return EPW_EINVAL;
+  if (!k_grid || k_grid[0] <= 0 || k_grid[1] <= 0 || k_grid[2] <= 0)
+    return h->fail(EPW_EINVAL, "epw_interp_interpolate_grid_host: k_grid must hold three positive sizes");
+  return interpolate_host_impl(h, nullptr, k_grid, k_shift, (int64_t)k_grid[0] * k_grid[1] * k_grid[2], q_list, nq, kq_map,
+                               eps_k, eps_kq, omega_q, g2, cuda_stream);
 }
 
 int epw_interp_get_stage_times(epw_interp_t h, double *ms, int n) {
@@ -696,10 +939,23 @@ int epw_interp_get_stage_launches(epw_interp_t h, int64_t *counts, int n) {
 
 int64_t epw_interp_last_launch_count(epw_interp_t h) { return h ? h->launches : 0; }
 
+int epw_interp_get_eigh_rotations(epw_interp_t h, uint64_t *counts, int n) {
+  if (!h || !counts || n <= 0) return EPW_EINVAL;
+  const int m = std::min(n, 3);
+  for (int i = 0; i < m; i++) counts[i] = 0;
+  if (!h->workctr.p) return m;
+  CU_OR_FAIL(h, cudaSetDevice(h->cfg.device), "cudaSetDevice");
+  CU_OR_FAIL(h, cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize");
+  unsigned long long v[3];
+  CU_OR_FAIL(h, cudaMemcpy(v, h->workctr.p, sizeof(v), cudaMemcpyDeviceToHost), "cudaMemcpy work counters");
+  for (int i = 0; i < m; i++) counts[i] = v[i];
+  return m;
+}
+
 int epw_interp_last_plan(epw_interp_t h, int64_t *plan, int n) {
   if (!h || !plan || n <= 0) return EPW_EINVAL;
-  const int64_t v[3] = {h->last_path, h->last_qb, h->last_kchunk};
-  const int m = std::min(n, 3);
+  const int64_t v[4] = {h->last_path, h->last_qb, h->last_kchunk, h->last_kmode};
+  const int m = std::min(n, 4);
   for (int i = 0; i < m; i++) plan[i] = v[i];
   return m;
 }

@@ -4,7 +4,8 @@
 // Two-sided cyclic Jacobi, A <- J^dagger A J, V <- V J, on a Hermitian matrix held in PACKED form: the real diagonal
 // d[i] and the strict upper triangle u[i][j] = a_ij (i < j); a_ji = conj(a_ij) is implied, so one plane rotation costs
 // (n-2) column-pair updates for A instead of the 2n of the full row + column pass, plus n for the rows of V.
-//   a_pq = r e^{i phi}, tau = (a_qq - a_pp)/(2r), t = sgn(tau)/(|tau| + sqrt(1 + tau^2)), c = 1/sqrt(1 + t^2), s = t c,
+//   a_pq = r e^{i phi}, tau = (a_qq - a_pp)/(2r), t = sgn(tau)/(|tau| + sqrt(1 + tau^2)), c = 1/sqrt(1 + t^2), s = t c
+//   (evaluated in the equivalent half-angle form, see jacobi_rotate_packed),
 //   S = s e^{i phi},  J = [[c, S], [-conj(S), c]] on rows/columns (p, q)           (same convention as eigh_jacobi.cu)
 //   a_pp <- a_pp - t r,  a_qq <- a_qq + t r,  a_pq <- 0,
 //   (a_jp, a_jq) <- (c a_jp - conj(S) a_jq,  S a_jp + c a_jq)   for every j not in {p, q},
@@ -60,18 +61,19 @@ __host__ __device__ __forceinline__ PlaneRot jacobi_rotate_packed(double (&d)[N]
   const c128 apq = u[p][q];
   const double r2 = fma(apq.x, apq.x, apq.y * apq.y);
   const bool live = r2 >= 1e-280;
-  const double inv_r = jp_rsqrt(live ? r2 : 1.0);
-  const double r = r2 * inv_r;
-  const double tau = 0.5 * (d[q] - d[p]) * inv_r;
-  const double w = sqrt(fma(tau, tau, 1.0));
-  const double t = copysign(1.0 / (fabs(tau) + w), tau);
-  const double c = jp_rsqrt(fma(t, t, 1.0));
-  const double sor = t * c * inv_r;
+  // half-angle form of the same rotation (tan 2 theta = r / a, |theta| <= pi/4): two dependent rsqrt instead of
+  // rsqrt -> sqrt -> divide -> rsqrt, and no subtraction anywhere (cos 2 theta in [0,1], x in [1/2, 1]):
+  //   h = 1/sqrt(a^2 + r^2), cos 2theta = |a| h, c = sqrt(x), x = (1 + cos 2theta)/2, S = sgn(a) a_pq h / (2c), t r = sgn(a) r^2 h / (2x)
+  const double a = 0.5 * (d[q] - d[p]);
+  const double h = jp_rsqrt(live ? fma(a, a, r2) : 1.0);
+  const double x = fma(0.5 * fabs(a), h, 0.5);
+  const double rc = jp_rsqrt(x);
+  const double sor = copysign(0.5 * h * rc, a);
   PlaneRot R;
-  R.c = live ? c : 1.0;
+  R.c = live ? x * rc : 1.0;
   R.sr = live ? sor * apq.x : 0.0;
   R.si = live ? sor * apq.y : 0.0;
-  const double tr = live ? t * r : 0.0;
+  const double tr = live ? copysign(0.5 * r2 * h * (rc * rc), a) : 0.0;
   d[p] -= tr;
   d[q] += tr;
   if (live) u[p][q] = make_double2(0.0, 0.0);

@@ -345,7 +345,9 @@ def test_rotate_g2_large(epw):
 # ---------------------------------------------------------------------------------------------------------
 # whole path
 # ---------------------------------------------------------------------------------------------------------
-def run_gpu(epw, w, k_list, q_list, kq_map=None, q_batch=0, host_api=False, path=0, workspace_bytes=0):
+def run_gpu(epw, w, k_list, q_list, kq_map=None, q_batch=0, host_api=False, path=0, workspace_bytes=0, grid=None,
+            shift=None):
+    """grid = (N1, N2, N3): call the uniform-grid entry point (k_list is then only used for its length)."""
     h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_, q_batch=q_batch, path=path, workspace_bytes=workspace_bytes)
     try:
         h.set_operators_from_host(w)
@@ -355,10 +357,18 @@ def run_gpu(epw, w, k_list, q_list, kq_map=None, q_batch=0, host_api=False, path
             eps_kq = np.empty((nq, nk, w.nbnd))
             om = np.empty((nq, w.nmodes))
             g2 = np.empty((nq, nk, w.nmodes, w.nbnd, w.nbnd))
-            epw.epw_interp_interpolate_host(h.h, np.ascontiguousarray(k_list), nk, np.ascontiguousarray(q_list), nq,
-                                            kq_map, eps_k, eps_kq, om, g2)
+            if grid is not None:
+                epw.epw_interp_interpolate_grid_host(h.h, grid, shift, np.ascontiguousarray(q_list), nq, kq_map, eps_k,
+                                                     eps_kq, om, g2)
+            else:
+                epw.epw_interp_interpolate_host(h.h, np.ascontiguousarray(k_list), nk, np.ascontiguousarray(q_list), nq,
+                                                kq_map, eps_k, eps_kq, om, g2)
             return eps_k, eps_kq, om, g2
-        out = h.interpolate(dev(k_list), dev(q_list), None if kq_map is None else dev(kq_map))
+        if grid is not None:
+            out = h.interpolate_grid(grid, dev(q_list), k_shift=shift, kq_map=None if kq_map is None else dev(kq_map))
+            assert epw.epw_interp_last_plan(h.h)["k_mode"] == ("list" if path == 2 or w.nbnd > 16 else "grid")
+        else:
+            out = h.interpolate(dev(k_list), dev(q_list), None if kq_map is None else dev(kq_map))
         epw.epw_interp_sync(h.h)
         return [None if t is None else t.cpu().numpy() for t in out]
     finally:
@@ -395,6 +405,67 @@ def test_reduced_shapes(epw, shape):
         w = synth.make_custom("odd", 5, 3, (1, 2, 0), 1.0, 0.1, 1.0, (9, 1, 17), ("random", 2, 3), seed=13)
     ref = oracle.interpolate(w.H_R, w.D_R, w.g_full(), w.Re, w.w_e, w.Rp, w.w_p, w.k_list, w.q_list)
     assert_path_close(run_gpu(epw, w, w.k_list, w.q_list), ref)
+
+
+# ---- uniform-grid entry point (factorised S2, csrc/re_to_k_grid.cu) ----------------------------------------
+def test_grid_config0_both_kq_modes_and_host_api(epw):
+    """configs[0] through epw_interp_interpolate_grid: all 4,096 pairs with kq_map, per-pair H(k+q), host buffers."""
+    w = synth.make_config(0)
+    ref = oracle.interpolate(w.H_R, w.D_R, w.g_full(), w.Re, w.w_e, w.Rp, w.w_p, w.k_list, w.q_list)
+    assert_path_close(run_gpu(epw, w, w.k_list, w.q_list, w.kq_map, grid=w.k_grid), ref)
+    assert_path_close(run_gpu(epw, w, w.k_list, w.q_list, None, grid=w.k_grid), ref)
+    ql = w.q_list[:5] + [0.01, 0.02, 0.03]
+    ref = oracle.interpolate(w.H_R, w.D_R, w.g_full(), w.Re, w.w_e, w.Rp, w.w_p, w.k_list, ql)
+    assert_path_close(run_gpu(epw, w, w.k_list, ql, None, grid=w.k_grid, host_api=True, q_batch=3), ref)
+
+
+@pytest.mark.parametrize("shape", ["si", "mos2", "odd", "chunks", "large-forced"])
+def test_grid_reduced_shapes(epw, shape):
+    """Reduced configs 1-3 through the grid entry point: ragged tiles in every axis pass, 2-D and skewed lattices,
+    several i1-plane chunks (workspace cap), and the large-Nb family (which expands the grid to a list)."""
+    ws, path = 0, 0
+    if shape == "si":
+        w = synth.make_custom("si-r", 8, 6, (2, 2, 2), 1.5, 0.1, 1.5, (7, 6, 5), ("random", 3, 3), seed=11)
+    elif shape == "mos2":
+        w = synth.make_custom("mos2-r", 11, 9, (3, 3, 0), 2.0, 0.1, 2.0, (15, 13, 1), ("random", 3, 2), seed=12)
+    elif shape == "odd":
+        w = synth.make_custom("odd", 5, 3, (1, 2, 0), 1.0, 0.1, 1.0, (9, 1, 17), ("random", 2, 3), seed=13)
+    elif shape == "chunks":
+        w = synth.make_custom("chunks", 4, 3, (1, 1, 1), 1.0, 0.1, 1.0, (11, 3, 4), ("random", 2, 3), seed=14)
+        ws = 16 * 12 * (16 * 3 + 16) * 3 + 100   # three i1 planes of [g~ | H(k+q)] per chunk -> 4 chunks, ragged last
+    else:
+        w = synth.make_custom("mos2-l", 11, 9, (2, 2, 0), 2.0, 0.1, 2.0, (13, 11, 1), ("random", 2, 2), seed=23)
+        path = 2
+    ref = oracle.interpolate(w.H_R, w.D_R, w.g_full(), w.Re, w.w_e, w.Rp, w.w_p, w.k_list, w.q_list)
+    assert_path_close(run_gpu(epw, w, w.k_list, w.q_list, grid=w.k_grid, workspace_bytes=ws, path=path), ref)
+
+
+def test_grid_shifted_and_sparse_lattice_list(epw):
+    """A shifted grid k = (i + s)/N and an Re list that is NOT a full box (vectors removed, order shuffled, non-unit
+    Wigner-Seitz weights): the box scatter must leave zeros where the list has no vector."""
+    w = synth.make_custom("sparse", 4, 3, (2, 1, 1), 1.0, 0.1, 1.0, (6, 5, 4), ("random", 2, 3), seed=31)
+    rng = np.random.default_rng(3)
+    keep = rng.permutation(w.ne)[: w.ne - 11]
+    g = np.ascontiguousarray(w.g_full()[:, :, keep])
+
+    class Sub:
+        nbnd, nmodes, ne, np_ = w.nbnd, w.nmodes, len(keep), w.np_
+        H_R, D_R = np.ascontiguousarray(w.H_R[keep]), w.D_R
+        Re, Rp, w_p = np.ascontiguousarray(w.Re[keep]), w.Rp, w.w_p
+        w_e = rng.uniform(0.3, 1.0, size=len(keep))
+        slab_elems = w.nbnd * w.nbnd * len(keep) * w.nmodes
+
+        @staticmethod
+        def g_slabs(ip, cnt):
+            return np.ascontiguousarray(g[ip:ip + cnt])
+
+    shift = (0.5, 0.25, 0.125)
+    k_list = (np.stack(np.meshgrid(*[np.arange(n) for n in w.k_grid], indexing="ij"), -1).reshape(-1, 3)
+              + np.array(shift)) / np.array(w.k_grid)
+    ref = oracle.interpolate(Sub.H_R, Sub.D_R, g, Sub.Re, Sub.w_e, Sub.Rp, Sub.w_p, k_list, w.q_list)
+    assert_path_close(run_gpu(epw, Sub, k_list, w.q_list, grid=w.k_grid, shift=shift), ref)
+    # and the same k-points as a list through the dense contraction
+    assert_path_close(run_gpu(epw, Sub, k_list, w.q_list), ref)
 
 
 def test_large_path_forced_on_config0(epw):
@@ -478,13 +549,13 @@ def test_errors_are_reported(epw):
 # ---------------------------------------------------------------------------------------------------------
 # full-size configurations, in the launch configuration bench.py times: sampled pairs against the oracle
 # ---------------------------------------------------------------------------------------------------------
-def check_sampled_pairs(epw, w, q_idx, k_idx, q_batch=0):
+def check_sampled_pairs(epw, w, q_idx, k_idx, q_batch=0, grid=False):
     """Run the library on ALL k of workload w and the q-points q_idx (one interpolate call, as bench.py does), then
     compare eps_k, omega_q, eps_kq and |g|^2 on the sampled (q, k) pairs with the oracle computed pair by pair."""
     g = w.g_full()
     ql = np.ascontiguousarray(w.q_list[q_idx])
     kq_map = None if w.kq_map is None else np.ascontiguousarray(w.kq_map[q_idx])
-    eps_k, eps_kq, om, g2 = run_gpu(epw, w, w.k_list, ql, kq_map, q_batch=q_batch)
+    eps_k, eps_kq, om, g2 = run_gpu(epw, w, w.k_list, ql, kq_map, q_batch=q_batch, grid=w.k_grid if grid else None)
     worst = 0.0
     for jq in range(len(q_idx)):
         e_ref, om_ref = oracle.phonon(w.D_R, w.Rp, w.w_p, ql[jq])
@@ -518,6 +589,18 @@ def test_config1_full_size_sampled(epw):
     q_idx = [0, 1, 2, 3, 500, 501, 998, 999]
     worst = check_sampled_pairs(epw, w, q_idx, sample_k(w.nk))
     print(f"config 1 full size: worst |g|^2 deviation {worst:.3f} x tolerance")
+
+
+@pytest.mark.parametrize("cfg,q_idx", [(1, [0, 1, 2, 3, 500, 501, 998, 999]), (2, [0, 1000, 1999]), (3, [0, 255])])
+def test_grid_full_size_sampled(epw, cfg, q_idx):
+    """configs[1..3] at full size through the uniform-grid entry point (what bench.py times by default)."""
+    w = synth.make_config(cfg)
+    k_idx = sample_k(w.nk, 16)
+    slab = w.k_grid[1] * w.k_grid[2]
+    k_idx = sorted(set(k_idx) | {slab - 1, slab, 63 * slab + 5 if 63 * slab + 5 < w.nk else 0,
+                                 64 * slab if 64 * slab < w.nk else 0})  # i1-plane and chunk edges
+    worst = check_sampled_pairs(epw, w, q_idx, k_idx, grid=True)
+    print(f"config {cfg} full size (grid): worst |g|^2 deviation {worst:.3f} x tolerance")
 
 
 def test_config2_full_size_sampled(epw):
