@@ -41,6 +41,7 @@ def parse_args():
     ap.add_argument("--nq-step", type=int, default=0,
                     help="q-points per step (per GPU); 0 = 8, reduced so that the |g|^2 buffer of a step stays below 20 GB")
     ap.add_argument("--q-batch", type=int, default=0, help="library q_batch for S1 (0 = default)")
+    ap.add_argument("--grid-unfused", action="store_true", help="EPW_FLAG_GRID_UNFUSED: keep g~ in HBM between S2 and S4b")
     ap.add_argument("--k-mode", default="grid", choices=["grid", "list"],
                     help="grid: epw_interp_interpolate_grid (the configs' k-points ARE uniform grids; factorised S2); "
                          "list: epw_interp_interpolate on the same k-points as a plain list (dense DMMA S2)")
@@ -226,7 +227,8 @@ def main():
     nk, E = w.nk, w.elements_per_pair
     nq_step = args.nq_step or max(1, min(8, int((20 << 30) // (8 * nk * E))))
     nq_step = min(nq_step, w.nq)
-    h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_, device=local_rank, q_batch=args.q_batch)
+    h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_, device=local_rank, q_batch=args.q_batch,
+                      flags=epw.EPW_FLAG_GRID_UNFUSED if args.grid_unfused else 0)
     t0 = time.perf_counter()
     h.set_operators_from_host(w)  # upload once; resident for the whole run
     torch.cuda.synchronize()
@@ -320,7 +322,7 @@ def main():
         def stage_table(mm):
             """Algorithmic work of the algorithm actually executed / CUDA-event time of the stage."""
             plan, stage_ms, stage_launches, rot = mm["plan"], mm["stage_ms"], mm["stage_launches"], mm["rotations"]
-            large, grid = plan["path"] == "large", plan["k_mode"] == "grid"
+            large, grid, fused = plan["path"] == "large", plan["k_mode"].startswith("grid"), plan["k_mode"] == "grid-fused"
             nsteps = args.steps
             pairs = float(nk) * nq_step * nsteps
             nq_tot = float(nq_step) * nsteps
@@ -333,16 +335,26 @@ def main():
             if grid:
                 N1, N2, N3 = w.k_grid
                 L1, L2, L3 = Lbox
-                mults = L1 * L2 * N3 * L3 + L1 * N2 * N3 * L2 + float(nk) * L1          # per column and q
-                byts = 16.0 * ncols * ((L1 * L2 * L3 + L1 * L2 * N3) + (L1 * L2 * N3 + L1 * N2 * N3) + (L1 * N2 * N3 + nk))
-                spec["S2_re_to_k"] = ("hbm", "zgemm_strided_kernel (3 axis passes)", byts * nq_tot, hbm, "GB/s",
-                                      {"flops": 8.0 * ncols * mults * nq_tot})
+                # the last axis pass runs on all columns, or (fused form) only on the Nb^2 H(k+q) columns
+                nc_last = (ncols - E) if fused else ncols
+                mults = ncols * (L1 * L2 * N3 * L3 + L1 * N2 * N3 * L2) + nc_last * float(nk) * L1     # per q
+                byts = 16.0 * (ncols * ((L1 * L2 * L3 + L1 * L2 * N3) + (L1 * L2 * N3 + L1 * N2 * N3))
+                               + nc_last * (L1 * N2 * N3 + nk))
+                spec["S2_re_to_k"] = ("hbm", "zgemm_strided_kernel (axis passes)", byts * nq_tot, hbm, "GB/s",
+                                      {"flops": 8.0 * mults * nq_tot})
             else:
                 spec["S2_re_to_k"] = ("tensor", "zgemm_strided_kernel" if large else "zgemm_dmma_kernel",
                                       8.0 * ncols * ne * pairs, dmma, "TFLOP/s", {})
-            spec["S4b_rotate_g2"] = ("tensor", "zgemm_strided_kernel" if large else "rotate_g2_dmma_kernel",
-                                     16.0 * nb ** 3 * nm * pairs, dmma, "TFLOP/s",
-                                     {"hbm_bytes": (16.0 * (E + 2 * nb * nb) + 8.0 * E) * pairs})
+            if fused:
+                # last axis pass of S2 (8 L1 E flops per pair, plain DFMA) + both rotation products (DMMA): one FP64 pipe
+                spec["S4b_rotate_g2"] = ("tensor", "grid_rotate_g2_kernel", (8.0 * Lbox[0] * E + 16.0 * nb ** 3 * nm) * pairs,
+                                         dmma, "TFLOP/s",
+                                         {"hbm_bytes": (32.0 * nb * nb + 8.0 * E) * pairs
+                                                       + 16.0 * E * Lbox[0] * w.k_grid[1] * w.k_grid[2] * nq_tot})
+            else:
+                spec["S4b_rotate_g2"] = ("tensor", "zgemm_strided_kernel" if large else "rotate_g2_dmma_kernel",
+                                         16.0 * nb ** 3 * nm * pairs, dmma, "TFLOP/s",
+                                         {"hbm_bytes": (16.0 * (E + 2 * nb * nb) + 8.0 * E) * pairs})
             spec["S4a_mode_rotation"] = ("tensor" if large else "alu",
                                          "zgemm_strided_kernel" if large else ("box_scatter_kernel" if grid else "pack_b_kernel"),
                                          8.0 * nb * nb * nm * nm * ne * nq_tot, dmma if large else dfma, "TFLOP/s", {})

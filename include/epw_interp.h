@@ -56,6 +56,8 @@ typedef struct {
   int32_t device;         /* CUDA device ordinal */
   int32_t q_batch;        /* q-points contracted per pass over g(Re,Rp) in S1 (1..8); 0 = library default */
   int32_t path;           /* EPW_PATH_AUTO (0): chosen from Nb, Nm; EPW_PATH_SMALL / EPW_PATH_LARGE force one (tests) */
+  int32_t flags;          /* 0, or EPW_FLAG_GRID_UNFUSED: on a uniform grid keep the last axis pass of S2 and S4b as two
+                             kernels with g~ in HBM (tests, debug getters) instead of the fused kernel */
   size_t workspace_bytes; /* cap on the library's scratch HBM; 0 = library chooses from free memory */
   double degen_tol;       /* informational (gap below which callers should sum |g|^2 over a subspace); unused inside */
   double omega_min;       /* modes with omega_q,nu <= omega_min give |g|^2 = 0 (acoustic modes at Gamma); default 0 */
@@ -65,6 +67,7 @@ typedef struct {
  * LARGE: S4a, S2 and both halves of S4b are FP64 tensor-path contractions that read their operand in place
  * (any Nb; configs[4], Nb = 192, Nm = 288).  Same results; AUTO picks by size. */
 enum { EPW_PATH_AUTO = 0, EPW_PATH_SMALL = 1, EPW_PATH_LARGE = 2 };
+enum { EPW_FLAG_GRID_UNFUSED = 1 };
 
 /* Create / destroy a handle.  *out is set to NULL on failure. */
 int epw_interp_create(epw_interp_t *out, const epw_interp_config *cfg);
@@ -165,8 +168,9 @@ int epw_interp_get_eigh_rotations(epw_interp_t h, uint64_t *counts, int n);
 int64_t epw_interp_last_launch_count(epw_interp_t h);
 
 /* How the last interpolate call was executed: plan[0] = EPW_PATH_SMALL or EPW_PATH_LARGE, plan[1] = q-points per pass
- * over g(Re,Rp) in S1, plan[2] = k-points per chunk of S2 / S3b / S4b, plan[3] = 1 if S2 ran in its factorised
- * uniform-grid form, 0 for the dense k-list contraction.  Returns the number of entries written. */
+ * over g(Re,Rp) in S1, plan[2] = k-points per chunk of S2 / S3b / S4b, plan[3] = 0 for the dense k-list contraction, 1 if S2 ran in its
+ * factorised uniform-grid form with g~ written to HBM, 2 if its last axis pass was fused with S4b (g~ never leaves
+ * the SM; times and launches of that kernel are booked under stage 6).  Returns the number of entries written. */
 int epw_interp_last_plan(epw_interp_t h, int64_t *plan, int n);
 
 /*

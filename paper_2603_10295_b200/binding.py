@@ -21,6 +21,7 @@ LIB_PATH = os.path.join(PKG, "libepw_interp.so")
 
 EPW_OK, EPW_EINVAL, EPW_ENOMEM, EPW_ECUDA, EPW_ENOTCONVERGED, EPW_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 EPW_PATH_AUTO, EPW_PATH_SMALL, EPW_PATH_LARGE = 0, 1, 2
+EPW_FLAG_GRID_UNFUSED = 1
 EPW_NUM_STAGES = 9
 STAGE_NAMES = ["S0_phase_tables", "S1_rp_to_q", "phonon_Dq_eig_S4a_pack", "Hk_eig", "S2_re_to_k_dmma", "Hkq_eig",
                "S4b_rotate_g2", "total", "S4a_mode_rotation"]
@@ -46,7 +47,7 @@ class EpwError(RuntimeError):
 
 class epw_interp_config(ctypes.Structure):
     _fields_ = [("nbnd", c_int32), ("nmodes", c_int32), ("ne", c_int32), ("np", c_int32), ("device", c_int32),
-                ("q_batch", c_int32), ("path", c_int32), ("workspace_bytes", c_size_t), ("degen_tol", c_double), ("omega_min", c_double)]
+                ("q_batch", c_int32), ("path", c_int32), ("flags", c_int32), ("workspace_bytes", c_size_t), ("degen_tol", c_double), ("omega_min", c_double)]
 
 
 _lib = None
@@ -127,8 +128,8 @@ def epw_version() -> str:
 
 
 def epw_interp_create(nbnd, nmodes, ne, np_, device=0, q_batch=0, workspace_bytes=0, degen_tol=1e-6, omega_min=0.0,
-                      path=EPW_PATH_AUTO):
-    cfg = epw_interp_config(nbnd, nmodes, ne, np_, device, q_batch, path, workspace_bytes, degen_tol, omega_min)
+                      path=EPW_PATH_AUTO, flags=0):
+    cfg = epw_interp_config(nbnd, nmodes, ne, np_, device, q_batch, path, flags, workspace_bytes, degen_tol, omega_min)
     h = c_void_p()
     _check(load_library().epw_interp_create(byref(h), byref(cfg)))
     return h
@@ -214,7 +215,7 @@ def epw_interp_last_plan(h) -> dict:
     buf = (c_int64 * 4)()
     _check(load_library().epw_interp_last_plan(h, buf, 4), h)
     return {"path": "large" if buf[0] == EPW_PATH_LARGE else "small", "q_batch": int(buf[1]), "k_chunk": int(buf[2]),
-            "k_mode": "grid" if buf[3] else "list"}
+            "k_mode": ("list", "grid", "grid-fused")[int(buf[3])]}
 
 
 def epw_interp_debug_get(h, what, dst_host):
@@ -276,10 +277,10 @@ class EpwInterp:
     """Owns one library handle.  `workload` is a synth.Workload-like object (numpy operators on the host)."""
 
     def __init__(self, nbnd, nmodes, ne, np_, device=0, q_batch=0, workspace_bytes=0, omega_min=0.0,
-                 path=EPW_PATH_AUTO):
+                 path=EPW_PATH_AUTO, flags=0):
         self.nbnd, self.nmodes, self.ne, self.np = nbnd, nmodes, ne, np_
         self.device = device
-        self.h = epw_interp_create(nbnd, nmodes, ne, np_, device, q_batch, workspace_bytes, 1e-6, omega_min, path)
+        self.h = epw_interp_create(nbnd, nmodes, ne, np_, device, q_batch, workspace_bytes, 1e-6, omega_min, path, flags)
 
     def close(self):
         if self.h is not None:

@@ -126,6 +126,11 @@ cudaError_t launch_box_scatter(const c128 *g1, const c128 *e, const double *omeg
                                const c128 *phase_qe, const double *w_e, const int32_t *box_idx, int64_t box_size, int nbb,
                                int nm, int ne, int ncols_g, int ncols_h, c128 *X, cudaStream_t st);
 cudaError_t launch_grid_axis_phase(int N, int i0, int cnt, double shift, int lo, int L, c128 *P, cudaStream_t st);
+// last axis pass of the grid form fused with S4b and |g|^2 (grid_rotate_g2.cu)
+bool grid_rotate_g2_supported(int nb, int nm, int L1);
+cudaError_t launch_grid_rotate_g2(const c128 *T2, int64_t slab, int ncols, int L1, const c128 *P1c, int cnt,
+                                  const c128 *Uk, const c128 *Ukq, const int32_t *kq_idx, int nb, int nm, int num_sms,
+                                  double *g2, cudaStream_t st);
 cudaError_t launch_grid_klist(const int32_t N[3], const double s[3], double *k_list, cudaStream_t st);
 
 cudaError_t launch_rotate_g2(const c128 *gt, int64_t stride_gt, const c128 *Uk, const c128 *Ukq, const int32_t *kq_idx,

@@ -92,7 +92,7 @@ struct epw_interp {
   // uniform-grid form of S2 (re_to_k_grid.cu): bounding box of the Re list, box-ordered operand and axis passes
   int box_lo[3] = {0, 0, 0}, box_L[3] = {1, 1, 1};
   int64_t box_size = 1;
-  DevBuf boxidx, X, T1, T2, Ptmp, P1pack, P2pack, P3pack, klist_gen;
+  DevBuf boxidx, X, T1, T2, Ptmp, P1raw, P1pack, P2pack, P3pack, klist_gen;
   DevBuf workctr;  // 3 x u64: plane rotations executed by the register-resident eigensolvers for H(k), H(k+q), D(q)
   // route the eigensolver work counter to slot i (0 H(k), 1 H(k+q), 2 D(q)) while stage timing is on; -1 = off
   void count_into(int slot) {
@@ -380,6 +380,10 @@ int epw_interp_create(epw_interp_t *out, const epw_interp_config *cfg) {
     g_create_error = "epw_interp_create: path must be EPW_PATH_AUTO, EPW_PATH_SMALL or EPW_PATH_LARGE";
     return EPW_EINVAL;
   }
+  if (cfg->flags & ~EPW_FLAG_GRID_UNFUSED) {
+    g_create_error = "epw_interp_create: unknown bit in flags";
+    return EPW_EINVAL;
+  }
   if (cfg->q_batch < 0 || cfg->q_batch > 8) {
     g_create_error = "epw_interp_create: q_batch must be in 0..8";
     return EPW_EINVAL;
@@ -425,7 +429,7 @@ void epw_interp_destroy(epw_interp_t h) {
                    &h->Uk, &h->Pq, &h->Pqe, &h->Dq, &h->eq, &h->g1, &h->Bpack, &h->C, &h->Ukq, &h->epskq_scratch,
                    &h->status, &h->eig_scratch, &h->hs_k, &h->hs_q, &h->hs_map, &h->hs_epsk, &h->hs_epskq,
                    &h->hs_omega, &h->hs_g2, &h->Pk, &h->BpackPk, &h->UpackK, &h->UpackKH, &h->BpackE,
-                   &h->ghat, &h->T, &h->Hkq, &h->boxidx, &h->X, &h->T1, &h->T2, &h->Ptmp, &h->P1pack, &h->P2pack,
+                   &h->ghat, &h->T, &h->Hkq, &h->boxidx, &h->X, &h->T1, &h->T2, &h->Ptmp, &h->P1raw, &h->P1pack, &h->P2pack,
                    &h->P3pack, &h->klist_gen, &h->workctr};
   for (DevBuf *b : all) b->release();
   for (cudaEvent_t ev : h->ev_pool) cudaEventDestroy(ev);
@@ -595,6 +599,9 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   int64_t slab = 0;          // k-points per i1 plane
   int cs = 0, nchunks = 1;   // i1 planes per k-chunk
   int KB1 = 0, NTc = 0;
+  // grid mode: the last axis pass is fused with S4b (grid_rotate_g2.cu) unless the caller asked for the two-kernel form
+  const bool fused = grid && !(h->cfg.flags & EPW_FLAG_GRID_UNFUSED) && grid_rotate_g2_supported(nb, nm, h->box_L[0]);
+  const int ncolsC = fused ? ncols_h : ncols;   // columns of the [g~ | H(k+q)] buffer that reach HBM
   if (!grid) {
     // k-chunk: one chunk of [g~ | H(k+q)] (16*ncols bytes per k) must stay L2-resident for the eigensolve and the
     // rotation that follow it, and its tile count should fill whole waves of the persistent contraction kernel
@@ -612,9 +619,11 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
     // k-chunk = whole i1 planes.  The last axis pass writes 64 complex columns (i1 values) per tile: prefer chunks of
     // a multiple of 64 planes (or all of them); 512 MB of [g~ | H(k+q)] per chunk unless that gives fewer than 16 planes.
     slab = (int64_t)grid->N[1] * grid->N[2];
-    const size_t plane_bytes = (size_t)slab * ncols * 16;
-    int64_t fit = (int64_t)(std::min(cap, (size_t)512 << 20) / plane_bytes);
-    if (fit < 16 && cap > ((size_t)512 << 20)) fit = std::min<int64_t>(64, (int64_t)(cap / plane_bytes));
+    // per-k workspace of a chunk: [g~ | H(k+q)] (unfused) or only the H(k+q) block (fused), plus U_{k+q} and eps
+    const size_t plane_bytes = (size_t)slab * ((fused ? ncols_h : ncols) + (kq_map ? 0 : nbb + nb)) * 16 + 16;
+    const size_t soft = fused ? ((size_t)2 << 30) : ((size_t)512 << 20);
+    int64_t fit = (int64_t)(std::min(cap, soft) / plane_bytes);
+    if (fit < 16 && cap > soft) fit = std::min<int64_t>(64, (int64_t)(cap / plane_bytes));
     if (fit < 1) return h->fail(EPW_ENOMEM, "epw_interp_interpolate_grid: workspace_bytes too small for one i1 plane of g~");
     if (fit >= grid->N[0]) fit = grid->N[0];
     else if (fit > 64) fit = fit / 64 * 64;
@@ -644,6 +653,7 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
     CU_OR_FAIL(h, h->P2pack.reserve(sizeof(double) * (size_t)ceil_div(2 * (int64_t)grid->N[1], GEMM_BN) *
                                     ceil_div(2 * (int64_t)L[1], GEMM_BK) * GEMM_CHUNK), "cudaMalloc P2pack");
     CU_OR_FAIL(h, h->P1pack.reserve(sizeof(double) * (size_t)nchunks * NTc * KB1 * GEMM_CHUNK), "cudaMalloc P1pack");
+    CU_OR_FAIL(h, h->P1raw.reserve(sizeof(c128) * (size_t)nchunks * L[0] * cs), "cudaMalloc P1raw");
   }
   CU_OR_FAIL(h, h->Hk.reserve(sizeof(c128) * (size_t)nk * nbb), "cudaMalloc Hk");
   CU_OR_FAIL(h, h->Uk.reserve(sizeof(c128) * (size_t)nk * nbb), "cudaMalloc Uk");
@@ -652,7 +662,7 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   CU_OR_FAIL(h, h->Dq.reserve(sizeof(c128) * (size_t)QB * nmm), "cudaMalloc Dq");
   CU_OR_FAIL(h, h->eq.reserve(sizeof(c128) * (size_t)QB * nmm), "cudaMalloc e_q");
   CU_OR_FAIL(h, h->g1.reserve(sizeof(c128) * (size_t)QB * h->rows), "cudaMalloc g(Re,q)");
-  CU_OR_FAIL(h, h->C.reserve(sizeof(c128) * (size_t)c_rows * ncols), "cudaMalloc g~");
+  if (ncolsC) CU_OR_FAIL(h, h->C.reserve(sizeof(c128) * (size_t)c_rows * ncolsC), "cudaMalloc g~");
   if (!kq_map) CU_OR_FAIL(h, h->Ukq.reserve(sizeof(c128) * (size_t)c_rows * nbb), "cudaMalloc Ukq");
   if (!kq_map && !eps_kq) CU_OR_FAIL(h, h->epskq_scratch.reserve(sizeof(double) * (size_t)c_rows * nb), "cudaMalloc eps scratch");
   CU_OR_FAIL(h, h->status.reserve(sizeof(int32_t)), "cudaMalloc status");
@@ -663,7 +673,8 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   CU_OR_FAIL(h, cudaMemsetAsync(h->status.p, 0, sizeof(int32_t), st), "memset status");
   h->last_nk = nk;
   h->last_c_rows = c_rows;
-  h->last_ncols = ncols;
+  h->last_ncols = ncolsC;
+  h->last_kmode = grid ? (fused ? 2 : 1) : 0;
   h->last_path = EPW_PATH_SMALL;
   h->last_qb = QB;
   h->last_kchunk = kchunk;
@@ -708,9 +719,9 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
     }
     for (int ci = 0; ci < nchunks; ci++) {
       const int cnt = std::min(cs, grid->N[0] - ci * cs);
-      LAUNCH(h, launch_grid_axis_phase(grid->N[0], ci * cs, cnt, grid->s[0], h->box_lo[0], L[0], h->Ptmp.as<c128>(), st),
-             "axis phases");
-      LAUNCH(h, launch_pack_b_strided(h->Ptmp.as<c128>(), cnt, 1, 0, 1, 0, nullptr, 0.0, L[0], cnt,
+      c128 *raw = h->P1raw.as<c128>() + (int64_t)ci * L[0] * cs;   // [L1][cnt], kept for the fused kernel
+      LAUNCH(h, launch_grid_axis_phase(grid->N[0], ci * cs, cnt, grid->s[0], h->box_lo[0], L[0], raw, st), "axis phases");
+      LAUNCH(h, launch_pack_b_strided(raw, cnt, 1, 0, 1, 0, nullptr, 0.0, L[0], cnt,
                                       h->P1pack.as<double>() + (int64_t)ci * NTc * KB1 * GEMM_CHUNK, st),
              "pack axis phases");
     }
@@ -795,15 +806,25 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
       for (int64_t k0 = 0; k0 < nk; k0 += kchunk) {
         const int64_t kn = std::min(kchunk, nk - k0);
         const int64_t crow = k0 % c_rows;
-        c128 *Cc = h->C.as<c128>() + crow * ncols;
+        c128 *Cc = h->C.as<c128>() + crow * ncolsC;
         // ---- S2: Re -> k contraction (+ H(k+q) columns) ----
         sp = h->begin_span(4, st);
-        if (!grid)
+        if (!grid) {
           LAUNCH(h, launch_zgemm_dmma(h->Apack.as<double>() + (k0 / GEMM_BM) * (int64_t)KB * GEMM_CHUNK, Bq, Cc, kn, ncols,
                                       KB, ncols, h->num_sms, st),
                  "zgemm S2");
-        else
+        } else if (!fused) {
           LAUNCH(h, grid_pass_c(ncols, (int)(k0 / kchunk), Cc), "grid pass S2");
+        } else if (ncols_h) {
+          // fused form: only the H(k+q) columns of the last axis pass go to HBM (the eigensolver's input)
+          const int ci = (int)(k0 / kchunk);
+          const int cnt = std::min(cs, grid->N[0] - ci * cs);
+          const int64_t Mh = slab * nbb;
+          LAUNCH(h, launch_zgemm_strided(h->T2.as<c128>() + ncols_g, nbb, ncols, slab * ncols, 0,
+                                         h->P1pack.as<double>() + (int64_t)ci * NTc * KB1 * GEMM_CHUNK, nullptr, Cc, Mh, 0, 1,
+                                         Mh, 0, 0, Mh, cnt, L[0], 1, h->num_sms, st),
+                 "grid pass H(k+q)");
+        }
         h->end_span(sp, st);
         const c128 *Ukq_ptr;
         const int32_t *kq_idx = nullptr;
@@ -824,7 +845,7 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
           c128 *Ukq_c = h->Ukq.as<c128>() + crow * nbb;
           double *eps_dst = eps_kq ? eps_kq + (q * nk + k0) * nb : h->epskq_scratch.as<double>() + crow * nb;
           h->count_into(1);
-          LAUNCH(h, launch_eigh_batched(Cc + ncols_g, ncols, nb, kn, eps_dst, Ukq_c, 0, h->status.as<int32_t>(),
+          LAUNCH(h, launch_eigh_batched(Cc + (ncolsC - ncols_h), ncolsC, nb, kn, eps_dst, Ukq_c, 0, h->status.as<int32_t>(),
                                         h->eig_scratch.as<c128>(), st),
                  "eigh H(k+q)");
           h->count_into(-1);
@@ -833,9 +854,18 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
         }
         // ---- S4b: band rotation + |g|^2 ----
         sp = h->begin_span(6, st);
-        LAUNCH(h, launch_rotate_g2(Cc, ncols, h->Uk.as<c128>() + k0 * nbb, Ukq_ptr, kq_idx, nb, nm, kn,
-                                   g2 + (q * nk + k0) * E, st),
-               "rotate_g2");
+        if (!fused) {
+          LAUNCH(h, launch_rotate_g2(Cc, ncols, h->Uk.as<c128>() + k0 * nbb, Ukq_ptr, kq_idx, nb, nm, kn,
+                                     g2 + (q * nk + k0) * E, st),
+                 "rotate_g2");
+        } else {
+          const int ci = (int)(k0 / kchunk);
+          const int cnt = std::min(cs, grid->N[0] - ci * cs);
+          LAUNCH(h, launch_grid_rotate_g2(h->T2.as<c128>(), slab, ncols, L[0], h->P1raw.as<c128>() + (int64_t)ci * L[0] * cs,
+                                          cnt, h->Uk.as<c128>() + k0 * nbb, Ukq_ptr, kq_idx, nb, nm, h->num_sms,
+                                          g2 + (q * nk + k0) * E, st),
+                 "grid_rotate_g2");
+        }
         h->end_span(sp, st);
       }
     }

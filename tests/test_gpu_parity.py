@@ -346,9 +346,11 @@ def test_rotate_g2_large(epw):
 # whole path
 # ---------------------------------------------------------------------------------------------------------
 def run_gpu(epw, w, k_list, q_list, kq_map=None, q_batch=0, host_api=False, path=0, workspace_bytes=0, grid=None,
-            shift=None):
-    """grid = (N1, N2, N3): call the uniform-grid entry point (k_list is then only used for its length)."""
-    h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_, q_batch=q_batch, path=path, workspace_bytes=workspace_bytes)
+            shift=None, flags=0):
+    """grid = (N1, N2, N3): call the uniform-grid entry point (k_list is then only used for its length);
+    flags = EPW_FLAG_GRID_UNFUSED keeps the last axis pass and the rotation as two kernels."""
+    h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_, q_batch=q_batch, path=path, workspace_bytes=workspace_bytes,
+                      flags=flags)
     try:
         h.set_operators_from_host(w)
         if host_api:
@@ -366,7 +368,8 @@ def run_gpu(epw, w, k_list, q_list, kq_map=None, q_batch=0, host_api=False, path
             return eps_k, eps_kq, om, g2
         if grid is not None:
             out = h.interpolate_grid(grid, dev(q_list), k_shift=shift, kq_map=None if kq_map is None else dev(kq_map))
-            assert epw.epw_interp_last_plan(h.h)["k_mode"] == ("list" if path == 2 or w.nbnd > 16 else "grid")
+            want = "list" if path == 2 or w.nbnd > 16 else ("grid" if flags else "grid-fused")
+            assert epw.epw_interp_last_plan(h.h)["k_mode"] == want
         else:
             out = h.interpolate(dev(k_list), dev(q_list), None if kq_map is None else dev(kq_map))
         epw.epw_interp_sync(h.h)
@@ -412,15 +415,17 @@ def test_grid_config0_both_kq_modes_and_host_api(epw):
     """configs[0] through epw_interp_interpolate_grid: all 4,096 pairs with kq_map, per-pair H(k+q), host buffers."""
     w = synth.make_config(0)
     ref = oracle.interpolate(w.H_R, w.D_R, w.g_full(), w.Re, w.w_e, w.Rp, w.w_p, w.k_list, w.q_list)
-    assert_path_close(run_gpu(epw, w, w.k_list, w.q_list, w.kq_map, grid=w.k_grid), ref)
-    assert_path_close(run_gpu(epw, w, w.k_list, w.q_list, None, grid=w.k_grid), ref)
+    for flags in (0, 1):
+        assert_path_close(run_gpu(epw, w, w.k_list, w.q_list, w.kq_map, grid=w.k_grid, flags=flags), ref)
+        assert_path_close(run_gpu(epw, w, w.k_list, w.q_list, None, grid=w.k_grid, flags=flags), ref)
     ql = w.q_list[:5] + [0.01, 0.02, 0.03]
     ref = oracle.interpolate(w.H_R, w.D_R, w.g_full(), w.Re, w.w_e, w.Rp, w.w_p, w.k_list, ql)
     assert_path_close(run_gpu(epw, w, w.k_list, ql, None, grid=w.k_grid, host_api=True, q_batch=3), ref)
 
 
-@pytest.mark.parametrize("shape", ["si", "mos2", "odd", "chunks", "large-forced"])
-def test_grid_reduced_shapes(epw, shape):
+@pytest.mark.parametrize("flags", [0, 1])
+@pytest.mark.parametrize("shape", ["si", "mos2", "odd", "chunks", "large-forced", "modes-split"])
+def test_grid_reduced_shapes(epw, shape, flags):
     """Reduced configs 1-3 through the grid entry point: ragged tiles in every axis pass, 2-D and skewed lattices,
     several i1-plane chunks (workspace cap), and the large-Nb family (which expands the grid to a list)."""
     ws, path = 0, 0
@@ -432,12 +437,16 @@ def test_grid_reduced_shapes(epw, shape):
         w = synth.make_custom("odd", 5, 3, (1, 2, 0), 1.0, 0.1, 1.0, (9, 1, 17), ("random", 2, 3), seed=13)
     elif shape == "chunks":
         w = synth.make_custom("chunks", 4, 3, (1, 1, 1), 1.0, 0.1, 1.0, (11, 3, 4), ("random", 2, 3), seed=14)
-        ws = 16 * 12 * (16 * 3 + 16) * 3 + 100   # three i1 planes of [g~ | H(k+q)] per chunk -> 4 chunks, ragged last
+        # three i1 planes (12 k each) of per-k workspace per chunk -> 4 chunks, ragged last
+        ws = (16 * 12 * ((16 * 3 if flags else 0) + 16 + 16 + 4) + 16) * 3 + 100
+    elif shape == "modes-split":
+        # Nb = 13, Nm = 12, L1 = 7: the fused kernel cannot hold all modes of a cell in shared memory -> mode groups
+        w = synth.make_custom("modes", 13, 12, (3, 1, 0), 1.0, 0.1, 1.0, (10, 3, 1), ("random", 2, 2), seed=15)
     else:
         w = synth.make_custom("mos2-l", 11, 9, (2, 2, 0), 2.0, 0.1, 2.0, (13, 11, 1), ("random", 2, 2), seed=23)
         path = 2
     ref = oracle.interpolate(w.H_R, w.D_R, w.g_full(), w.Re, w.w_e, w.Rp, w.w_p, w.k_list, w.q_list)
-    assert_path_close(run_gpu(epw, w, w.k_list, w.q_list, grid=w.k_grid, workspace_bytes=ws, path=path), ref)
+    assert_path_close(run_gpu(epw, w, w.k_list, w.q_list, grid=w.k_grid, workspace_bytes=ws, path=path, flags=flags), ref)
 
 
 def test_grid_shifted_and_sparse_lattice_list(epw):
@@ -464,6 +473,7 @@ def test_grid_shifted_and_sparse_lattice_list(epw):
               + np.array(shift)) / np.array(w.k_grid)
     ref = oracle.interpolate(Sub.H_R, Sub.D_R, g, Sub.Re, Sub.w_e, Sub.Rp, Sub.w_p, k_list, w.q_list)
     assert_path_close(run_gpu(epw, Sub, k_list, w.q_list, grid=w.k_grid, shift=shift), ref)
+    assert_path_close(run_gpu(epw, Sub, k_list, w.q_list, grid=w.k_grid, shift=shift, flags=1), ref)
     # and the same k-points as a list through the dense contraction
     assert_path_close(run_gpu(epw, Sub, k_list, w.q_list), ref)
 
