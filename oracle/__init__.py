@@ -61,6 +61,7 @@ def lib():
         L.oracle_interpolate.restype = i
         L.oracle_eq7_direct.argtypes = [i, i, i, i, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         L.oracle_eq6_wannier_from_bloch.argtypes = [i, i, i, i, vp, vp, i, vp, i, vp, vp, vp]
+        L.oracle_eq6_unrotate.argtypes = [i, i, vp, vp, vp, vp, vp, vp]
         for name in ("oracle_g_bytes",):
             getattr(L, name).argtypes = [f64] * 4
             getattr(L, name).restype = f64
@@ -226,6 +227,17 @@ def eq6_wannier_from_bloch(G, kc, qc, Re, Rp) -> np.ndarray:
     ne, np_ = Re.shape[0], Rp.shape[0]
     out = np.empty((np_, nm, ne, nb, nb), dtype=np.complex128)
     lib().oracle_eq6_wannier_from_bloch(nb, nm, ne, np_, _p(G), _p(kc), nkc, _p(qc), nqc, _p(Re), _p(Rp), _p(out))
+    return out
+
+
+def eq6_unrotate(g, Ukq_cm, Uk_cm, e_cm, omega) -> np.ndarray:
+    """Gauge part of Eq. 6 for one (k',q') block: Bloch g [nu][n][m] -> Wannier-gauge g~ [ka][n'][m']."""
+    g = _c(g, np.complex128)
+    nm, nb, _ = g.shape
+    Ukq_cm, Uk_cm, e_cm = _c(Ukq_cm, np.complex128), _c(Uk_cm, np.complex128), _c(e_cm, np.complex128)
+    omega = _c(omega, np.float64)
+    out = np.empty_like(g)
+    lib().oracle_eq6_unrotate(nb, nm, _p(g), _p(Ukq_cm), _p(Uk_cm), _p(e_cm), _p(omega), _p(out))
     return out
 
 

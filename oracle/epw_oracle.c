@@ -364,6 +364,44 @@ void oracle_eq6_wannier_from_bloch(int nb, int nm, int ne, int np, const zc *G, 
 }
 
 /* ---------------------------------------------------------------------------------------------
+ * Gauge part of Eq. 6: the factors U*_{mm'k'+q'} U_{nn'k'} u^-1_{nu,ka}(q') that take one
+ * coarse-grid Bloch-representation block back to the Wannier gauge before the two inverse Fourier sums.
+ * With [reading G4] paper-U = V^dagger (V = eigenvector columns) U*_{mm'} = V[m',m], U_{nn'} = conj(V[n',n]), and with
+ * [reading G3] u = e/sqrt(2 omega) (e unitary) u^-1_{nu,ka} = sqrt(2 omega_nu) conj(e[ka,nu]):
+ *   g~_{m'n' ka} = sum_{m n nu} Ukq[m',m] g_{mn nu} conj(Uk[n',n]) sqrt(2 omega_nu) conj(e[ka,nu])
+ * g [m + Nb*(n + Nb*nu)] -> gt [m' + Nb*(n' + Nb*ka)].  The exact inverse of oracle_mode_rotate followed by
+ * oracle_band_rotate (for omega > 0).
+ * ------------------------------------------------------------------------------------------- */
+void oracle_eq6_unrotate(int nb, int nm, const zc *g, const zc *Ukq, const zc *Uk, const zc *e, const double *omega,
+                         zc *gt) {
+  const int nbb = nb * nb;
+  zc *T = (zc *)malloc(sizeof(zc) * nbb);
+  zc *gw = (zc *)malloc(sizeof(zc) * nbb * nm);   /* Wannier band gauge, still mode basis */
+  for (int nu = 0; nu < nm; nu++) {
+    const zc *gn = g + (int64_t)nbb * nu;
+    for (int n = 0; n < nb; n++)
+      for (int mp = 0; mp < nb; mp++) {
+        zc s = 0.0;
+        for (int m = 0; m < nb; m++) s += Ukq[mp + nb * m] * gn[m + nb * n];
+        T[mp + nb * n] = s;
+      }
+    for (int np_ = 0; np_ < nb; np_++)
+      for (int mp = 0; mp < nb; mp++) {
+        zc s = 0.0;
+        for (int n = 0; n < nb; n++) s += T[mp + nb * n] * conj(Uk[np_ + nb * n]);
+        gw[mp + nb * np_ + (int64_t)nbb * nu] = s;
+      }
+  }
+  for (int ka = 0; ka < nm; ka++)
+    for (int el = 0; el < nbb; el++) {
+      zc s = 0.0;
+      for (int nu = 0; nu < nm; nu++) s += gw[el + (int64_t)nbb * nu] * sqrt(2.0 * omega[nu]) * conj(e[ka + nm * nu]);
+      gt[el + (int64_t)nbb * ka] = s;
+    }
+  free(T); free(gw);
+}
+
+/* ---------------------------------------------------------------------------------------------
  * Bookkeeping helpers pinned by the paper's printed numbers.
  * ------------------------------------------------------------------------------------------- */
 /* Table III caption: size of g(Re,Rp) = 16 Nb^2 Nm Ne Np bytes. */

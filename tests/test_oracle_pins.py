@@ -498,3 +498,28 @@ def test_silicon_size_and_eq12_ratio_as_printed():
     eq12 = 1 / nk + (1 / np_) * (1 + 2 / ne + nm / ne)
     assert abs(ratio - eq12) / eq12 < 0.02  # Eq. 12 drops the small terms of Eq. 8 ("approximately")
     assert abs(ratio * denom - 1) < 0.02
+
+
+# ---------------------------------------------------------------------------------------------
+# Gauge part of Eq. 6 (Bloch -> Wannier), the step before the hot path.
+# ---------------------------------------------------------------------------------------------
+def test_eq6_unrotate_matches_matrix_algebra_and_inverts_the_forward_rotations():
+    """Pin (textbook matrix algebra + invariant): PAPER.md:L78-80 with reading G4 gives, per mode,
+    g~_nu = V_{k+q} g_nu V_k^dagger, then g~_ka = sum_nu g~_nu sqrt(2 omega_nu) conj(e[ka,nu]) -- written here with
+    numpy matmul on mathematical matrices; and it must undo oracle_mode_rotate + oracle_band_rotate (both pinned
+    above), including which index carries k+q and where the conjugates sit."""
+    nb, nm = 4, 3
+    Ukq, Uk, e = random_unitary_cm(nb), random_unitary_cm(nb), random_unitary_cm(nm)
+    omega = np.array([0.7, 1.3, 2.1])
+    g = crandn(nm, nb, nb)  # [nu][n][m]
+    got = oracle.eq6_unrotate(g, Ukq, Uk, e, omega)
+    Vkq, Vk, E = cm(Ukq), cm(Uk), cm(e)  # mathematical matrices [row, col]
+    gw = np.stack([Vkq @ g[nu].T @ Vk.conj().T for nu in range(nm)])  # [nu][m'][n']
+    ref = np.einsum("vab,kv->kab", gw * np.sqrt(2 * omega)[:, None, None], E.conj())  # [ka][m'][n']
+    np.testing.assert_allclose(got, np.swapaxes(ref, 1, 2), rtol=0, atol=1e-14)
+    # inverse of the forward rotations
+    gt = crandn(nm, nb, nb)  # [ka][n'][m']
+    fwd = oracle.band_rotate(oracle.mode_rotate(gt, e, omega), Ukq, Uk)
+    np.testing.assert_allclose(oracle.eq6_unrotate(fwd, Ukq, Uk, e, omega), gt, rtol=0, atol=1e-13)
+    # transposing a U or swapping k <-> k+q is detected
+    assert np.abs(oracle.eq6_unrotate(fwd, Uk, Ukq, e, omega) - gt).max() > 1e-2
