@@ -50,6 +50,9 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-klist-arm", action="store_true", help="skip the extra list-mode measurement of --k-mode grid")
     ap.add_argument("--stages", action="store_true", help="also print per-stage device times to stderr")
+    ap.add_argument("--eq6", action="store_true",
+                    help="time Eq. 6 (Bloch -> Wannier, epw_wannier_from_bloch) on coarse grids that match the config's "
+                         "R sets instead of the interpolation path; prints its own JSON line")
     return ap.parse_args()
 
 
@@ -200,10 +203,61 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------------------
 # B200 arm
 # ------------------------------------------------------------------------------------------------------------
+def run_eq6(args):
+    """Eq. 6 at the size of the config's operator: coarse k', q' grids with one lattice vector per residue class
+    (so that the transform is the exact inverse of the interpolation), random coarse-grid data on the device."""
+    import torch
+
+    import paper_2603_10295_b200 as epw
+    import synth
+
+    torch.cuda.set_device(0)
+    w = synth.make_config(args.config)
+    Nc = [int(w.Re[:, d].max() - w.Re[:, d].min() + 1) for d in range(3)]
+    ax = [np.arange(n) / n for n in Nc]
+    kc = np.stack(np.meshgrid(*ax, indexing="ij"), axis=-1).reshape(-1, 3)
+    nkc = nqc = len(kc)
+    nb, nm = w.nbnd, w.nmodes
+    G = torch.randn((nqc, nkc, nm, nb, nb, 2), dtype=torch.float64, device="cuda")
+    out = torch.empty((w.np_, nm, w.ne, nb, nb, 2), dtype=torch.float64, device="cuda")
+    kd, Red, Rpd = torch.from_numpy(kc).cuda(), torch.from_numpy(w.Re).cuda(), torch.from_numpy(w.Rp).cuda()
+
+    def call():
+        epw.epw_wannier_from_bloch(G, kd, nkc, kd, nqc, Red, w.ne, Rpd, w.np_, nb, nm, out)
+
+    for _ in range(args.warmup):
+        call()
+    torch.cuda.synchronize()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(args.steps):
+        call()
+    ev1.record()
+    torch.cuda.synchronize()
+    ms = ev0.elapsed_time(ev1) / args.steps
+    E = nb * nb * nm
+    flops = 8.0 * E * (float(w.ne) * nkc * nqc + float(w.ne) * w.np_ * nqc)
+    peaks = epw.epw_probe_peaks(0)
+    print(json.dumps({
+        "metric": "Eq. 6 Bloch->Wannier: g(Re,Rp) elements/s (FP64)", "value": E * w.ne * w.np_ / (ms * 1e-3),
+        "unit": "elements/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+        "higher_is_better": True, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"Eq. 6 for the operator of configs[{w.index}]: {nkc} k' x {nqc} q' coarse points "
+                               f"({'x'.join(map(str, Nc))} grids), Nb={nb} Nm={nm} Ne={w.ne} Np={w.np_}; includes the "
+                               "call's own workspace allocation and phase tables"},
+        "roofline": {"bound": "tensor", "kernel": "zgemm_strided_kernel (2 launches)", "achieved": flops / (ms * 1e-3) / 1e12,
+                     "peak": peaks["fp64_dmma_tflops"], "unit": "TFLOP/s",
+                     "frac": flops / (ms * 1e-3) / 1e12 / peaks["fp64_dmma_tflops"], "traffic": None},
+    }))
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+        return
+    if args.eq6:
+        run_eq6(args)
         return
 
     import torch

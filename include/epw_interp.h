@@ -251,6 +251,31 @@ int epw_zgemm_strided(const void *A, int64_t a_rb, int64_t a_bs, int64_t a_ks, i
 int epw_rotate_g2(const void *gt, int64_t stride_gt, const void *Uk, const void *Ukq, const int32_t *kq_idx,
                   int32_t nb, int32_t nm, int64_t nk, double *g2, void *cuda_stream);
 
+/* -------------------------------------------------------------------------------------------------
+ * Eq. 6, the step before the hot path: coarse-grid Bloch representation -> g(Re,Rp).
+ * Device pointers; both calls synchronise the stream before returning (temporary workspace).
+ * ----------------------------------------------------------------------------------------------- */
+
+/* Gauge part of Eq. 6 for every (k',q') block of a coarse grid:
+ *   gt[iq][ik][ka][n'][m'] = sum_{m n nu} Ukq[iq][ik][m',m] g[iq][ik][nu][n][m] conj(Uk[ik][n',n]) sqrt(2 omega[iq][nu]) conj(e[iq][ka,nu])
+ * (the inverse of S4a + S4b; paper-U = V^dagger, u = e/sqrt(2 omega): DESIGN.md readings G3, G4).
+ *   g_bloch c128 [nqc][nkc][Nm][Nb][Nb] (m fastest), Uk c128 [nkc][Nb][Nb], Ukq c128 [nqc][nkc][Nb][Nb] (column-major,
+ *   columns = eigenvectors), e_q c128 [nqc][Nm][Nm] (columns = mode eigenvectors), omega_q f64 [nqc][Nm] (> 0),
+ *   gt_out c128 [nqc][nkc][Nm][Nb][Nb] (may not alias g_bloch). */
+int epw_eq6_unrotate(const void *g_bloch, const void *Uk, const void *Ukq, const void *e_q, const double *omega_q,
+                     int32_t nb, int32_t nm, int64_t nkc, int64_t nqc, void *gt_out, void *cuda_stream);
+
+/* The two inverse Fourier sums of Eq. 6 in the Wannier gauge:
+ *   g_RR[ip][ka][ie][n'][m'] = 1/(Ne Np) sum_{iq,ik} gt[iq][ik][ka][n'][m'] exp(-2 pi i (q'_iq . Rp_ip + k'_ik . Re_ie))
+ * with the normalisation as printed in the paper (Ne, Np = numbers of lattice vectors; for one vector per residue
+ * class of the coarse grids this is the exact inverse of the interpolation).
+ *   gt c128 [nqc][nkc][Nm][Nb][Nb], kc f64 [nkc][3], qc f64 [nqc][3] (crystal coordinates), Re int32 [ne][3],
+ *   Rp int32 [np][3]; g_RR_out c128 [np][Nm][ne][Nb][Nb] -- the layout epw_interp_set_wannier_operators takes.
+ * Runs as two in-place FP64 tensor-path contractions (zgemm_strided.cu) with conjugated phase tables. */
+int epw_wannier_from_bloch(const void *gt, const double *kc, int64_t nkc, const double *qc, int64_t nqc, const int32_t *Re,
+                           int32_t ne, const int32_t *Rp, int32_t np, int32_t nb, int32_t nm, void *g_RR_out,
+                           void *cuda_stream);
+
 /* Roofline denominators measured on this device ("Measurement"): FP64 tensor (DMMA m8n8k4) TFLOP/s,
  * plain DFMA TFLOP/s and HBM read / copy GB/s from tight probe kernels.  out[0..3]; returns 0 or a status. */
 int epw_probe_peaks(int32_t device, double *out4);

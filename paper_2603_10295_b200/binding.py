@@ -35,6 +35,7 @@ EXPORTED_SYMBOLS = [
     "epw_interp_enable_stage_timing", "epw_interp_get_stage_launches", "epw_interp_last_launch_count", "epw_interp_get_eigh_rotations", "epw_interp_last_plan", "epw_interp_debug_get", "epw_interp_last_error",
     "epw_phase_table", "epw_rp_to_q", "epw_interp_operator", "epw_eigh_batched", "epw_eigh_batched_algo", "epw_zgemm", "epw_zgemm_strided",
     "epw_rotate_g2",
+    "epw_eq6_unrotate", "epw_wannier_from_bloch",
     "epw_probe_peaks", "epw_version",
 ]
 
@@ -94,6 +95,8 @@ def load_library() -> ctypes.CDLL:
                                         c_int64, vp, c_int64, c_int64, c_int64, c_int64, c_int64, c_int, c_int64,
                                         c_int32, c_int32, c_int64, vp]
         L.epw_rotate_g2.argtypes = [vp, c_int64, vp, vp, vp, c_int32, c_int32, c_int64, vp, vp]
+        L.epw_eq6_unrotate.argtypes = [vp, vp, vp, vp, vp, c_int32, c_int32, c_int64, c_int64, vp, vp]
+        L.epw_wannier_from_bloch.argtypes = [vp, vp, c_int64, vp, c_int64, vp, c_int32, vp, c_int32, c_int32, c_int32, vp, vp]
         L.epw_probe_peaks.argtypes = [c_int32, POINTER(c_double)]
         L.epw_version.restype = c_char_p
         _lib = L
@@ -265,6 +268,16 @@ def epw_zgemm_strided(A, a_rb, a_bs, a_ks, a_batch, B, b_sr, b_sn, b_batch, b_co
 def epw_rotate_g2(gt, stride_gt, Uk, Ukq, kq_idx, nb, nm, nk, g2, stream=None):
     _check(load_library().epw_rotate_g2(_ptr(gt), stride_gt, _ptr(Uk), _ptr(Ukq), _ptr(kq_idx), nb, nm, nk, _ptr(g2),
                                         _stream() if stream is None else stream))
+
+
+def epw_eq6_unrotate(g_bloch, Uk, Ukq, e_q, omega_q, nb, nm, nkc, nqc, gt_out, stream=None):
+    _check(load_library().epw_eq6_unrotate(_ptr(g_bloch), _ptr(Uk), _ptr(Ukq), _ptr(e_q), _ptr(omega_q), nb, nm, nkc, nqc,
+                                           _ptr(gt_out), _stream() if stream is None else stream))
+
+
+def epw_wannier_from_bloch(gt, kc, nkc, qc, nqc, Re, ne, Rp, np_, nb, nm, g_RR_out, stream=None):
+    _check(load_library().epw_wannier_from_bloch(_ptr(gt), _ptr(kc), nkc, _ptr(qc), nqc, _ptr(Re), ne, _ptr(Rp), np_, nb,
+                                                 nm, _ptr(g_RR_out), _stream() if stream is None else stream))
 
 
 def epw_probe_peaks(device=0) -> dict:

@@ -138,6 +138,14 @@ cudaError_t launch_rotate_g2(const c128 *gt, int64_t stride_gt, const c128 *Uk, 
 
 bool rotate_g2_small_supported(int nb, int nm);  // Nb <= 16 and the T staging buffer of one pair fits shared memory
 
+// Eq. 6, Bloch -> Wannier (bloch_to_wannier.cu)
+cudaError_t launch_eq6_unrotate(const c128 *g, const c128 *Uk, const c128 *Ukq, const c128 *e, const double *omega, int nb,
+                                int nm, int64_t nkc, int64_t nqc, c128 *tmp, c128 *gt, cudaStream_t st);
+cudaError_t launch_wannier_from_bloch(const c128 *gt, const double *kc, int64_t nkc, const double *qc, int64_t nqc,
+                                      const int32_t *Re, int ne, const int32_t *Rp, int np, int nb, int nm, double *wk,
+                                      double *wq, c128 *Pk, c128 *Pq, double *BpackK, double *BpackQ, int32_t *zero_gather,
+                                      c128 *g1, c128 *g_RR, int num_sms, cudaStream_t st);
+
 int probe_peaks(int device, double *out4);
 
 }  // namespace epw

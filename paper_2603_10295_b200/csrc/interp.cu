@@ -1145,6 +1145,56 @@ int epw_rotate_g2(const void *gt, int64_t stride_gt, const void *Uk, const void 
   return rc;
 }
 
+int epw_eq6_unrotate(const void *g_bloch, const void *Uk, const void *Ukq, const void *e_q, const double *omega_q,
+                     int32_t nb, int32_t nm, int64_t nkc, int64_t nqc, void *gt_out, void *cuda_stream) {
+  if (!g_bloch || !Uk || !Ukq || !e_q || !omega_q || !gt_out || nb <= 0 || nm <= 0 || nkc <= 0 || nqc <= 0)
+    return EPW_EINVAL;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  c128 *tmp = nullptr;
+  if (cudaMalloc(&tmp, sizeof(c128) * (size_t)nkc * nqc * nb * nb * nm) != cudaSuccess) return EPW_ENOMEM;
+  const cudaError_t e = launch_eq6_unrotate(reinterpret_cast<const c128 *>(g_bloch), reinterpret_cast<const c128 *>(Uk),
+                                            reinterpret_cast<const c128 *>(Ukq), reinterpret_cast<const c128 *>(e_q),
+                                            omega_q, nb, nm, nkc, nqc, tmp, reinterpret_cast<c128 *>(gt_out), st);
+  cudaStreamSynchronize(st);
+  cudaFree(tmp);
+  return rc_of(e);
+}
+
+int epw_wannier_from_bloch(const void *gt, const double *kc, int64_t nkc, const double *qc, int64_t nqc, const int32_t *Re,
+                           int32_t ne, const int32_t *Rp, int32_t np, int32_t nb, int32_t nm, void *g_RR_out,
+                           void *cuda_stream) {
+  if (!gt || !kc || !qc || !Re || !Rp || !g_RR_out || nkc <= 0 || nqc <= 0 || ne <= 0 || np <= 0 || nb <= 0 || nm <= 0)
+    return EPW_EINVAL;
+  if (nkc > 2147483647LL / 2 || nqc > 2147483647LL / 2) return EPW_EINVAL;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  int dev = 0, nsm = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  const size_t rows = (size_t)nb * nb * nm * ne;
+  const size_t packK = (size_t)ceil_div(2 * (int64_t)ne, GEMM_BN) * ceil_div(2 * nkc, GEMM_BK) * GEMM_CHUNK;
+  const size_t packQ = (size_t)ceil_div(2 * (int64_t)np, GEMM_BN) * ceil_div(2 * nqc, GEMM_BK) * GEMM_CHUNK;
+  // one allocation, carved up (all pieces 16-byte aligned)
+  auto al = [](size_t b) { return (b + 255) & ~(size_t)255; };
+  const size_t sz[] = {al(sizeof(double) * ne), al(sizeof(double) * np), al(sizeof(c128) * nkc * ne),
+                       al(sizeof(c128) * nqc * np), al(sizeof(double) * packK), al(sizeof(double) * packQ),
+                       al(sizeof(int32_t) * nqc), al(sizeof(c128) * nqc * rows)};
+  size_t total = 0;
+  for (size_t b : sz) total += b;
+  char *ws = nullptr;
+  if (cudaMalloc(&ws, total) != cudaSuccess) return EPW_ENOMEM;
+  char *p[8];
+  size_t off = 0;
+  for (int i = 0; i < 8; i++) { p[i] = ws + off; off += sz[i]; }
+  const cudaError_t e = launch_wannier_from_bloch(
+      reinterpret_cast<const c128 *>(gt), kc, nkc, qc, nqc, Re, ne, Rp, np, nb, nm, reinterpret_cast<double *>(p[0]),
+      reinterpret_cast<double *>(p[1]), reinterpret_cast<c128 *>(p[2]), reinterpret_cast<c128 *>(p[3]),
+      reinterpret_cast<double *>(p[4]), reinterpret_cast<double *>(p[5]), reinterpret_cast<int32_t *>(p[6]),
+      reinterpret_cast<c128 *>(p[7]), reinterpret_cast<c128 *>(g_RR_out), nsm, st);
+  cudaStreamSynchronize(st);
+  cudaFree(ws);
+  return rc_of(e);
+}
+
 int epw_probe_peaks(int32_t device, double *out4) {
   if (!out4) return EPW_EINVAL;
   return probe_peaks(device, out4);
