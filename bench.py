@@ -41,6 +41,10 @@ def parse_args():
     ap.add_argument("--nq-step", type=int, default=0,
                     help="q-points per step (per GPU); 0 = 8, reduced so that the |g|^2 buffer of a step stays below 20 GB")
     ap.add_argument("--q-batch", type=int, default=0, help="library q_batch for S1 (0 = default)")
+    ap.add_argument("--rp-shard", action="store_true",
+                    help="NEXT-1 (PAPER.md:L186-188): g(Re,Rp) split by Rp over the ranks; per step every rank contracts "
+                         "its slabs for the q-points of ALL ranks, one NCCL reduce-scatter of g(Re,q) hands each rank the "
+                         "summed g(Re,q) of its own q-points, and the rest of the path runs unchanged")
     ap.add_argument("--grid-unfused", action="store_true", help="EPW_FLAG_GRID_UNFUSED: keep g~ in HBM between S2 and S4b")
     ap.add_argument("--k-mode", default="grid", choices=["grid", "list"],
                     help="grid: epw_interp_interpolate_grid (the configs' k-points ARE uniform grids; factorised S2); "
@@ -284,7 +288,8 @@ def main():
     h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_, device=local_rank, q_batch=args.q_batch,
                       flags=epw.EPW_FLAG_GRID_UNFUSED if args.grid_unfused else 0)
     t0 = time.perf_counter()
-    h.set_operators_from_host(w)  # upload once; resident for the whole run
+    # upload once; resident for the whole run; with --rp-shard only this rank's Rp slabs
+    h.set_operators_from_host(w, rp_range=shard.rp_ranges(w.np_, world)[rank] if args.rp_shard else None)
     torch.cuda.synchronize()
     t_upload = time.perf_counter() - t0
 
@@ -307,8 +312,26 @@ def main():
     g2 = torch.empty((nq_step, nk, w.nmodes, w.nbnd, w.nbnd), dtype=torch.float64, device="cuda")  # reused every step
 
     use_grid = args.k_mode == "grid"
+    if args.rp_shard:
+        args.no_e2e = True   # the host-buffer entry point has no Rp-sharded form
+    rows = w.slab_elems
+    q_all_dev = None
+    if args.rp_shard:
+        # the q-points of every rank for each step (rank r owns block r of the step's world*nq_step points)
+        q_all_dev = [torch.from_numpy(np.ascontiguousarray(
+            w.q_list[np.concatenate([shard.q_block(s, world, r, nq_step, w.nq) for r in range(world)])])).cuda()
+            for s in range(total_steps)]
+        g1_part = torch.empty((world * nq_step, rows, 2), dtype=torch.float64, device="cuda")
+        g1_mine = torch.empty((nq_step, rows, 2), dtype=torch.float64, device="cuda")
 
     def step(s, grid=None):
+        if args.rp_shard:
+            epw.epw_interp_rp_to_q_partial(h.h, q_all_dev[s], world * nq_step, g1_part)
+            if world > 1:
+                dist.reduce_scatter_tensor(g1_mine, g1_part, op=dist.ReduceOp.SUM)   # the one exchange step, on the stream
+                epw.epw_interp_set_gq(h.h, g1_mine)
+            else:
+                epw.epw_interp_set_gq(h.h, g1_part)
         if use_grid if grid is None else grid:
             epw.epw_interp_interpolate_grid(h.h, w.k_grid, None, q_dev[s], nq_step,
                                             None if map_dev is None else map_dev[s], eps_k, eps_kq, omega, g2)
@@ -526,7 +549,8 @@ def main():
             "config": {
                 "workload": f"BASELINE.json configs[{w.index}] {w.name}: Nb={w.nbnd} Nm={w.nmodes} Ne={w.ne} Np={w.np_} "
                             f"Nk={nk} ({'x'.join(map(str, w.k_grid))}), {nq_step} q per step per GPU ({w.q_desc})",
-                "global_batch_pairs": world * nk * nq_step, "parallelism": f"q-sharded x{world}",
+                "global_batch_pairs": world * nk * nq_step, "parallelism": (f"g(Re,Rp) Rp-sharded x{world} + reduce-scatter of g(Re,q) over q" if args.rp_shard
+                                                                      else f"q-sharded x{world}"),
                 "k_mode": ("uniform grid -> epw_interp_interpolate_grid" if use_grid else "k-list -> epw_interp_interpolate"),
                 "l2": "inputs larger than L2: g(Re,Rp) %.0f MB streamed per q-batch, phase table %.0f MB, |g|^2 output %.0f MB "
                       "per step" % (w.g_bytes / 1e6, 16.0 * nk * w.ne / 1e6, 8.0 * elements_per_step / 1e6),

@@ -136,6 +136,26 @@ int epw_interp_interpolate_grid_host(epw_interp_t h, const int32_t *k_grid, cons
                                      int64_t nq, const int32_t *kq_map, double *eps_k, double *eps_kq, double *omega_q,
                                      double *g2, void *cuda_stream);
 
+/*
+ * g(Re,Rp) split over several GPUs by Rp (the paper's pool level for operators larger than one GPU's memory,
+ * PAPER.md:L186-188, Table III; SURVEY.md 8(e) variant B / 8(f) NEXT-1).  Eq. 9 is a sum over Rp, so each
+ * rank contracts its own slabs and the partial g(Re,q) are summed across ranks -- the paper does D2H + mp_sum on the
+ * host (L514, L522); here the partial sums stay on the device and the caller all-reduces them on the same stream
+ * (NCCL through torch.distributed: the one real exchange step of the path).  After the sum every rank holds the full
+ * g(Re,q) and runs the rest of the path on ITS share of the k-points (outputs are disjoint).
+ *
+ *   epw_interp_set_rp_shard     before uploading g: this handle keeps only slabs [ip_start, ip_start+ip_count) of g_RR
+ *                               (H_R, D_R, Re, Rp and the weights are still the complete lists).
+ *   epw_interp_rp_to_q_partial  S0 + S1 over the handle's slabs: g1_partial c128 [nq][Nb^2 Nm Ne] (device, caller-owned),
+ *                               asynchronous on cuda_stream.  q_list f64 [nq][3] device.
+ *   epw_interp_set_gq           the NEXT epw_interp_interpolate / _grid call takes g(Re,q) from g1_reduced (device,
+ *                               c128 [nq][Nb^2 Nm Ne], the same nq and q order as that call) instead of running S1;
+ *                               NULL restores the normal path.  The buffer must stay valid until that call completes.
+ */
+int epw_interp_set_rp_shard(epw_interp_t h, int32_t ip_start, int32_t ip_count);
+int epw_interp_rp_to_q_partial(epw_interp_t h, const double *q_list, int64_t nq, void *g1_partial, void *cuda_stream);
+int epw_interp_set_gq(epw_interp_t h, const void *g1_reduced);
+
 /* Wait for the handle's last enqueued work and report deferred device-side status (EPW_ENOTCONVERGED, EPW_ECUDA). */
 int epw_interp_sync(epw_interp_t h);
 

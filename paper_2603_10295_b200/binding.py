@@ -36,6 +36,7 @@ EXPORTED_SYMBOLS = [
     "epw_phase_table", "epw_rp_to_q", "epw_interp_operator", "epw_eigh_batched", "epw_eigh_batched_algo", "epw_zgemm", "epw_zgemm_strided",
     "epw_rotate_g2",
     "epw_eq6_unrotate", "epw_wannier_from_bloch",
+    "epw_interp_set_rp_shard", "epw_interp_rp_to_q_partial", "epw_interp_set_gq",
     "epw_probe_peaks", "epw_version",
 ]
 
@@ -73,6 +74,9 @@ def load_library() -> ctypes.CDLL:
         L.epw_interp_interpolate_host.argtypes = [vp, vp, c_int64, vp, c_int64, vp, vp, vp, vp, vp, vp]
         L.epw_interp_interpolate_grid.argtypes = [vp, vp, vp, vp, c_int64, vp, vp, vp, vp, vp, vp]
         L.epw_interp_interpolate_grid_host.argtypes = [vp, vp, vp, vp, c_int64, vp, vp, vp, vp, vp, vp]
+        L.epw_interp_set_rp_shard.argtypes = [vp, c_int32, c_int32]
+        L.epw_interp_rp_to_q_partial.argtypes = [vp, vp, c_int64, vp, vp]
+        L.epw_interp_set_gq.argtypes = [vp, vp]
         L.epw_interp_sync.argtypes = [vp]
         L.epw_interp_get_stage_times.argtypes = [vp, POINTER(c_double), c_int]
         L.epw_interp_enable_stage_timing.argtypes = [vp, c_int]
@@ -182,6 +186,19 @@ def epw_interp_interpolate_grid_host(h, k_grid, k_shift, q_list, nq, kq_map, eps
     _check(load_library().epw_interp_interpolate_grid_host(h, g, s, _ptr(q_list), nq, _ptr(kq_map), _ptr(eps_k),
                                                            _ptr(eps_kq), _ptr(omega_q), _ptr(g2),
                                                            _stream() if stream is None else stream), h)
+
+
+def epw_interp_set_rp_shard(h, ip_start, ip_count):
+    _check(load_library().epw_interp_set_rp_shard(h, ip_start, ip_count), h)
+
+
+def epw_interp_rp_to_q_partial(h, q_list, nq, g1_partial, stream=None):
+    _check(load_library().epw_interp_rp_to_q_partial(h, _ptr(q_list), nq, _ptr(g1_partial),
+                                                     _stream() if stream is None else stream), h)
+
+
+def epw_interp_set_gq(h, g1_reduced):
+    _check(load_library().epw_interp_set_gq(h, _ptr(g1_reduced)), h)
 
 
 def epw_interp_sync(h):
@@ -306,13 +323,17 @@ class EpwInterp:
         except Exception:
             pass
 
-    def set_operators_from_host(self, w, slab_chunk_bytes=2 << 30):
-        """Upload H, D, R lists from a workload and stream g(Re,Rp) in Rp slabs (never holds all of g on the host)."""
+    def set_operators_from_host(self, w, slab_chunk_bytes=2 << 30, rp_range=None):
+        """Upload H, D, R lists from a workload and stream g(Re,Rp) in Rp slabs (never holds all of g on the host).
+        rp_range = (start, stop): keep only that Rp shard of g on this GPU (epw_interp_set_rp_shard)."""
+        lo, hi = (0, w.np_) if rp_range is None else rp_range
+        if rp_range is not None:
+            epw_interp_set_rp_shard(self.h, lo, hi - lo)
         epw_interp_set_wannier_operators(self.h, w.H_R, w.D_R, None, w.Re, w.w_e, w.Rp, w.w_p, 0)
         per_slab = 16 * w.slab_elems
         step = max(1, int(slab_chunk_bytes // per_slab))
-        for ip in range(0, w.np_, step):
-            cnt = min(step, w.np_ - ip)
+        for ip in range(lo, hi, step):
+            cnt = min(step, hi - ip)
             epw_interp_set_g_slabs(self.h, ip, cnt, w.g_slabs(ip, cnt), 0)
 
     def interpolate(self, k_list, q_list, kq_map=None, want_eps_kq=True):

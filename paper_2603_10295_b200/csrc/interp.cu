@@ -83,6 +83,10 @@ struct epw_interp {
   int q_batch = 4;
   bool operators_set = false;
   std::vector<char> slab_set;
+  // Rp shard (NEXT-1): this handle keeps only slabs [rp_lo, rp_lo + rp_cnt) of g(Re,Rp)
+  int rp_lo = 0, rp_cnt = 0;
+  bool sharded = false;
+  const c128 *ext_g1 = nullptr;  // g(Re,q) supplied by the caller (already summed over every rank's Rp) for this call
   // resident operators
   DevBuf g, H, D, Re, Rp, we, wp, ones;
   // per-call workspace
@@ -209,7 +213,7 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
   CU_OR_FAIL(h, h->Pq.reserve(sizeof(c128) * (size_t)QB * np), "cudaMalloc Pq");
   CU_OR_FAIL(h, h->Dq.reserve(sizeof(c128) * (size_t)QB * nmm), "cudaMalloc Dq");
   CU_OR_FAIL(h, h->eq.reserve(sizeof(c128) * (size_t)QB * nmm), "cudaMalloc e_q");
-  CU_OR_FAIL(h, h->g1.reserve(sizeof(c128) * (size_t)QB * h->rows), "cudaMalloc g(Re,q)");
+  if (!h->ext_g1) CU_OR_FAIL(h, h->g1.reserve(sizeof(c128) * (size_t)QB * h->rows), "cudaMalloc g(Re,q)");
   CU_OR_FAIL(h, h->BpackE.reserve(sizeof(double) * (size_t)NTm * KBm * GEMM_CHUNK), "cudaMalloc BpackE");
   CU_OR_FAIL(h, h->ghat.reserve(sizeof(c128) * (size_t)ne * E), "cudaMalloc g^(Re,q)");
   CU_OR_FAIL(h, h->C.reserve(sizeof(c128) * (size_t)kc * E), "cudaMalloc g~");
@@ -275,7 +279,9 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
              "phase_table(q,Re)");
     h->end_span(sp, st);
     sp = h->begin_span(1, st);
-    LAUNCH(h, launch_rp_to_q(h->g.as<c128>(), h->rows, np, h->Pq.as<c128>(), qb, h->g1.as<c128>(), st), "rp_to_q");
+    const c128 *g1b = h->ext_g1 ? h->ext_g1 + q0 * h->rows : h->g1.as<c128>();
+    if (!h->ext_g1)
+      LAUNCH(h, launch_rp_to_q(h->g.as<c128>(), h->rows, np, h->Pq.as<c128>(), qb, h->g1.as<c128>(), st), "rp_to_q");
     h->end_span(sp, st);
     sp = h->begin_span(2, st);
     LAUNCH(h, launch_interp_operator(h->D.as<c128>(), nm, np, h->Pq.as<c128>(), qb, h->Dq.as<c128>(), st), "D(q)");
@@ -293,7 +299,7 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
       LAUNCH(h, launch_pack_b_strided(h->eq.as<c128>() + (int64_t)iq * nmm, 1, nm, 0, 1, 0, omega_q + q * nm,
                                       h->cfg.omega_min, nm, nm, h->BpackE.as<double>(), st),
              "pack e_q");
-      LAUNCH(h, launch_zgemm_strided(h->g1.as<c128>() + (int64_t)iq * h->rows, xrows, 0, xrows, 0,
+      LAUNCH(h, launch_zgemm_strided(g1b + (int64_t)iq * h->rows, xrows, 0, xrows, 0,
                                      h->BpackE.as<double>(), nullptr, h->ghat.p, nbb, E, 1, nbb, 0, 0, xrows, nm, nm, 1,
                                      h->num_sms, st),
              "zgemm S4a");
@@ -417,6 +423,7 @@ int epw_interp_create(epw_interp_t *out, const epw_interp_config *cfg) {
   h->num_sms = prop.multiProcessorCount;
   h->q_batch = cfg->q_batch > 0 ? cfg->q_batch : 4;
   h->slab_set.assign(h->np, 0);
+  h->rp_cnt = h->np;
   *out = h;
   return EPW_OK;
 }
@@ -438,14 +445,14 @@ void epw_interp_destroy(epw_interp_t h) {
 
 int epw_interp_set_g_slabs(epw_interp_t h, int32_t ip_start, int32_t ip_count, const void *g_slabs, int on_device) {
   if (!h) return EPW_EINVAL;
-  if (!g_slabs || ip_start < 0 || ip_count <= 0 || ip_start + ip_count > h->np)
-    return h->fail(EPW_EINVAL, "epw_interp_set_g_slabs: bad slab range or null pointer");
+  if (!g_slabs || ip_start < h->rp_lo || ip_count <= 0 || ip_start + ip_count > h->rp_lo + h->rp_cnt)
+    return h->fail(EPW_EINVAL, "epw_interp_set_g_slabs: bad slab range (outside this handle's Rp shard) or null pointer");
   CU_OR_FAIL(h, cudaSetDevice(h->cfg.device), "cudaSetDevice");
-  const size_t total = (size_t)h->rows * h->np * sizeof(c128);
+  const size_t total = (size_t)h->rows * h->rp_cnt * sizeof(c128);
   CU_OR_FAIL(h, h->g.reserve(total), "cudaMalloc g(Re,Rp)");
   const size_t slab = (size_t)h->rows * sizeof(c128);
   CU_OR_FAIL(h,
-             cudaMemcpy(h->g.as<char>() + slab * ip_start, g_slabs, slab * ip_count,
+             cudaMemcpy(h->g.as<char>() + slab * (ip_start - h->rp_lo), g_slabs, slab * ip_count,
                         on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice),
              "cudaMemcpy g slabs");
   for (int i = 0; i < ip_count; i++) h->slab_set[ip_start + i] = 1;
@@ -499,7 +506,11 @@ int epw_interp_set_wannier_operators(epw_interp_t h, const void *H_R, const void
   fill_ones_kernel<<<(nmax + 255) / 256, 256>>>(h->ones.as<double>(), nmax);
   CU_OR_FAIL(h, cudaDeviceSynchronize(), "fill_ones");
   h->operators_set = true;
-  if (g_RR) return epw_interp_set_g_slabs(h, 0, h->np, g_RR, on_device);
+  if (g_RR) {
+    // g_RR holds every slab; a sharded handle keeps its own range only
+    const char *src = reinterpret_cast<const char *>(g_RR) + (size_t)h->rows * sizeof(c128) * h->rp_lo;
+    return epw_interp_set_g_slabs(h, h->rp_lo, h->rp_cnt, src, on_device);
+  }
   return EPW_OK;
 }
 
@@ -521,8 +532,13 @@ static int check_interpolate_args(epw_interp *h, const void *k_src, int64_t nk, 
   if (!k_src || !q_list || !eps_k || !omega_q || !g2 || nk <= 0 || nq <= 0)
     return h->fail(EPW_EINVAL, std::string(who) + ": null pointer or non-positive nk/nq");
   if (!h->operators_set) return h->fail(EPW_EINVAL, std::string(who) + ": operators not set");
-  for (int ip = 0; ip < h->np; ip++)
-    if (!h->slab_set[ip]) return h->fail(EPW_EINVAL, std::string(who) + ": g(Re,Rp) slab missing");
+  if (!h->ext_g1) {
+    if (h->sharded)
+      return h->fail(EPW_EINVAL, std::string(who) + ": this handle holds an Rp shard of g(Re,Rp); use "
+                                                   "epw_interp_rp_to_q_partial + an all-reduce + epw_interp_set_gq");
+    for (int ip = 0; ip < h->np; ip++)
+      if (!h->slab_set[ip]) return h->fail(EPW_EINVAL, std::string(who) + ": g(Re,Rp) slab missing");
+  }
   return EPW_OK;
 }
 
@@ -661,7 +677,7 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   CU_OR_FAIL(h, h->Pqe.reserve(sizeof(c128) * (size_t)QB * ne), "cudaMalloc Pqe");
   CU_OR_FAIL(h, h->Dq.reserve(sizeof(c128) * (size_t)QB * nmm), "cudaMalloc Dq");
   CU_OR_FAIL(h, h->eq.reserve(sizeof(c128) * (size_t)QB * nmm), "cudaMalloc e_q");
-  CU_OR_FAIL(h, h->g1.reserve(sizeof(c128) * (size_t)QB * h->rows), "cudaMalloc g(Re,q)");
+  if (!h->ext_g1) CU_OR_FAIL(h, h->g1.reserve(sizeof(c128) * (size_t)QB * h->rows), "cudaMalloc g(Re,q)");
   if (ncolsC) CU_OR_FAIL(h, h->C.reserve(sizeof(c128) * (size_t)c_rows * ncolsC), "cudaMalloc g~");
   if (!kq_map) CU_OR_FAIL(h, h->Ukq.reserve(sizeof(c128) * (size_t)c_rows * nbb), "cudaMalloc Ukq");
   if (!kq_map && !eps_kq) CU_OR_FAIL(h, h->epskq_scratch.reserve(sizeof(double) * (size_t)c_rows * nb), "cudaMalloc eps scratch");
@@ -764,7 +780,9 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
     h->end_span(sp, st);
     // ---- S1: Eq. 9 for the batch ----
     sp = h->begin_span(1, st);
-    LAUNCH(h, launch_rp_to_q(h->g.as<c128>(), h->rows, np, h->Pq.as<c128>(), qb, h->g1.as<c128>(), st), "rp_to_q");
+    const c128 *g1b = h->ext_g1 ? h->ext_g1 + q0 * h->rows : h->g1.as<c128>();
+    if (!h->ext_g1)
+      LAUNCH(h, launch_rp_to_q(h->g.as<c128>(), h->rows, np, h->Pq.as<c128>(), qb, h->g1.as<c128>(), st), "rp_to_q");
     h->end_span(sp, st);
     // ---- phonons: D(q), eigensolve, S4a hoisted into the B operand of S2 ----
     sp = h->begin_span(2, st);
@@ -779,7 +797,7 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
       sp = h->begin_span(8, st);
       for (int iq = 0; iq < qb; iq++)
         LAUNCH(h,
-               launch_pack_b(h->g1.as<c128>() + (int64_t)iq * h->rows, h->eq.as<c128>() + (int64_t)iq * nmm,
+               launch_pack_b(g1b + (int64_t)iq * h->rows, h->eq.as<c128>() + (int64_t)iq * nmm,
                              omega_q + (q0 + iq) * nm, h->cfg.omega_min, h->H.as<c128>(),
                              ncols_h ? h->Pqe.as<c128>() + (int64_t)iq * ne : nullptr, nbb, nm, ne, ncols_g, ncols_h,
                              h->Bpack.as<double>() + (int64_t)iq * NT * KB * GEMM_CHUNK, st),
@@ -792,7 +810,7 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
       const double *Bq = grid ? nullptr : h->Bpack.as<double>() + (int64_t)iq * NT * KB * GEMM_CHUNK;
       if (grid) {
         sp = h->begin_span(8, st);
-        LAUNCH(h, launch_box_scatter(h->g1.as<c128>() + (int64_t)iq * h->rows, h->eq.as<c128>() + (int64_t)iq * nmm,
+        LAUNCH(h, launch_box_scatter(g1b + (int64_t)iq * h->rows, h->eq.as<c128>() + (int64_t)iq * nmm,
                                      omega_q + q * nm, h->cfg.omega_min, h->H.as<c128>(),
                                      ncols_h ? h->Pqe.as<c128>() + (int64_t)iq * ne : nullptr, h->we.as<double>(),
                                      h->boxidx.as<int32_t>(), h->box_size, nbb, nm, ne, ncols_g, ncols_h,
@@ -875,6 +893,52 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
 }
 
 extern "C" {
+
+int epw_interp_set_rp_shard(epw_interp_t h, int32_t ip_start, int32_t ip_count) {
+  if (!h) return EPW_EINVAL;
+  if (ip_start < 0 || ip_count <= 0 || ip_start + ip_count > h->np)
+    return h->fail(EPW_EINVAL, "epw_interp_set_rp_shard: range outside [0, Np)");
+  if (h->g.p) return h->fail(EPW_EINVAL, "epw_interp_set_rp_shard: call before any g(Re,Rp) slab is uploaded");
+  h->rp_lo = ip_start;
+  h->rp_cnt = ip_count;
+  h->sharded = !(ip_start == 0 && ip_count == h->np);
+  return EPW_OK;
+}
+
+int epw_interp_rp_to_q_partial(epw_interp_t h, const double *q_list, int64_t nq, void *g1_partial, void *cuda_stream) {
+  if (!h) return EPW_EINVAL;
+  if (!q_list || !g1_partial || nq <= 0) return h->fail(EPW_EINVAL, "epw_interp_rp_to_q_partial: null pointer or nq <= 0");
+  if (!h->operators_set) return h->fail(EPW_EINVAL, "epw_interp_rp_to_q_partial: operators not set");
+  for (int ip = h->rp_lo; ip < h->rp_lo + h->rp_cnt; ip++)
+    if (!h->slab_set[ip]) return h->fail(EPW_EINVAL, "epw_interp_rp_to_q_partial: g(Re,Rp) slab of this shard missing");
+  CU_OR_FAIL(h, cudaSetDevice(h->cfg.device), "cudaSetDevice");
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  h->last_stream = st;
+  h->launches = 0;
+  const int QB = (int)std::min<int64_t>(h->q_batch, nq);
+  CU_OR_FAIL(h, h->Pq.reserve(sizeof(c128) * (size_t)QB * h->np), "cudaMalloc Pq");
+  c128 *out = reinterpret_cast<c128 *>(g1_partial);
+  for (int64_t q0 = 0; q0 < nq; q0 += QB) {
+    const int qb = (int)std::min<int64_t>(QB, nq - q0);
+    int sp = h->begin_span(0, st);
+    // phases of this shard's lattice vectors only: P[iq][ip - rp_lo]
+    LAUNCH(h, launch_phase_table(q_list + 3 * q0, qb, h->Rp.as<int32_t>() + 3 * h->rp_lo, h->wp.as<double>() + h->rp_lo,
+                                 h->rp_cnt, h->Pq.as<c128>(), st),
+           "phase_table(q,Rp shard)");
+    h->end_span(sp, st);
+    sp = h->begin_span(1, st);
+    LAUNCH(h, launch_rp_to_q(h->g.as<c128>(), h->rows, h->rp_cnt, h->Pq.as<c128>(), qb, out + q0 * h->rows, st),
+           "rp_to_q (partial)");
+    h->end_span(sp, st);
+  }
+  return EPW_OK;
+}
+
+int epw_interp_set_gq(epw_interp_t h, const void *g1_reduced) {
+  if (!h) return EPW_EINVAL;
+  h->ext_g1 = reinterpret_cast<const c128 *>(g1_reduced);
+  return EPW_OK;
+}
 
 int epw_interp_sync(epw_interp_t h) {
   if (!h) return EPW_EINVAL;
@@ -1180,8 +1244,13 @@ int epw_wannier_from_bloch(const void *gt, const double *kc, int64_t nkc, const 
                        al(sizeof(int32_t) * nqc), al(sizeof(c128) * nqc * rows)};
   size_t total = 0;
   for (size_t b : sz) total += b;
-  char *ws = nullptr;
-  if (cudaMalloc(&ws, total) != cudaSuccess) return EPW_ENOMEM;
+  // grow-only workspace kept between calls (cudaMalloc + cudaFree of ~1 GB cost more than the two contractions);
+  // like every stage-level entry point this call is not thread-safe
+  static DevBuf cache;
+  static int cache_dev = -1;
+  if (cache_dev != dev) { cache.release(); cache_dev = dev; }
+  if (cache.reserve(total) != cudaSuccess) return EPW_ENOMEM;
+  char *ws = cache.as<char>();
   char *p[8];
   size_t off = 0;
   for (int i = 0; i < 8; i++) { p[i] = ws + off; off += sz[i]; }
@@ -1191,7 +1260,6 @@ int epw_wannier_from_bloch(const void *gt, const double *kc, int64_t nkc, const 
       reinterpret_cast<double *>(p[4]), reinterpret_cast<double *>(p[5]), reinterpret_cast<int32_t *>(p[6]),
       reinterpret_cast<c128 *>(p[7]), reinterpret_cast<c128 *>(g_RR_out), nsm, st);
   cudaStreamSynchronize(st);
-  cudaFree(ws);
   return rc_of(e);
 }
 

@@ -64,3 +64,31 @@ def all_gather_rows(local, ranges, dist, device=None):
     parts = [torch.empty_like(pad) for _ in range(world)]
     dist.all_gather(parts, pad)
     return torch.cat([parts[r][: ranges[r][1] - ranges[r][0]] for r in range(world)], dim=0)
+
+
+def interpolate_rp_sharded(epw, handle, q_list, nq, rows, run_rest, dist=None, reduce_fn=None):
+    """One interpolation step with g(Re,Rp) split by Rp over the ranks: every rank contracts its own
+    slabs (`epw_interp_rp_to_q_partial`), the partial g(Re,q) are summed across ranks ON THE DEVICE and on the current
+    stream (NCCL all-reduce through torch.distributed -- the paper stages this through the host, L514-522), then
+    `run_rest()` (the caller's `epw_interp_interpolate[_grid]` on this rank's share of the k-points) runs with S1
+    replaced by the reduced g(Re,q).  `reduce_fn(tensor)` overrides the collective (tests on one GPU sum explicitly).
+    Returns the reduced g(Re,q) tensor [nq][rows][2] (kept alive by the caller until the stream has completed)."""
+    import torch
+
+    g1 = torch.empty((nq, rows, 2), dtype=torch.float64, device=q_list.device)
+    epw.epw_interp_rp_to_q_partial(handle, q_list, nq, g1)
+    if reduce_fn is not None:
+        g1 = reduce_fn(g1)
+    elif dist is not None and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(g1, op=dist.ReduceOp.SUM)
+    epw.epw_interp_set_gq(handle, g1)
+    try:
+        run_rest()
+    finally:
+        epw.epw_interp_set_gq(handle, None)
+    return g1
+
+
+def k_ranges(nk: int, world: int) -> list[tuple[int, int]]:
+    """After the all-reduce every rank holds g(Re,q) and interpolates its own contiguous share of the k-list."""
+    return q_ranges(nk, world)

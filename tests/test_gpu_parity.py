@@ -664,3 +664,57 @@ def test_config4_full_size_sampled(epw):
             print(f"config 4 full size, k {ik}: worst |g|^2 deviation {wst:.3f} x tolerance")
     finally:
         h.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# NEXT-1: g(Re,Rp) split by Rp over ranks.  One GPU here: the two "ranks" are two handles run
+# one after the other (no kernel waits on another), their partial g(Re,q) summed explicitly where NCCL would.
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("large", [False, True])
+def test_rp_sharded_two_handles(epw, large):
+    from paper_2603_10295_b200 import shard
+
+    if large:
+        w = synth.make_custom("zsnr-s", 18, 6, (3, 0, 0), 1.0, 0.05, 2.0, (40, 1, 1), ("random", 3, 1), seed=51)
+    else:
+        w = synth.make_custom("si-s", 8, 6, (1, 2, 1), 1.5, 0.1, 1.5, (6, 5, 4), ("random", 5, 3), seed=52)
+    ref = oracle.interpolate(w.H_R, w.D_R, w.g_full(), w.Re, w.w_e, w.Rp, w.w_p, w.k_list, w.q_list)
+    world = 2
+    rows = w.nbnd * w.nbnd * w.nmodes * w.ne
+    handles = []
+    try:
+        for r, (a, b) in enumerate(shard.rp_ranges(w.np_, world)):
+            h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_, q_batch=2)
+            h.set_operators_from_host(w, rp_range=(a, b))
+            handles.append(h)
+        # a sharded handle refuses the unsharded call
+        with pytest.raises(epw.EpwError):
+            handles[0].interpolate(dev(w.k_list), dev(w.q_list))
+        q_d = dev(w.q_list)
+        partial = []
+        for h in handles:
+            g1 = torch.empty((w.nq, rows, 2), dtype=torch.float64, device="cuda")
+            epw.epw_interp_rp_to_q_partial(h.h, q_d, w.nq, g1)
+            partial.append(g1)
+        total = partial[0] + partial[1]          # what dist.all_reduce(SUM) leaves on every rank
+        g1_ref = np.stack([oracle.rp_to_q(w.g_full(), w.Rp, w.w_p, q) for q in w.q_list]).reshape(w.nq, rows)
+        assert np.abs(znp(total) - g1_ref).max() <= 1e-13 * np.abs(g1_ref).max()
+        # each rank: the rest of the path on its own share of the k-points, through the helper bench / users call
+        outs = []
+        for r, (ka, kb) in enumerate(shard.k_ranges(w.nk, world)):
+            res = {}
+
+            def rest(h=handles[r], ka=ka, kb=kb):
+                res["out"] = h.interpolate(dev(w.k_list[ka:kb]), q_d)
+
+            shard.interpolate_rp_sharded(epw, handles[r].h, q_d, w.nq, rows, rest, reduce_fn=lambda t: total)
+            epw.epw_interp_sync(handles[r].h)
+            outs.append([t.cpu().numpy() for t in res["out"]])
+        eps_k = np.concatenate([o[0] for o in outs], axis=0)
+        eps_kq = np.concatenate([o[1] for o in outs], axis=1)
+        g2 = np.concatenate([o[3] for o in outs], axis=1)
+        assert_path_close((eps_k, eps_kq, outs[0][2], g2), ref)
+        np.testing.assert_array_equal(outs[0][2], outs[1][2])  # omega_q identical on both ranks
+    finally:
+        for h in handles:
+            h.close()

@@ -98,3 +98,50 @@ def test_q_sharded_run_world2_gloo(tmp_path):
     port = _free_port()
     mp.spawn(_worker, args=(2, port, str(tmp_path)), nprocs=2, join=True)
     assert (tmp_path / "ok").exists()
+
+
+def _worker_rp(rank: int, world: int, port: int, tmpdir: str):
+    """Rp-sharded variant: partial Eq. 9 per rank, all-reduce(SUM) of g(Re,q), then each rank
+    interpolates its share of the k-points.  Worker = the oracle; under test: rp_ranges / k_ranges / the collective."""
+    import torch
+    import torch.distributed as dist
+
+    sys.path.insert(0, ROOT)
+    import oracle
+    import synth
+
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    os.environ["OMP_NUM_THREADS"] = "1"
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        w = synth.make_custom("rp-shard", 2, 3, (1, 1, 0), 1.0, 0.1, 1.0, (3, 2, 1), ("random", 2, 2), seed=12)
+        g = w.g_full()
+        a, b = shard.rp_ranges(w.np_, world)[rank]
+        ka, kb = shard.k_ranges(w.nk, world)[rank]
+        g2_local = []
+        for q in w.q_list:
+            part = oracle.rp_to_q(g[a:b], w.Rp[a:b], w.w_p[a:b], q)           # this rank's slabs only
+            t = torch.from_numpy(part.view(np.float64).copy())
+            dist.all_reduce(t, op=dist.ReduceOp.SUM)                          # the one exchange step of the path
+            g1 = t.numpy().view(np.complex128).reshape(part.shape)
+            e_cm, om = oracle.phonon(w.D_R, w.Rp, w.w_p, q)
+            g2_local.append(np.stack([oracle.pair(g1, w.H_R, w.Re, w.w_e, e_cm, om, k, q)[0] for k in w.k_list[ka:kb]]))
+        g2_local = torch.from_numpy(np.stack(g2_local, axis=1))               # [nk_local][nq]...
+        g2_all = shard.all_gather_rows(g2_local, shard.k_ranges(w.nk, world), dist)
+        if rank == 0:
+            ref = oracle.interpolate(w.H_R, w.D_R, g, w.Re, w.w_e, w.Rp, w.w_p, w.k_list, w.q_list)[3]
+            got = np.swapaxes(g2_all.numpy(), 0, 1)
+            assert np.abs(got - ref).max() <= 1e-12 * np.abs(ref).max()
+            open(os.path.join(tmpdir, "ok_rp"), "w").write("ok")
+        dist.barrier()
+    finally:
+        dist.destroy_process_group()
+
+
+def test_rp_sharded_run_world2_gloo(tmp_path):
+    import torch.multiprocessing as mp
+
+    port = _free_port()
+    mp.spawn(_worker_rp, args=(2, port, str(tmp_path)), nprocs=2, join=True)
+    assert (tmp_path / "ok_rp").exists()
