@@ -62,6 +62,7 @@ def lib():
         L.oracle_eq7_direct.argtypes = [i, i, i, i, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         L.oracle_eq6_wannier_from_bloch.argtypes = [i, i, i, i, vp, vp, i, vp, i, vp, vp, vp]
         L.oracle_eq6_unrotate.argtypes = [i, i, vp, vp, vp, vp, vp, vp]
+        L.oracle_window_mask.argtypes = [i, i64, i64, vp, vp, f64, f64, vp]
         for name in ("oracle_g_bytes",):
             getattr(L, name).argtypes = [f64] * 4
             getattr(L, name).restype = f64
@@ -238,6 +239,15 @@ def eq6_unrotate(g, Ukq_cm, Uk_cm, e_cm, omega) -> np.ndarray:
     omega = _c(omega, np.float64)
     out = np.empty_like(g)
     lib().oracle_eq6_unrotate(nb, nm, _p(g), _p(Ukq_cm), _p(Uk_cm), _p(e_cm), _p(omega), _p(out))
+    return out
+
+
+def window_mask(eps_k, eps_kq, emin, emax) -> np.ndarray:
+    """Energy-window pre-screening: uint8 [nq][nk], 1 = pair kept."""
+    eps_k, eps_kq = _c(eps_k, np.float64), _c(eps_kq, np.float64)
+    nq, nk, nb = eps_kq.shape
+    out = np.empty((nq, nk), dtype=np.uint8)
+    lib().oracle_window_mask(nb, nk, nq, _p(eps_k), _p(eps_kq), float(emin), float(emax), _p(out))
     return out
 
 

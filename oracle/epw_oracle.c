@@ -402,6 +402,26 @@ void oracle_eq6_unrotate(int nb, int nm, const zc *g, const zc *Ukq, const zc *U
 }
 
 /* ---------------------------------------------------------------------------------------------
+ * Energy-window pre-screening: "skipping the calculation of the e-ph matrix elements involving
+ * states outside a ... energy window".  A pair (k,q) is KEPT iff the initial state and the final state can both lie in
+ * the window: some band of eps_k and some band of eps_{k+q} is in [emin, emax] (closed interval).
+ * mask[ik + nk*iq] = 1 (kept) or 0 (skipped; its |g|^2 block is reported as zeros).
+ * ------------------------------------------------------------------------------------------- */
+void oracle_window_mask(int nb, int64_t nk, int64_t nq, const double *eps_k, const double *eps_kq, double emin,
+                        double emax, unsigned char *mask) {
+  for (int64_t iq = 0; iq < nq; iq++)
+    for (int64_t ik = 0; ik < nk; ik++) {
+      int in_k = 0, in_kq = 0;
+      for (int b = 0; b < nb; b++) {
+        const double e1 = eps_k[b + nb * ik], e2 = eps_kq[b + nb * (ik + nk * iq)];
+        if (e1 >= emin && e1 <= emax) in_k = 1;
+        if (e2 >= emin && e2 <= emax) in_kq = 1;
+      }
+      mask[ik + nk * iq] = (unsigned char)(in_k && in_kq);
+    }
+}
+
+/* ---------------------------------------------------------------------------------------------
  * Bookkeeping helpers pinned by the paper's printed numbers.
  * ------------------------------------------------------------------------------------------- */
 /* Table III caption: size of g(Re,Rp) = 16 Nb^2 Nm Ne Np bytes. */

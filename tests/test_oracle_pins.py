@@ -523,3 +523,22 @@ def test_eq6_unrotate_matches_matrix_algebra_and_inverts_the_forward_rotations()
     np.testing.assert_allclose(oracle.eq6_unrotate(fwd, Ukq, Uk, e, omega), gt, rtol=0, atol=1e-13)
     # transposing a U or swapping k <-> k+q is detected
     assert np.abs(oracle.eq6_unrotate(fwd, Uk, Ukq, e, omega) - gt).max() > 1e-2
+
+
+# ---------------------------------------------------------------------------------------------
+# Energy-window pre-screening.
+# ---------------------------------------------------------------------------------------------
+def test_window_mask_hand_example_and_bruteforce():
+    """Pin (worked example + brute force): a pair is kept iff some band of eps_k AND some band of eps_{k+q} lies in
+    the closed window.  Hand example first, then random spectra against the one-line numpy statement."""
+    eps_k = np.array([[-1.0, 0.1, 2.0], [0.5, 0.6, 0.7], [-3.0, -2.0, 5.0]])            # k0 in, k1 out, k2 out for [0, 0.3]
+    eps_kq = np.array([[[0.3, 9.0, 9.0], [0.0, 0.0, 0.0], [0.2, 0.2, 0.2]],              # q0: kq in / in / in
+                       [[0.31, 9.0, 9.0], [0.1, 9.0, 9.0], [-0.01, 0.4, 1.0]]])          # q1: out / in / out
+    got = oracle.window_mask(eps_k, eps_kq, 0.0, 0.3)
+    np.testing.assert_array_equal(got, [[1, 0, 0], [0, 0, 0]])
+    got = oracle.window_mask(eps_k, eps_kq, 0.0, 0.5)                                     # edge value 0.5 is inside
+    np.testing.assert_array_equal(got, [[1, 1, 0], [1, 1, 0]])
+    ek, ekq = rng.uniform(-1, 1, (7, 4)), rng.uniform(-1, 1, (5, 7, 4))
+    ref = (((ek >= -0.2) & (ek <= 0.1)).any(-1)[None, :] & ((ekq >= -0.2) & (ekq <= 0.1)).any(-1)).astype(np.uint8)
+    np.testing.assert_array_equal(oracle.window_mask(ek, ekq, -0.2, 0.1), ref)
+    assert 0 < ref.sum() < ref.size
