@@ -41,6 +41,9 @@ def parse_args():
     ap.add_argument("--nq-step", type=int, default=0,
                     help="q-points per step (per GPU); 0 = 8, reduced so that the |g|^2 buffer of a step stays below 20 GB")
     ap.add_argument("--q-batch", type=int, default=0, help="library q_batch for S1 (0 = default)")
+    ap.add_argument("--energy-window", type=float, nargs=2, metavar=("EMIN", "EMAX"), default=None,
+                    help="NEXT-3 (PAPER.md:L241): pre-screen the pairs with this energy window (eV); the line then reports "
+                         "KEPT elements/s under its own metric name (not comparable with the unscreened headline)")
     ap.add_argument("--rp-shard", action="store_true",
                     help="NEXT-1 (PAPER.md:L186-188): g(Re,Rp) split by Rp over the ranks; per step every rank contracts "
                          "its slabs for the q-points of ALL ranks, one NCCL reduce-scatter of g(Re,q) hands each rank the "
@@ -312,6 +315,11 @@ def main():
     g2 = torch.empty((nq_step, nk, w.nmodes, w.nbnd, w.nbnd), dtype=torch.float64, device="cuda")  # reused every step
 
     use_grid = args.k_mode == "grid"
+    mask_dev = None
+    if args.energy_window:
+        mask_dev = torch.zeros((nq_step, nk), dtype=torch.uint8, device="cuda")
+        epw.epw_interp_set_energy_window(h.h, True, args.energy_window[0], args.energy_window[1], mask_dev)
+        args.no_e2e = True
     if args.rp_shard:
         args.no_e2e = True   # the host-buffer entry point has no Rp-sharded form
     rows = w.slab_elems
@@ -377,6 +385,12 @@ def main():
     ms, clocks, launches = m["ms"], m["clocks"], m["launches"]
     elements_per_step = nk * nq_step * E
     value = world * elements_per_step * args.steps / (ms * 1e-3)
+    window = None
+    if mask_dev is not None:
+        kept = float(mask_dev.float().mean().item())   # of the last step's pairs
+        window = {"emin": args.energy_window[0], "emax": args.energy_window[1], "kept_fraction_last_step": kept,
+                  "nominal_elements_per_s": value}
+        value *= kept
     # the same k-points handed over as a plain list (dense FP64 tensor-path S2), reported beside the grid arm
     m_list = measure(False, False) if (use_grid and not args.no_klist_arm) else None
 
@@ -543,7 +557,8 @@ def main():
 
     if rank == 0:
         line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "metric": METRIC if window is None else METRIC + " -- KEPT pairs only, energy-window pre-screening on",
+            "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {
@@ -557,7 +572,7 @@ def main():
                 "operator_upload_s": t_upload,
             },
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
-            "klist_path": klist_path, "cpu_baseline": cpu_baseline,
+            "klist_path": klist_path, "energy_window": window, "cpu_baseline": cpu_baseline,
         }
         print(json.dumps(line))
     h.close()

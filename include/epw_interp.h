@@ -137,6 +137,17 @@ int epw_interp_interpolate_grid_host(epw_interp_t h, const int32_t *k_grid, cons
                                      double *g2, void *cuda_stream);
 
 /*
+ * Energy-window pre-screening of the pairs ("skipping the calculation of the e-ph matrix elements
+ * involving states outside a 0.3 eV energy window").  While enabled, every following
+ * interpolate call keeps a pair (k,q) iff some band of eps_k AND some band of eps_{k+q} lies in the closed interval
+ * [emin, emax] (decided on the library's own FP64 eigenvalues, right after the eigensolves); the |g|^2 block of a
+ * skipped pair is written as zeros and its S4b work (and, on a uniform grid, the last axis pass of S2) is not done.
+ * eps_k, eps_kq and omega_q are still complete.  mask_out: NULL, or a device buffer uint8 [nq][nk] that receives
+ * 1 (kept) / 0 (skipped) for every pair of each call.  (To drop k-points altogether, pass the screened k-list.)
+ */
+int epw_interp_set_energy_window(epw_interp_t h, int enabled, double emin, double emax, uint8_t *mask_out);
+
+/*
  * g(Re,Rp) split over several GPUs by Rp (the paper's pool level for operators larger than one GPU's memory,
  * PAPER.md:L186-188, Table III; SURVEY.md 8(e) variant B / 8(f) NEXT-1).  Eq. 9 is a sum over Rp, so each
  * rank contracts its own slabs and the partial g(Re,q) are summed across ranks -- the paper does D2H + mp_sum on the

@@ -130,11 +130,18 @@ cudaError_t launch_grid_axis_phase(int N, int i0, int cnt, double shift, int lo,
 bool grid_rotate_g2_supported(int nb, int nm, int L1);
 cudaError_t launch_grid_rotate_g2(const c128 *T2, int64_t slab, int ncols, int L1, const c128 *P1c, int cnt,
                                   const c128 *Uk, const c128 *Ukq, const int32_t *kq_idx, int nb, int nm, int num_sms,
-                                  double *g2, cudaStream_t st);
+                                  const uint8_t *mask, double *g2, cudaStream_t st);
 cudaError_t launch_grid_klist(const int32_t N[3], const double s[3], double *k_list, cudaStream_t st);
 
+// mask (may be NULL): uint8 per pair, 0 = skipped by the energy-window pre-screening -> zeros, no arithmetic
 cudaError_t launch_rotate_g2(const c128 *gt, int64_t stride_gt, const c128 *Uk, const c128 *Ukq, const int32_t *kq_idx,
-                             int nb, int nm, int64_t nk, double *g2, cudaStream_t st);
+                             int nb, int nm, int64_t nk, const uint8_t *mask, double *g2, cudaStream_t st);
+// Energy-window pre-screening (window.cu): mask[ik] = some band of eps_k[ik] AND some band of
+// eps_{k+q}[ik] (= eps_kq[ik], or eps_k_all[kq_idx[ik]] when kq_idx is given) lies in [emin, emax].
+cudaError_t launch_window_mask(const double *eps_k, const double *eps_kq, const double *eps_k_all, const int32_t *kq_idx,
+                               int nb, int64_t nk, double emin, double emax, uint8_t *mask, cudaStream_t st);
+// g2 blocks (E doubles each) of the skipped pairs <- 0 (kernel families that cannot skip: large-Nb path)
+cudaError_t launch_zero_masked(const uint8_t *mask, int64_t nk, int64_t E, double *g2, cudaStream_t st);
 
 bool rotate_g2_small_supported(int nb, int nm);  // Nb <= 16 and the T staging buffer of one pair fits shared memory
 

@@ -34,7 +34,8 @@ template <int NB, int W>
 __global__ void __launch_bounds__(W * 32, 2)
     grid_rotate_g2_kernel(const c128 *__restrict__ T2, int64_t slab, int ncols, int L1, const c128 *__restrict__ P1c,
                           int cnt, int i1_per_cta, const c128 *__restrict__ Uk, const c128 *__restrict__ Ukq,
-                          const int32_t *__restrict__ kq_idx, int nm, int nug, double *__restrict__ g2) {
+                          const int32_t *__restrict__ kq_idx, int nm, int nug, const uint8_t *__restrict__ mask,
+                          double *__restrict__ g2) {
   constexpr int KS = (2 * NB + 3) / 4;  // k-steps of 4 real
   constexpr int NT = (2 * NB + 7) / 8;  // column tiles of 8 real
   constexpr int SP = grot_pitch(NB);
@@ -74,6 +75,12 @@ __global__ void __launch_bounds__(W * 32, 2)
   const int j_hi = j_lo + i1_per_cta < cnt ? j_lo + i1_per_cta : cnt;
   for (int j = j_lo + warp; j < j_hi; j += W) {
     const int64_t kc = (int64_t)j * slab + cell;   // k index relative to the chunk
+    if (mask != nullptr && mask[kc] == 0) {
+      // energy-window pre-screening: a skipped pair reports zeros and costs no arithmetic
+      double *dz = g2 + kc * E + (int64_t)nu0 * NBB;
+      for (int i = lane; i < rows * NB; i += 32) dz[i] = 0.0;
+      continue;
+    }
     if (lane < L1) sP[lane] = P1c[(int64_t)lane * cnt + j];
     // ---- B' = embedding of Uk, B'' = embedding of conj(Ukq); fragment (ks, nt): k-row 4 ks + t, column 8 nt + g ----
     double b1[KS][NT], b2[KS][NT];
@@ -165,7 +172,8 @@ __global__ void __launch_bounds__(W * 32, 2)
 
 template <int NB, int W>
 static cudaError_t launch_grot(const c128 *T2, int64_t slab, int ncols, int L1, const c128 *P1c, int cnt, const c128 *Uk,
-                               const c128 *Ukq, const int32_t *kq_idx, int nm, int num_sms, double *g2, cudaStream_t st) {
+                               const c128 *Ukq, const int32_t *kq_idx, int nm, int num_sms, const uint8_t *mask, double *g2,
+                               cudaStream_t st) {
   if (L1 > 32) return cudaErrorInvalidConfiguration;
   // modes per CTA: as many as keep (T2 rows + W staging buffers + phases) within ~100 KB, i.e. two CTAs per SM
   const size_t budget = (size_t)110 << 10;
@@ -191,7 +199,7 @@ static cudaError_t launch_grot(const c128 *T2, int64_t slab, int ncols, int L1, 
   if (slab > 2147483647LL || nsplit > 65535) return cudaErrorInvalidConfiguration;
   dim3 grid((unsigned)slab, (unsigned)ngroups, (unsigned)nsplit);
   grid_rotate_g2_kernel<NB, W><<<grid, W * 32, smem, st>>>(T2, slab, ncols, L1, P1c, cnt, i1_per_cta, Uk, Ukq, kq_idx, nm,
-                                                          nug, g2);
+                                                          nug, mask, g2);
   return cudaGetLastError();
 }
 
@@ -207,11 +215,11 @@ bool grid_rotate_g2_supported(int nb, int nm, int L1) {
 // i1 planes of this chunk; Uk, Ukq, kq_idx, g2 are relative to the first k of the chunk (k = j*slab + cell).
 cudaError_t launch_grid_rotate_g2(const c128 *T2, int64_t slab, int ncols, int L1, const c128 *P1c, int cnt,
                                   const c128 *Uk, const c128 *Ukq, const int32_t *kq_idx, int nb, int nm, int num_sms,
-                                  double *g2, cudaStream_t st) {
+                                  const uint8_t *mask, double *g2, cudaStream_t st) {
   if (slab <= 0 || cnt <= 0) return cudaSuccess;
   switch (nb) {
 #define EPW_GROT_CASE(NB_, W_) \
-  case NB_: return launch_grot<NB_, W_>(T2, slab, ncols, L1, P1c, cnt, Uk, Ukq, kq_idx, nm, num_sms, g2, st);
+  case NB_: return launch_grot<NB_, W_>(T2, slab, ncols, L1, P1c, cnt, Uk, Ukq, kq_idx, nm, num_sms, mask, g2, st);
     EPW_GROT_CASE(1, 8) EPW_GROT_CASE(2, 8) EPW_GROT_CASE(3, 8) EPW_GROT_CASE(4, 8) EPW_GROT_CASE(5, 8)
     EPW_GROT_CASE(6, 8) EPW_GROT_CASE(7, 8) EPW_GROT_CASE(8, 8) EPW_GROT_CASE(9, 4) EPW_GROT_CASE(10, 4)
     EPW_GROT_CASE(11, 4) EPW_GROT_CASE(12, 4) EPW_GROT_CASE(13, 4) EPW_GROT_CASE(14, 4) EPW_GROT_CASE(15, 4)

@@ -86,6 +86,11 @@ struct epw_interp {
   // Rp shard (NEXT-1): this handle keeps only slabs [rp_lo, rp_lo + rp_cnt) of g(Re,Rp)
   int rp_lo = 0, rp_cnt = 0;
   bool sharded = false;
+  // energy-window pre-screening (NEXT-3)
+  bool window_on = false;
+  double emin = 0.0, emax = 0.0;
+  uint8_t *mask_out = nullptr;   // caller's device buffer [nq][nk] or NULL
+  DevBuf maskbuf;
   const c128 *ext_g1 = nullptr;  // g(Re,q) supplied by the caller (already summed over every rank's Rp) for this call
   // resident operators
   DevBuf g, H, D, Re, Rp, we, wp, ones;
@@ -225,6 +230,7 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
     if (!eps_kq) CU_OR_FAIL(h, h->epskq_scratch.reserve(sizeof(double) * (size_t)nk * nb), "cudaMalloc eps scratch");
   }
   CU_OR_FAIL(h, h->status.reserve(sizeof(int32_t)), "cudaMalloc status");
+  if (h->window_on && !h->mask_out) CU_OR_FAIL(h, h->maskbuf.reserve((size_t)nk), "cudaMalloc mask");
   {
     const size_t need = std::max(eigh_large_scratch_bytes(nb, nk), eigh_large_scratch_bytes(nm, QB));
     if (need) CU_OR_FAIL(h, h->eig_scratch.reserve(need), "cudaMalloc eig scratch");
@@ -351,6 +357,14 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
                                        kq_map ? kq_map + q * nk + k0 : nullptr, g2 + (q * nk + k0) * E, MR, 0, nb, 1, E,
                                        1, MR, nb, nb, kn, h->num_sms, st),
                "zgemm S4b (U_{k+q}) + |g|^2");
+        if (h->window_on) {
+          // the in-place contractions of this kernel family cannot skip pairs: screened pairs are zeroed afterwards
+          uint8_t *m = (h->mask_out ? h->mask_out + q * nk : h->maskbuf.as<uint8_t>()) + k0;
+          const double *ekq = kq_map ? nullptr : (eps_kq ? eps_kq + (q * nk + k0) * nb : h->epskq_scratch.as<double>() + k0 * nb);
+          LAUNCH(h, launch_window_mask(eps_k + k0 * nb, ekq, eps_k, kq_map ? kq_map + q * nk + k0 : nullptr, nb, kn, h->emin,
+                                       h->emax, m, st), "window mask");
+          LAUNCH(h, launch_zero_masked(m, kn, E, g2 + (q * nk + k0) * E, st), "zero screened pairs");
+        }
         h->end_span(sp, st);
       }
     }
@@ -437,7 +451,7 @@ void epw_interp_destroy(epw_interp_t h) {
                    &h->status, &h->eig_scratch, &h->hs_k, &h->hs_q, &h->hs_map, &h->hs_epsk, &h->hs_epskq,
                    &h->hs_omega, &h->hs_g2, &h->Pk, &h->BpackPk, &h->UpackK, &h->UpackKH, &h->BpackE,
                    &h->ghat, &h->T, &h->Hkq, &h->boxidx, &h->X, &h->T1, &h->T2, &h->Ptmp, &h->P1raw, &h->P1pack, &h->P2pack,
-                   &h->P3pack, &h->klist_gen, &h->workctr};
+                   &h->P3pack, &h->klist_gen, &h->workctr, &h->maskbuf};
   for (DevBuf *b : all) b->release();
   for (cudaEvent_t ev : h->ev_pool) cudaEventDestroy(ev);
   delete h;
@@ -682,6 +696,7 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   if (!kq_map) CU_OR_FAIL(h, h->Ukq.reserve(sizeof(c128) * (size_t)c_rows * nbb), "cudaMalloc Ukq");
   if (!kq_map && !eps_kq) CU_OR_FAIL(h, h->epskq_scratch.reserve(sizeof(double) * (size_t)c_rows * nb), "cudaMalloc eps scratch");
   CU_OR_FAIL(h, h->status.reserve(sizeof(int32_t)), "cudaMalloc status");
+  if (h->window_on && !h->mask_out) CU_OR_FAIL(h, h->maskbuf.reserve((size_t)nk), "cudaMalloc mask");
   {
     const size_t need = std::max(eigh_large_scratch_bytes(nb, nk), eigh_large_scratch_bytes(nm, QB));
     if (need) CU_OR_FAIL(h, h->eig_scratch.reserve(need), "cudaMalloc eig scratch");
@@ -870,17 +885,28 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
           h->end_span(sp, st);
           Ukq_ptr = Ukq_c;
         }
+        // ---- energy-window pre-screening of the pairs of this chunk ----
+        const uint8_t *mask = nullptr;
+        if (h->window_on) {
+          uint8_t *m = h->mask_out ? h->mask_out + q * nk + k0 : h->maskbuf.as<uint8_t>();
+          const double *ekq = kq_map ? nullptr
+                                     : (eps_kq ? eps_kq + (q * nk + k0) * nb : h->epskq_scratch.as<double>() + crow * nb);
+          sp = h->begin_span(5, st);
+          LAUNCH(h, launch_window_mask(eps_k + k0 * nb, ekq, eps_k, kq_idx, nb, kn, h->emin, h->emax, m, st), "window mask");
+          h->end_span(sp, st);
+          mask = m;
+        }
         // ---- S4b: band rotation + |g|^2 ----
         sp = h->begin_span(6, st);
         if (!fused) {
-          LAUNCH(h, launch_rotate_g2(Cc, ncols, h->Uk.as<c128>() + k0 * nbb, Ukq_ptr, kq_idx, nb, nm, kn,
+          LAUNCH(h, launch_rotate_g2(Cc, ncols, h->Uk.as<c128>() + k0 * nbb, Ukq_ptr, kq_idx, nb, nm, kn, mask,
                                      g2 + (q * nk + k0) * E, st),
                  "rotate_g2");
         } else {
           const int ci = (int)(k0 / kchunk);
           const int cnt = std::min(cs, grid->N[0] - ci * cs);
           LAUNCH(h, launch_grid_rotate_g2(h->T2.as<c128>(), slab, ncols, L[0], h->P1raw.as<c128>() + (int64_t)ci * L[0] * cs,
-                                          cnt, h->Uk.as<c128>() + k0 * nbb, Ukq_ptr, kq_idx, nb, nm, h->num_sms,
+                                          cnt, h->Uk.as<c128>() + k0 * nbb, Ukq_ptr, kq_idx, nb, nm, h->num_sms, mask,
                                           g2 + (q * nk + k0) * E, st),
                  "grid_rotate_g2");
         }
@@ -893,6 +919,16 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
 }
 
 extern "C" {
+
+int epw_interp_set_energy_window(epw_interp_t h, int enabled, double emin, double emax, uint8_t *mask_out) {
+  if (!h) return EPW_EINVAL;
+  if (enabled && !(emin <= emax)) return h->fail(EPW_EINVAL, "epw_interp_set_energy_window: need emin <= emax");
+  h->window_on = enabled != 0;
+  h->emin = emin;
+  h->emax = emax;
+  h->mask_out = enabled ? mask_out : nullptr;
+  return EPW_OK;
+}
 
 int epw_interp_set_rp_shard(epw_interp_t h, int32_t ip_start, int32_t ip_count) {
   if (!h) return EPW_EINVAL;
@@ -1190,7 +1226,7 @@ int epw_rotate_g2(const void *gt, int64_t stride_gt, const void *Uk, const void 
   if (!gt || !Uk || !Ukq || !g2 || nb <= 0 || nm <= 0 || nk < 0) return EPW_EINVAL;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
   const cudaError_t e = launch_rotate_g2(reinterpret_cast<const c128 *>(gt), stride_gt, reinterpret_cast<const c128 *>(Uk),
-                                         reinterpret_cast<const c128 *>(Ukq), kq_idx, nb, nm, nk, g2, st);
+                                         reinterpret_cast<const c128 *>(Ukq), kq_idx, nb, nm, nk, nullptr, g2, st);
   if (e != cudaErrorInvalidConfiguration) return rc_of(e);
   // large (Nb, Nm): T[(nu,m')][n] = sum_n' g~[(nu,m')][n'] U_k[n'][n];  |g|^2[(nu,n)][m] = |sum_m' T[(nu,n)][m'] conj(Ukq[m'][m])|^2
   cudaGetLastError();

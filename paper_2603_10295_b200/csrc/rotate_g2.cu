@@ -30,7 +30,7 @@ template <int NB, int WPP>
 __global__ void __launch_bounds__(ROT_THREADS)
     rotate_g2_dmma_kernel(const c128 *__restrict__ gt, int64_t stride_gt, const c128 *__restrict__ Uk,
                           const c128 *__restrict__ Ukq, const int32_t *__restrict__ kq_idx, int nm, int64_t nk,
-                          double *__restrict__ g2) {
+                          const uint8_t *__restrict__ mask, double *__restrict__ g2) {
   constexpr int KS = (2 * NB + 3) / 4;  // k-steps of 4 real
   constexpr int NT = (2 * NB + 7) / 8;  // column tiles of 8 real
   constexpr int SP = rot_pitch(NB);
@@ -53,6 +53,14 @@ __global__ void __launch_bounds__(ROT_THREADS)
     const int64_t ik = (pass * gridDim.x + blockIdx.x) * PPC + slot;
     const bool have = ik < nk;
     const int64_t ikc = have ? ik : 0;
+    // energy-window pre-screening: a skipped pair reports zeros and costs no arithmetic.  The decision is
+    // uniform over the WPP warps of a pair; with WPP > 1 every warp still takes the two block-wide barriers below.
+    const bool skip = mask != nullptr && have && mask[ikc] == 0;
+    if (skip) {
+      double *dz = g2 + ikc * (int64_t)rows * NB;
+      for (int i = sub * 32 + lane; i < rows * NB; i += WPP * 32) dz[i] = 0.0;
+    }
+    if (skip && WPP == 1) continue;
     // ---- B' = embedding of Uk, B'' = embedding of conj(Ukq); fragment (ks, nt): k-row 4 ks + t, column 8 nt + g ----
     double b1[KS][NT], b2[KS][NT];
     {
@@ -76,7 +84,7 @@ __global__ void __launch_bounds__(ROT_THREADS)
     }
     // ---- product 1: T[(nu,m')][n] ----
     const double *gsrc = reinterpret_cast<const double *>(gt + ikc * stride_gt);
-    for (int mt = sub; mt < MT; mt += WPP) {
+    for (int mt = sub; mt < (skip ? 0 : MT); mt += WPP) {
       const int row = 8 * mt + g;
       const bool rv = row < rows;
       const int nu = row / NB, mp = row - nu * NB;
@@ -107,7 +115,7 @@ __global__ void __launch_bounds__(ROT_THREADS)
     else __syncthreads();
     // ---- product 2: |sum_m' T[(nu,n)][m'] conj(Ukq[m'][m])|^2 ----
     double *dst = g2 + ikc * (int64_t)rows * NB;
-    for (int mt = sub; mt < MT; mt += WPP) {
+    for (int mt = sub; mt < (skip ? 0 : MT); mt += WPP) {
       const int row = 8 * mt + g;
       const double *arow = sT + (size_t)row * SP * 2 + t;
       double acc[NT][2];
@@ -134,7 +142,7 @@ __global__ void __launch_bounds__(ROT_THREADS)
 
 template <int NB, int WPP>
 static cudaError_t launch_rot(const c128 *gt, int64_t stride_gt, const c128 *Uk, const c128 *Ukq, const int32_t *kq_idx,
-                              int nm, int64_t nk, double *g2, size_t smem_per_pair, cudaStream_t st) {
+                              int nm, int64_t nk, const uint8_t *mask, double *g2, size_t smem_per_pair, cudaStream_t st) {
   constexpr int PPC = ROT_WARPS / WPP;
   const size_t smem = smem_per_pair * PPC;
   if (smem > 48 * 1024) {
@@ -144,20 +152,21 @@ static cudaError_t launch_rot(const c128 *gt, int64_t stride_gt, const c128 *Uk,
   }
   const int64_t want = ceil_div(nk, PPC);
   const int64_t grid = want < 148 * 16 ? want : 148 * 16;
-  rotate_g2_dmma_kernel<NB, WPP><<<(unsigned)grid, ROT_THREADS, smem, st>>>(gt, stride_gt, Uk, Ukq, kq_idx, nm, nk, g2);
+  rotate_g2_dmma_kernel<NB, WPP><<<(unsigned)grid, ROT_THREADS, smem, st>>>(gt, stride_gt, Uk, Ukq, kq_idx, nm, nk, mask, g2);
   return cudaGetLastError();
 }
 
 template <int NB>
 static cudaError_t launch_rot_nb(const c128 *gt, int64_t stride_gt, const c128 *Uk, const c128 *Ukq,
-                                 const int32_t *kq_idx, int nm, int64_t nk, double *g2, cudaStream_t st) {
+                                 const int32_t *kq_idx, int nm, int64_t nk, const uint8_t *mask, double *g2,
+                                 cudaStream_t st) {
   const int MT = (nm * NB + 7) / 8;
   const size_t per_pair = sizeof(c128) * (size_t)MT * 8 * rot_pitch(NB);
   if (per_pair > (size_t)200 * 1024) return cudaErrorInvalidConfiguration;
   // one warp per pair while four staging buffers fit comfortably; otherwise 2 or 4 warps share a pair
-  if (per_pair <= (size_t)12 * 1024) return launch_rot<NB, 1>(gt, stride_gt, Uk, Ukq, kq_idx, nm, nk, g2, per_pair, st);
-  if (per_pair <= (size_t)24 * 1024) return launch_rot<NB, 2>(gt, stride_gt, Uk, Ukq, kq_idx, nm, nk, g2, per_pair, st);
-  return launch_rot<NB, 4>(gt, stride_gt, Uk, Ukq, kq_idx, nm, nk, g2, per_pair, st);
+  if (per_pair <= (size_t)12 * 1024) return launch_rot<NB, 1>(gt, stride_gt, Uk, Ukq, kq_idx, nm, nk, mask, g2, per_pair, st);
+  if (per_pair <= (size_t)24 * 1024) return launch_rot<NB, 2>(gt, stride_gt, Uk, Ukq, kq_idx, nm, nk, mask, g2, per_pair, st);
+  return launch_rot<NB, 4>(gt, stride_gt, Uk, Ukq, kq_idx, nm, nk, mask, g2, per_pair, st);
 }
 
 bool rotate_g2_small_supported(int nb, int nm) {
@@ -167,11 +176,11 @@ bool rotate_g2_small_supported(int nb, int nm) {
 }
 
 cudaError_t launch_rotate_g2(const c128 *gt, int64_t stride_gt, const c128 *Uk, const c128 *Ukq, const int32_t *kq_idx,
-                             int nb, int nm, int64_t nk, double *g2, cudaStream_t st) {
+                             int nb, int nm, int64_t nk, const uint8_t *mask, double *g2, cudaStream_t st) {
   if (nk <= 0) return cudaSuccess;
   switch (nb) {
 #define EPW_ROT_CASE(NB_) \
-  case NB_: return launch_rot_nb<NB_>(gt, stride_gt, Uk, Ukq, kq_idx, nm, nk, g2, st);
+  case NB_: return launch_rot_nb<NB_>(gt, stride_gt, Uk, Ukq, kq_idx, nm, nk, mask, g2, st);
     EPW_ROT_CASE(1) EPW_ROT_CASE(2) EPW_ROT_CASE(3) EPW_ROT_CASE(4) EPW_ROT_CASE(5) EPW_ROT_CASE(6) EPW_ROT_CASE(7)
     EPW_ROT_CASE(8) EPW_ROT_CASE(9) EPW_ROT_CASE(10) EPW_ROT_CASE(11) EPW_ROT_CASE(12) EPW_ROT_CASE(13)
     EPW_ROT_CASE(14) EPW_ROT_CASE(15) EPW_ROT_CASE(16)

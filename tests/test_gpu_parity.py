@@ -718,3 +718,65 @@ def test_rp_sharded_two_handles(epw, large):
     finally:
         for h in handles:
             h.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# NEXT-3: energy-window pre-screening of the pairs
+# ---------------------------------------------------------------------------------------------------------
+def pick_window(eps_all, frac_lo=0.48, frac_hi=0.52, margin=1e-6):
+    """A window whose edges are at least `margin` away from every eigenvalue, so that the keep / skip decision is the
+    same on both sides although their eigenvalues differ in the last digits (floats deciding an integer)."""
+    v = np.sort(np.asarray(eps_all).ravel())
+    lo, hi = v[int(frac_lo * len(v))], v[int(frac_hi * len(v))]
+    for edge in ("lo", "hi"):
+        x = lo if edge == "lo" else hi
+        while np.abs(v - x).min() < margin:
+            x += 3.3 * margin
+        lo, hi = (x, hi) if edge == "lo" else (lo, x)
+    return float(lo), float(hi)
+
+
+@pytest.mark.parametrize("mode", ["grid-fused", "grid-unfused", "list", "list-kqmap", "large"])
+def test_energy_window_screening(epw, mode):
+    if mode == "large":
+        w = synth.make_custom("zsnr-w", 18, 5, (2, 0, 0), 1.0, 0.05, 2.0, (30, 1, 1), ("random", 3, 1), seed=61)
+    else:
+        w = synth.make_config(0)
+    ql = w.q_list[:6] if mode == "list-kqmap" else (w.q_list[:6] + ([0.013, 0.007, 0.021] if mode != "large" else 0.0))
+    kq_map = np.ascontiguousarray(w.kq_map[:6]) if mode == "list-kqmap" else None
+    ref = oracle.interpolate(w.H_R, w.D_R, w.g_full(), w.Re, w.w_e, w.Rp, w.w_p, w.k_list, ql)
+    emin, emax = pick_window(np.concatenate([ref[0].ravel(), ref[1].ravel()]))
+    mask_ref = oracle.window_mask(ref[0], ref[1], emin, emax)
+    assert 0.02 < mask_ref.mean() < 0.95      # the window really screens, and really keeps
+    g2_ref = ref[3] * mask_ref[:, :, None, None, None]
+    h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_, q_batch=4,
+                      flags=epw.EPW_FLAG_GRID_UNFUSED if mode == "grid-unfused" else 0)
+    try:
+        h.set_operators_from_host(w)
+        mask_d = torch.full((len(ql), w.nk), 7, dtype=torch.uint8, device="cuda")
+        epw.epw_interp_set_energy_window(h.h, True, emin, emax, mask_d)
+        if mode.startswith("grid"):
+            out = h.interpolate_grid(w.k_grid, dev(ql))
+        else:
+            out = h.interpolate(dev(w.k_list), dev(ql), None if kq_map is None else dev(kq_map))
+        epw.epw_interp_sync(h.h)
+        eps_k, eps_kq, om, g2 = [t.cpu().numpy() for t in out]
+        np.testing.assert_array_equal(mask_d.cpu().numpy(), mask_ref)        # integer decision: bit-exact
+        assert (g2[mask_ref == 0] == 0.0).all()                              # skipped pairs report exact zeros
+        kept = [(iq, ik) for iq in range(len(ql)) for ik in range(w.nk) if mask_ref[iq, ik]]
+        assert_path_close((eps_k, eps_kq, om, g2), (ref[0], ref[1], ref[2], g2_ref), pairs=kept)
+        # switching the window off restores the full result (no internal mask buffer this time)
+        epw.epw_interp_set_energy_window(h.h, False)
+        out = h.interpolate_grid(w.k_grid, dev(ql)) if mode.startswith("grid") else \
+            h.interpolate(dev(w.k_list), dev(ql), None if kq_map is None else dev(kq_map))
+        epw.epw_interp_sync(h.h)
+        assert_path_close([t.cpu().numpy() for t in out], ref, pairs=kept[:50] + [(0, 0), (len(ql) - 1, w.nk - 1)])
+        # internal mask buffer (mask_out = NULL)
+        epw.epw_interp_set_energy_window(h.h, True, emin, emax, None)
+        out = h.interpolate_grid(w.k_grid, dev(ql)) if mode.startswith("grid") else \
+            h.interpolate(dev(w.k_list), dev(ql), None if kq_map is None else dev(kq_map))
+        epw.epw_interp_sync(h.h)
+        g2b = out[3].cpu().numpy()
+        assert (g2b[mask_ref == 0] == 0.0).all() and np.array_equal(g2b != 0, g2 != 0)
+    finally:
+        h.close()
