@@ -3,12 +3,16 @@
 
 Metric (BASELINE.json): interpolated |g(k,q)|^2 elements/s in FP64, elements = Nk * Nq * Nb^2 * Nm.
 Workload at N = 1: BASELINE.json configs[1] ("Si-like production": Nb=8, Nm=6, Ne=Np=343, 40^3 k grid, random q).
-A step = one epw_interp_interpolate call over ALL 64,000 k and a batch of `--nq-step` q-points: every stage of the
-path (S0 phase tables, S1 Rp->q, D(q)/H(k)/H(k+q) + eigensolves, S4a, S2 Re->k on the FP64 tensor path, S4b + |g|^2).
+A step = one interpolate call over ALL 64,000 k and a batch of `--nq-step` q-points: every stage of the path (S0 phase
+tables, S1 Rp->q, D(q)/H(k)/H(k+q) + eigensolves, S4a, S2 Re->k, S4b + |g|^2).  `--k-mode grid` (default) hands the k-points
+over as the uniform grid they are (epw_interp_interpolate_grid: factorised S2); `--k-mode list` as a plain list (dense FP64
+tensor-path S2); in grid mode the list form is timed as well and reported as `klist_path`.
 With N > 1 the q-points are sharded over ranks (the paper's image level: no communication inside
-the loop) -> weak scaling, no data-path collective.
+the loop) -> weak scaling, no data-path collective; `--rp-shard` splits g(Re,Rp) by Rp instead (one reduce-scatter per step).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--nq-step Q] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--nq-step Q] [--k-mode grid|list] [--impl reference]
+    python bench.py --eq6 [--config I]                 Eq. 6 (Bloch -> Wannier), own JSON line
+    python bench.py --energy-window EMIN EMAX          with pair pre-screening, own metric name
 
 `--impl reference` times the CPU oracle (oracle/, plain C) on the host cores on a bounded sample of the same
 workload; it is a deliberately slow baseline, not a target.
