@@ -43,7 +43,7 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (default 1 = Si-like production)")
     ap.add_argument("--nq-step", type=int, default=0,
-                    help="q-points per step (per GPU); 0 = 8, reduced so that the |g|^2 buffer of a step stays below 20 GB")
+                    help="q-points per step (per GPU); 0 = 32, reduced so that the |g|^2 buffer of a step stays below 40 GB")
     ap.add_argument("--q-batch", type=int, default=0, help="library q_batch for S1 (0 = default)")
     ap.add_argument("--energy-window", type=float, nargs=2, metavar=("EMIN", "EMAX"), default=None,
                     help="NEXT-3 (PAPER.md:L241): pre-screen the pairs with this energy window (eV); the line then reports "
@@ -290,7 +290,9 @@ def main():
 
     w = synth.make_config(args.config)
     nk, E = w.nk, w.elements_per_pair
-    nq_step = args.nq_step or max(1, min(8, int((20 << 30) // (8 * nk * E))))
+    # q-points per interpolate call: the k side (phases, H(k), U_k) is computed once per call, so a caller batches as
+    # many q as its |g|^2 buffer allows; here at most 32 q and at most 40 GB of output per step
+    nq_step = args.nq_step or max(1, min(32, int((40 << 30) // (8 * nk * E))))
     nq_step = min(nq_step, w.nq)
     h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_, device=local_rank, q_batch=args.q_batch,
                       flags=epw.EPW_FLAG_GRID_UNFUSED if args.grid_unfused else 0)
