@@ -108,6 +108,7 @@ struct epw_interp {
     eigh_set_work_counter(timing && slot >= 0 && workctr.p ? workctr.as<unsigned long long>() + slot : nullptr);
   }
   int last_kmode = 0;
+  int64_t last_eq_slot = 0;  // slot of the last q of the last call inside the e_q buffer (debug getter)
   // host-entry staging
   DevBuf hs_k, hs_q, hs_map, hs_epsk, hs_epskq, hs_omega, hs_g2;
   // bookkeeping of the last call
@@ -240,6 +241,7 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
   h->last_c_rows = kc;
   h->last_ncols = (int)E;
   h->last_path = EPW_PATH_LARGE;
+  h->last_eq_slot = (nq - 1) % QB;
   h->last_qb = QB;
   h->last_kchunk = kc;
 
@@ -435,7 +437,7 @@ int epw_interp_create(epw_interp_t *out, const epw_interp_config *cfg) {
   h->nmm = h->nm * h->nm;
   h->rows = (int64_t)h->nbb * h->ne * h->nm;
   h->num_sms = prop.multiProcessorCount;
-  h->q_batch = cfg->q_batch > 0 ? cfg->q_batch : 4;
+  h->q_batch = cfg->q_batch > 0 ? cfg->q_batch : 8;
   h->slab_set.assign(h->np, 0);
   h->rp_cnt = h->np;
   *out = h;
@@ -687,10 +689,11 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   }
   CU_OR_FAIL(h, h->Hk.reserve(sizeof(c128) * (size_t)nk * nbb), "cudaMalloc Hk");
   CU_OR_FAIL(h, h->Uk.reserve(sizeof(c128) * (size_t)nk * nbb), "cudaMalloc Uk");
-  CU_OR_FAIL(h, h->Pq.reserve(sizeof(c128) * (size_t)QB * np), "cudaMalloc Pq");
-  CU_OR_FAIL(h, h->Pqe.reserve(sizeof(c128) * (size_t)QB * ne), "cudaMalloc Pqe");
-  CU_OR_FAIL(h, h->Dq.reserve(sizeof(c128) * (size_t)QB * nmm), "cudaMalloc Dq");
-  CU_OR_FAIL(h, h->eq.reserve(sizeof(c128) * (size_t)QB * nmm), "cudaMalloc e_q");
+  // the q side is small (16 (Np + Ne + 2 Nm^2) bytes per q): phases, D(q) and its eigen-system for ALL q of the call at once
+  CU_OR_FAIL(h, h->Pq.reserve(sizeof(c128) * (size_t)nq * np), "cudaMalloc Pq");
+  CU_OR_FAIL(h, h->Pqe.reserve(sizeof(c128) * (size_t)nq * ne), "cudaMalloc Pqe");
+  CU_OR_FAIL(h, h->Dq.reserve(sizeof(c128) * (size_t)nq * nmm), "cudaMalloc Dq");
+  CU_OR_FAIL(h, h->eq.reserve(sizeof(c128) * (size_t)nq * nmm), "cudaMalloc e_q");
   if (!h->ext_g1) CU_OR_FAIL(h, h->g1.reserve(sizeof(c128) * (size_t)QB * h->rows), "cudaMalloc g(Re,q)");
   if (ncolsC) CU_OR_FAIL(h, h->C.reserve(sizeof(c128) * (size_t)c_rows * ncolsC), "cudaMalloc g~");
   if (!kq_map) CU_OR_FAIL(h, h->Ukq.reserve(sizeof(c128) * (size_t)c_rows * nbb), "cudaMalloc Ukq");
@@ -698,7 +701,7 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   CU_OR_FAIL(h, h->status.reserve(sizeof(int32_t)), "cudaMalloc status");
   if (h->window_on && !h->mask_out) CU_OR_FAIL(h, h->maskbuf.reserve((size_t)nk), "cudaMalloc mask");
   {
-    const size_t need = std::max(eigh_large_scratch_bytes(nb, nk), eigh_large_scratch_bytes(nm, QB));
+    const size_t need = std::max(eigh_large_scratch_bytes(nb, nk), eigh_large_scratch_bytes(nm, nq));
     if (need) CU_OR_FAIL(h, h->eig_scratch.reserve(need), "cudaMalloc eig scratch");
   }
   CU_OR_FAIL(h, cudaMemsetAsync(h->status.p, 0, sizeof(int32_t), st), "memset status");
@@ -706,6 +709,7 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   h->last_c_rows = c_rows;
   h->last_ncols = ncolsC;
   h->last_kmode = grid ? (fused ? 2 : 1) : 0;
+  h->last_eq_slot = nq - 1;
   h->last_path = EPW_PATH_SMALL;
   h->last_qb = QB;
   h->last_kchunk = kchunk;
@@ -782,39 +786,39 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   h->count_into(-1);
   h->end_span(sp, st);
 
+  // ---- q side (once per call): S0 phases of every q, D(q), phonon eigen-systems ----
+  sp = h->begin_span(0, st);
+  LAUNCH(h, launch_phase_table(q_list, nq, h->Rp.as<int32_t>(), h->wp.as<double>(), np, h->Pq.as<c128>(), st),
+         "phase_table(q,Rp)");
+  if (ncols_h)
+    LAUNCH(h, launch_phase_table(q_list, nq, h->Re.as<int32_t>(), h->ones.as<double>(), ne, h->Pqe.as<c128>(), st),
+           "phase_table(q,Re)");
+  h->end_span(sp, st);
+  sp = h->begin_span(2, st);
+  LAUNCH(h, launch_interp_operator(h->D.as<c128>(), nm, np, h->Pq.as<c128>(), nq, h->Dq.as<c128>(), st), "D(q)");
+  h->count_into(2);
+  LAUNCH(h, launch_eigh_batched(h->Dq.as<c128>(), nmm, nm, nq, omega_q, h->eq.as<c128>(), 1, h->status.as<int32_t>(),
+                                h->eig_scratch.as<c128>(), st),
+         "eigh D(q)");
+  h->count_into(-1);
+  h->end_span(sp, st);
+
   for (int64_t q0 = 0; q0 < nq; q0 += QB) {
     const int qb = (int)std::min<int64_t>(QB, nq - q0);
-    // ---- S0 for this q batch ----
-    sp = h->begin_span(0, st);
-    LAUNCH(h, launch_phase_table(q_list + 3 * q0, qb, h->Rp.as<int32_t>(), h->wp.as<double>(), np, h->Pq.as<c128>(), st),
-           "phase_table(q,Rp)");
-    if (ncols_h)
-      LAUNCH(h, launch_phase_table(q_list + 3 * q0, qb, h->Re.as<int32_t>(), h->ones.as<double>(), ne,
-                                   h->Pqe.as<c128>(), st),
-             "phase_table(q,Re)");
-    h->end_span(sp, st);
+    const c128 *Pq_b = h->Pq.as<c128>() + q0 * np, *Pqe_b = h->Pqe.as<c128>() + q0 * ne, *eq_b = h->eq.as<c128>() + q0 * nmm;
     // ---- S1: Eq. 9 for the batch ----
     sp = h->begin_span(1, st);
     const c128 *g1b = h->ext_g1 ? h->ext_g1 + q0 * h->rows : h->g1.as<c128>();
     if (!h->ext_g1)
-      LAUNCH(h, launch_rp_to_q(h->g.as<c128>(), h->rows, np, h->Pq.as<c128>(), qb, h->g1.as<c128>(), st), "rp_to_q");
-    h->end_span(sp, st);
-    // ---- phonons: D(q), eigensolve, S4a hoisted into the B operand of S2 ----
-    sp = h->begin_span(2, st);
-    LAUNCH(h, launch_interp_operator(h->D.as<c128>(), nm, np, h->Pq.as<c128>(), qb, h->Dq.as<c128>(), st), "D(q)");
-    h->count_into(2);
-    LAUNCH(h, launch_eigh_batched(h->Dq.as<c128>(), nmm, nm, qb, omega_q + q0 * nm, h->eq.as<c128>(), 1,
-                                  h->status.as<int32_t>(), h->eig_scratch.as<c128>(), st),
-           "eigh D(q)");
-    h->count_into(-1);
+      LAUNCH(h, launch_rp_to_q(h->g.as<c128>(), h->rows, np, Pq_b, qb, h->g1.as<c128>(), st), "rp_to_q");
     h->end_span(sp, st);
     if (!grid) {
       sp = h->begin_span(8, st);
       for (int iq = 0; iq < qb; iq++)
         LAUNCH(h,
-               launch_pack_b(g1b + (int64_t)iq * h->rows, h->eq.as<c128>() + (int64_t)iq * nmm,
+               launch_pack_b(g1b + (int64_t)iq * h->rows, eq_b + (int64_t)iq * nmm,
                              omega_q + (q0 + iq) * nm, h->cfg.omega_min, h->H.as<c128>(),
-                             ncols_h ? h->Pqe.as<c128>() + (int64_t)iq * ne : nullptr, nbb, nm, ne, ncols_g, ncols_h,
+                             ncols_h ? Pqe_b + (int64_t)iq * ne : nullptr, nbb, nm, ne, ncols_g, ncols_h,
                              h->Bpack.as<double>() + (int64_t)iq * NT * KB * GEMM_CHUNK, st),
                "pack_b");
       h->end_span(sp, st);
@@ -825,9 +829,9 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
       const double *Bq = grid ? nullptr : h->Bpack.as<double>() + (int64_t)iq * NT * KB * GEMM_CHUNK;
       if (grid) {
         sp = h->begin_span(8, st);
-        LAUNCH(h, launch_box_scatter(g1b + (int64_t)iq * h->rows, h->eq.as<c128>() + (int64_t)iq * nmm,
+        LAUNCH(h, launch_box_scatter(g1b + (int64_t)iq * h->rows, eq_b + (int64_t)iq * nmm,
                                      omega_q + q * nm, h->cfg.omega_min, h->H.as<c128>(),
-                                     ncols_h ? h->Pqe.as<c128>() + (int64_t)iq * ne : nullptr, h->we.as<double>(),
+                                     ncols_h ? Pqe_b + (int64_t)iq * ne : nullptr, h->we.as<double>(),
                                      h->boxidx.as<int32_t>(), h->box_size, nbb, nm, ne, ncols_g, ncols_h,
                                      h->X.as<c128>(), st),
                "box_scatter");
@@ -1106,7 +1110,10 @@ int64_t epw_interp_debug_get(epw_interp_t h, int what, void *dst, size_t bytes) 
     case EPW_DBG_H_K: need = sizeof(c128) * nbb * h->last_nk; src = h->Hk.p; break;
     case EPW_DBG_U_K: need = sizeof(c128) * nbb * h->last_nk; src = h->Uk.p; break;
     case EPW_DBG_U_KQ: need = sizeof(c128) * nbb * std::min(h->last_nk, h->last_c_rows); src = h->Ukq.p; break;
-    case EPW_DBG_E_Q: need = sizeof(c128) * (size_t)h->nmm; src = h->eq.p; break;
+    case EPW_DBG_E_Q:
+      need = sizeof(c128) * (size_t)h->nmm;
+      src = h->eq.p ? h->eq.as<c128>() + h->last_eq_slot * h->nmm : nullptr;
+      break;
     case EPW_DBG_G_TILDE: {
       // strided copy: rows of the g~ buffer are ncols wide, the first Nb^2 Nm entries are g~
       const int64_t rowsC = std::min(h->last_nk, h->last_c_rows);
