@@ -30,8 +30,8 @@ __host__ __device__ constexpr int grot_t2_pitch(int nb) { return nb == 8 ? 8 : g
 template <int NB>
 __device__ __forceinline__ int grot_t2_pos(int np_, int mp) { return NB == 8 ? (mp ^ ((np_ & 1) << 2)) : mp; }
 
-template <int NB, int W>
-__global__ void __launch_bounds__(W * 32, 2)
+template <int NB, int W, int MINB>
+__global__ void __launch_bounds__(W * 32, MINB)
     grid_rotate_g2_kernel(const c128 *__restrict__ T2, int64_t slab, int ncols, int L1, const c128 *__restrict__ P1c,
                           int cnt, int i1_per_cta, const c128 *__restrict__ Uk, const c128 *__restrict__ Ukq,
                           const int32_t *__restrict__ kq_idx, int nm, int nug, const uint8_t *__restrict__ mask,
@@ -170,13 +170,13 @@ __global__ void __launch_bounds__(W * 32, 2)
   }
 }
 
-template <int NB, int W>
+template <int NB, int W, int MINB>
 static cudaError_t launch_grot(const c128 *T2, int64_t slab, int ncols, int L1, const c128 *P1c, int cnt, const c128 *Uk,
                                const c128 *Ukq, const int32_t *kq_idx, int nm, int num_sms, const uint8_t *mask, double *g2,
                                cudaStream_t st) {
   if (L1 > 32) return cudaErrorInvalidConfiguration;
   // modes per CTA: as many as keep (T2 rows + W staging buffers + phases) within ~100 KB, i.e. two CTAs per SM
-  const size_t budget = (size_t)110 << 10;
+  const size_t budget = MINB == 2 ? ((size_t)110 << 10) : ((size_t)220 << 10);
   int nug = 0;
   size_t smem = 0;
   for (int n = nm; n >= 1; n--) {
@@ -185,7 +185,7 @@ static cudaError_t launch_grot(const c128 *T2, int64_t slab, int ncols, int L1, 
     if (need <= budget) { nug = n; smem = need; break; }
   }
   if (nug == 0) return cudaErrorInvalidConfiguration;
-  cudaError_t e = cudaFuncSetAttribute(grid_rotate_g2_kernel<NB, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaError_t e = cudaFuncSetAttribute(grid_rotate_g2_kernel<NB, W, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   const int ngroups = (nm + nug - 1) / nug;
   // split the i1 walk so that the grid has a few waves of (2 CTAs per SM)
@@ -198,17 +198,17 @@ static cudaError_t launch_grot(const c128 *T2, int64_t slab, int ncols, int L1, 
   nsplit = ceil_div(cnt, i1_per_cta);
   if (slab > 2147483647LL || nsplit > 65535) return cudaErrorInvalidConfiguration;
   dim3 grid((unsigned)slab, (unsigned)ngroups, (unsigned)nsplit);
-  grid_rotate_g2_kernel<NB, W><<<grid, W * 32, smem, st>>>(T2, slab, ncols, L1, P1c, cnt, i1_per_cta, Uk, Ukq, kq_idx, nm,
+  grid_rotate_g2_kernel<NB, W, MINB><<<grid, W * 32, smem, st>>>(T2, slab, ncols, L1, P1c, cnt, i1_per_cta, Uk, Ukq, kq_idx, nm,
                                                           nug, mask, g2);
   return cudaGetLastError();
 }
 
 bool grid_rotate_g2_supported(int nb, int nm, int L1) {
   if (nb < 1 || nb > 16 || L1 > 32) return false;
-  const int W = nb <= 8 ? 8 : 4;
+  const int W = 8;
   const size_t need = sizeof(c128) * ((size_t)L1 * nb * grot_t2_pitch(nb) + (size_t)W * L1 + (size_t)W * (((size_t)nb + 7) / 8) * 8 * grot_pitch(nb));
   (void)nm;
-  return need <= ((size_t)110 << 10);
+  return need <= (nb <= 8 ? ((size_t)110 << 10) : ((size_t)220 << 10));
 }
 
 // T2 c128 [L1][slab][ncols] (the g columns are the first Nb^2 Nm of each row); P1c c128 [L1][cnt]: phases of the cnt
@@ -219,11 +219,11 @@ cudaError_t launch_grid_rotate_g2(const c128 *T2, int64_t slab, int ncols, int L
   if (slab <= 0 || cnt <= 0) return cudaSuccess;
   switch (nb) {
 #define EPW_GROT_CASE(NB_, W_) \
-  case NB_: return launch_grot<NB_, W_>(T2, slab, ncols, L1, P1c, cnt, Uk, Ukq, kq_idx, nm, num_sms, mask, g2, st);
+  case NB_: return launch_grot<NB_, W_, (NB_ <= 8 ? 2 : 1)>(T2, slab, ncols, L1, P1c, cnt, Uk, Ukq, kq_idx, nm, num_sms, mask, g2, st);
     EPW_GROT_CASE(1, 8) EPW_GROT_CASE(2, 8) EPW_GROT_CASE(3, 8) EPW_GROT_CASE(4, 8) EPW_GROT_CASE(5, 8)
-    EPW_GROT_CASE(6, 8) EPW_GROT_CASE(7, 8) EPW_GROT_CASE(8, 8) EPW_GROT_CASE(9, 4) EPW_GROT_CASE(10, 4)
-    EPW_GROT_CASE(11, 4) EPW_GROT_CASE(12, 4) EPW_GROT_CASE(13, 4) EPW_GROT_CASE(14, 4) EPW_GROT_CASE(15, 4)
-    EPW_GROT_CASE(16, 4)
+    EPW_GROT_CASE(6, 8) EPW_GROT_CASE(7, 8) EPW_GROT_CASE(8, 8) EPW_GROT_CASE(9, 8) EPW_GROT_CASE(10, 8)
+    EPW_GROT_CASE(11, 8) EPW_GROT_CASE(12, 8) EPW_GROT_CASE(13, 8) EPW_GROT_CASE(14, 8) EPW_GROT_CASE(15, 8)
+    EPW_GROT_CASE(16, 8)
 #undef EPW_GROT_CASE
     default: return cudaErrorInvalidConfiguration;
   }
