@@ -143,6 +143,11 @@ def epw_interp_create(nbnd, nmodes, ne, np_, device=0, q_batch=0, workspace_byte
     return h
 
 
+def epw_interp_last_error(h=None) -> str:
+    msg = load_library().epw_interp_last_error(h)
+    return msg.decode() if msg else ""
+
+
 def epw_interp_destroy(h):
     load_library().epw_interp_destroy(h)
 
