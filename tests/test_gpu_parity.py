@@ -781,3 +781,71 @@ def test_energy_window_screening(epw, mode):
         assert (g2b[mask_ref == 0] == 0.0).all() and np.array_equal(g2b != 0, g2 != 0)
     finally:
         h.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# degenerate cases of the method
+# ---------------------------------------------------------------------------------------------------------
+class _Wl:
+    """Minimal workload object for EpwInterp.set_operators_from_host built from explicit arrays."""
+
+    def __init__(self, H_R, D_R, g, Re, Rp, w_e=None, w_p=None):
+        self.H_R, self.D_R, self._g, self.Re, self.Rp = H_R, D_R, np.ascontiguousarray(g), Re, Rp
+        self.nbnd, self.nmodes, self.ne, self.np_ = H_R.shape[1], D_R.shape[1], len(Re), len(Rp)
+        self.w_e = np.ones(self.ne) if w_e is None else w_e
+        self.w_p = np.ones(self.np_) if w_p is None else w_p
+        self.slab_elems = self.nbnd * self.nbnd * self.ne * self.nmodes
+
+    def g_slabs(self, ip, cnt):
+        return np.ascontiguousarray(self._g[ip:ip + cnt])
+
+    def g_full(self):
+        return self._g
+
+
+@pytest.mark.parametrize("route", ["list", "grid", "large"])
+def test_exactly_degenerate_bands_and_modes(epw, route):
+    """H(R) = 1_2 (x) h(R) and D(R) = 1_2 (x) d(R): every band and every mode is exactly two-fold degenerate at every k, q,
+    so individual |g_mn nu|^2 are not unique (reading G10) -- compare sums over the degenerate blocks."""
+    base = synth.make_custom("deg", 3, 2, (1, 1, 0), 1.0, 0.1, 1.0, (5, 4, 1), ("random", 3, 2), seed=71)
+    H = np.stack([np.kron(np.eye(2), base.H_R[i].T).T for i in range(base.ne)])   # column-major storage [j][i]
+    D = np.stack([np.kron(np.eye(2), base.D_R[i].T).T for i in range(base.np_)])
+    nb, nm = 6, 4
+    g = 0.1 * crandn(base.np_, nm, base.ne, nb, nb) * np.exp(-np.linalg.norm(base.Re, axis=1))[None, None, :, None, None]
+    w = _Wl(np.ascontiguousarray(H), np.ascontiguousarray(D), g, base.Re, base.Rp)
+    ref = oracle.interpolate(w.H_R, w.D_R, g, w.Re, w.w_e, w.Rp, w.w_p, base.k_list, base.q_list)
+    assert np.abs(ref[0][:, 0] - ref[0][:, 1]).max() < 1e-9        # the spectrum really is pairwise degenerate
+    kw = dict(path=2) if route == "large" else (dict(grid=base.k_grid) if route == "grid" else {})
+    assert_path_close(run_gpu(epw, w, base.k_list, base.q_list, **kw), ref)
+
+
+@pytest.mark.parametrize("route", ["list", "grid", "large"])
+def test_omega_min_cutoff_and_tiny_lists(epw, route):
+    """Modes with omega <= omega_min report |g|^2 = 0 exactly (reading G12); one k and one q; nq not a multiple of the S1
+    batch."""
+    w = synth.make_custom("cut", 4, 5, (1, 1, 1), 1.0, 0.1, 1.0, (3, 2, 2), ("random", 11, 3), seed=72)
+    g = w.g_full()
+    om = oracle.interpolate(w.H_R, w.D_R, g, w.Re, w.w_e, w.Rp, w.w_p, w.k_list[:1], w.q_list)[2]
+    omega_min = float(np.sort(om.ravel())[len(om.ravel()) // 3]) + 1e-7     # cuts about a third of the modes
+    ref = oracle.interpolate(w.H_R, w.D_R, g, w.Re, w.w_e, w.Rp, w.w_p, w.k_list, w.q_list, omega_min=omega_min)
+    assert (ref[3] == 0).any() and (ref[3] != 0).any()
+    h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_, omega_min=omega_min, path=2 if route == "large" else 0, q_batch=4)
+    try:
+        h.set_operators_from_host(w)
+        out = h.interpolate_grid(w.k_grid, dev(w.q_list)) if route == "grid" else h.interpolate(dev(w.k_list), dev(w.q_list))
+        epw.epw_interp_sync(h.h)
+        got = [t.cpu().numpy() for t in out]
+        assert_path_close(got, ref)
+        assert np.array_equal(got[3] == 0, ref[3] == 0)
+        # one k, one q
+        k1, q1 = w.k_list[5:6], w.q_list[3:4]
+        ref1 = oracle.interpolate(w.H_R, w.D_R, g, w.Re, w.w_e, w.Rp, w.w_p, k1, q1, omega_min=omega_min)
+        out = h.interpolate(dev(k1), dev(q1))
+        epw.epw_interp_sync(h.h)
+        assert_path_close([t.cpu().numpy() for t in out], ref1)
+        if route == "grid":   # a 1 x 1 x 1 "grid" with a shift = the single point k1
+            out = h.interpolate_grid((1, 1, 1), dev(q1), k_shift=tuple(k1[0]))
+            epw.epw_interp_sync(h.h)
+            assert_path_close([t.cpu().numpy() for t in out], ref1)
+    finally:
+        h.close()
