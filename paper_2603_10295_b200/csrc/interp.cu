@@ -216,16 +216,18 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
   CU_OR_FAIL(h, h->BpackPk.reserve(sizeof(double) * (size_t)NTk * KBe * GEMM_CHUNK), "cudaMalloc BpackPk");
   CU_OR_FAIL(h, h->UpackK.reserve(sizeof(double) * (size_t)nk * upack), "cudaMalloc UpackK");
   CU_OR_FAIL(h, h->UpackKH.reserve(sizeof(double) * (size_t)nk * upack), "cudaMalloc UpackKH");
-  CU_OR_FAIL(h, h->Pq.reserve(sizeof(c128) * (size_t)QB * np), "cudaMalloc Pq");
-  CU_OR_FAIL(h, h->Dq.reserve(sizeof(c128) * (size_t)QB * nmm), "cudaMalloc Dq");
-  CU_OR_FAIL(h, h->eq.reserve(sizeof(c128) * (size_t)QB * nmm), "cudaMalloc e_q");
+  // the q side is small next to g: phases, D(q) and its eigen-system for ALL q of the call at once (a 288 x 288 solve
+  // occupies one thread-block cluster; one at a time would leave the rest of the GPU idle)
+  CU_OR_FAIL(h, h->Pq.reserve(sizeof(c128) * (size_t)nq * np), "cudaMalloc Pq");
+  CU_OR_FAIL(h, h->Dq.reserve(sizeof(c128) * (size_t)nq * nmm), "cudaMalloc Dq");
+  CU_OR_FAIL(h, h->eq.reserve(sizeof(c128) * (size_t)nq * nmm), "cudaMalloc e_q");
   if (!h->ext_g1) CU_OR_FAIL(h, h->g1.reserve(sizeof(c128) * (size_t)QB * h->rows), "cudaMalloc g(Re,q)");
   CU_OR_FAIL(h, h->BpackE.reserve(sizeof(double) * (size_t)NTm * KBm * GEMM_CHUNK), "cudaMalloc BpackE");
   CU_OR_FAIL(h, h->ghat.reserve(sizeof(c128) * (size_t)ne * E), "cudaMalloc g^(Re,q)");
   CU_OR_FAIL(h, h->C.reserve(sizeof(c128) * (size_t)kc * E), "cudaMalloc g~");
   CU_OR_FAIL(h, h->T.reserve(sizeof(c128) * (size_t)kc * E), "cudaMalloc T");
   if (!kq_map) {
-    CU_OR_FAIL(h, h->Pqe.reserve(sizeof(c128) * (size_t)QB * ne), "cudaMalloc Pqe");
+    CU_OR_FAIL(h, h->Pqe.reserve(sizeof(c128) * (size_t)nq * ne), "cudaMalloc Pqe");
     CU_OR_FAIL(h, h->Hkq.reserve(sizeof(c128) * (size_t)nk * nbb), "cudaMalloc Hkq");
     CU_OR_FAIL(h, h->Ukq.reserve(sizeof(c128) * (size_t)nk * nbb), "cudaMalloc Ukq");
     if (!eps_kq) CU_OR_FAIL(h, h->epskq_scratch.reserve(sizeof(double) * (size_t)nk * nb), "cudaMalloc eps scratch");
@@ -233,7 +235,7 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
   CU_OR_FAIL(h, h->status.reserve(sizeof(int32_t)), "cudaMalloc status");
   if (h->window_on && !h->mask_out) CU_OR_FAIL(h, h->maskbuf.reserve((size_t)nk), "cudaMalloc mask");
   {
-    const size_t need = std::max(eigh_large_scratch_bytes(nb, nk), eigh_large_scratch_bytes(nm, QB));
+    const size_t need = std::max(eigh_large_scratch_bytes(nb, nk), eigh_large_scratch_bytes(nm, nq));
     if (need) CU_OR_FAIL(h, h->eig_scratch.reserve(need), "cudaMalloc eig scratch");
   }
   CU_OR_FAIL(h, cudaMemsetAsync(h->status.p, 0, sizeof(int32_t), st), "memset status");
@@ -241,7 +243,7 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
   h->last_c_rows = kc;
   h->last_ncols = (int)E;
   h->last_path = EPW_PATH_LARGE;
-  h->last_eq_slot = (nq - 1) % QB;
+  h->last_eq_slot = nq - 1;
   h->last_qb = QB;
   h->last_kchunk = kc;
 
@@ -276,35 +278,37 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
            "pack conj U_k");
   h->end_span(sp, st);
 
+  // ---- q side, once per call ----
+  sp = h->begin_span(0, st);
+  LAUNCH(h, launch_phase_table(q_list, nq, h->Rp.as<int32_t>(), h->wp.as<double>(), np, h->Pq.as<c128>(), st),
+         "phase_table(q,Rp)");
+  if (!kq_map)
+    LAUNCH(h, launch_phase_table(q_list, nq, h->Re.as<int32_t>(), h->ones.as<double>(), ne, h->Pqe.as<c128>(), st),
+           "phase_table(q,Re)");
+  h->end_span(sp, st);
+  sp = h->begin_span(2, st);
+  LAUNCH(h, launch_interp_operator(h->D.as<c128>(), nm, np, h->Pq.as<c128>(), nq, h->Dq.as<c128>(), st), "D(q)");
+  h->count_into(2);
+  LAUNCH(h, launch_eigh_batched(h->Dq.as<c128>(), nmm, nm, nq, omega_q, h->eq.as<c128>(), 1, h->status.as<int32_t>(),
+                                h->eig_scratch.as<c128>(), st),
+         "eigh D(q)");
+  h->count_into(-1);
+  h->end_span(sp, st);
+
   for (int64_t q0 = 0; q0 < nq; q0 += QB) {
     const int qb = (int)std::min<int64_t>(QB, nq - q0);
-    sp = h->begin_span(0, st);
-    LAUNCH(h, launch_phase_table(q_list + 3 * q0, qb, h->Rp.as<int32_t>(), h->wp.as<double>(), np, h->Pq.as<c128>(), st),
-           "phase_table(q,Rp)");
-    if (!kq_map)
-      LAUNCH(h, launch_phase_table(q_list + 3 * q0, qb, h->Re.as<int32_t>(), h->ones.as<double>(), ne,
-                                   h->Pqe.as<c128>(), st),
-             "phase_table(q,Re)");
-    h->end_span(sp, st);
+    const c128 *Pq_b = h->Pq.as<c128>() + q0 * np, *Pqe_b = h->Pqe.as<c128>() + q0 * ne, *eq_b = h->eq.as<c128>() + q0 * nmm;
     sp = h->begin_span(1, st);
     const c128 *g1b = h->ext_g1 ? h->ext_g1 + q0 * h->rows : h->g1.as<c128>();
     if (!h->ext_g1)
-      LAUNCH(h, launch_rp_to_q(h->g.as<c128>(), h->rows, np, h->Pq.as<c128>(), qb, h->g1.as<c128>(), st), "rp_to_q");
-    h->end_span(sp, st);
-    sp = h->begin_span(2, st);
-    LAUNCH(h, launch_interp_operator(h->D.as<c128>(), nm, np, h->Pq.as<c128>(), qb, h->Dq.as<c128>(), st), "D(q)");
-    h->count_into(2);
-    LAUNCH(h, launch_eigh_batched(h->Dq.as<c128>(), nmm, nm, qb, omega_q + q0 * nm, h->eq.as<c128>(), 1,
-                                  h->status.as<int32_t>(), h->eig_scratch.as<c128>(), st),
-           "eigh D(q)");
-    h->count_into(-1);
+      LAUNCH(h, launch_rp_to_q(h->g.as<c128>(), h->rows, np, Pq_b, qb, h->g1.as<c128>(), st), "rp_to_q");
     h->end_span(sp, st);
 
     for (int iq = 0; iq < qb; iq++) {
       const int64_t q = q0 + iq;
       // ---- S4a (hoisted): g^(Re,q)[Re][nu][n'][m'] = sum_ka g(Re,q)[ka][Re][n'][m'] e_q[ka][nu] / sqrt(2 omega_nu) ----
       sp = h->begin_span(8, st);
-      LAUNCH(h, launch_pack_b_strided(h->eq.as<c128>() + (int64_t)iq * nmm, 1, nm, 0, 1, 0, omega_q + q * nm,
+      LAUNCH(h, launch_pack_b_strided(eq_b + (int64_t)iq * nmm, 1, nm, 0, 1, 0, omega_q + q * nm,
                                       h->cfg.omega_min, nm, nm, h->BpackE.as<double>(), st),
              "pack e_q");
       LAUNCH(h, launch_zgemm_strided(g1b + (int64_t)iq * h->rows, xrows, 0, xrows, 0,
@@ -317,7 +321,7 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
         // ---- off-grid q: H(k+q) for every k, eigensolve, packed conj(U_{k+q}) ----
         sp = h->begin_span(5, st);
         LAUNCH(h,
-               launch_pack_b(nullptr, nullptr, nullptr, 0.0, h->H.as<c128>(), h->Pqe.as<c128>() + (int64_t)iq * ne, nbb,
+               launch_pack_b(nullptr, nullptr, nullptr, 0.0, h->H.as<c128>(), Pqe_b + (int64_t)iq * ne, nbb,
                              nm, ne, 0, nbb, h->BpackH.as<double>(), st),
                "pack_b(H e^{iqR})");
         LAUNCH(h, launch_zgemm_dmma(h->Apack.as<double>(), h->BpackH.as<double>(), h->Hkq.as<c128>(), nk, nbb, KBe, nbb,
