@@ -111,7 +111,9 @@ int epw_interp_interpolate(epw_interp_t h, const double *k_list, int64_t nk, con
 
 /*
  * Same computation with HOST buffers (pinned or pageable): copies k_list, q_list, kq_map to the device, runs the
- * path, copies eps_k, eps_kq (if non-NULL), omega_q and g2 back, and returns after the stream has completed.
+ * path, copies eps_k, eps_kq (if non-NULL), omega_q and g2 back, and returns after everything has completed.
+ * The g2 / eps_kq slices of each finished q are copied on an internal second stream while the next q is computed
+ * (pinned host buffers make that copy asynchronous; pageable ones still work).
  */
 int epw_interp_interpolate_host(epw_interp_t h, const double *k_list, int64_t nk, const double *q_list, int64_t nq,
                                 const int32_t *kq_map, double *eps_k, double *eps_kq, double *omega_q, double *g2,

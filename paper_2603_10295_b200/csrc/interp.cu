@@ -109,6 +109,31 @@ struct epw_interp {
   }
   int last_kmode = 0;
   int64_t last_eq_slot = 0;  // slot of the last q of the last call inside the e_q buffer (debug getter)
+  // host-entry output drain: while a host-buffer call runs, the |g|^2 and eps_kq slices of every finished q are copied
+  // to the caller's host buffers on a second stream, overlapping the device-to-host link with the next q's kernels
+  struct HostSink { double *g2 = nullptr, *eps_kq = nullptr; bool active = false; } sink;
+  cudaStream_t copy_stream = nullptr;
+  std::vector<cudaEvent_t> sink_ev;
+  size_t sink_ev_used = 0;
+  int drain_q(int64_t q, int64_t nk, int64_t E, const double *g2_dev, const double *eps_kq_dev, cudaStream_t st) {
+    if (!sink.active) return EPW_OK;
+    if (sink_ev_used == sink_ev.size()) {
+      cudaEvent_t ev;
+      if (cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) != cudaSuccess) return EPW_ECUDA;
+      sink_ev.push_back(ev);
+    }
+    cudaEvent_t ev = sink_ev[sink_ev_used++];
+    cudaError_t e = cudaEventRecord(ev, st);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(copy_stream, ev, 0);
+    if (e == cudaSuccess)
+      e = cudaMemcpyAsync(sink.g2 + q * nk * E, g2_dev + q * nk * E, sizeof(double) * (size_t)(nk * E),
+                          cudaMemcpyDeviceToHost, copy_stream);
+    if (e == cudaSuccess && sink.eps_kq && eps_kq_dev)
+      e = cudaMemcpyAsync(sink.eps_kq + q * nk * nb, eps_kq_dev + q * nk * nb, sizeof(double) * (size_t)(nk * nb),
+                          cudaMemcpyDeviceToHost, copy_stream);
+    if (e != cudaSuccess) return cuda_fail(e, "drain D2H");
+    return EPW_OK;
+  }
   // host-entry staging
   DevBuf hs_k, hs_q, hs_map, hs_epsk, hs_epskq, hs_omega, hs_g2;
   // bookkeeping of the last call
@@ -373,6 +398,7 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
         }
         h->end_span(sp, st);
       }
+      { const int rc = h->drain_q(q, nk, E, g2, eps_kq, st); if (rc != EPW_OK) return rc; }
     }
   }
   h->end_span(t_total, st);
@@ -460,6 +486,8 @@ void epw_interp_destroy(epw_interp_t h) {
                    &h->P3pack, &h->klist_gen, &h->workctr, &h->maskbuf};
   for (DevBuf *b : all) b->release();
   for (cudaEvent_t ev : h->ev_pool) cudaEventDestroy(ev);
+  for (cudaEvent_t ev : h->sink_ev) cudaEventDestroy(ev);
+  if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
   delete h;
 }
 
@@ -920,6 +948,7 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
         }
         h->end_span(sp, st);
       }
+      { const int rc = h->drain_q(q, nk, E, g2, eps_kq, st); if (rc != EPW_OK) return rc; }
     }
   }
   h->end_span(t_total, st);
@@ -1019,19 +1048,26 @@ static int interpolate_host_impl(epw_interp_t h, const double *k_list, const int
     CU_OR_FAIL(h, cudaMemcpyAsync(h->hs_map.p, kq_map, sizeof(int32_t) * nk * nq, cudaMemcpyHostToDevice, st), "H2D map");
   const int32_t *map_d = kq_map ? h->hs_map.as<int32_t>() : nullptr;
   double *epskq_d = eps_kq ? h->hs_epskq.as<double>() : nullptr;
+  // |g|^2 (and eps_kq) leave the device q by q on a second stream while the next q is being computed
+  if (!h->copy_stream) CU_OR_FAIL(h, cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking), "cudaStreamCreate");
+  h->sink.g2 = g2;
+  h->sink.eps_kq = eps_kq;
+  h->sink.active = true;
+  h->sink_ev_used = 0;
   const int rc = k_list ? epw_interp_interpolate(h, h->hs_k.as<double>(), nk, h->hs_q.as<double>(), nq, map_d,
                                                  h->hs_epsk.as<double>(), epskq_d, h->hs_omega.as<double>(),
                                                  h->hs_g2.as<double>(), cuda_stream)
                         : epw_interp_interpolate_grid(h, k_grid, k_shift, h->hs_q.as<double>(), nq, map_d,
                                                       h->hs_epsk.as<double>(), epskq_d, h->hs_omega.as<double>(),
                                                       h->hs_g2.as<double>(), cuda_stream);
-  if (rc != EPW_OK) return rc;
+  h->sink.active = false;
+  if (rc != EPW_OK) {
+    cudaStreamSynchronize(h->copy_stream);
+    return rc;
+  }
   CU_OR_FAIL(h, cudaMemcpyAsync(eps_k, h->hs_epsk.p, sizeof(double) * nk * h->nb, cudaMemcpyDeviceToHost, st), "D2H eps_k");
-  if (eps_kq)
-    CU_OR_FAIL(h, cudaMemcpyAsync(eps_kq, h->hs_epskq.p, sizeof(double) * nk * nq * h->nb, cudaMemcpyDeviceToHost, st),
-               "D2H eps_kq");
   CU_OR_FAIL(h, cudaMemcpyAsync(omega_q, h->hs_omega.p, sizeof(double) * nq * h->nm, cudaMemcpyDeviceToHost, st), "D2H omega");
-  CU_OR_FAIL(h, cudaMemcpyAsync(g2, h->hs_g2.p, sizeof(double) * E * nk * nq, cudaMemcpyDeviceToHost, st), "D2H g2");
+  CU_OR_FAIL(h, cudaStreamSynchronize(h->copy_stream), "cudaStreamSynchronize(copy)");
   return epw_interp_sync(h);
 }
 
