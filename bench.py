@@ -437,7 +437,7 @@ def main():
                 mults = ncols * (L1 * L2 * N3 * L3 + L1 * N2 * N3 * L2) + nc_last * float(nk) * L1     # per q
                 byts = 16.0 * (ncols * ((L1 * L2 * L3 + L1 * L2 * N3) + (L1 * L2 * N3 + L1 * N2 * N3))
                                + nc_last * (L1 * N2 * N3 + nk))
-                spec["S2_re_to_k"] = ("hbm", "zgemm_strided_kernel (axis passes)", byts * nq_tot, hbm, "GB/s",
+                spec["S2_re_to_k"] = ("hbm", "axis_pass_kernel (axis passes)", byts * nq_tot, hbm, "GB/s",
                                       {"flops": 8.0 * mults * nq_tot})
             else:
                 spec["S2_re_to_k"] = ("tensor", "zgemm_strided_kernel" if large else "zgemm_dmma_kernel",

@@ -131,6 +131,10 @@ bool grid_rotate_g2_supported(int nb, int nm, int L1);
 cudaError_t launch_grid_rotate_g2(const c128 *T2, int64_t slab, int ncols, int L1, const c128 *P1c, int cnt,
                                   const c128 *Uk, const c128 *Ukq, const int32_t *kq_idx, int nb, int nm, int num_sms,
                                   const uint8_t *mask, double *g2, cudaStream_t st);
+// one axis pass as a streaming kernel (K = L_d <= 32); P c128 [K][N] row-major (unpacked phases)
+bool axis_pass_supported(int K);
+cudaError_t launch_axis_pass(const c128 *A, int64_t a_rb, int64_t a_bs, int64_t a_ks, int64_t M, const c128 *P, int K, int N,
+                             c128 *C, int64_t c_rb, int64_t c_bs, int64_t c_cs, int num_sms, cudaStream_t st);
 cudaError_t launch_grid_klist(const int32_t N[3], const double s[3], double *k_list, cudaStream_t st);
 
 // mask (may be NULL): uint8 per pair, 0 = skipped by the energy-window pre-screening -> zeros, no arithmetic

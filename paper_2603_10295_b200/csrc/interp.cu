@@ -101,7 +101,7 @@ struct epw_interp {
   // uniform-grid form of S2 (re_to_k_grid.cu): bounding box of the Re list, box-ordered operand and axis passes
   int box_lo[3] = {0, 0, 0}, box_L[3] = {1, 1, 1};
   int64_t box_size = 1;
-  DevBuf boxidx, X, T1, T2, Ptmp, P1raw, P1pack, P2pack, P3pack, klist_gen;
+  DevBuf boxidx, X, T1, T2, Ptmp, P1raw, P2raw, P3raw, P1pack, P2pack, P3pack, klist_gen;
   DevBuf workctr;  // 3 x u64: plane rotations executed by the register-resident eigensolvers for H(k), H(k+q), D(q)
   // route the eigensolver work counter to slot i (0 H(k), 1 H(k+q), 2 D(q)) while stage timing is on; -1 = off
   void count_into(int slot) {
@@ -482,7 +482,7 @@ void epw_interp_destroy(epw_interp_t h) {
                    &h->Uk, &h->Pq, &h->Pqe, &h->Dq, &h->eq, &h->g1, &h->Bpack, &h->C, &h->Ukq, &h->epskq_scratch,
                    &h->status, &h->eig_scratch, &h->hs_k, &h->hs_q, &h->hs_map, &h->hs_epsk, &h->hs_epskq,
                    &h->hs_omega, &h->hs_g2, &h->Pk, &h->BpackPk, &h->UpackK, &h->UpackKH, &h->BpackE,
-                   &h->ghat, &h->T, &h->Hkq, &h->boxidx, &h->X, &h->T1, &h->T2, &h->Ptmp, &h->P1raw, &h->P1pack, &h->P2pack,
+                   &h->ghat, &h->T, &h->Hkq, &h->boxidx, &h->X, &h->T1, &h->T2, &h->Ptmp, &h->P1raw, &h->P2raw, &h->P3raw, &h->P1pack, &h->P2pack,
                    &h->P3pack, &h->klist_gen, &h->workctr, &h->maskbuf};
   for (DevBuf *b : all) b->release();
   for (cudaEvent_t ev : h->ev_pool) cudaEventDestroy(ev);
@@ -718,6 +718,8 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
                                     ceil_div(2 * (int64_t)L[1], GEMM_BK) * GEMM_CHUNK), "cudaMalloc P2pack");
     CU_OR_FAIL(h, h->P1pack.reserve(sizeof(double) * (size_t)nchunks * NTc * KB1 * GEMM_CHUNK), "cudaMalloc P1pack");
     CU_OR_FAIL(h, h->P1raw.reserve(sizeof(c128) * (size_t)nchunks * L[0] * cs), "cudaMalloc P1raw");
+    CU_OR_FAIL(h, h->P2raw.reserve(sizeof(c128) * (size_t)L[1] * grid->N[1]), "cudaMalloc P2raw");
+    CU_OR_FAIL(h, h->P3raw.reserve(sizeof(c128) * (size_t)L[2] * grid->N[2]), "cudaMalloc P3raw");
   }
   CU_OR_FAIL(h, h->Hk.reserve(sizeof(c128) * (size_t)nk * nbb), "cudaMalloc Hk");
   CU_OR_FAIL(h, h->Uk.reserve(sizeof(c128) * (size_t)nk * nbb), "cudaMalloc Uk");
@@ -747,13 +749,23 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   h->last_kchunk = kchunk;
 
   // the two leading axis passes of the factorised S2: X [L1][L2][L3][nc] -> T1 [L1][L2][N3][nc] -> T2 [L1][N2][N3][nc]
+  // Axis passes: a streaming kernel when the box extent is small (always, for Wigner-Seitz lists), else the in-place
+  // tensor-path contraction with the packed phase table.
   auto grid_pass_ab = [&](int nc) -> cudaError_t {
     const int64_t N2 = grid->N[1], N3 = grid->N[2];
-    cudaError_t e = launch_zgemm_strided(h->X.as<c128>(), nc, (int64_t)L[2] * nc, nc, 0, h->P3pack.as<double>(), nullptr,
-                                         h->T1.p, nc, N3 * nc, 1, nc, 0, 0, (int64_t)L[0] * L[1] * nc, (int)N3, L[2], 1,
-                                         h->num_sms, st);
+    cudaError_t e;
+    if (axis_pass_supported(L[2]))
+      e = launch_axis_pass(h->X.as<c128>(), nc, (int64_t)L[2] * nc, nc, (int64_t)L[0] * L[1] * nc, h->P3raw.as<c128>(), L[2],
+                           (int)N3, h->T1.as<c128>(), nc, N3 * nc, nc, h->num_sms, st);
+    else
+      e = launch_zgemm_strided(h->X.as<c128>(), nc, (int64_t)L[2] * nc, nc, 0, h->P3pack.as<double>(), nullptr, h->T1.p, nc,
+                               N3 * nc, 1, nc, 0, 0, (int64_t)L[0] * L[1] * nc, (int)N3, L[2], 1, h->num_sms, st);
     if (e != cudaSuccess) return e;
     h->launches++;
+    if (axis_pass_supported(L[1]))
+      return launch_axis_pass(h->T1.as<c128>(), N3 * nc, (int64_t)L[1] * N3 * nc, N3 * nc, (int64_t)L[0] * N3 * nc,
+                              h->P2raw.as<c128>(), L[1], (int)N2, h->T2.as<c128>(), N3 * nc, N2 * N3 * nc, N3 * nc,
+                              h->num_sms, st);
     return launch_zgemm_strided(h->T1.as<c128>(), N3 * nc, (int64_t)L[1] * N3 * nc, N3 * nc, 0, h->P2pack.as<double>(),
                                 nullptr, h->T2.p, N3 * nc, N2 * N3 * nc, 1, N3 * nc, 0, 0, (int64_t)L[0] * N3 * nc,
                                 (int)N2, L[1], 1, h->num_sms, st);
@@ -762,6 +774,9 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   auto grid_pass_c = [&](int nc, int ci, c128 *out) -> cudaError_t {
     const int cnt = std::min(cs, grid->N[0] - ci * cs);
     const int64_t Mrows = slab * nc;
+    if (axis_pass_supported(L[0]))
+      return launch_axis_pass(h->T2.as<c128>(), Mrows, 0, Mrows, Mrows, h->P1raw.as<c128>() + (int64_t)ci * L[0] * cs, L[0],
+                              cnt, out, Mrows, 0, Mrows, h->num_sms, st);
     return launch_zgemm_strided(h->T2.as<c128>(), Mrows, 0, Mrows, 0,
                                 h->P1pack.as<double>() + (int64_t)ci * NTc * KB1 * GEMM_CHUNK, nullptr, out, Mrows, 0, 1,
                                 Mrows, 0, 0, Mrows, cnt, L[0], 1, h->num_sms, st);
@@ -779,9 +794,10 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
     struct Axis { int d; DevBuf *pack; };
     const Axis ax[2] = {{2, &h->P3pack}, {1, &h->P2pack}};
     for (const Axis &a : ax) {
-      LAUNCH(h, launch_grid_axis_phase(grid->N[a.d], 0, grid->N[a.d], grid->s[a.d], h->box_lo[a.d], L[a.d],
-                                       h->Ptmp.as<c128>(), st), "axis phases");
-      LAUNCH(h, launch_pack_b_strided(h->Ptmp.as<c128>(), grid->N[a.d], 1, 0, 1, 0, nullptr, 0.0, L[a.d], grid->N[a.d],
+      c128 *raw = (a.d == 2 ? h->P3raw : h->P2raw).as<c128>();   // [L_d][N_d], kept for the streaming axis pass
+      LAUNCH(h, launch_grid_axis_phase(grid->N[a.d], 0, grid->N[a.d], grid->s[a.d], h->box_lo[a.d], L[a.d], raw, st),
+             "axis phases");
+      LAUNCH(h, launch_pack_b_strided(raw, grid->N[a.d], 1, 0, 1, 0, nullptr, 0.0, L[a.d], grid->N[a.d],
                                       a.pack->as<double>(), st), "pack axis phases");
     }
     for (int ci = 0; ci < nchunks; ci++) {
@@ -889,10 +905,15 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
           const int ci = (int)(k0 / kchunk);
           const int cnt = std::min(cs, grid->N[0] - ci * cs);
           const int64_t Mh = slab * nbb;
-          LAUNCH(h, launch_zgemm_strided(h->T2.as<c128>() + ncols_g, nbb, ncols, slab * ncols, 0,
-                                         h->P1pack.as<double>() + (int64_t)ci * NTc * KB1 * GEMM_CHUNK, nullptr, Cc, Mh, 0, 1,
-                                         Mh, 0, 0, Mh, cnt, L[0], 1, h->num_sms, st),
-                 "grid pass H(k+q)");
+          if (axis_pass_supported(L[0]))
+            LAUNCH(h, launch_axis_pass(h->T2.as<c128>() + ncols_g, nbb, ncols, slab * ncols, Mh,
+                                       h->P1raw.as<c128>() + (int64_t)ci * L[0] * cs, L[0], cnt, Cc, Mh, 0, Mh, h->num_sms, st),
+                   "grid pass H(k+q)");
+          else
+            LAUNCH(h, launch_zgemm_strided(h->T2.as<c128>() + ncols_g, nbb, ncols, slab * ncols, 0,
+                                           h->P1pack.as<double>() + (int64_t)ci * NTc * KB1 * GEMM_CHUNK, nullptr, Cc, Mh, 0,
+                                           1, Mh, 0, 0, Mh, cnt, L[0], 1, h->num_sms, st),
+                   "grid pass H(k+q)");
         }
         h->end_span(sp, st);
         const c128 *Ukq_ptr;

@@ -11,8 +11,8 @@
 // (7^3 vectors, 40^3 grid).  X is the B operand of the dense path, B_q[Re][c] = w_e(Re) [ g^(Re,q) | e^{2 pi i q.Re} H(Re) ],
 // scattered into the bounding box [L1][L2][L3] of the Re list (zeros where the list has no vector); the result C is
 // the same [k][c] array the dense kernel writes, so the eigensolver and the rotation that follow are unchanged.
-// Each pass is one launch of the in-place strided FP64 tensor-path contraction (zgemm_strided.cu) with a tiny packed
-// phase table as its B operand; the last pass is bound by writing C (16 ncols bytes per k) to HBM, not by arithmetic.
+// Each pass is one launch of the streaming kernel at the end of this file (or, for box extents above 32, of the in-place
+// FP64 tensor-path contraction of zgemm_strided.cu); a pass is bound by writing its output to HBM, not by arithmetic.
 // The result equals the plain definition up to rounding order (sums re-associated axis by axis).
 #include "common.cuh"
 
@@ -112,6 +112,88 @@ cudaError_t launch_grid_klist(const int32_t N[3], const double s[3], double *k_l
   const int64_t blocks = ceil_div(nk, 256);
   grid_klist_kernel<<<(unsigned)(blocks < 148 * 8 ? blocks : 148 * 8), 256, 0, st>>>(N[0], N[1], N[2], s[0], s[1], s[2],
                                                                                     k_list);
+  return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// One axis pass as a streaming kernel:  C[blk][col][off] = sum_{r < K} A[blk][r][off] * P[r][col]
+//   A element (row, r) at  A + (row / a_rb) * a_bs + (row % a_rb) + r * a_ks      (rows contiguous for fixed r)
+//   C element (row, col) at C + (row / c_rb) * c_bs + (row % c_rb) + col * c_cs
+// K = L_d is 7..13 here: the pass reads each input once, writes N_d outputs per input and does 4 K DFMA per output --
+// it is bound by the write stream, and a tensor-core tile pipeline (load -> DMMA -> epilogue per tile, one CTA per SM)
+// only adds latency (43 us against a 14 us memory time for the axis-2 pass of configs[1]).  Here a thread keeps the K
+// inputs of two adjacent rows in registers, takes the phases by broadcast from shared memory and streams the columns
+// out with fully coalesced 16-byte stores; blockIdx.y splits the columns so that small passes still fill the GPU.
+// ---------------------------------------------------------------------------------------------------------------
+template <int KMAX>
+__global__ void __launch_bounds__(256)
+    axis_pass_kernel(const c128 *__restrict__ A, int64_t a_rb, int64_t a_bs, int64_t a_ks, int64_t M,
+                     const c128 *__restrict__ P, int K, int N, int cols_per_y, c128 *__restrict__ C, int64_t c_rb,
+                     int64_t c_bs, int64_t c_cs) {
+  extern __shared__ double2 sPh[];  // [K][ncol] of this column group
+  const int col0 = blockIdx.y * cols_per_y;
+  const int ncol = N - col0 < cols_per_y ? N - col0 : cols_per_y;
+  for (int e = threadIdx.x; e < K * ncol; e += blockDim.x) {
+    const int r = e / ncol, c = e - r * ncol;
+    sPh[e] = P[(int64_t)r * N + col0 + c];
+  }
+  __syncthreads();
+  const int64_t row0 = 2 * (blockIdx.x * (int64_t)blockDim.x + threadIdx.x);
+  if (row0 >= M) return;
+  const bool two = row0 + 1 < M;
+  const int64_t row1 = two ? row0 + 1 : row0;
+  const int64_t b0 = row0 / a_rb, b1 = row1 / a_rb;
+  const c128 *src0 = A + b0 * a_bs + (row0 - b0 * a_rb), *src1 = A + b1 * a_bs + (row1 - b1 * a_rb);
+  c128 x0[KMAX], x1[KMAX];
+#pragma unroll
+  for (int r = 0; r < KMAX; r++) {
+    x0[r] = r < K ? src0[(int64_t)r * a_ks] : cmake(0.0, 0.0);
+    x1[r] = r < K ? src1[(int64_t)r * a_ks] : cmake(0.0, 0.0);
+  }
+  const int64_t d0 = row0 / c_rb, d1 = row1 / c_rb;
+  c128 *dst0 = C + d0 * c_bs + (row0 - d0 * c_rb) + (int64_t)col0 * c_cs;
+  c128 *dst1 = C + d1 * c_bs + (row1 - d1 * c_rb) + (int64_t)col0 * c_cs;
+  for (int c = 0; c < ncol; c++) {
+    c128 y0 = cmake(0.0, 0.0), y1 = cmake(0.0, 0.0);
+#pragma unroll
+    for (int r = 0; r < KMAX; r++) {
+      if (r < K) {
+        const c128 ph = sPh[r * ncol + c];
+        cfma(y0, x0[r], ph);
+        cfma(y1, x1[r], ph);
+      }
+    }
+    dst0[(int64_t)c * c_cs] = y0;
+    if (two) dst1[(int64_t)c * c_cs] = y1;
+  }
+}
+
+bool axis_pass_supported(int K) { return K >= 1 && K <= 32; }
+
+cudaError_t launch_axis_pass(const c128 *A, int64_t a_rb, int64_t a_bs, int64_t a_ks, int64_t M, const c128 *P, int K, int N,
+                             c128 *C, int64_t c_rb, int64_t c_bs, int64_t c_cs, int num_sms, cudaStream_t st) {
+  if (M <= 0 || N <= 0 || K <= 0) return cudaSuccess;
+  if (K > 32) return cudaErrorInvalidValue;
+  const int64_t bx = ceil_div(ceil_div(M, 2), 256);
+  // split the columns while the row blocks alone would not give every SM a few CTAs
+  int ny = 1;
+  while (bx * ny < 4 * (int64_t)num_sms && ny < N && N / (ny + 1) >= 8) ny++;
+  const int cols_per_y = (int)ceil_div(N, ny);
+  ny = (int)ceil_div(N, cols_per_y);
+  const size_t smem = sizeof(double2) * (size_t)K * cols_per_y;
+  dim3 grid((unsigned)bx, (unsigned)ny);
+#define EPW_AXIS_LAUNCH(KM)                                                                                          \
+  do {                                                                                                               \
+    if (smem > 48 * 1024) {                                                                                          \
+      cudaError_t e = cudaFuncSetAttribute(axis_pass_kernel<KM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+      if (e != cudaSuccess) return e;                                                                                \
+    }                                                                                                                \
+    axis_pass_kernel<KM><<<grid, 256, smem, st>>>(A, a_rb, a_bs, a_ks, M, P, K, N, cols_per_y, C, c_rb, c_bs, c_cs);    \
+  } while (0)
+  if (K <= 8) EPW_AXIS_LAUNCH(8);
+  else if (K <= 16) EPW_AXIS_LAUNCH(16);
+  else EPW_AXIS_LAUNCH(32);
+#undef EPW_AXIS_LAUNCH
   return cudaGetLastError();
 }
 
