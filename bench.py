@@ -39,8 +39,8 @@ UNIT = "elements/s"
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=6)
-    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=40)
+    ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (default 1 = Si-like production)")
     ap.add_argument("--nq-step", type=int, default=0,
                     help="q-points per step (per GPU); 0 = 32, reduced so that the |g|^2 buffer of a step stays below 40 GB")
