@@ -63,6 +63,7 @@ def lib():
         L.oracle_eq6_wannier_from_bloch.argtypes = [i, i, i, i, vp, vp, i, vp, i, vp, vp, vp]
         L.oracle_eq6_unrotate.argtypes = [i, i, vp, vp, vp, vp, vp, vp]
         L.oracle_window_mask.argtypes = [i, i64, i64, vp, vp, f64, f64, vp]
+        L.oracle_selfenergy_accumulate.argtypes = [i, i, i64, i64, vp, vp, vp, vp, vp, f64, f64, f64, vp]
         for name in ("oracle_g_bytes",):
             getattr(L, name).argtypes = [f64] * 4
             getattr(L, name).restype = f64
@@ -248,6 +249,18 @@ def window_mask(eps_k, eps_kq, emin, emax) -> np.ndarray:
     nq, nk, nb = eps_kq.shape
     out = np.empty((nq, nk), dtype=np.uint8)
     lib().oracle_window_mask(nb, nk, nq, _p(eps_k), _p(eps_kq), float(emin), float(emax), _p(out))
+    return out
+
+
+def selfenergy_accumulate(g2, eps_k, eps_kq, omega, w_q, mu, kT, sigma, out=None) -> np.ndarray:
+    """Im Sigma_nk accumulator (NEXT-4 consumer, reading G18): g2 [nq][nk][Nm][Nb][Nb] -> out [nk][Nb] (+=)."""
+    g2, eps_k, eps_kq, omega = _c(g2, np.float64), _c(eps_k, np.float64), _c(eps_kq, np.float64), _c(omega, np.float64)
+    nq, nk, nm, nb, _ = g2.shape
+    w_q = None if w_q is None else _c(w_q, np.float64)
+    if out is None:
+        out = np.zeros((nk, nb), dtype=np.float64)
+    lib().oracle_selfenergy_accumulate(nb, nm, nk, nq, _p(g2), _p(eps_k), _p(eps_kq), _p(omega), _p(w_q), float(mu),
+                                       float(kT), float(sigma), _p(out))
     return out
 
 

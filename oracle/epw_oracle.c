@@ -422,6 +422,41 @@ void oracle_window_mask(int nb, int64_t nk, int64_t nq, const double *eps_k, con
 }
 
 /* ---------------------------------------------------------------------------------------------
+ * A consumer of |g|^2.  The paper names the consumers -- "ab initio Boltzmann transport",
+ * "electron self-energy" -- but prints no formula for them; [reading, G18] the
+ * imaginary part of the Fan-Migdal electron self-energy in its usual double-sum form with Gaussian-broadened energy
+ * conservation is taken, per initial state (n,k):
+ *   Im Sigma_nk += pi sum_q w_q sum_{m,nu} |g_{mn nu}(k,q)|^2 [ (n_qnu + f_mk+q)     delta_s(e_nk - e_mk+q + w_qnu)
+ *                                                           + (n_qnu + 1 - f_mk+q) delta_s(e_nk - e_mk+q - w_qnu) ]
+ *   delta_s(x) = exp(-(x/s)^2) / (s sqrt(pi)),  n = 1/(exp(w/kT) - 1),  f = 1/(exp((e - mu)/kT) + 1);
+ * modes with w <= 0 are skipped.  out[n + Nb*ik] is ACCUMULATED (+=).  g2 [nq][nk][Nm][Nb(n)][Nb(m)].
+ * ------------------------------------------------------------------------------------------- */
+void oracle_selfenergy_accumulate(int nb, int nm, int64_t nk, int64_t nq, const double *g2, const double *eps_k,
+                                  const double *eps_kq, const double *omega, const double *w_q, double mu, double kT,
+                                  double sigma, double *out) {
+  const double pi = 3.14159265358979323846;
+  for (int64_t iq = 0; iq < nq; iq++)
+    for (int64_t ik = 0; ik < nk; ik++)
+      for (int n = 0; n < nb; n++) {
+        const double e1 = eps_k[n + nb * ik];
+        double s = 0.0;
+        for (int nu = 0; nu < nm; nu++) {
+          const double w = omega[nu + nm * iq];
+          if (!(w > 0.0)) continue;
+          const double bose = 1.0 / (exp(w / kT) - 1.0);
+          for (int m = 0; m < nb; m++) {
+            const double e2 = eps_kq[m + nb * (ik + nk * iq)];
+            const double f = 1.0 / (exp((e2 - mu) / kT) + 1.0);
+            const double xa = (e1 - e2 + w) / sigma, xe = (e1 - e2 - w) / sigma;
+            const double da = exp(-xa * xa) / (sigma * sqrt(pi)), de = exp(-xe * xe) / (sigma * sqrt(pi));
+            s += g2[m + nb * (n + nb * (nu + nm * (ik + nk * iq)))] * ((bose + f) * da + (bose + 1.0 - f) * de);
+          }
+        }
+        out[n + nb * ik] += pi * (w_q ? w_q[iq] : 1.0) * s;
+      }
+}
+
+/* ---------------------------------------------------------------------------------------------
  * Bookkeeping helpers pinned by the paper's printed numbers.
  * ------------------------------------------------------------------------------------------- */
 /* Table III caption: size of g(Re,Rp) = 16 Nb^2 Nm Ne Np bytes. */

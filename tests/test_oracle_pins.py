@@ -542,3 +542,43 @@ def test_window_mask_hand_example_and_bruteforce():
     ref = (((ek >= -0.2) & (ek <= 0.1)).any(-1)[None, :] & ((ekq >= -0.2) & (ekq <= 0.1)).any(-1)).astype(np.uint8)
     np.testing.assert_array_equal(oracle.window_mask(ek, ekq, -0.2, 0.1), ref)
     assert 0 < ref.sum() < ref.size
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-4 consumer: Im Sigma_nk accumulator (reading G18; the paper names the consumer, not its formula)
+# ---------------------------------------------------------------------------------------------
+def test_selfenergy_energy_integral_linearity_and_zero_temperature_selection():
+    """Pins that do not retype the formula:
+    (1) each broadened delta integrates to one, so the integral of Im Sigma over the initial-state energy is
+        pi w |g|^2 (2 n_B + 1) -- the Fermi factors cancel between absorption and emission;
+    (2) linear in |g|^2 and in w_q, additive over q, accumulating into `out`;
+    (3) T -> 0: an electron above a filled sea can only EMIT (final energy e - w, which must be empty), never absorb;
+        an initial state inside the sea only scatters into the empty state reached by ABSORPTION if that is what
+        energy conservation selects -- fixes which delta carries which occupation factor and the sign of w."""
+    nb, nm = 1, 1
+    w, e2, mu, kT, sigma, g2v, wq = 0.05, 0.3, 0.1, 0.02, 0.004, 0.7, 0.25
+    es = np.linspace(e2 - 0.2, e2 + 0.2, 4001)            # the "k-points": a fine grid of initial-state energies
+    g2 = np.full((1, len(es), nm, nb, nb), g2v)
+    out = oracle.selfenergy_accumulate(g2, es[:, None], np.full((1, len(es), 1), e2), [[w]], [wq], mu, kT, sigma)
+    nB = 1.0 / np.expm1(w / kT)
+    integral = np.sum(out[:, 0]) * (es[1] - es[0])    # peaks are far inside the grid; rectangle rule on smooth Gaussians
+    assert abs(integral - np.pi * wq * g2v * (2 * nB + 1)) < 1e-9 * integral
+    # the two peaks sit at e2 - w (absorption: e + w = e2) and e2 + w (emission: e - w = e2)
+    below, above = es < e2, es > e2
+    peaks = [es[below][np.argmax(out[below, 0])], es[above][np.argmax(out[above, 0])]]
+    np.testing.assert_allclose(peaks, [e2 - w, e2 + w], atol=2e-4)
+    # (2) linearity / additivity / accumulation
+    out2 = oracle.selfenergy_accumulate(np.concatenate([g2, 3 * g2]), es[:, None], np.full((2, len(es), 1), e2),
+                                        [[w], [w]], [wq, 2 * wq], mu, kT, sigma, out=out.copy())
+    np.testing.assert_allclose(out2, out * (1 + 1 + 6), rtol=1e-12, atol=1e-300)   # atol: denormal tails of the Gaussians
+    # (3) zero temperature: final state e2 EMPTY (above mu): only the emission peak (e = e2 + w) survives, weight 1
+    cold = oracle.selfenergy_accumulate(g2, es[:, None], np.full((1, len(es), 1), e2), [[w]], [1.0], mu, 1e-5, sigma)
+    lo, hi = es < e2, es > e2
+    assert cold[lo, 0].max() < 1e-12 * cold[hi, 0].max()
+    assert abs(np.sum(cold[hi, 0]) * (es[1] - es[0]) - np.pi * g2v) < 1e-9
+    # final state FILLED (below mu): only the absorption peak (e = e2 - w) survives
+    cold2 = oracle.selfenergy_accumulate(g2, es[:, None], np.full((1, len(es), 1), e2), [[w]], [1.0], e2 + 1.0, 1e-5, sigma)
+    assert cold2[hi, 0].max() < 1e-12 * cold2[lo, 0].max()
+    assert abs(np.sum(cold2[lo, 0]) * (es[1] - es[0]) - np.pi * g2v) < 1e-9
+    # modes with omega <= 0 do not contribute
+    assert not oracle.selfenergy_accumulate(g2, es[:, None], np.full((1, len(es), 1), e2), [[-0.01]], None, mu, kT, sigma).any()
