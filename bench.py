@@ -48,6 +48,9 @@ def parse_args():
     ap.add_argument("--energy-window", type=float, nargs=2, metavar=("EMIN", "EMAX"), default=None,
                     help="NEXT-3 (PAPER.md:L241): pre-screen the pairs with this energy window (eV); the line then reports "
                          "KEPT elements/s under its own metric name (not comparable with the unscreened headline)")
+    ap.add_argument("--consumer", action="store_true",
+                    help="NEXT-4: reduce |g|^2 on the device into the Im Sigma_nk accumulator (g2 = NULL: the Nk x Nq output "
+                         "never exists); own metric name")
     ap.add_argument("--rp-shard", action="store_true",
                     help="NEXT-1 (PAPER.md:L186-188): g(Re,Rp) split by Rp over the ranks; per step every rank contracts "
                          "its slabs for the q-points of ALL ranks, one NCCL reduce-scatter of g(Re,q) hands each rank the "
@@ -326,6 +329,12 @@ def main():
         mask_dev = torch.zeros((nq_step, nk), dtype=torch.uint8, device="cuda")
         epw.epw_interp_set_energy_window(h.h, True, args.energy_window[0], args.energy_window[1], mask_dev)
         args.no_e2e = True
+    acc_dev = None
+    if args.consumer:
+        acc_dev = torch.zeros((nk, w.nbnd), dtype=torch.float64, device="cuda")
+        # chemical potential in the middle of the bands of the first k-point, room temperature, 20 meV broadening
+        epw.epw_interp_set_selfenergy_consumer(h.h, True, 0.0, 0.025, 0.02, None, acc_dev)
+        args.no_e2e = True
     if args.rp_shard:
         args.no_e2e = True   # the host-buffer entry point has no Rp-sharded form
     rows = w.slab_elems
@@ -346,12 +355,13 @@ def main():
                 epw.epw_interp_set_gq(h.h, g1_mine)
             else:
                 epw.epw_interp_set_gq(h.h, g1_part)
+        g2_arg, ekq_arg = (None, None) if args.consumer else (g2, eps_kq)
         if use_grid if grid is None else grid:
             epw.epw_interp_interpolate_grid(h.h, w.k_grid, None, q_dev[s], nq_step,
-                                            None if map_dev is None else map_dev[s], eps_k, eps_kq, omega, g2)
+                                            None if map_dev is None else map_dev[s], eps_k, ekq_arg, omega, g2_arg)
         else:
             epw.epw_interp_interpolate(h.h, k_dev, nk, q_dev[s], nq_step, None if map_dev is None else map_dev[s],
-                                       eps_k, eps_kq, omega, g2)
+                                       eps_k, ekq_arg, omega, g2_arg)
 
     def barrier():
         if world > 1:
@@ -563,7 +573,8 @@ def main():
 
     if rank == 0:
         line = {
-            "metric": METRIC if window is None else METRIC + " -- KEPT pairs only, energy-window pre-screening on",
+            "metric": (METRIC + " -- reduced on the device into Im Sigma_nk (no |g|^2 output)" if args.consumer else
+                       METRIC if window is None else METRIC + " -- KEPT pairs only, energy-window pre-screening on"),
             "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",

@@ -150,6 +150,21 @@ int epw_interp_interpolate_grid_host(epw_interp_t h, const int32_t *k_grid, cons
 int epw_interp_set_energy_window(epw_interp_t h, int enabled, double emin, double emax, uint8_t *mask_out);
 
 /*
+ * A consumer of |g|^2 on the device: while enabled, every following interpolate call adds, for
+ * each of its pairs, the contribution of that pair to the imaginary part of the Fan-Migdal electron self-energy
+ *   Im Sigma_nk += pi w_q sum_{m,nu} |g_{mn nu}(k,q)|^2 [ (n_qnu + f_mk+q) delta_s(e_nk - e_mk+q + w_qnu)
+ *                                                      + (n_qnu + 1 - f_mk+q) delta_s(e_nk - e_mk+q - w_qnu) ]
+ * (delta_s(x) = exp(-(x/s)^2)/(s sqrt(pi)), Bose n at kT, Fermi f at (mu, kT), modes with omega <= 0 skipped) -- the
+ * paper names this consumer without printing it: DESIGN.md reading G18.
+ *   w_q      NULL (weight 1) or device f64 [nq of the call]: weight of every q-point of the call
+ *   im_sigma device f64 [nk][Nb], ACCUMULATED (+=) by every call: the caller zeroes it and may sum over many calls
+ * With the consumer enabled the g2 argument of the interpolate calls may be NULL: the library then keeps |g|^2 of one q
+ * at a time in its own scratch (8 Nb^2 Nm nk bytes) and the 8 Nb^2 Nm nk nq byte output never exists.
+ */
+int epw_interp_set_selfenergy_consumer(epw_interp_t h, int enabled, double mu, double kT, double sigma, const double *w_q,
+                                       double *im_sigma);
+
+/*
  * g(Re,Rp) split over several GPUs by Rp (the paper's pool level for operators larger than one GPU's memory,
  * PAPER.md:L186-188, Table III; SURVEY.md 8(e) variant B / 8(f) NEXT-1).  Eq. 9 is a sum over Rp, so each
  * rank contracts its own slabs and the partial g(Re,q) are summed across ranks -- the paper does D2H + mp_sum on the

@@ -36,7 +36,7 @@ EXPORTED_SYMBOLS = [
     "epw_phase_table", "epw_rp_to_q", "epw_interp_operator", "epw_eigh_batched", "epw_eigh_batched_algo", "epw_zgemm", "epw_zgemm_strided",
     "epw_rotate_g2",
     "epw_eq6_unrotate", "epw_wannier_from_bloch",
-    "epw_interp_set_energy_window", "epw_interp_set_rp_shard", "epw_interp_rp_to_q_partial", "epw_interp_set_gq",
+    "epw_interp_set_energy_window", "epw_interp_set_selfenergy_consumer", "epw_interp_set_rp_shard", "epw_interp_rp_to_q_partial", "epw_interp_set_gq",
     "epw_probe_peaks", "epw_version",
 ]
 
@@ -75,6 +75,7 @@ def load_library() -> ctypes.CDLL:
         L.epw_interp_interpolate_grid.argtypes = [vp, vp, vp, vp, c_int64, vp, vp, vp, vp, vp, vp]
         L.epw_interp_interpolate_grid_host.argtypes = [vp, vp, vp, vp, c_int64, vp, vp, vp, vp, vp, vp]
         L.epw_interp_set_energy_window.argtypes = [vp, c_int, c_double, c_double, vp]
+        L.epw_interp_set_selfenergy_consumer.argtypes = [vp, c_int, c_double, c_double, c_double, vp, vp]
         L.epw_interp_set_rp_shard.argtypes = [vp, c_int32, c_int32]
         L.epw_interp_rp_to_q_partial.argtypes = [vp, vp, c_int64, vp, vp]
         L.epw_interp_set_gq.argtypes = [vp, vp]
@@ -196,6 +197,11 @@ def epw_interp_interpolate_grid_host(h, k_grid, k_shift, q_list, nq, kq_map, eps
 
 def epw_interp_set_energy_window(h, enabled, emin=0.0, emax=0.0, mask_out=None):
     _check(load_library().epw_interp_set_energy_window(h, int(bool(enabled)), float(emin), float(emax), _ptr(mask_out)), h)
+
+
+def epw_interp_set_selfenergy_consumer(h, enabled, mu=0.0, kT=1.0, sigma=1.0, w_q=None, im_sigma=None):
+    _check(load_library().epw_interp_set_selfenergy_consumer(h, int(bool(enabled)), float(mu), float(kT), float(sigma),
+                                                             _ptr(w_q), _ptr(im_sigma)), h)
 
 
 def epw_interp_set_rp_shard(h, ip_start, ip_count):

@@ -157,6 +157,12 @@ cudaError_t launch_wannier_from_bloch(const c128 *gt, const double *kc, int64_t 
                                       double *wq, c128 *Pk, c128 *Pq, double *BpackK, double *BpackQ, int32_t *zero_gather,
                                       c128 *g1, c128 *g_RR, int num_sms, cudaStream_t st);
 
+// NEXT-4 consumer (consumer.cu): Im Sigma_nk += ... over the pairs (k = 0..nk-1, q = iq) of one |g|^2 slab
+cudaError_t launch_selfenergy_accumulate(const double *g2q, const double *eps_k, const double *eps_kq,
+                                         const double *eps_k_all, const int32_t *kq_idx, const double *omega_q,
+                                         const double *w_q, int64_t iq, double mu, double kT, double sigma, int nb, int nm,
+                                         int64_t nk, double *out, cudaStream_t st);
+
 int probe_peaks(int device, double *out4);
 
 }  // namespace epw

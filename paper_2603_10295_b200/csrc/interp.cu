@@ -91,6 +91,9 @@ struct epw_interp {
   double emin = 0.0, emax = 0.0;
   uint8_t *mask_out = nullptr;   // caller's device buffer [nq][nk] or NULL
   DevBuf maskbuf;
+  // NEXT-4 consumer: Im Sigma_nk accumulator
+  struct Consumer { bool on = false; double mu = 0, kT = 0, sigma = 0; const double *w_q = nullptr; double *out = nullptr; } cons;
+  DevBuf g2_scratch;   // |g|^2 of one q when the caller passes g2 = NULL (consumer on)
   const c128 *ext_g1 = nullptr;  // g(Re,q) supplied by the caller (already summed over every rank's Rp) for this call
   // resident operators
   DevBuf g, H, D, Re, Rp, we, wp, ones;
@@ -210,6 +213,10 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
                              cudaStream_t st) {
   const int nb = h->nb, nm = h->nm, ne = h->ne, np = h->np, nbb = h->nbb, nmm = h->nmm;
   const int64_t E = (int64_t)nbb * nm;        // elements per (k,q) pair
+  if (!g2) CU_OR_FAIL(h, h->g2_scratch.reserve(sizeof(double) * (size_t)nk * E), "cudaMalloc |g|^2 scratch");
+  double *const g2_base = g2 ? g2 : h->g2_scratch.as<double>();
+  const int64_t g2_qs = g2 ? nk * E : 0;
+  auto G2 = [&](int64_t q, int64_t k0) { return g2_base + q * g2_qs + k0 * E; };
   const int64_t xrows = (int64_t)ne * nbb;    // rows of the S4a contraction
   const int64_t MR = (int64_t)nm * nb;        // rows of the two S4b contractions
   const int KBe = (int)ceil_div(2 * (int64_t)ne, GEMM_BK), KBb = (int)ceil_div(2 * (int64_t)nb, GEMM_BK);
@@ -385,7 +392,7 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
                                        h->T.p, MR, 0, nb, 1, E, 0, MR, nb, nb, kn, h->num_sms, st),
                "zgemm S4b (U_k)");
         LAUNCH(h, launch_zgemm_strided(h->T.as<c128>(), nb, nbb, nb, E, kq_map ? Bconj : Bconj + k0 * upack,
-                                       kq_map ? kq_map + q * nk + k0 : nullptr, g2 + (q * nk + k0) * E, MR, 0, nb, 1, E,
+                                       kq_map ? kq_map + q * nk + k0 : nullptr, G2(q, k0), MR, 0, nb, 1, E,
                                        1, MR, nb, nb, kn, h->num_sms, st),
                "zgemm S4b (U_{k+q}) + |g|^2");
         if (h->window_on) {
@@ -394,11 +401,18 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
           const double *ekq = kq_map ? nullptr : (eps_kq ? eps_kq + (q * nk + k0) * nb : h->epskq_scratch.as<double>() + k0 * nb);
           LAUNCH(h, launch_window_mask(eps_k + k0 * nb, ekq, eps_k, kq_map ? kq_map + q * nk + k0 : nullptr, nb, kn, h->emin,
                                        h->emax, m, st), "window mask");
-          LAUNCH(h, launch_zero_masked(m, kn, E, g2 + (q * nk + k0) * E, st), "zero screened pairs");
+          LAUNCH(h, launch_zero_masked(m, kn, E, G2(q, k0), st), "zero screened pairs");
+        }
+        if (h->cons.on) {
+          const double *ekq = kq_map ? nullptr : (eps_kq ? eps_kq + (q * nk + k0) * nb : h->epskq_scratch.as<double>() + k0 * nb);
+          LAUNCH(h, launch_selfenergy_accumulate(G2(q, k0), eps_k + k0 * nb, ekq, eps_k, kq_map ? kq_map + q * nk + k0 : nullptr,
+                                                 omega_q + q * nm, h->cons.w_q, q, h->cons.mu, h->cons.kT, h->cons.sigma, nb,
+                                                 nm, kn, h->cons.out + k0 * nb, st),
+                 "Im Sigma accumulate");
         }
         h->end_span(sp, st);
       }
-      { const int rc = h->drain_q(q, nk, E, g2, eps_kq, st); if (rc != EPW_OK) return rc; }
+      if (g2) { const int rc = h->drain_q(q, nk, E, g2, eps_kq, st); if (rc != EPW_OK) return rc; }
     }
   }
   h->end_span(t_total, st);
@@ -483,7 +497,7 @@ void epw_interp_destroy(epw_interp_t h) {
                    &h->status, &h->eig_scratch, &h->hs_k, &h->hs_q, &h->hs_map, &h->hs_epsk, &h->hs_epskq,
                    &h->hs_omega, &h->hs_g2, &h->Pk, &h->BpackPk, &h->UpackK, &h->UpackKH, &h->BpackE,
                    &h->ghat, &h->T, &h->Hkq, &h->boxidx, &h->X, &h->T1, &h->T2, &h->Ptmp, &h->P1raw, &h->P2raw, &h->P3raw, &h->P1pack, &h->P2pack,
-                   &h->P3pack, &h->klist_gen, &h->workctr, &h->maskbuf};
+                   &h->P3pack, &h->klist_gen, &h->workctr, &h->maskbuf, &h->g2_scratch};
   for (DevBuf *b : all) b->release();
   for (cudaEvent_t ev : h->ev_pool) cudaEventDestroy(ev);
   for (cudaEvent_t ev : h->sink_ev) cudaEventDestroy(ev);
@@ -577,7 +591,7 @@ int epw_interp_enable_stage_timing(epw_interp_t h, int on) {
 
 static int check_interpolate_args(epw_interp *h, const void *k_src, int64_t nk, const double *q_list, int64_t nq,
                                   const double *eps_k, const double *omega_q, const double *g2, const char *who) {
-  if (!k_src || !q_list || !eps_k || !omega_q || !g2 || nk <= 0 || nq <= 0)
+  if (!k_src || !q_list || !eps_k || !omega_q || (!g2 && !h->cons.on) || nk <= 0 || nq <= 0)
     return h->fail(EPW_EINVAL, std::string(who) + ": null pointer or non-positive nk/nq");
   if (!h->operators_set) return h->fail(EPW_EINVAL, std::string(who) + ": operators not set");
   if (!h->ext_g1) {
@@ -656,6 +670,11 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   const int QB = (int)std::min<int64_t>(h->q_batch, nq);
   const int64_t E = (int64_t)ncols_g;
   const size_t cap = h->cfg.workspace_bytes ? h->cfg.workspace_bytes : ((size_t)6 << 30);
+  // |g|^2 of pair (q, k0..): the caller's buffer, or (consumer on, g2 = NULL) the library's one-q scratch
+  if (!g2) CU_OR_FAIL(h, h->g2_scratch.reserve(sizeof(double) * (size_t)nk * E), "cudaMalloc |g|^2 scratch");
+  double *const g2_base = g2 ? g2 : h->g2_scratch.as<double>();
+  const int64_t g2_qs = g2 ? nk * E : 0;
+  auto G2 = [&](int64_t q, int64_t k0) { return g2_base + q * g2_qs + k0 * E; };
 
   int64_t kchunk, c_rows;
   // grid mode: extents of the three axis passes (re_to_k_grid.cu)
@@ -957,19 +976,27 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
         sp = h->begin_span(6, st);
         if (!fused) {
           LAUNCH(h, launch_rotate_g2(Cc, ncols, h->Uk.as<c128>() + k0 * nbb, Ukq_ptr, kq_idx, nb, nm, kn, mask,
-                                     g2 + (q * nk + k0) * E, st),
+                                     G2(q, k0), st),
                  "rotate_g2");
         } else {
           const int ci = (int)(k0 / kchunk);
           const int cnt = std::min(cs, grid->N[0] - ci * cs);
           LAUNCH(h, launch_grid_rotate_g2(h->T2.as<c128>(), slab, ncols, L[0], h->P1raw.as<c128>() + (int64_t)ci * L[0] * cs,
                                           cnt, h->Uk.as<c128>() + k0 * nbb, Ukq_ptr, kq_idx, nb, nm, h->num_sms, mask,
-                                          g2 + (q * nk + k0) * E, st),
+                                          G2(q, k0), st),
                  "grid_rotate_g2");
+        }
+        if (h->cons.on) {
+          const double *ekq = kq_map ? nullptr
+                                     : (eps_kq ? eps_kq + (q * nk + k0) * nb : h->epskq_scratch.as<double>() + crow * nb);
+          LAUNCH(h, launch_selfenergy_accumulate(G2(q, k0), eps_k + k0 * nb, ekq, eps_k, kq_idx, omega_q + q * nm,
+                                                 h->cons.w_q, q, h->cons.mu, h->cons.kT, h->cons.sigma, nb, nm, kn,
+                                                 h->cons.out + k0 * nb, st),
+                 "Im Sigma accumulate");
         }
         h->end_span(sp, st);
       }
-      { const int rc = h->drain_q(q, nk, E, g2, eps_kq, st); if (rc != EPW_OK) return rc; }
+      if (g2) { const int rc = h->drain_q(q, nk, E, g2, eps_kq, st); if (rc != EPW_OK) return rc; }
     }
   }
   h->end_span(t_total, st);
@@ -977,6 +1004,20 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
 }
 
 extern "C" {
+
+int epw_interp_set_selfenergy_consumer(epw_interp_t h, int enabled, double mu, double kT, double sigma, const double *w_q,
+                                       double *im_sigma) {
+  if (!h) return EPW_EINVAL;
+  if (enabled && (!(kT > 0.0) || !(sigma > 0.0) || !im_sigma))
+    return h->fail(EPW_EINVAL, "epw_interp_set_selfenergy_consumer: need kT > 0, sigma > 0 and an output buffer");
+  h->cons.on = enabled != 0;
+  h->cons.mu = mu;
+  h->cons.kT = kT;
+  h->cons.sigma = sigma;
+  h->cons.w_q = enabled ? w_q : nullptr;
+  h->cons.out = enabled ? im_sigma : nullptr;
+  return EPW_OK;
+}
 
 int epw_interp_set_energy_window(epw_interp_t h, int enabled, double emin, double emax, uint8_t *mask_out) {
   if (!h) return EPW_EINVAL;

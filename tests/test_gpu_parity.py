@@ -849,3 +849,64 @@ def test_omega_min_cutoff_and_tiny_lists(epw, route):
             assert_path_close([t.cpu().numpy() for t in out], ref1)
     finally:
         h.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# NEXT-4: a consumer of |g|^2 on the device (Im Sigma_nk accumulator, reading G18)
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("mode", ["grid-fused-nog2", "grid-unfused", "list", "list-kqmap-nog2", "large", "large-nog2"])
+def test_selfenergy_consumer(epw, mode):
+    if mode.startswith("large"):
+        w = synth.make_custom("zsnr-se", 18, 5, (2, 0, 0), 1.0, 0.05, 2.0, (24, 1, 1), ("random", 5, 1), seed=81)
+        ql, kq_map = w.q_list, None
+    else:
+        w = synth.make_config(0)
+        ql = w.q_list[:6] if "kqmap" in mode else w.q_list[:6] + [0.013, 0.007, 0.021]
+        kq_map = np.ascontiguousarray(w.kq_map[:6]) if "kqmap" in mode else None
+    nq = len(ql)
+    ref = oracle.interpolate(w.H_R, w.D_R, w.g_full(), w.Re, w.w_e, w.Rp, w.w_p, w.k_list, ql)
+    mu = float(np.median(ref[0]))
+    kT, sigma = 0.05, 0.08
+    wq = np.random.default_rng(5).uniform(0.5, 1.5, size=nq)
+    want = oracle.selfenergy_accumulate(ref[3], ref[0], ref[1], ref[2], wq, mu, kT, sigma)
+    want2 = oracle.selfenergy_accumulate(ref[3][:2], ref[0], ref[1][:2], ref[2][:2], None, mu, kT, sigma, out=want.copy())
+    h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_, q_batch=4, path=2 if mode.startswith("large") else 0,
+                      flags=epw.EPW_FLAG_GRID_UNFUSED if mode == "grid-unfused" else 0)
+    try:
+        h.set_operators_from_host(w)
+        acc = torch.zeros((w.nk, w.nbnd), dtype=torch.float64, device="cuda")
+        wq_d = dev(wq)
+        epw.epw_interp_set_selfenergy_consumer(h.h, True, mu, kT, sigma, wq_d, acc)
+        nog2 = mode.endswith("nog2")
+        eps_k = torch.empty((w.nk, w.nbnd), dtype=torch.float64, device="cuda")
+        om = torch.empty((nq, w.nmodes), dtype=torch.float64, device="cuda")
+        g2 = None if nog2 else torch.empty((nq, w.nk, w.nmodes, w.nbnd, w.nbnd), dtype=torch.float64, device="cuda")
+        q_d, k_d = dev(ql), dev(w.k_list)
+        map_d = None if kq_map is None else dev(kq_map)
+
+        def call(nq_call, eps_kq):
+            if mode.startswith("grid"):
+                epw.epw_interp_interpolate_grid(h.h, w.k_grid, None, q_d, nq_call, map_d, eps_k, eps_kq, om, g2)
+            else:
+                epw.epw_interp_interpolate(h.h, k_d, w.nk, q_d, nq_call, map_d, eps_k, eps_kq, om, g2)
+            epw.epw_interp_sync(h.h)
+
+        call(nq, None)   # eps_kq = NULL: the consumer reads the library's own eigenvalues
+        got = acc.cpu().numpy()
+        assert np.abs(got - want).max() <= 1e-8 * np.abs(want).max()
+        if g2 is not None:   # |g|^2 is still delivered when the caller asks for it
+            assert_path_close((eps_k.cpu().numpy(), ref[1], om.cpu().numpy(), g2.cpu().numpy()), ref,   # eps_kq not requested
+                              pairs=[(0, 0), (nq - 1, w.nk - 1), (2, 7)])
+        # a second call accumulates (first two q again, unit weights)
+        epw.epw_interp_set_selfenergy_consumer(h.h, True, mu, kT, sigma, None, acc)
+        eps_kq = torch.empty((2, w.nk, w.nbnd), dtype=torch.float64, device="cuda")
+        call(2, eps_kq)
+        got2 = acc.cpu().numpy()
+        assert np.abs(got2 - want2).max() <= 1e-8 * np.abs(want2).max()
+        # g2 = NULL without a consumer is an error
+        epw.epw_interp_set_selfenergy_consumer(h.h, False)
+        if nog2:
+            with pytest.raises(epw.EpwError):
+                call(2, eps_kq)
+    finally:
+        h.close()
