@@ -135,6 +135,9 @@ cudaError_t launch_grid_rotate_g2(const c128 *T2, int64_t slab, int ncols, int L
 bool axis_pass_supported(int K);
 cudaError_t launch_axis_pass(const c128 *A, int64_t a_rb, int64_t a_bs, int64_t a_ks, int64_t M, const c128 *P, int K, int N,
                              c128 *C, int64_t c_rb, int64_t c_bs, int64_t c_cs, int num_sms, cudaStream_t st);
+cudaError_t launch_axis_pass_p(const c128 *A, int64_t a_rb, int64_t a_bs, int64_t a_ks, int64_t M, const c128 *P,
+                               int64_t p_rs, int64_t p_cs, int K, int N, c128 *C, int64_t c_rb, int64_t c_bs, int64_t c_cs,
+                               int num_sms, cudaStream_t st);
 cudaError_t launch_grid_klist(const int32_t N[3], const double s[3], double *k_list, cudaStream_t st);
 
 // mask (may be NULL): uint8 per pair, 0 = skipped by the energy-window pre-screening -> zeros, no arithmetic

@@ -125,56 +125,63 @@ cudaError_t launch_grid_klist(const int32_t N[3], const double s[3], double *k_l
 // inputs of two adjacent rows in registers, takes the phases by broadcast from shared memory and streams the columns
 // out with fully coalesced 16-byte stores; blockIdx.y splits the columns so that small passes still fill the GPU.
 // ---------------------------------------------------------------------------------------------------------------
-template <int KMAX>
+template <int KMAX, int R>
 __global__ void __launch_bounds__(256)
     axis_pass_kernel(const c128 *__restrict__ A, int64_t a_rb, int64_t a_bs, int64_t a_ks, int64_t M,
-                     const c128 *__restrict__ P, int K, int N, int cols_per_y, c128 *__restrict__ C, int64_t c_rb,
-                     int64_t c_bs, int64_t c_cs) {
+                     const c128 *__restrict__ P, int64_t p_rs, int64_t p_cs, int K, int N, int cols_per_y,
+                     c128 *__restrict__ C, int64_t c_rb, int64_t c_bs, int64_t c_cs) {
   extern __shared__ double2 sPh[];  // [K][ncol] of this column group
   const int col0 = blockIdx.y * cols_per_y;
   const int ncol = N - col0 < cols_per_y ? N - col0 : cols_per_y;
   for (int e = threadIdx.x; e < K * ncol; e += blockDim.x) {
     const int r = e / ncol, c = e - r * ncol;
-    sPh[e] = P[(int64_t)r * N + col0 + c];
+    sPh[e] = P[(int64_t)r * p_rs + (int64_t)(col0 + c) * p_cs];
   }
   __syncthreads();
-  const int64_t row0 = 2 * (blockIdx.x * (int64_t)blockDim.x + threadIdx.x);
+  const int64_t row0 = R * (blockIdx.x * (int64_t)blockDim.x + threadIdx.x);
   if (row0 >= M) return;
-  const bool two = row0 + 1 < M;
-  const int64_t row1 = two ? row0 + 1 : row0;
-  const int64_t b0 = row0 / a_rb, b1 = row1 / a_rb;
-  const c128 *src0 = A + b0 * a_bs + (row0 - b0 * a_rb), *src1 = A + b1 * a_bs + (row1 - b1 * a_rb);
-  c128 x0[KMAX], x1[KMAX];
+  c128 x[R][KMAX];
+  c128 *dst[R];
+  bool have[R];
 #pragma unroll
-  for (int r = 0; r < KMAX; r++) {
-    x0[r] = r < K ? src0[(int64_t)r * a_ks] : cmake(0.0, 0.0);
-    x1[r] = r < K ? src1[(int64_t)r * a_ks] : cmake(0.0, 0.0);
+  for (int i = 0; i < R; i++) {
+    have[i] = row0 + i < M;
+    const int64_t row = have[i] ? row0 + i : row0;
+    const int64_t b = row / a_rb;
+    const c128 *src = A + b * a_bs + (row - b * a_rb);
+#pragma unroll
+    for (int r = 0; r < KMAX; r++) x[i][r] = r < K ? src[(int64_t)r * a_ks] : cmake(0.0, 0.0);
+    const int64_t d = row / c_rb;
+    dst[i] = C + d * c_bs + (row - d * c_rb) + (int64_t)col0 * c_cs;
   }
-  const int64_t d0 = row0 / c_rb, d1 = row1 / c_rb;
-  c128 *dst0 = C + d0 * c_bs + (row0 - d0 * c_rb) + (int64_t)col0 * c_cs;
-  c128 *dst1 = C + d1 * c_bs + (row1 - d1 * c_rb) + (int64_t)col0 * c_cs;
   for (int c = 0; c < ncol; c++) {
-    c128 y0 = cmake(0.0, 0.0), y1 = cmake(0.0, 0.0);
+    c128 y[R];
+#pragma unroll
+    for (int i = 0; i < R; i++) y[i] = cmake(0.0, 0.0);
 #pragma unroll
     for (int r = 0; r < KMAX; r++) {
       if (r < K) {
         const c128 ph = sPh[r * ncol + c];
-        cfma(y0, x0[r], ph);
-        cfma(y1, x1[r], ph);
+#pragma unroll
+        for (int i = 0; i < R; i++) cfma(y[i], x[i][r], ph);
       }
     }
-    dst0[(int64_t)c * c_cs] = y0;
-    if (two) dst1[(int64_t)c * c_cs] = y1;
+#pragma unroll
+    for (int i = 0; i < R; i++)
+      if (have[i]) dst[i][(int64_t)c * c_cs] = y[i];
   }
 }
 
 bool axis_pass_supported(int K) { return K >= 1 && K <= 32; }
 
-cudaError_t launch_axis_pass(const c128 *A, int64_t a_rb, int64_t a_bs, int64_t a_ks, int64_t M, const c128 *P, int K, int N,
-                             c128 *C, int64_t c_rb, int64_t c_bs, int64_t c_cs, int num_sms, cudaStream_t st) {
+// P element (r, col) at P + r * p_rs + col * p_cs (c128 elements)
+cudaError_t launch_axis_pass_p(const c128 *A, int64_t a_rb, int64_t a_bs, int64_t a_ks, int64_t M, const c128 *P,
+                               int64_t p_rs, int64_t p_cs, int K, int N, c128 *C, int64_t c_rb, int64_t c_bs, int64_t c_cs,
+                               int num_sms, cudaStream_t st) {
   if (M <= 0 || N <= 0 || K <= 0) return cudaSuccess;
   if (K > 32) return cudaErrorInvalidValue;
-  const int64_t bx = ceil_div(ceil_div(M, 2), 256);
+  const int R = K <= 16 ? 2 : 1;   // rows per thread: the K inputs of every row live in registers
+  const int64_t bx = ceil_div(ceil_div(M, R), 256);
   // split the columns while the row blocks alone would not give every SM a few CTAs
   int ny = 1;
   while (bx * ny < 4 * (int64_t)num_sms && ny < N && N / (ny + 1) >= 8) ny++;
@@ -182,19 +189,26 @@ cudaError_t launch_axis_pass(const c128 *A, int64_t a_rb, int64_t a_bs, int64_t 
   ny = (int)ceil_div(N, cols_per_y);
   const size_t smem = sizeof(double2) * (size_t)K * cols_per_y;
   dim3 grid((unsigned)bx, (unsigned)ny);
-#define EPW_AXIS_LAUNCH(KM)                                                                                          \
+#define EPW_AXIS_LAUNCH(KM, RR)                                                                                       \
   do {                                                                                                               \
     if (smem > 48 * 1024) {                                                                                          \
-      cudaError_t e = cudaFuncSetAttribute(axis_pass_kernel<KM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+      cudaError_t e =                                                                                                \
+          cudaFuncSetAttribute(axis_pass_kernel<KM, RR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);    \
       if (e != cudaSuccess) return e;                                                                                \
     }                                                                                                                \
-    axis_pass_kernel<KM><<<grid, 256, smem, st>>>(A, a_rb, a_bs, a_ks, M, P, K, N, cols_per_y, C, c_rb, c_bs, c_cs);    \
+    axis_pass_kernel<KM, RR><<<grid, 256, smem, st>>>(A, a_rb, a_bs, a_ks, M, P, p_rs, p_cs, K, N, cols_per_y, C, c_rb, \
+                                                      c_bs, c_cs);                                                   \
   } while (0)
-  if (K <= 8) EPW_AXIS_LAUNCH(8);
-  else if (K <= 16) EPW_AXIS_LAUNCH(16);
-  else EPW_AXIS_LAUNCH(32);
+  if (K <= 8) EPW_AXIS_LAUNCH(8, 2);
+  else if (K <= 16) EPW_AXIS_LAUNCH(16, 2);
+  else EPW_AXIS_LAUNCH(32, 1);
 #undef EPW_AXIS_LAUNCH
   return cudaGetLastError();
+}
+
+cudaError_t launch_axis_pass(const c128 *A, int64_t a_rb, int64_t a_bs, int64_t a_ks, int64_t M, const c128 *P, int K, int N,
+                             c128 *C, int64_t c_rb, int64_t c_bs, int64_t c_cs, int num_sms, cudaStream_t st) {
+  return launch_axis_pass_p(A, a_rb, a_bs, a_ks, M, P, N, 1, K, N, C, c_rb, c_bs, c_cs, num_sms, st);
 }
 
 }  // namespace epw
