@@ -82,27 +82,31 @@ __global__ void __launch_bounds__(W * 32, MINB)
       continue;
     }
     if (lane < L1) sP[lane] = P1c[(int64_t)lane * cnt + j];
-    // ---- B' = embedding of Uk, B'' = embedding of conj(Ukq); fragment (ks, nt): k-row 4 ks + t, column 8 nt + g ----
+    // ---- B' = embedding of Uk (product 1); fragment (ks, nt): k-row 4 ks + t, column 8 nt + g.  For Nb > 8 the
+    //      embedding B'' of conj(Ukq) is built only after product 1 (its lines are prefetched into L1 here), which
+    //      keeps one fragment set live at a time and lets 12 warps share the SM instead of 8. ----
+    constexpr bool LATE_B2 = NB > 8;
+    const c128 *uk = Uk + kc * NBB;
+    const c128 *ukq = Ukq + (kq_idx ? (int64_t)kq_idx[kc] : kc) * NBB;
     double b1[KS][NT], b2[KS][NT];
-    {
-      const c128 *uk = Uk + kc * NBB;
-      const c128 *ukq = Ukq + (kq_idx ? (int64_t)kq_idx[kc] : kc) * NBB;
-#pragma unroll
-      for (int ks = 0; ks < KS; ks++)
-#pragma unroll
-        for (int nt = 0; nt < NT; nt++) {
-          const int r = 2 * ks + (t >> 1), a = t & 1;   // complex row (n' or m'), real sub-row
-          const int c = 4 * nt + (g >> 1), b = g & 1;   // complex column (n or m), real sub-column
-          c128 x = make_double2(0.0, 0.0), y = make_double2(0.0, 0.0);
-          if (r < NB && c < NB) {
-            x = uk[r + NB * c];
-            y = ukq[r + NB * c];
-          }
-          y.y = -y.y;  // conj(Ukq)
-          b1[ks][nt] = a == 0 ? (b ? x.y : x.x) : (b ? x.x : -x.y);
-          b2[ks][nt] = a == 0 ? (b ? y.y : y.x) : (b ? y.x : -y.y);
-        }
+    if (LATE_B2) {
+      if (lane * 8 < NBB) asm volatile("prefetch.global.L1 [%0];" ::"l"(ukq + lane * 8));
     }
+#pragma unroll
+    for (int ks = 0; ks < KS; ks++)
+#pragma unroll
+      for (int nt = 0; nt < NT; nt++) {
+        const int r = 2 * ks + (t >> 1), a = t & 1;   // complex row (n' or m'), real sub-row
+        const int c = 4 * nt + (g >> 1), b = g & 1;   // complex column (n or m), real sub-column
+        c128 x = make_double2(0.0, 0.0), y = make_double2(0.0, 0.0);
+        if (r < NB && c < NB) {
+          x = uk[r + NB * c];
+          if (!LATE_B2) y = ukq[r + NB * c];
+        }
+        y.y = -y.y;  // conj(Ukq)
+        b1[ks][nt] = a == 0 ? (b ? x.y : x.x) : (b ? x.x : -x.y);
+        if (!LATE_B2) b2[ks][nt] = a == 0 ? (b ? y.y : y.x) : (b ? y.x : -y.y);
+      }
     __syncwarp();
     // ---- last axis pass + product 1: T[(nu,m')][n] = sum_n' g~[nu][n'][m'] Uk[n'][n] ----
     for (int mt = 0; mt < MT; mt++) {
@@ -144,6 +148,19 @@ __global__ void __launch_bounds__(W * 32, MINB)
       }
     }
     __syncwarp();
+    if (LATE_B2) {
+#pragma unroll
+      for (int ks = 0; ks < KS; ks++)
+#pragma unroll
+        for (int nt = 0; nt < NT; nt++) {
+          const int r = 2 * ks + (t >> 1), a = t & 1;
+          const int c = 4 * nt + (g >> 1), b = g & 1;
+          c128 y = make_double2(0.0, 0.0);
+          if (r < NB && c < NB) y = ukq[r + NB * c];
+          y.y = -y.y;  // conj(Ukq)
+          b2[ks][nt] = a == 0 ? (b ? y.y : y.x) : (b ? y.x : -y.y);
+        }
+    }
     // ---- product 2: |sum_m' T[(nu,n)][m'] conj(Ukq[m'][m])|^2 ----
     double *dst = g2 + kc * E + (int64_t)nu0 * NBB;
     for (int mt = 0; mt < MT; mt++) {
@@ -205,7 +222,7 @@ static cudaError_t launch_grot(const c128 *T2, int64_t slab, int ncols, int L1, 
 
 bool grid_rotate_g2_supported(int nb, int nm, int L1) {
   if (nb < 1 || nb > 16 || L1 > 32) return false;
-  const int W = 8;
+  const int W = nb <= 8 ? 8 : 12;
   const size_t need = sizeof(c128) * ((size_t)L1 * nb * grot_t2_pitch(nb) + (size_t)W * L1 + (size_t)W * (((size_t)nb + 7) / 8) * 8 * grot_pitch(nb));
   (void)nm;
   return need <= (nb <= 8 ? ((size_t)110 << 10) : ((size_t)220 << 10));
@@ -221,9 +238,9 @@ cudaError_t launch_grid_rotate_g2(const c128 *T2, int64_t slab, int ncols, int L
 #define EPW_GROT_CASE(NB_, W_) \
   case NB_: return launch_grot<NB_, W_, (NB_ <= 8 ? 2 : 1)>(T2, slab, ncols, L1, P1c, cnt, Uk, Ukq, kq_idx, nm, num_sms, mask, g2, st);
     EPW_GROT_CASE(1, 8) EPW_GROT_CASE(2, 8) EPW_GROT_CASE(3, 8) EPW_GROT_CASE(4, 8) EPW_GROT_CASE(5, 8)
-    EPW_GROT_CASE(6, 8) EPW_GROT_CASE(7, 8) EPW_GROT_CASE(8, 8) EPW_GROT_CASE(9, 8) EPW_GROT_CASE(10, 8)
-    EPW_GROT_CASE(11, 8) EPW_GROT_CASE(12, 8) EPW_GROT_CASE(13, 8) EPW_GROT_CASE(14, 8) EPW_GROT_CASE(15, 8)
-    EPW_GROT_CASE(16, 8)
+    EPW_GROT_CASE(6, 8) EPW_GROT_CASE(7, 8) EPW_GROT_CASE(8, 8) EPW_GROT_CASE(9, 12) EPW_GROT_CASE(10, 12)
+    EPW_GROT_CASE(11, 12) EPW_GROT_CASE(12, 12) EPW_GROT_CASE(13, 12) EPW_GROT_CASE(14, 12) EPW_GROT_CASE(15, 12)
+    EPW_GROT_CASE(16, 12)
 #undef EPW_GROT_CASE
     default: return cudaErrorInvalidConfiguration;
   }
