@@ -7,7 +7,7 @@
 //
 // sm_100a has no tcgen05 kind for FP64: the FP64 tensor instruction is the warp-level DMMA (mma.sync m8n8k4.f64,
 // SASS DMMA.8x8x4; the m16n8k{4,8,16}.f64 shapes lower to the same instruction), measured at 37.0 TFLOP/s on this
-// B200 = 64 FMA/clk/SM (profiles/r01_fp64_probe.md).  The kernel is built around that:
+// B200 = 64 FMA/clk/SM (epw_probe_peaks, printed in every bench line).  The kernel is built around that:
 //   * complex product as a real GEMM with interleaved re/im (common.cuh): 4 real FMA per complex MAC, no waste;
 //   * both operands are pre-packed in fragment order, so a (tile, k-block) chunk is ONE 16 KB 1-D bulk TMA copy
 //     (cp.async.bulk ... mbarrier::complete_tx, SASS UBLKCP) and every fragment load is a conflict-free LDS.128;
