@@ -183,7 +183,7 @@ def sample_size(w):
     E = w.elements_per_pair
     if E > 1_000_000:
         return 1, 2     # configs[4]: ~50 s per pair in the oracle's plain loops
-    return (4, 4096) if E < 2000 else (4, 512)
+    return (8, 8192) if E < 2000 else (4, 512)
 
 
 def run_reference(args):
