@@ -910,3 +910,22 @@ def test_selfenergy_consumer(epw, mode):
                 call(2, eps_kq)
     finally:
         h.close()
+
+
+@pytest.mark.parametrize("delta", [3e-7, 1e-4])
+@pytest.mark.parametrize("route", ["list", "grid"])
+def test_nearly_degenerate_bands(epw, route, delta):
+    """Bands split by delta: 3e-7 eV (inside the 1e-6 eV degeneracy window: compared as block sums) and 1e-4 eV (resolved
+    individually: the eigenvectors must then be accurate to ~ eps / delta)."""
+    base = synth.make_custom("ndeg", 3, 3, (1, 1, 0), 1.0, 0.1, 1.0, (5, 4, 1), ("random", 3, 2), seed=73)
+    H = np.stack([np.kron(np.eye(2), base.H_R[i].T).T for i in range(base.ne)])
+    i0 = [i for i, r in enumerate(base.Re) if not r.any()][0]
+    H[i0] += np.diag([0, 0, 0, delta, delta, delta])
+    nb, nm = 6, 3
+    g = 0.1 * crandn(base.np_, nm, base.ne, nb, nb) * np.exp(-np.linalg.norm(base.Re, axis=1))[None, None, :, None, None]
+    w = _Wl(np.ascontiguousarray(H), base.D_R, g, base.Re, base.Rp)
+    ref = oracle.interpolate(w.H_R, w.D_R, g, w.Re, w.w_e, w.Rp, w.w_p, base.k_list, base.q_list)
+    gaps = np.diff(ref[0], axis=1)
+    assert np.abs(gaps - delta).min() < 1e-9            # the splitting is really there
+    kw = dict(grid=base.k_grid) if route == "grid" else {}
+    assert_path_close(run_gpu(epw, w, base.k_list, base.q_list, **kw), ref)
