@@ -56,6 +56,7 @@ def parse_args():
                          "its slabs for the q-points of ALL ranks, one NCCL reduce-scatter of g(Re,q) hands each rank the "
                          "summed g(Re,q) of its own q-points, and the rest of the path runs unchanged")
     ap.add_argument("--grid-unfused", action="store_true", help="EPW_FLAG_GRID_UNFUSED: keep g~ in HBM between S2 and S4b")
+    ap.add_argument("--grid-fused", action="store_true", help="EPW_FLAG_GRID_FUSED: force the fused last-pass + rotation kernel")
     ap.add_argument("--k-mode", default="grid", choices=["grid", "list"],
                     help="grid: epw_interp_interpolate_grid (the configs' k-points ARE uniform grids; factorised S2); "
                          "list: epw_interp_interpolate on the same k-points as a plain list (dense DMMA S2)")
@@ -298,7 +299,7 @@ def main():
     nq_step = args.nq_step or max(1, min(32, int((40 << 30) // (8 * nk * E))))
     nq_step = min(nq_step, w.nq)
     h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_, device=local_rank, q_batch=args.q_batch,
-                      flags=epw.EPW_FLAG_GRID_UNFUSED if args.grid_unfused else 0)
+                      flags=epw.EPW_FLAG_GRID_UNFUSED if args.grid_unfused else (epw.EPW_FLAG_GRID_FUSED if args.grid_fused else 0))
     t0 = time.perf_counter()
     # upload once; resident for the whole run; with --rp-shard only this rank's Rp slabs
     h.set_operators_from_host(w, rp_range=shard.rp_ranges(w.np_, world)[rank] if args.rp_shard else None)

@@ -56,8 +56,9 @@ typedef struct {
   int32_t device;         /* CUDA device ordinal */
   int32_t q_batch;        /* q-points contracted per pass over g(Re,Rp) in S1 (1..8); 0 = library default */
   int32_t path;           /* EPW_PATH_AUTO (0): chosen from Nb, Nm; EPW_PATH_SMALL / EPW_PATH_LARGE force one (tests) */
-  int32_t flags;          /* 0, or EPW_FLAG_GRID_UNFUSED: on a uniform grid keep the last axis pass of S2 and S4b as two
-                             kernels with g~ in HBM (tests, debug getters) instead of the fused kernel */
+  int32_t flags;          /* 0: on a uniform grid the library chooses between the fused kernel (last axis pass of S2 + S4b,
+                             g~ never in HBM; chosen for Nb <= 8) and the two-kernel form (chosen for 9 <= Nb <= 16, where
+                             it measures faster); EPW_FLAG_GRID_UNFUSED / EPW_FLAG_GRID_FUSED force one of them */
   size_t workspace_bytes; /* cap on the library's scratch HBM; 0 = library chooses from free memory */
   double degen_tol;       /* informational (gap below which callers should sum |g|^2 over a subspace); unused inside */
   double omega_min;       /* modes with omega_q,nu <= omega_min give |g|^2 = 0 (acoustic modes at Gamma); default 0 */
@@ -67,7 +68,7 @@ typedef struct {
  * LARGE: S4a, S2 and both halves of S4b are FP64 tensor-path contractions that read their operand in place
  * (any Nb; configs[4], Nb = 192, Nm = 288).  Same results; AUTO picks by size. */
 enum { EPW_PATH_AUTO = 0, EPW_PATH_SMALL = 1, EPW_PATH_LARGE = 2 };
-enum { EPW_FLAG_GRID_UNFUSED = 1 };
+enum { EPW_FLAG_GRID_UNFUSED = 1, EPW_FLAG_GRID_FUSED = 2 };
 
 /* Create / destroy a handle.  *out is set to NULL on failure. */
 int epw_interp_create(epw_interp_t *out, const epw_interp_config *cfg);

@@ -21,7 +21,7 @@ LIB_PATH = os.path.join(PKG, "libepw_interp.so")
 
 EPW_OK, EPW_EINVAL, EPW_ENOMEM, EPW_ECUDA, EPW_ENOTCONVERGED, EPW_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 EPW_PATH_AUTO, EPW_PATH_SMALL, EPW_PATH_LARGE = 0, 1, 2
-EPW_FLAG_GRID_UNFUSED = 1
+EPW_FLAG_GRID_UNFUSED, EPW_FLAG_GRID_FUSED = 1, 2
 EPW_NUM_STAGES = 9
 STAGE_NAMES = ["S0_phase_tables", "S1_rp_to_q", "phonon_Dq_eig_S4a_pack", "Hk_eig", "S2_re_to_k_dmma", "Hkq_eig",
                "S4b_rotate_g2", "total", "S4a_mode_rotation"]

@@ -446,7 +446,8 @@ int epw_interp_create(epw_interp_t *out, const epw_interp_config *cfg) {
     g_create_error = "epw_interp_create: path must be EPW_PATH_AUTO, EPW_PATH_SMALL or EPW_PATH_LARGE";
     return EPW_EINVAL;
   }
-  if (cfg->flags & ~EPW_FLAG_GRID_UNFUSED) {
+  if ((cfg->flags & ~(EPW_FLAG_GRID_UNFUSED | EPW_FLAG_GRID_FUSED)) ||
+      cfg->flags == (EPW_FLAG_GRID_UNFUSED | EPW_FLAG_GRID_FUSED)) {
     g_create_error = "epw_interp_create: unknown bit in flags";
     return EPW_EINVAL;
   }
@@ -683,7 +684,10 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   int cs = 0, nchunks = 1;   // i1 planes per k-chunk
   int KB1 = 0, NTc = 0;
   // grid mode: the last axis pass is fused with S4b (grid_rotate_g2.cu) unless the caller asked for the two-kernel form
-  const bool fused = grid && !(h->cfg.flags & EPW_FLAG_GRID_UNFUSED) && grid_rotate_g2_supported(nb, nm, h->box_L[0]);
+  // measured (bench.py --grid-unfused, configs[1..3]): the fused kernel wins for Nb = 8 (21.5 vs 22.2 ms, 128 vs 136 ms),
+  // the two-kernel form for Nb = 11 (22.9 vs 25.4 ms: 8-row DMMA tiles and mode groups fit Nb = 11 badly)
+  const bool want_fused = (h->cfg.flags & EPW_FLAG_GRID_FUSED) || (!(h->cfg.flags & EPW_FLAG_GRID_UNFUSED) && nb <= 8);
+  const bool fused = grid && want_fused && grid_rotate_g2_supported(nb, nm, h->box_L[0]);
   const int ncolsC = fused ? ncols_h : ncols;   // columns of the [g~ | H(k+q)] buffer that reach HBM
   if (!grid) {
     // k-chunk: one chunk of [g~ | H(k+q)] (16*ncols bytes per k) must stay L2-resident for the eigensolve and the

@@ -368,7 +368,8 @@ def run_gpu(epw, w, k_list, q_list, kq_map=None, q_batch=0, host_api=False, path
             return eps_k, eps_kq, om, g2
         if grid is not None:
             out = h.interpolate_grid(grid, dev(q_list), k_shift=shift, kq_map=None if kq_map is None else dev(kq_map))
-            want = "list" if path == 2 or w.nbnd > 16 else ("grid" if flags else "grid-fused")
+            fused = flags == 2 or (flags == 0 and w.nbnd <= 8)
+            want = "list" if path == 2 or w.nbnd > 16 else ("grid-fused" if fused else "grid")
             assert epw.epw_interp_last_plan(h.h)["k_mode"] == want
         else:
             out = h.interpolate(dev(k_list), dev(q_list), None if kq_map is None else dev(kq_map))
@@ -423,7 +424,7 @@ def test_grid_config0_both_kq_modes_and_host_api(epw):
     assert_path_close(run_gpu(epw, w, w.k_list, ql, None, grid=w.k_grid, host_api=True, q_batch=3), ref)
 
 
-@pytest.mark.parametrize("flags", [0, 1])
+@pytest.mark.parametrize("flags", [0, 1, 2])
 @pytest.mark.parametrize("shape", ["si", "mos2", "odd", "chunks", "large-forced", "modes-split"])
 def test_grid_reduced_shapes(epw, shape, flags):
     """Reduced configs 1-3 through the grid entry point: ragged tiles in every axis pass, 2-D and skewed lattices,
@@ -438,7 +439,7 @@ def test_grid_reduced_shapes(epw, shape, flags):
     elif shape == "chunks":
         w = synth.make_custom("chunks", 4, 3, (1, 1, 1), 1.0, 0.1, 1.0, (11, 3, 4), ("random", 2, 3), seed=14)
         # three i1 planes (12 k each) of per-k workspace per chunk -> 4 chunks, ragged last
-        ws = (16 * 12 * ((16 * 3 if flags else 0) + 16 + 16 + 4) + 16) * 3 + 100
+        ws = (16 * 12 * ((16 * 3 if flags == 1 else 0) + 16 + 16 + 4) + 16) * 3 + 100
     elif shape == "modes-split":
         # Nb = 13, Nm = 12, L1 = 7: the fused kernel cannot hold all modes of a cell in shared memory -> mode groups
         w = synth.make_custom("modes", 13, 12, (3, 1, 0), 1.0, 0.1, 1.0, (10, 3, 1), ("random", 2, 2), seed=15)
