@@ -84,15 +84,35 @@ __global__ void __launch_bounds__(ROT_THREADS)
     }
     // ---- product 1: T[(nu,m')][n] ----
     const double *gsrc = reinterpret_cast<const double *>(gt + ikc * stride_gt);
+    // A' fragments of tile mt: lane (g,t) holds one real component of g~[nu][n' = 2ks + t/2][m'] for row (nu,m') = 8 mt + g.
+    // The fragments of the NEXT tile are requested before the DMMAs of the current one (software pipeline): with loads
+    // issued only at their point of use a warp had 4 x 256 bytes in flight and the kernel ran at half the HBM rate.
+    auto load_a = [&](int mt, double (&dst)[KS]) {
+      const int row = 8 * mt + g;
+      const bool rv = row < rows;
+      const int nu = row / NB, mp = row - nu * NB;
+#pragma unroll
+      for (int ks = 0; ks < KS; ks++) {
+        const int np_ = 2 * ks + (t >> 1);
+        dst[ks] = (rv && np_ < NB) ? gsrc[(((int64_t)nu * NB + np_) * NB + mp) * 2 + (t & 1)] : 0.0;
+      }
+    };
+    // (only when one warp owns the pair, i.e. small Nb: for Nb > 8 the extra registers cost more occupancy than the
+    // pipeline gains)
+    constexpr bool PIPE = WPP == 1;
+    double a_next[KS];
+    if (PIPE && !skip && sub < MT) load_a(sub, a_next);
     for (int mt = sub; mt < (skip ? 0 : MT); mt += WPP) {
       const int row = 8 * mt + g;
       const bool rv = row < rows;
       const int nu = row / NB, mp = row - nu * NB;
       double a[KS];
+      if (PIPE) {
 #pragma unroll
-      for (int ks = 0; ks < KS; ks++) {
-        const int np_ = 2 * ks + (t >> 1);
-        a[ks] = (rv && np_ < NB) ? gsrc[(((int64_t)nu * NB + np_) * NB + mp) * 2 + (t & 1)] : 0.0;
+        for (int ks = 0; ks < KS; ks++) a[ks] = a_next[ks];
+        if (mt + WPP < MT) load_a(mt + WPP, a_next);
+      } else {
+        load_a(mt, a);
       }
       double acc[NT][2];
 #pragma unroll
