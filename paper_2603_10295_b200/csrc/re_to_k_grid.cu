@@ -122,8 +122,9 @@ cudaError_t launch_grid_klist(const int32_t N[3], const double s[3], double *k_l
 // K = L_d is 7..13 here: the pass reads each input once, writes N_d outputs per input and does 4 K DFMA per output --
 // it is bound by the write stream, and a tensor-core tile pipeline (load -> DMMA -> epilogue per tile, one CTA per SM)
 // only adds latency (43 us against a 14 us memory time for the axis-2 pass of configs[1]).  Here a thread keeps the K
-// inputs of two adjacent rows in registers, takes the phases by broadcast from shared memory and streams the columns
-// out with fully coalesced 16-byte stores; blockIdx.y splits the columns so that small passes still fill the GPU.
+// inputs of its row in registers (R rows per thread is a template parameter; one row measured best: more threads in
+// flight beat fewer phase loads per FMA), takes the phases by broadcast from shared memory and streams the columns out
+// with fully coalesced 16-byte stores; blockIdx.y splits the columns so that small passes still fill the GPU.
 // ---------------------------------------------------------------------------------------------------------------
 template <int KMAX, int R>
 __global__ void __launch_bounds__(256)
@@ -180,7 +181,7 @@ cudaError_t launch_axis_pass_p(const c128 *A, int64_t a_rb, int64_t a_bs, int64_
                                int num_sms, cudaStream_t st) {
   if (M <= 0 || N <= 0 || K <= 0) return cudaSuccess;
   if (K > 32) return cudaErrorInvalidValue;
-  const int R = K <= 16 ? 2 : 1;   // rows per thread: the K inputs of every row live in registers
+  const int R = 1;   // rows per thread (see the kernel comment)   // rows per thread: the K inputs of every row live in registers (96 / ~90 / ~160 per thread)
   const int64_t bx = ceil_div(ceil_div(M, R), 256);
   // split the columns while the row blocks alone would not give every SM a few CTAs
   int ny = 1;
@@ -199,8 +200,8 @@ cudaError_t launch_axis_pass_p(const c128 *A, int64_t a_rb, int64_t a_bs, int64_
     axis_pass_kernel<KM, RR><<<grid, 256, smem, st>>>(A, a_rb, a_bs, a_ks, M, P, p_rs, p_cs, K, N, cols_per_y, C, c_rb, \
                                                       c_bs, c_cs);                                                   \
   } while (0)
-  if (K <= 8) EPW_AXIS_LAUNCH(8, 2);
-  else if (K <= 16) EPW_AXIS_LAUNCH(16, 2);
+  if (K <= 8) EPW_AXIS_LAUNCH(8, 1);
+  else if (K <= 16) EPW_AXIS_LAUNCH(16, 1);
   else EPW_AXIS_LAUNCH(32, 1);
 #undef EPW_AXIS_LAUNCH
   return cudaGetLastError();
