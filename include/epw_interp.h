@@ -56,9 +56,9 @@ typedef struct {
   int32_t device;         /* CUDA device ordinal */
   int32_t q_batch;        /* q-points contracted per pass over g(Re,Rp) in S1 (1..8); 0 = library default */
   int32_t path;           /* EPW_PATH_AUTO (0): chosen from Nb, Nm; EPW_PATH_SMALL / EPW_PATH_LARGE force one (tests) */
-  int32_t flags;          /* 0: on a uniform grid the library chooses between the fused kernel (last axis pass of S2 + S4b,
-                             g~ never in HBM; chosen for Nb <= 8) and the two-kernel form (chosen for 9 <= Nb <= 16, where
-                             it measures faster); EPW_FLAG_GRID_UNFUSED / EPW_FLAG_GRID_FUSED force one of them */
+  int32_t flags;          /* 0 or EPW_FLAG_GRID_UNFUSED: on a uniform grid the last axis pass of S2 writes g~ and rotate_g2 reads
+                             it (two kernels; measured as fast as or faster than the alternative at every config);
+                             EPW_FLAG_GRID_FUSED: one kernel does the last axis pass and S4b, g~ never reaches HBM (Nb <= 16) */
   size_t workspace_bytes; /* cap on the library's scratch HBM; 0 = library chooses from free memory */
   double degen_tol;       /* informational (gap below which callers should sum |g|^2 over a subspace); unused inside */
   double omega_min;       /* modes with omega_q,nu <= omega_min give |g|^2 = 0 (acoustic modes at Gamma); default 0 */

@@ -684,9 +684,10 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   int cs = 0, nchunks = 1;   // i1 planes per k-chunk
   int KB1 = 0, NTc = 0;
   // grid mode: the last axis pass is fused with S4b (grid_rotate_g2.cu) unless the caller asked for the two-kernel form
-  // measured (bench.py --grid-unfused, configs[1..3]): the fused kernel wins for Nb = 8 (21.5 vs 22.2 ms, 128 vs 136 ms),
-  // the two-kernel form for Nb = 11 (22.9 vs 25.4 ms: 8-row DMMA tiles and mode groups fit Nb = 11 badly)
-  const bool want_fused = (h->cfg.flags & EPW_FLAG_GRID_FUSED) || (!(h->cfg.flags & EPW_FLAG_GRID_UNFUSED) && nb <= 8);
+  // measured (bench.py --grid-fused / --grid-unfused, configs[1..3]): with the streaming axis passes and the pipelined
+  // rotation kernel the two-kernel form is as fast as the fused kernel for Nb = 8 (21.27 vs 21.28 ms, 123.0 vs 125.4 ms)
+  // and faster for Nb = 11 (20.9 vs 25.4 ms), so it is the default; the fused kernel stays available by flag
+  const bool want_fused = (h->cfg.flags & EPW_FLAG_GRID_FUSED) != 0;
   const bool fused = grid && want_fused && grid_rotate_g2_supported(nb, nm, h->box_L[0]);
   const int ncolsC = fused ? ncols_h : ncols;   // columns of the [g~ | H(k+q)] buffer that reach HBM
   if (!grid) {

@@ -368,7 +368,7 @@ def run_gpu(epw, w, k_list, q_list, kq_map=None, q_batch=0, host_api=False, path
             return eps_k, eps_kq, om, g2
         if grid is not None:
             out = h.interpolate_grid(grid, dev(q_list), k_shift=shift, kq_map=None if kq_map is None else dev(kq_map))
-            fused = flags == 2 or (flags == 0 and w.nbnd <= 8)
+            fused = flags == 2
             want = "list" if path == 2 or w.nbnd > 16 else ("grid-fused" if fused else "grid")
             assert epw.epw_interp_last_plan(h.h)["k_mode"] == want
         else:
@@ -416,7 +416,7 @@ def test_grid_config0_both_kq_modes_and_host_api(epw):
     """configs[0] through epw_interp_interpolate_grid: all 4,096 pairs with kq_map, per-pair H(k+q), host buffers."""
     w = synth.make_config(0)
     ref = oracle.interpolate(w.H_R, w.D_R, w.g_full(), w.Re, w.w_e, w.Rp, w.w_p, w.k_list, w.q_list)
-    for flags in (0, 1):
+    for flags in (0, 2):
         assert_path_close(run_gpu(epw, w, w.k_list, w.q_list, w.kq_map, grid=w.k_grid, flags=flags), ref)
         assert_path_close(run_gpu(epw, w, w.k_list, w.q_list, None, grid=w.k_grid, flags=flags), ref)
     ql = w.q_list[:5] + [0.01, 0.02, 0.03]
@@ -439,7 +439,7 @@ def test_grid_reduced_shapes(epw, shape, flags):
     elif shape == "chunks":
         w = synth.make_custom("chunks", 4, 3, (1, 1, 1), 1.0, 0.1, 1.0, (11, 3, 4), ("random", 2, 3), seed=14)
         # three i1 planes (12 k each) of per-k workspace per chunk -> 4 chunks, ragged last
-        ws = (16 * 12 * ((16 * 3 if flags == 1 else 0) + 16 + 16 + 4) + 16) * 3 + 100
+        ws = (16 * 12 * ((16 * 3 if flags != 2 else 0) + 16 + 16 + 4) + 16) * 3 + 100
     elif shape == "modes-split":
         # Nb = 13, Nm = 12, L1 = 7: the fused kernel cannot hold all modes of a cell in shared memory -> mode groups
         w = synth.make_custom("modes", 13, 12, (3, 1, 0), 1.0, 0.1, 1.0, (10, 3, 1), ("random", 2, 2), seed=15)
@@ -474,7 +474,7 @@ def test_grid_shifted_and_sparse_lattice_list(epw):
               + np.array(shift)) / np.array(w.k_grid)
     ref = oracle.interpolate(Sub.H_R, Sub.D_R, g, Sub.Re, Sub.w_e, Sub.Rp, Sub.w_p, k_list, w.q_list)
     assert_path_close(run_gpu(epw, Sub, k_list, w.q_list, grid=w.k_grid, shift=shift), ref)
-    assert_path_close(run_gpu(epw, Sub, k_list, w.q_list, grid=w.k_grid, shift=shift, flags=1), ref)
+    assert_path_close(run_gpu(epw, Sub, k_list, w.q_list, grid=w.k_grid, shift=shift, flags=2), ref)
     # and the same k-points as a list through the dense contraction
     assert_path_close(run_gpu(epw, Sub, k_list, w.q_list), ref)
 
@@ -560,13 +560,14 @@ def test_errors_are_reported(epw):
 # ---------------------------------------------------------------------------------------------------------
 # full-size configurations, in the launch configuration bench.py times: sampled pairs against the oracle
 # ---------------------------------------------------------------------------------------------------------
-def check_sampled_pairs(epw, w, q_idx, k_idx, q_batch=0, grid=False):
+def check_sampled_pairs(epw, w, q_idx, k_idx, q_batch=0, grid=False, flags=0):
     """Run the library on ALL k of workload w and the q-points q_idx (one interpolate call, as bench.py does), then
     compare eps_k, omega_q, eps_kq and |g|^2 on the sampled (q, k) pairs with the oracle computed pair by pair."""
     g = w.g_full()
     ql = np.ascontiguousarray(w.q_list[q_idx])
     kq_map = None if w.kq_map is None else np.ascontiguousarray(w.kq_map[q_idx])
-    eps_k, eps_kq, om, g2 = run_gpu(epw, w, w.k_list, ql, kq_map, q_batch=q_batch, grid=w.k_grid if grid else None)
+    eps_k, eps_kq, om, g2 = run_gpu(epw, w, w.k_list, ql, kq_map, q_batch=q_batch, grid=w.k_grid if grid else None,
+                                    flags=flags)
     worst = 0.0
     for jq in range(len(q_idx)):
         e_ref, om_ref = oracle.phonon(w.D_R, w.Rp, w.w_p, ql[jq])
@@ -613,6 +614,9 @@ def test_grid_full_size_sampled(epw, cfg, q_idx):
                                  64 * slab if 64 * slab < w.nk else 0})  # i1-plane and chunk edges
     worst = check_sampled_pairs(epw, w, q_idx, k_idx, grid=True)
     print(f"config {cfg} full size (grid): worst |g|^2 deviation {worst:.3f} x tolerance")
+    if cfg == 1:   # and the fused kernel at full size
+        worst = check_sampled_pairs(epw, w, q_idx[:4], k_idx, grid=True, flags=2)
+        print(f"config {cfg} full size (grid, fused kernel): worst |g|^2 deviation {worst:.3f} x tolerance")
 
 
 def test_config2_full_size_sampled(epw):
@@ -740,6 +744,7 @@ def pick_window(eps_all, frac_lo=0.48, frac_hi=0.52, margin=1e-6):
 
 @pytest.mark.parametrize("mode", ["grid-fused", "grid-unfused", "list", "list-kqmap", "large"])
 def test_energy_window_screening(epw, mode):
+    fl = {"grid-fused": 2, "grid-unfused": 1}.get(mode, 0)
     if mode == "large":
         w = synth.make_custom("zsnr-w", 18, 5, (2, 0, 0), 1.0, 0.05, 2.0, (30, 1, 1), ("random", 3, 1), seed=61)
     else:
@@ -751,8 +756,7 @@ def test_energy_window_screening(epw, mode):
     mask_ref = oracle.window_mask(ref[0], ref[1], emin, emax)
     assert 0.02 < mask_ref.mean() < 0.95      # the window really screens, and really keeps
     g2_ref = ref[3] * mask_ref[:, :, None, None, None]
-    h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_, q_batch=4,
-                      flags=epw.EPW_FLAG_GRID_UNFUSED if mode == "grid-unfused" else 0)
+    h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_, q_batch=4, flags=fl)
     try:
         h.set_operators_from_host(w)
         mask_d = torch.full((len(ql), w.nk), 7, dtype=torch.uint8, device="cuda")
@@ -872,7 +876,7 @@ def test_selfenergy_consumer(epw, mode):
     want = oracle.selfenergy_accumulate(ref[3], ref[0], ref[1], ref[2], wq, mu, kT, sigma)
     want2 = oracle.selfenergy_accumulate(ref[3][:2], ref[0], ref[1][:2], ref[2][:2], None, mu, kT, sigma, out=want.copy())
     h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_, q_batch=4, path=2 if mode.startswith("large") else 0,
-                      flags=epw.EPW_FLAG_GRID_UNFUSED if mode == "grid-unfused" else 0)
+                      flags=2 if mode.startswith("grid-fused") else (1 if mode == "grid-unfused" else 0))
     try:
         h.set_operators_from_host(w)
         acc = torch.zeros((w.nk, w.nbnd), dtype=torch.float64, device="cuda")
