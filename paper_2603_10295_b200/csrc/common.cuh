@@ -70,25 +70,24 @@ cudaError_t launch_phase_pack_a(const double *x, int64_t nx, const int32_t *R, c
 cudaError_t launch_rp_to_q(const c128 *g, int64_t rows, int np, const c128 *Pq, int nq, c128 *g1, cudaStream_t st);
 cudaError_t launch_interp_operator(const c128 *OpR, int n, int nr, const c128 *P, int64_t nx, c128 *out,
                                    cudaStream_t st);
+// `work` (may be NULL): device word that accumulates the number of plane rotations executed (matrix-rotations), so that
+// the FP64 work of a solve can be stated (the sweep count is data dependent).
 cudaError_t launch_eigh_batched(const c128 *A, int64_t stride_a, int n, int64_t batch, double *evals, c128 *V,
-                                int sqrt_mode, int32_t *status, c128 *scratch_large, cudaStream_t st);
+                                int sqrt_mode, int32_t *status, c128 *scratch_large, unsigned long long *work,
+                                cudaStream_t st);
 size_t eigh_large_scratch_bytes(int n, int64_t batch);
 // same with an explicit kernel choice (EPW_EIGH_AUTO / _WARP / _THREAD / _COLS, include/epw_interp.h)
 cudaError_t launch_eigh_batched_algo(const c128 *A, int64_t stride_a, int n, int64_t batch, double *evals, c128 *V,
-                                     int sqrt_mode, int32_t *status, c128 *scratch_large, int algo, cudaStream_t st);
-// Optional work counter of the two register-resident solvers: a device word that accumulates the number of plane
-// rotations executed (matrix-rotations), so that their FP64 work can be stated (the sweep count is data dependent).
-// NULL (default) = not counted.  Process-wide; set by the handle while stage timing is on.
-void eigh_set_work_counter(unsigned long long *dev_counter);
-unsigned long long *eigh_work_counter();
+                                     int sqrt_mode, int32_t *status, c128 *scratch_large, int algo,
+                                     unsigned long long *work, cudaStream_t st);
 // column-pair one-sided solver (eigh_cols.cu), n in 9..16
 bool eigh_cols_supported(int n);
 cudaError_t launch_eigh_cols(const c128 *A, int64_t stride_a, int n, int64_t batch, double *evals, c128 *V,
-                             int sqrt_mode, int32_t *status, cudaStream_t st);
+                             int sqrt_mode, int32_t *status, unsigned long long *work, cudaStream_t st);
 // thread-per-matrix register-resident solver (eigh_thread.cu), n in 2..8
 bool eigh_thread_supported(int n);
 cudaError_t launch_eigh_thread(const c128 *A, int64_t stride_a, int n, int64_t batch, double *evals, c128 *V,
-                               int sqrt_mode, int32_t *status, cudaStream_t st);
+                               int sqrt_mode, int32_t *status, unsigned long long *work, cudaStream_t st);
 
 // Build the packed B' operand for one q:
 //   complex column c <  nm*nbb : sum_ka g1[ka][r][el] * e[ka + nm*nu] * amp[nu]     (c = nu*nbb + el)   (S4a hoisted)

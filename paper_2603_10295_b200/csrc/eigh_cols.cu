@@ -231,29 +231,29 @@ __global__ void __launch_bounds__(ColsCfg<NN>::THREADS, (NN <= 12 ? 2 : 1))
 
 template <int NN>
 static cudaError_t launch_cols_n(const c128 *A, int64_t stride_a, int64_t batch, double *evals, c128 *V, int sqrt_mode,
-                                 int32_t *status, cudaStream_t st) {
+                                 int32_t *status, unsigned long long *work, cudaStream_t st) {
   typedef ColsCfg<NN> Cfg;
   cudaError_t e = cudaFuncSetAttribute(eigh_cols_kernel<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
   if (e != cudaSuccess) return e;
   eigh_cols_kernel<NN><<<(unsigned)ceil_div(batch, 32), Cfg::THREADS, Cfg::SMEM, st>>>(A, stride_a, batch, evals, V,
-                                                                                      sqrt_mode, status, eigh_work_counter());
+                                                                                      sqrt_mode, status, work);
   return cudaGetLastError();
 }
 
 bool eigh_cols_supported(int n) { return n >= 9 && n <= 16; }
 
 cudaError_t launch_eigh_cols(const c128 *A, int64_t stride_a, int n, int64_t batch, double *evals, c128 *V,
-                             int sqrt_mode, int32_t *status, cudaStream_t st) {
+                             int sqrt_mode, int32_t *status, unsigned long long *work, cudaStream_t st) {
   if (batch <= 0) return cudaSuccess;
   switch (n) {
-    case 9: return launch_cols_n<9>(A, stride_a, batch, evals, V, sqrt_mode, status, st);
-    case 10: return launch_cols_n<10>(A, stride_a, batch, evals, V, sqrt_mode, status, st);
-    case 11: return launch_cols_n<11>(A, stride_a, batch, evals, V, sqrt_mode, status, st);
-    case 12: return launch_cols_n<12>(A, stride_a, batch, evals, V, sqrt_mode, status, st);
-    case 13: return launch_cols_n<13>(A, stride_a, batch, evals, V, sqrt_mode, status, st);
-    case 14: return launch_cols_n<14>(A, stride_a, batch, evals, V, sqrt_mode, status, st);
-    case 15: return launch_cols_n<15>(A, stride_a, batch, evals, V, sqrt_mode, status, st);
-    case 16: return launch_cols_n<16>(A, stride_a, batch, evals, V, sqrt_mode, status, st);
+    case 9: return launch_cols_n<9>(A, stride_a, batch, evals, V, sqrt_mode, status, work, st);
+    case 10: return launch_cols_n<10>(A, stride_a, batch, evals, V, sqrt_mode, status, work, st);
+    case 11: return launch_cols_n<11>(A, stride_a, batch, evals, V, sqrt_mode, status, work, st);
+    case 12: return launch_cols_n<12>(A, stride_a, batch, evals, V, sqrt_mode, status, work, st);
+    case 13: return launch_cols_n<13>(A, stride_a, batch, evals, V, sqrt_mode, status, work, st);
+    case 14: return launch_cols_n<14>(A, stride_a, batch, evals, V, sqrt_mode, status, work, st);
+    case 15: return launch_cols_n<15>(A, stride_a, batch, evals, V, sqrt_mode, status, work, st);
+    case 16: return launch_cols_n<16>(A, stride_a, batch, evals, V, sqrt_mode, status, work, st);
     default: return cudaErrorInvalidValue;
   }
 }

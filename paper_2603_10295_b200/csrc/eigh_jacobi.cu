@@ -607,27 +607,25 @@ size_t eigh_large_scratch_bytes(int n, int64_t batch) {
   return (size_t)eigh_large_grid(batch) * 2 * (size_t)n * n * sizeof(c128);
 }
 
-static unsigned long long *g_work_counter = nullptr;
-void eigh_set_work_counter(unsigned long long *dev_counter) { g_work_counter = dev_counter; }
-unsigned long long *eigh_work_counter() { return g_work_counter; }
-
 cudaError_t launch_eigh_batched(const c128 *A, int64_t stride_a, int n, int64_t batch, double *evals, c128 *V,
-                                int sqrt_mode, int32_t *status, c128 *scratch_large, cudaStream_t st) {
-  return launch_eigh_batched_algo(A, stride_a, n, batch, evals, V, sqrt_mode, status, scratch_large, EPW_EIGH_AUTO, st);
+                                int sqrt_mode, int32_t *status, c128 *scratch_large, unsigned long long *work,
+                                cudaStream_t st) {
+  return launch_eigh_batched_algo(A, stride_a, n, batch, evals, V, sqrt_mode, status, scratch_large, EPW_EIGH_AUTO, work, st);
 }
 
 // Kernel choice: the thread-per-matrix solver needs tens of thousands of matrices to fill the GPU (32 matrices per
 // 64-thread CTA) and is the throughput kernel of the per-pair H(k+q) solves; small batches (H(k) of a tiny grid, D(q)
 // of a q-batch) finish sooner on the warp-per-matrix kernel, which spreads one matrix over 32 lanes.
 cudaError_t launch_eigh_batched_algo(const c128 *A, int64_t stride_a, int n, int64_t batch, double *evals, c128 *V,
-                                     int sqrt_mode, int32_t *status, c128 *scratch_large, int algo, cudaStream_t st) {
+                                     int sqrt_mode, int32_t *status, c128 *scratch_large, int algo,
+                                     unsigned long long *work, cudaStream_t st) {
   if (batch <= 0) return cudaSuccess;
   if (algo == EPW_EIGH_THREAD && !eigh_thread_supported(n)) return cudaErrorInvalidValue;
   if (algo == EPW_EIGH_THREAD || (algo == EPW_EIGH_AUTO && eigh_thread_supported(n) && batch >= 2048))
-    return launch_eigh_thread(A, stride_a, n, batch, evals, V, sqrt_mode, status, st);
+    return launch_eigh_thread(A, stride_a, n, batch, evals, V, sqrt_mode, status, work, st);
   if (algo == EPW_EIGH_COLS && !eigh_cols_supported(n)) return cudaErrorInvalidValue;
   if (algo == EPW_EIGH_COLS || (algo == EPW_EIGH_AUTO && eigh_cols_supported(n) && batch >= 2048))
-    return launch_eigh_cols(A, stride_a, n, batch, evals, V, sqrt_mode, status, st);
+    return launch_eigh_cols(A, stride_a, n, batch, evals, V, sqrt_mode, status, work, st);
   if (n <= EIGH_SMALL_MAX_N) {
     const int ld = n | 1, half = (n + (n & 1)) >> 1;
     size_t per_warp = (size_t)(2 * ld * n) * sizeof(c128) + (size_t)half * sizeof(Rot) + (size_t)n * sizeof(double);

@@ -106,9 +106,9 @@ struct epw_interp {
   int64_t box_size = 1;
   DevBuf boxidx, X, T1, T2, Ptmp, P1raw, P2raw, P3raw, P1pack, P2pack, P3pack, klist_gen;
   DevBuf workctr;  // 3 x u64: plane rotations executed by the register-resident eigensolvers for H(k), H(k+q), D(q)
-  // route the eigensolver work counter to slot i (0 H(k), 1 H(k+q), 2 D(q)) while stage timing is on; -1 = off
-  void count_into(int slot) {
-    eigh_set_work_counter(timing && slot >= 0 && workctr.p ? workctr.as<unsigned long long>() + slot : nullptr);
+  // eigensolver work counter of slot i (0 H(k), 1 H(k+q), 2 D(q)) while stage timing is on, else NULL
+  unsigned long long *work_slot(int slot) const {
+    return timing && workctr.p ? workctr.as<unsigned long long>() + slot : nullptr;
   }
   int last_kmode = 0;
   int64_t last_eq_slot = 0;  // slot of the last q of the last call inside the e_q buffer (debug getter)
@@ -298,11 +298,9 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
   LAUNCH(h, launch_zgemm_dmma(h->Apack.as<double>(), h->BpackH.as<double>(), h->Hk.as<c128>(), nk, nbb, KBe, nbb,
                               h->num_sms, st),
          "zgemm H(k)");
-  h->count_into(0);
   LAUNCH(h, launch_eigh_batched(h->Hk.as<c128>(), nbb, nb, nk, eps_k, h->Uk.as<c128>(), 0, h->status.as<int32_t>(),
-                                h->eig_scratch.as<c128>(), st),
+                                h->eig_scratch.as<c128>(), h->work_slot(0), st),
          "eigh H(k)");
-  h->count_into(-1);
   LAUNCH(h, launch_pack_b_strided(h->Uk.as<c128>(), 1, nb, nbb, nk, 0, nullptr, 0.0, nb, nb, h->UpackK.as<double>(), st),
          "pack U_k");
   if (kq_map)
@@ -320,11 +318,9 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
   h->end_span(sp, st);
   sp = h->begin_span(2, st);
   LAUNCH(h, launch_interp_operator(h->D.as<c128>(), nm, np, h->Pq.as<c128>(), nq, h->Dq.as<c128>(), st), "D(q)");
-  h->count_into(2);
   LAUNCH(h, launch_eigh_batched(h->Dq.as<c128>(), nmm, nm, nq, omega_q, h->eq.as<c128>(), 1, h->status.as<int32_t>(),
-                                h->eig_scratch.as<c128>(), st),
+                                h->eig_scratch.as<c128>(), h->work_slot(2), st),
          "eigh D(q)");
-  h->count_into(-1);
   h->end_span(sp, st);
 
   for (int64_t q0 = 0; q0 < nq; q0 += QB) {
@@ -360,11 +356,9 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
                                     h->num_sms, st),
                "zgemm H(k+q)");
         double *eps_dst = eps_kq ? eps_kq + q * nk * nb : h->epskq_scratch.as<double>();
-        h->count_into(1);
         LAUNCH(h, launch_eigh_batched(h->Hkq.as<c128>(), nbb, nb, nk, eps_dst, h->Ukq.as<c128>(), 0,
-                                      h->status.as<int32_t>(), h->eig_scratch.as<c128>(), st),
+                                      h->status.as<int32_t>(), h->eig_scratch.as<c128>(), h->work_slot(1), st),
                "eigh H(k+q)");
-        h->count_into(-1);
         LAUNCH(h, launch_pack_b_strided(h->Ukq.as<c128>(), 1, nb, nbb, nk, 1, nullptr, 0.0, nb, nb,
                                         h->UpackKH.as<double>(), st),
                "pack conj U_{k+q}");
@@ -851,11 +845,9 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
     for (int ci = 0; ci < nchunks; ci++)
       LAUNCH(h, grid_pass_c(nbb, ci, h->Hk.as<c128>() + (int64_t)ci * kchunk * nbb), "grid pass H(k)");
   }
-  h->count_into(0);
   LAUNCH(h, launch_eigh_batched(h->Hk.as<c128>(), nbb, nb, nk, eps_k, h->Uk.as<c128>(), 0, h->status.as<int32_t>(),
-                                h->eig_scratch.as<c128>(), st),
+                                h->eig_scratch.as<c128>(), h->work_slot(0), st),
          "eigh H(k)");
-  h->count_into(-1);
   h->end_span(sp, st);
 
   // ---- q side (once per call): S0 phases of every q, D(q), phonon eigen-systems ----
@@ -868,11 +860,9 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   h->end_span(sp, st);
   sp = h->begin_span(2, st);
   LAUNCH(h, launch_interp_operator(h->D.as<c128>(), nm, np, h->Pq.as<c128>(), nq, h->Dq.as<c128>(), st), "D(q)");
-  h->count_into(2);
   LAUNCH(h, launch_eigh_batched(h->Dq.as<c128>(), nmm, nm, nq, omega_q, h->eq.as<c128>(), 1, h->status.as<int32_t>(),
-                                h->eig_scratch.as<c128>(), st),
+                                h->eig_scratch.as<c128>(), h->work_slot(2), st),
          "eigh D(q)");
-  h->count_into(-1);
   h->end_span(sp, st);
 
   for (int64_t q0 = 0; q0 < nq; q0 += QB) {
@@ -958,11 +948,9 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
           sp = h->begin_span(5, st);
           c128 *Ukq_c = h->Ukq.as<c128>() + crow * nbb;
           double *eps_dst = eps_kq ? eps_kq + (q * nk + k0) * nb : h->epskq_scratch.as<double>() + crow * nb;
-          h->count_into(1);
           LAUNCH(h, launch_eigh_batched(Cc + (ncolsC - ncols_h), ncolsC, nb, kn, eps_dst, Ukq_c, 0, h->status.as<int32_t>(),
-                                        h->eig_scratch.as<c128>(), st),
+                                        h->eig_scratch.as<c128>(), h->work_slot(1), st),
                  "eigh H(k+q)");
-          h->count_into(-1);
           h->end_span(sp, st);
           Ukq_ptr = Ukq_c;
         }
@@ -1279,7 +1267,7 @@ int epw_eigh_batched_algo(const void *A, int64_t stride_a, int32_t n, int64_t ba
   const size_t need = eigh_large_scratch_bytes(n, batch);
   if (need && cudaMalloc(&scratch, need) != cudaSuccess) return EPW_ENOMEM;
   const cudaError_t e = launch_eigh_batched_algo(reinterpret_cast<const c128 *>(A), stride_a, n, batch, evals,
-                                                 reinterpret_cast<c128 *>(V), sqrt_mode, status, scratch, algo, st);
+                                                 reinterpret_cast<c128 *>(V), sqrt_mode, status, scratch, algo, nullptr, st);
   if (scratch) {  // stage-level convenience path: wait so the scratch can be released
     cudaStreamSynchronize(st);
     cudaFree(scratch);
