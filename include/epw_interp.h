@@ -54,14 +54,17 @@ typedef struct {
   int32_t ne;             /* Ne: number of electron Wigner-Seitz vectors Re */
   int32_t np;             /* Np: number of phonon Wigner-Seitz vectors Rp */
   int32_t device;         /* CUDA device ordinal */
-  int32_t q_batch;        /* q-points contracted per pass over g(Re,Rp) in S1 (1..8); 0 = library default */
+  int32_t q_batch;        /* q-points contracted per pass over g(Re,Rp) in S1 (1..8); 0 = library default (8); lowered by the
+                             library when the [Np][q_batch] phase table would not fit shared memory (Np > 1,760 at 8);
+                             Np > 14,080 is EPW_EUNSUPPORTED */
   int32_t path;           /* EPW_PATH_AUTO (0): chosen from Nb, Nm; EPW_PATH_SMALL / EPW_PATH_LARGE force one (tests) */
   int32_t flags;          /* 0 or EPW_FLAG_GRID_UNFUSED: on a uniform grid the last axis pass of S2 writes g~ and rotate_g2 reads
                              it (two kernels; measured as fast as or faster than the alternative at every config);
                              EPW_FLAG_GRID_FUSED: one kernel does the last axis pass and S4b, g~ never reaches HBM (Nb <= 16) */
   size_t workspace_bytes; /* cap on the library's scratch HBM; 0 = library chooses from free memory */
   double degen_tol;       /* informational (gap below which callers should sum |g|^2 over a subspace); unused inside */
-  double omega_min;       /* modes with omega_q,nu <= omega_min give |g|^2 = 0 (acoustic modes at Gamma); default 0 */
+  double omega_min;       /* modes with omega_q,nu <= omega_min give |g|^2 = 0 (acoustic modes at Gamma); default 0;
+                             must be >= 0 (create fails with EPW_EINVAL otherwise: soft modes are reported with negative omega) */
 } epw_interp_config;
 
 /* Kernel families of the path.  SMALL: a whole (k,q) pair lives in shared memory (Nb <= 16, configs[0..3]).
@@ -185,7 +188,9 @@ int epw_interp_set_rp_shard(epw_interp_t h, int32_t ip_start, int32_t ip_count);
 int epw_interp_rp_to_q_partial(epw_interp_t h, const double *q_list, int64_t nq, void *g1_partial, void *cuda_stream);
 int epw_interp_set_gq(epw_interp_t h, const void *g1_reduced);
 
-/* Wait for the handle's last enqueued work and report deferred device-side status (EPW_ENOTCONVERGED, EPW_ECUDA). */
+/* Wait for the handle's last enqueued work and report deferred device-side status (EPW_ENOTCONVERGED, EPW_ECUDA).
+ * The convergence flag is sticky: it is set by any eigensolve of any call enqueued since the last epw_interp_sync and is
+ * read and cleared only here, so one sync after several asynchronous calls reports a failure in any of them. */
 int epw_interp_sync(epw_interp_t h);
 
 /*

@@ -63,7 +63,7 @@ cudaError_t launch_eq6_unrotate(const c128 *g, const c128 *Uk, const c128 *Ukq, 
   const int64_t total = nblocks * nb * nb * nm;
   if (total <= 0) return cudaSuccess;
   const int64_t want = ceil_div(total, 256);
-  const unsigned grid = (unsigned)(want < 148 * 32 ? want : 148 * 32);
+  const unsigned grid = grid_cap(want, 32);
   eq6_unrotate_kernel<<<grid, 256, 0, st>>>(0, g, Uk, Ukq, e, omega, nb, nm, nkc, nblocks, gt);
   eq6_unrotate_kernel<<<grid, 256, 0, st>>>(1, gt, Uk, Ukq, e, omega, nb, nm, nkc, nblocks, tmp);
   eq6_unrotate_kernel<<<grid, 256, 0, st>>>(2, tmp, Uk, Ukq, e, omega, nb, nm, nkc, nblocks, gt);

@@ -33,6 +33,23 @@ __device__ __forceinline__ double cabs2(c128 a) { return a.x * a.x + a.y * a.y; 
 static inline int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
 static inline int64_t round_up(int64_t a, int64_t b) { return ceil_div(a, b) * b; }
 
+// SM count of the CURRENT device (grid sizing of the streaming kernels); looked up once per device ordinal.
+static inline int device_sm_count() {
+  static int cache[64] = {0};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return 148;
+  if (dev >= 0 && dev < 64 && cache[dev] > 0) return cache[dev];
+  int n = 0;
+  if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) return 148;
+  if (dev >= 0 && dev < 64) cache[dev] = n;
+  return n;
+}
+// grid of a grid-stride kernel: `blocks` CTAs, at most `per_sm` per SM of the current device
+static inline unsigned grid_cap(int64_t blocks, int per_sm) {
+  const int64_t cap = (int64_t)device_sm_count() * per_sm;
+  return (unsigned)(blocks < cap ? blocks : cap);
+}
+
 // ---- DMMA GEMM operand packing (see zgemm_dmma.cu for the kernel and DESIGN.md "Data layout") -----------------
 // Real embedding of a complex contraction C = A B:
 //   A'[m][2r+a]     = (a ? Im : Re) A[m][r]
@@ -68,6 +85,7 @@ cudaError_t launch_phase_table(const double *x, int64_t nx, const int32_t *R, co
 cudaError_t launch_phase_pack_a(const double *x, int64_t nx, const int32_t *R, const double *w, int nr, double *Apack,
                                 cudaStream_t st);
 cudaError_t launch_rp_to_q(const c128 *g, int64_t rows, int np, const c128 *Pq, int nq, c128 *g1, cudaStream_t st);
+int rp_to_q_max_nq(int np);   // q-points per pass whose phase table fits shared memory (<= 8; 0 = unsupported Np)
 cudaError_t launch_interp_operator(const c128 *OpR, int n, int nr, const c128 *P, int64_t nx, c128 *out,
                                    cudaStream_t st);
 // `work` (may be NULL): device word that accumulates the number of plane rotations executed (matrix-rotations), so that

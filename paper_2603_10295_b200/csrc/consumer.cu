@@ -5,7 +5,7 @@
 // part of the Fan-Migdal self-energy with Gaussian-broadened energy conservation,
 //   Im Sigma_nk += pi w_q sum_{m,nu} |g_{mn nu}(k,q)|^2 [ (n_qnu + f_mk+q)     delta_s(e_nk - e_mk+q + w_qnu)
 //                                                      + (n_qnu + 1 - f_mk+q) delta_s(e_nk - e_mk+q - w_qnu) ],
-//   delta_s(x) = exp(-(x/s)^2)/(s sqrt(pi)),  n = 1/(exp(w/kT) - 1),  f = 1/(exp((e - mu)/kT) + 1),  modes with w <= 0 skipped.
+//   delta_s(x) = exp(-(x/s)^2)/(s sqrt(pi)),  n = 1/expm1(w/kT),  f = 1/(exp((e - mu)/kT) + 1),  modes with w <= 0 skipped.
 // One thread per (k, n); the sum over (nu, m) runs in a fixed order and q-points are accumulated in call order on one
 // stream, so the result is deterministic.  With the consumer on, the caller may pass g2 = NULL: the library then keeps
 // |g|^2 of one q at a time in its own scratch and nothing of size Nk Nq ever exists.
@@ -41,7 +41,7 @@ __global__ void __launch_bounds__(256)
         // realistic broadening are skipped without evaluating any exponential
         const bool ka = xa * xa < 50.0, ke = xe * xe < 50.0;
         if (!ka && !ke) continue;
-        if (bose < 0.0) bose = 1.0 / (exp(w / kT) - 1.0);
+        if (bose < 0.0) bose = 1.0 / expm1(w / kT);   // expm1: no cancellation when w << kT
         const double f = 1.0 / (exp((em - mu) / kT) + 1.0);
         const double da = ka ? exp(-xa * xa) : 0.0, de = ke ? exp(-xe * xe) : 0.0;
         s += row[m] * ((bose + f) * da + (bose + 1.0 - f) * de);
@@ -57,7 +57,7 @@ cudaError_t launch_selfenergy_accumulate(const double *g2q, const double *eps_k,
                                          int64_t nk, double *out, cudaStream_t st) {
   if (nk <= 0) return cudaSuccess;
   const int64_t blocks = ceil_div(nk * nb, 256);
-  selfenergy_accumulate_kernel<<<(unsigned)(blocks < 148 * 16 ? blocks : 148 * 16), 256, 0, st>>>(
+  selfenergy_accumulate_kernel<<<grid_cap(blocks, 16), 256, 0, st>>>(
       g2q, eps_k, eps_kq, eps_k_all, kq_idx, omega_q, w_q, iq, mu, kT, sigma, nb, nm, nk, out);
   return cudaGetLastError();
 }

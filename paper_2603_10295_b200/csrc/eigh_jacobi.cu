@@ -589,7 +589,7 @@ static int eigh_cluster_plan(int n, int64_t batch, int *nr_out, size_t *smem_out
                         sizeof(RotB) * (size_t)half;
     if (smem > (size_t)220 * 1024) continue;
     if (best == 0) best = cs;                      // smallest cluster that fits: best throughput for large batches
-    if (batch * cs <= 148) best = cs;              // few matrices: spread each one over more SMs
+    if (batch * cs <= device_sm_count()) best = cs;              // few matrices: spread each one over more SMs
   }
   if (best) {
     const int nr = (n + best - 1) / best, hp = (half + best - 1) / best;
@@ -600,7 +600,10 @@ static int eigh_cluster_plan(int n, int64_t batch, int *nr_out, size_t *smem_out
   return best;
 }
 
-static int eigh_large_grid(int64_t batch) { return (int)(batch < 148 ? batch : 148); }
+static int eigh_large_grid(int64_t batch) {
+  const int nsm = device_sm_count();
+  return (int)(batch < nsm ? batch : nsm);
+}
 
 size_t eigh_large_scratch_bytes(int n, int64_t batch) {
   if (n <= EIGH_SMALL_MAX_N) return 0;

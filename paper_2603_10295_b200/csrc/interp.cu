@@ -8,6 +8,7 @@
 #include <algorithm>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -79,7 +80,7 @@ struct epw_interp {
   epw_interp_config cfg{};
   int nb = 0, nm = 0, ne = 0, np = 0, nbb = 0, nmm = 0;
   int64_t rows = 0;  // Nb^2 Ne Nm = rows of Fig. 13's A(m,n)
-  int num_sms = 148;
+  int num_sms = 0;   // set by epw_interp_create from the device
   int q_batch = 4;
   bool operators_set = false;
   std::vector<char> slab_set;
@@ -156,6 +157,23 @@ struct epw_interp {
     last_error = msg;
     return code;
   }
+  // q-points per pass of S1: the configured batch, clamped so that the [Np][QB] phase table fits shared memory
+  int s1_batch(int64_t nq, int *qb_out) {
+    const int fit = rp_to_q_max_nq(np);
+    if (fit == 0)
+      return fail(EPW_EUNSUPPORTED, "Np = " + std::to_string(np) + " lattice vectors: the phase table of one q-point "
+                                    "exceeds the shared memory of an SM (S1 supports Np <= 14080)");
+    *qb_out = (int)std::min<int64_t>(std::min(q_batch, fit), nq);
+    return EPW_OK;
+  }
+  // The convergence flag is STICKY: every eigensolve of every enqueued call may set it, only epw_interp_sync reads and
+  // clears it, so a caller that enqueues several calls before one sync still learns of a failure in any of them.
+  int ensure_status() {
+    if (status.p) return EPW_OK;
+    cudaError_t e = status.reserve(sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMemset(status.p, 0, sizeof(int32_t));
+    return e == cudaSuccess ? EPW_OK : cuda_fail(e, "cudaMalloc status");
+  }
   int cuda_fail(cudaError_t e, const char *where) {
     last_error = std::string(where) + ": " + cudaGetErrorString(e);
     return e == cudaErrorMemoryAllocation ? EPW_ENOMEM : EPW_ECUDA;
@@ -228,7 +246,8 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
   const int64_t upack = (int64_t)NTb * KBb * GEMM_CHUNK;  // doubles of one packed Nb x Nb operand
 
   // q per pass over g(Re,Rp): g(Re,q) is 16 Nb^2 Nm Ne bytes per q here (2.9 GB for configs[4]); keep the batch <= 8 GB
-  int QB = (int)std::min<int64_t>(h->q_batch, nq);
+  int QB = 1;
+  { const int rc = h->s1_batch(nq, &QB); if (rc != EPW_OK) return rc; }
   {
     const size_t per_q = sizeof(c128) * (size_t)h->rows;
     QB = (int)std::max<int64_t>(1, std::min<int64_t>(QB, (int64_t)(((size_t)8 << 30) / per_q)));
@@ -264,13 +283,12 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
     CU_OR_FAIL(h, h->Ukq.reserve(sizeof(c128) * (size_t)nk * nbb), "cudaMalloc Ukq");
     if (!eps_kq) CU_OR_FAIL(h, h->epskq_scratch.reserve(sizeof(double) * (size_t)nk * nb), "cudaMalloc eps scratch");
   }
-  CU_OR_FAIL(h, h->status.reserve(sizeof(int32_t)), "cudaMalloc status");
+  { const int rc = h->ensure_status(); if (rc != EPW_OK) return rc; }
   if (h->window_on && !h->mask_out) CU_OR_FAIL(h, h->maskbuf.reserve((size_t)nk), "cudaMalloc mask");
   {
     const size_t need = std::max(eigh_large_scratch_bytes(nb, nk), eigh_large_scratch_bytes(nm, nq));
     if (need) CU_OR_FAIL(h, h->eig_scratch.reserve(need), "cudaMalloc eig scratch");
   }
-  CU_OR_FAIL(h, cudaMemsetAsync(h->status.p, 0, sizeof(int32_t), st), "memset status");
   h->last_nk = nk;
   h->last_c_rows = kc;
   h->last_ncols = (int)E;
@@ -366,7 +384,7 @@ static int interpolate_large(epw_interp *h, const double *k_list, int64_t nk, co
       } else if (eps_kq) {
         sp = h->begin_span(5, st);
         h->launches++;
-        gather_eps_kernel<<<(unsigned)std::min<int64_t>(ceil_div(nk * nb, 256), 148 * 8), 256, 0, st>>>(
+        gather_eps_kernel<<<grid_cap(ceil_div(nk * nb, 256), 8), 256, 0, st>>>(
             eps_k, kq_map + q * nk, nb, nk, eps_kq + q * nk * nb);
         CU_OR_FAIL(h, cudaGetLastError(), "gather_eps");
         h->end_span(sp, st);
@@ -445,6 +463,10 @@ int epw_interp_create(epw_interp_t *out, const epw_interp_config *cfg) {
     g_create_error = "epw_interp_create: unknown bit in flags";
     return EPW_EINVAL;
   }
+  if (!(cfg->omega_min >= 0.0)) {   // also rejects NaN
+    g_create_error = "epw_interp_create: omega_min must be >= 0 (a negative cut-off would let soft modes into 1/sqrt(2 omega))";
+    return EPW_EINVAL;
+  }
   if (cfg->q_batch < 0 || cfg->q_batch > 8) {
     g_create_error = "epw_interp_create: q_batch must be in 0..8";
     return EPW_EINVAL;
@@ -486,7 +508,7 @@ int epw_interp_create(epw_interp_t *out, const epw_interp_config *cfg) {
 void epw_interp_destroy(epw_interp_t h) {
   if (!h) return;
   cudaSetDevice(h->cfg.device);
-  if (h->last_stream || true) cudaDeviceSynchronize();
+  cudaDeviceSynchronize();   // kernels of this handle may still be reading its buffers
   DevBuf *all[] = {&h->g, &h->H, &h->D, &h->Re, &h->Rp, &h->we, &h->wp, &h->ones, &h->Apack, &h->BpackH, &h->Hk,
                    &h->Uk, &h->Pq, &h->Pqe, &h->Dq, &h->eq, &h->g1, &h->Bpack, &h->C, &h->Ukq, &h->epskq_scratch,
                    &h->status, &h->eig_scratch, &h->hs_k, &h->hs_q, &h->hs_map, &h->hs_epsk, &h->hs_epskq,
@@ -662,7 +684,8 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   const int NT = (int)ceil_div(2 * (int64_t)ncols, GEMM_BN);
   const int NTH = (int)ceil_div(2 * (int64_t)nbb, GEMM_BN);
   const int64_t MT = ceil_div(nk, GEMM_BM);
-  const int QB = (int)std::min<int64_t>(h->q_batch, nq);
+  int QB = 1;
+  { const int rc = h->s1_batch(nq, &QB); if (rc != EPW_OK) return rc; }
   const int64_t E = (int64_t)ncols_g;
   const size_t cap = h->cfg.workspace_bytes ? h->cfg.workspace_bytes : ((size_t)6 << 30);
   // |g|^2 of pair (q, k0..): the caller's buffer, or (consumer on, g2 = NULL) the library's one-q scratch
@@ -750,13 +773,12 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   if (ncolsC) CU_OR_FAIL(h, h->C.reserve(sizeof(c128) * (size_t)c_rows * ncolsC), "cudaMalloc g~");
   if (!kq_map) CU_OR_FAIL(h, h->Ukq.reserve(sizeof(c128) * (size_t)c_rows * nbb), "cudaMalloc Ukq");
   if (!kq_map && !eps_kq) CU_OR_FAIL(h, h->epskq_scratch.reserve(sizeof(double) * (size_t)c_rows * nb), "cudaMalloc eps scratch");
-  CU_OR_FAIL(h, h->status.reserve(sizeof(int32_t)), "cudaMalloc status");
+  { const int rc = h->ensure_status(); if (rc != EPW_OK) return rc; }
   if (h->window_on && !h->mask_out) CU_OR_FAIL(h, h->maskbuf.reserve((size_t)nk), "cudaMalloc mask");
   {
     const size_t need = std::max(eigh_large_scratch_bytes(nb, nk), eigh_large_scratch_bytes(nm, nq));
     if (need) CU_OR_FAIL(h, h->eig_scratch.reserve(need), "cudaMalloc eig scratch");
   }
-  CU_OR_FAIL(h, cudaMemsetAsync(h->status.p, 0, sizeof(int32_t), st), "memset status");
   h->last_nk = nk;
   h->last_c_rows = c_rows;
   h->last_ncols = ncolsC;
@@ -938,7 +960,7 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
           if (eps_kq) {
             sp = h->begin_span(5, st);
             h->launches++;
-            gather_eps_kernel<<<(unsigned)std::min<int64_t>(ceil_div(kn * nb, 256), 148 * 8), 256, 0, st>>>(
+            gather_eps_kernel<<<grid_cap(ceil_div(kn * nb, 256), 8), 256, 0, st>>>(
                 eps_k, kq_idx, nb, kn, eps_kq + (q * nk + k0) * nb);
             CU_OR_FAIL(h, cudaGetLastError(), "gather_eps");
             h->end_span(sp, st);
@@ -1043,7 +1065,8 @@ int epw_interp_rp_to_q_partial(epw_interp_t h, const double *q_list, int64_t nq,
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
   h->last_stream = st;
   h->launches = 0;
-  const int QB = (int)std::min<int64_t>(h->q_batch, nq);
+  int QB = 1;
+  { const int rc = h->s1_batch(nq, &QB); if (rc != EPW_OK) return rc; }
   CU_OR_FAIL(h, h->Pq.reserve(sizeof(c128) * (size_t)QB * h->np), "cudaMalloc Pq");
   c128 *out = reinterpret_cast<c128 *>(g1_partial);
   for (int64_t q0 = 0; q0 < nq; q0 += QB) {
@@ -1075,7 +1098,11 @@ int epw_interp_sync(epw_interp_t h) {
   if (h->status.p) {
     int32_t s = 0;
     CU_OR_FAIL(h, cudaMemcpy(&s, h->status.p, sizeof(s), cudaMemcpyDeviceToHost), "cudaMemcpy status");
-    if (s) return h->fail(EPW_ENOTCONVERGED, "a Jacobi eigensolve did not converge within the sweep limit");
+    if (s) {
+      CU_OR_FAIL(h, cudaMemset(h->status.p, 0, sizeof(int32_t)), "memset status");   // read once, then cleared
+      return h->fail(EPW_ENOTCONVERGED, "a Jacobi eigensolve did not converge within the sweep limit (in this or an "
+                                        "earlier call since the last epw_interp_sync)");
+    }
   }
   return EPW_OK;
 }
@@ -1230,7 +1257,11 @@ int64_t epw_interp_debug_get(epw_interp_t h, int what, void *dst, size_t bytes) 
 // ---------------------------------------------------------------------------------------------------------
 // stage-level entry points
 // ---------------------------------------------------------------------------------------------------------
-static int rc_of(cudaError_t e) { return e == cudaSuccess ? EPW_OK : (e == cudaErrorInvalidValue ? EPW_EINVAL : EPW_ECUDA); }
+static int rc_of(cudaError_t e) {
+  if (e == cudaSuccess) return EPW_OK;
+  if (e == cudaErrorInvalidValue) return EPW_EINVAL;
+  return e == cudaErrorInvalidConfiguration ? EPW_EUNSUPPORTED : EPW_ECUDA;   // a launcher refused the shape
+}
 
 int epw_phase_table(const double *x_list, int64_t nx, const int32_t *R, const double *w, int32_t nr, void *P_out,
                     void *cuda_stream) {
@@ -1278,9 +1309,7 @@ int epw_eigh_batched_algo(const void *A, int64_t stride_a, int32_t n, int64_t ba
 int epw_zgemm(const void *A, const void *B, void *C, int64_t M, int32_t N, int32_t K, int64_t ldc, void *cuda_stream) {
   if (!A || !B || !C || M <= 0 || N <= 0 || K <= 0 || ldc < N) return EPW_EINVAL;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
-  int dev = 0, nsm = 148;
-  cudaGetDevice(&dev);
-  cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  const int nsm = device_sm_count();
   const int KB = (int)ceil_div(2 * (int64_t)K, GEMM_BK);
   const int NT = (int)ceil_div(2 * (int64_t)N, GEMM_BN);
   const int64_t MT = ceil_div(M, GEMM_BM);
@@ -1306,9 +1335,7 @@ int epw_zgemm_strided(const void *A, int64_t a_rb, int64_t a_bs, int64_t a_ks, i
   if (!A || !B || !C || M <= 0 || N <= 0 || K <= 0 || batch <= 0 || a_rb <= 0 || c_rb <= 0 || nb_mats <= 0)
     return EPW_EINVAL;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
-  int dev = 0, nsm = 148;
-  cudaGetDevice(&dev);
-  cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  const int nsm = device_sm_count();
   const int KB = (int)ceil_div(2 * (int64_t)K, GEMM_BK);
   const int NT = (int)ceil_div(2 * (int64_t)N, GEMM_BN);
   double *Bp = nullptr;
@@ -1369,9 +1396,7 @@ int epw_wannier_from_bloch(const void *gt, const double *kc, int64_t nkc, const 
     return EPW_EINVAL;
   if (nkc > 2147483647LL / 2 || nqc > 2147483647LL / 2) return EPW_EINVAL;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
-  int dev = 0, nsm = 148;
-  cudaGetDevice(&dev);
-  cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  const int nsm = device_sm_count();
   const size_t rows = (size_t)nb * nb * nm * ne;
   const size_t packK = (size_t)ceil_div(2 * (int64_t)ne, GEMM_BN) * ceil_div(2 * nkc, GEMM_BK) * GEMM_CHUNK;
   const size_t packQ = (size_t)ceil_div(2 * (int64_t)np, GEMM_BN) * ceil_div(2 * nqc, GEMM_BK) * GEMM_CHUNK;
@@ -1382,11 +1407,14 @@ int epw_wannier_from_bloch(const void *gt, const double *kc, int64_t nkc, const 
                        al(sizeof(int32_t) * nqc), al(sizeof(c128) * nqc * rows)};
   size_t total = 0;
   for (size_t b : sz) total += b;
-  // grow-only workspace kept between calls (cudaMalloc + cudaFree of ~1 GB cost more than the two contractions);
-  // like every stage-level entry point this call is not thread-safe
-  static DevBuf cache;
-  static int cache_dev = -1;
-  if (cache_dev != dev) { cache.release(); cache_dev = dev; }
+  // grow-only workspace kept between calls, one per device (cudaMalloc + cudaFree of ~1 GB cost more than the two
+  // contractions); concurrent callers are serialised by the lock, which is held until the stream has drained
+  static std::mutex cache_mu;
+  static DevBuf cache_of[64];
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return EPW_ECUDA;
+  std::lock_guard<std::mutex> lock(cache_mu);
+  DevBuf &cache = cache_of[dev];
   if (cache.reserve(total) != cudaSuccess) return EPW_ENOMEM;
   char *ws = cache.as<char>();
   char *p[8];

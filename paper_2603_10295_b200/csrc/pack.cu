@@ -30,7 +30,7 @@ cudaError_t launch_interp_operator(const c128 *OpR, int n, int nr, const c128 *P
   if (nx <= 0) return cudaSuccess;
   const int64_t total = nx * n * n;
   const int64_t blocks = ceil_div(total, 256);
-  interp_operator_kernel<<<(unsigned)(blocks < 148 * 32 ? blocks : 148 * 32), 256, 0, st>>>(OpR, n * n, nr, P, nx, out);
+  interp_operator_kernel<<<grid_cap(blocks, 32), 256, 0, st>>>(OpR, n * n, nr, P, nx, out);
   return cudaGetLastError();
 }
 

@@ -69,7 +69,7 @@ cudaError_t launch_phase_table(const double *x, int64_t nx, const int32_t *R, co
                                cudaStream_t st) {
   if (nx <= 0 || nr <= 0) return cudaSuccess;
   const int64_t total = nx * nr;
-  const int grid = (int)(ceil_div(total, 256) < 148 * 16 ? ceil_div(total, 256) : 148 * 16);
+  const int grid = grid_cap(ceil_div(total, 256), 16);
   phase_table_kernel<<<grid, 256, 0, st>>>(x, nx, R, w, nr, P);
   return cudaGetLastError();
 }

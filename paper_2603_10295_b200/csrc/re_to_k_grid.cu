@@ -65,7 +65,7 @@ cudaError_t launch_box_scatter(const c128 *g1, const c128 *e, const double *omeg
     if (e0 != cudaSuccess) return e0;
   }
   const int64_t blocks = ceil_div((int64_t)ne * ncols, 256);
-  box_scatter_kernel<<<(unsigned)(blocks < 148 * 16 ? blocks : 148 * 16), 256, 0, st>>>(
+  box_scatter_kernel<<<grid_cap(blocks, 16), 256, 0, st>>>(
       g1, e, omega, omega_min, H_R, phase_qe, w_e, box_idx, nbb, nm, ne, ncols_g, ncols_h, X);
   return cudaGetLastError();
 }
@@ -110,7 +110,7 @@ __global__ void __launch_bounds__(256) grid_klist_kernel(int N1, int N2, int N3,
 cudaError_t launch_grid_klist(const int32_t N[3], const double s[3], double *k_list, cudaStream_t st) {
   const int64_t nk = (int64_t)N[0] * N[1] * N[2];
   const int64_t blocks = ceil_div(nk, 256);
-  grid_klist_kernel<<<(unsigned)(blocks < 148 * 8 ? blocks : 148 * 8), 256, 0, st>>>(N[0], N[1], N[2], s[0], s[1], s[2],
+  grid_klist_kernel<<<grid_cap(blocks, 8), 256, 0, st>>>(N[0], N[1], N[2], s[0], s[1], s[2],
                                                                                     k_list);
   return cudaGetLastError();
 }

@@ -171,8 +171,8 @@ static cudaError_t launch_rot(const c128 *gt, int64_t stride_gt, const c128 *Uk,
     if (e != cudaSuccess) return e;
   }
   const int64_t want = ceil_div(nk, PPC);
-  const int64_t grid = want < 148 * 16 ? want : 148 * 16;
-  rotate_g2_dmma_kernel<NB, WPP><<<(unsigned)grid, ROT_THREADS, smem, st>>>(gt, stride_gt, Uk, Ukq, kq_idx, nm, nk, mask, g2);
+  const unsigned grid = grid_cap(want, 16);
+  rotate_g2_dmma_kernel<NB, WPP><<<grid, ROT_THREADS, smem, st>>>(gt, stride_gt, Uk, Ukq, kq_idx, nm, nk, mask, g2);
   return cudaGetLastError();
 }
 

@@ -164,9 +164,7 @@ static cudaError_t launch_nq(const c128 *g, int64_t rows, int np, const c128 *Pq
 
 template <int NQ>
 static cudaError_t launch_nq_tma(const c128 *g, int64_t rows, int np, const c128 *Pq, c128 *g1, cudaStream_t st) {
-  int dev = 0, nsm = 148;
-  cudaGetDevice(&dev);
-  cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  const int nsm = device_sm_count();
   // row-tile height: the multiple of 32 in [256, 512] whose tile count fills whole waves best
   int RB = RP_MAX_RB;
   double best = -1.0;
@@ -197,7 +195,17 @@ static cudaError_t launch_nq(const c128 *g, int64_t rows, int np, const c128 *Pq
   return cudaGetLastError();
 }
 
+// The kernels keep the phase table [np][NQ] of a pass in shared memory (16 np NQ bytes): the largest NQ <= 8 that fits
+// the 227 KB a CTA may use, 0 if not even one q-point fits (Np > ~14,000).
+int rp_to_q_max_nq(int np) {
+  const size_t limit = (size_t)220 * 1024;
+  for (int nq = 8; nq >= 1; nq--)
+    if (sizeof(double2) * (size_t)np * nq <= limit) return nq;
+  return 0;
+}
+
 cudaError_t launch_rp_to_q(const c128 *g, int64_t rows, int np, const c128 *Pq, int nq, c128 *g1, cudaStream_t st) {
+  if (nq > rp_to_q_max_nq(np)) return cudaErrorInvalidConfiguration;
   switch (nq) {
     case 1: return launch_nq<1>(g, rows, np, Pq, g1, st);
     case 2: return launch_nq<2>(g, rows, np, Pq, g1, st);

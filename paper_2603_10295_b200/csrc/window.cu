@@ -27,7 +27,7 @@ cudaError_t launch_window_mask(const double *eps_k, const double *eps_kq, const 
                                int nb, int64_t nk, double emin, double emax, uint8_t *mask, cudaStream_t st) {
   if (nk <= 0) return cudaSuccess;
   const int64_t blocks = ceil_div(nk, 256);
-  window_mask_kernel<<<(unsigned)(blocks < 148 * 8 ? blocks : 148 * 8), 256, 0, st>>>(eps_k, eps_kq, eps_k_all, kq_idx, nb, nk,
+  window_mask_kernel<<<grid_cap(blocks, 8), 256, 0, st>>>(eps_k, eps_kq, eps_k_all, kq_idx, nb, nk,
                                                                                    emin, emax, mask);
   return cudaGetLastError();
 }
@@ -43,7 +43,7 @@ __global__ void __launch_bounds__(256)
 
 cudaError_t launch_zero_masked(const uint8_t *mask, int64_t nk, int64_t E, double *g2, cudaStream_t st) {
   if (nk <= 0) return cudaSuccess;
-  zero_masked_kernel<<<(unsigned)(nk < 148 * 16 ? nk : 148 * 16), 256, 0, st>>>(mask, nk, E, g2);
+  zero_masked_kernel<<<grid_cap(nk, 16), 256, 0, st>>>(mask, nk, E, g2);
   return cudaGetLastError();
 }
 

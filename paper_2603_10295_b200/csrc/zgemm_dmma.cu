@@ -131,12 +131,11 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1)
 cudaError_t launch_zgemm_dmma(const double *Apack, const double *Bpack, c128 *C, int64_t M, int N, int KB, int64_t ldc,
                               int num_sms, cudaStream_t st) {
   if (M <= 0 || N <= 0 || KB <= 0) return cudaSuccess;
-  static bool attr_set = false;
-  if (!attr_set) {
+  // the shared-memory opt-in is a per-device attribute: set it on every launch (cheap) instead of caching it per process
+  {
     cudaError_t e = cudaFuncSetAttribute(zgemm_dmma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)GEMM_SMEM_BYTES);
     if (e != cudaSuccess) return e;
-    attr_set = true;
   }
   const int NT = (int)ceil_div(2 * (int64_t)N, GEMM_BN);
   const int64_t MT = ceil_div(M, GEMM_BM);

@@ -184,12 +184,11 @@ cudaError_t launch_zgemm_strided(const c128 *A, int64_t a_rb, int64_t a_bs, int6
                                  int64_t batch, int num_sms, cudaStream_t st) {
   if (M <= 0 || N <= 0 || K <= 0 || batch <= 0) return cudaSuccess;
   if (a_rb <= 0 || c_rb <= 0) return cudaErrorInvalidValue;
-  static bool attr_set = false;
-  if (!attr_set) {
+  // the shared-memory opt-in is a per-device attribute: set it on every launch (cheap) instead of caching it per process
+  {
     cudaError_t e = cudaFuncSetAttribute(zgemm_strided_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)SA_SMEM_BYTES);
     if (e != cudaSuccess) return e;
-    attr_set = true;
   }
   StridedGemmParams p;
   p.A = A; p.a_rb = a_rb; p.a_bs = a_bs; p.a_ks = a_ks; p.a_batch = a_batch;

@@ -65,3 +65,15 @@ def test_no_cpu_fallback():
     for f in os.listdir(os.path.join(ROOT, "paper_2603_10295_b200", "csrc")):
         assert "oracle" not in open(os.path.join(ROOT, "paper_2603_10295_b200", "csrc", f)).read().replace(
             "Nothing in here is used by oracle/", "")
+
+
+def test_create_rejects_a_negative_or_nan_omega_min():
+    """Argument validation happens before the device is touched, so it is checkable on a CPU box: a negative cut-off
+    would let soft modes (reported with negative omega) into 1/sqrt(2 omega)."""
+    import paper_2603_10295_b200 as epw
+
+    for bad in (-1e-3, float("nan")):
+        with pytest.raises(epw.EpwError) as e:
+            epw.epw_interp_create(8, 6, 27, 27, omega_min=bad)
+        assert e.value.code == epw.binding.EPW_EINVAL
+        assert "omega_min" in str(e.value)

@@ -934,3 +934,59 @@ def test_nearly_degenerate_bands(epw, route, delta):
     assert np.abs(gaps - delta).min() < 1e-9            # the splitting is really there
     kw = dict(grid=base.k_grid) if route == "grid" else {}
     assert_path_close(run_gpu(epw, w, base.k_list, base.q_list, **kw), ref)
+
+
+def test_many_lattice_vectors_clamp_the_s1_batch(epw):
+    """Np = 2,197 (a 13^3 Wigner-Seitz box): the [Np][8] phase table of the default S1 batch does not fit shared memory,
+    so the library lowers the batch (6 q per pass here) instead of failing; 9 q = one full and one ragged pass."""
+    w = synth.make_custom("many-R", 1, 1, (6, 6, 6), 2.0, 0.1, 2.0, (2, 3, 1), ("random", 9, 3), seed=41)
+    assert w.np_ == 2197
+    ref = oracle.interpolate(w.H_R, w.D_R, w.g_full(), w.Re, w.w_e, w.Rp, w.w_p, w.k_list, w.q_list)
+    h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_)
+    try:
+        h.set_operators_from_host(w)
+        out = h.interpolate(dev(w.k_list), dev(w.q_list))
+        epw.epw_interp_sync(h.h)
+        assert epw.epw_interp_last_plan(h.h)["q_batch"] == 6
+        assert_path_close([t.cpu().numpy() for t in out], ref)
+        out = h.interpolate_grid(w.k_grid, dev(w.q_list))
+        epw.epw_interp_sync(h.h)
+        assert_path_close([t.cpu().numpy() for t in out], ref)
+    finally:
+        h.close()
+
+
+def test_two_handles_from_two_threads_count_their_own_rotations(epw):
+    """include/epw_interp.h: distinct handles are independent.  Two handles with stage timing on, driven from two host
+    threads on two streams at the same time, must report the rotation counts (and results) of their serial runs."""
+    import threading
+
+    ws = [synth.make_custom("si-a", 8, 6, (1, 1, 1), 1.5, 0.1, 1.5, (12, 12, 16), ("random", 3, 3), seed=51),
+          synth.make_custom("si-b", 6, 3, (1, 1, 1), 1.0, 0.1, 1.0, (16, 12, 12), ("random", 2, 3), seed=52)]
+
+    def run(w, stream, out):
+        with torch.cuda.stream(stream):
+            h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_)
+            try:
+                h.set_operators_from_host(w)
+                epw.epw_interp_enable_stage_timing(h.h, True)
+                for _ in range(3):
+                    res = h.interpolate_grid(w.k_grid, dev(w.q_list))
+                epw.epw_interp_sync(h.h)
+                out["rot"] = epw.epw_interp_get_eigh_rotations(h.h)
+                out["g2"] = res[3].cpu().numpy()
+            finally:
+                h.close()
+
+    serial = [dict(), dict()]
+    for w, o in zip(ws, serial):
+        run(w, torch.cuda.Stream(), o)
+    par = [dict(), dict()]
+    th = [threading.Thread(target=run, args=(w, torch.cuda.Stream(), o)) for w, o in zip(ws, par)]
+    for t in th:
+        t.start()
+    for t in th:
+        t.join()
+    for s, p in zip(serial, par):
+        assert s["rot"]["Hkq"] > 0 and s["rot"] == p["rot"]
+        assert np.array_equal(s["g2"], p["g2"])
