@@ -145,6 +145,11 @@ cudaError_t launch_box_scatter(const c128 *g1, const c128 *e, const double *omeg
 cudaError_t launch_grid_axis_phase(int N, int i0, int cnt, double shift, int lo, int L, c128 *P, cudaStream_t st);
 // last axis pass of the grid form fused with S4b and |g|^2 (grid_rotate_g2.cu)
 bool grid_rotate_g2_supported(int nb, int nm, int L1);
+// the same on the FP64 tensor path throughout (grid_fused.cu): pass as a DMMA product over quads of i1, then S4b
+bool grid_fused_supported(int nb, int nm, int L1);
+cudaError_t launch_grid_fused(const c128 *T2, int64_t slab, int ncols, int L1, const c128 *P1c, int cnt, const c128 *Uk,
+                              const c128 *Ukq, const int32_t *kq_idx, int nb, int nm, int num_sms, const uint8_t *mask,
+                              double *g2, cudaStream_t st);
 cudaError_t launch_grid_rotate_g2(const c128 *T2, int64_t slab, int ncols, int L1, const c128 *P1c, int cnt,
                                   const c128 *Uk, const c128 *Ukq, const int32_t *kq_idx, int nb, int nm, int num_sms,
                                   const uint8_t *mask, double *g2, cudaStream_t st);

@@ -705,7 +705,7 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   // rotation kernel the two-kernel form is as fast as the fused kernel for Nb = 8 (21.27 vs 21.28 ms, 123.0 vs 125.4 ms)
   // and faster for Nb = 11 (20.9 vs 25.4 ms), so it is the default; the fused kernel stays available by flag
   const bool want_fused = (h->cfg.flags & EPW_FLAG_GRID_FUSED) != 0;
-  const bool fused = grid && want_fused && grid_rotate_g2_supported(nb, nm, h->box_L[0]);
+  const bool fused = grid && want_fused && grid_fused_supported(nb, nm, h->box_L[0]);
   const int ncolsC = fused ? ncols_h : ncols;   // columns of the [g~ | H(k+q)] buffer that reach HBM
   if (!grid) {
     // k-chunk: one chunk of [g~ | H(k+q)] (16*ncols bytes per k) must stay L2-resident for the eigensolve and the
@@ -996,10 +996,10 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
         } else {
           const int ci = (int)(k0 / kchunk);
           const int cnt = std::min(cs, grid->N[0] - ci * cs);
-          LAUNCH(h, launch_grid_rotate_g2(h->T2.as<c128>(), slab, ncols, L[0], h->P1raw.as<c128>() + (int64_t)ci * L[0] * cs,
+          LAUNCH(h, launch_grid_fused(h->T2.as<c128>(), slab, ncols, L[0], h->P1raw.as<c128>() + (int64_t)ci * L[0] * cs,
                                           cnt, h->Uk.as<c128>() + k0 * nbb, Ukq_ptr, kq_idx, nb, nm, h->num_sms, mask,
                                           G2(q, k0), st),
-                 "grid_rotate_g2");
+                 "grid_fused");
         }
         if (h->cons.on) {
           const double *ekq = kq_map ? nullptr
