@@ -58,9 +58,9 @@ typedef struct {
                              library when the [Np][q_batch] phase table would not fit shared memory (Np > 1,760 at 8);
                              Np > 14,080 is EPW_EUNSUPPORTED */
   int32_t path;           /* EPW_PATH_AUTO (0): chosen from Nb, Nm; EPW_PATH_SMALL / EPW_PATH_LARGE force one (tests) */
-  int32_t flags;          /* 0 or EPW_FLAG_GRID_UNFUSED: on a uniform grid the last axis pass of S2 writes g~ and rotate_g2 reads
-                             it (two kernels; measured as fast as or faster than the alternative at every config);
-                             EPW_FLAG_GRID_FUSED: one kernel does the last axis pass and S4b, g~ never reaches HBM (Nb <= 16) */
+  int32_t flags;          /* 0: on a uniform grid the library picks the faster form of the last axis pass of S2 + S4b: ONE kernel
+                             (g~ never reaches HBM) for Nb <= 8, two kernels (the pass writes g~, rotate_g2 reads it) above;
+                             EPW_FLAG_GRID_FUSED / EPW_FLAG_GRID_UNFUSED force the one-kernel (Nb <= 16) / two-kernel form */
   size_t workspace_bytes; /* cap on the library's scratch HBM; 0 = library chooses from free memory */
   double degen_tol;       /* informational (gap below which callers should sum |g|^2 over a subspace); unused inside */
   double omega_min;       /* modes with omega_q,nu <= omega_min give |g|^2 = 0 (acoustic modes at Gamma); default 0;
@@ -147,7 +147,8 @@ int epw_interp_interpolate_grid_host(epw_interp_t h, const int32_t *k_grid, cons
  * involving states outside a 0.3 eV energy window").  While enabled, every following
  * interpolate call keeps a pair (k,q) iff some band of eps_k AND some band of eps_{k+q} lies in the closed interval
  * [emin, emax] (decided on the library's own FP64 eigenvalues, right after the eigensolves); the |g|^2 block of a
- * skipped pair is written as zeros and its S4b work (and, on a uniform grid, the last axis pass of S2) is not done.
+ * skipped pair is written as zeros and its S4b work is not done (the one-kernel grid form works on quads of four
+ * consecutive i1: a quad is skipped when all four of its pairs are).
  * eps_k, eps_kq and omega_q are still complete.  mask_out: NULL, or a device buffer uint8 [nq][nk] that receives
  * 1 (kept) / 0 (skipped) for every pair of each call.  (To drop k-points altogether, pass the screened k-list.)
  */

@@ -18,6 +18,8 @@
 // the U fragments of the four pairs stay in registers over all modes when Nb <= 8.
 // HBM traffic per pair: 32 Nb^2 (the two U) + 8 Nb^2 Nm (output) bytes; T2 (16 Nb^2 Nm L1 N2 N3 bytes per q) is L2-resident.
 // FP64 work per pair: 8 L1 Nb^2 Nm (pass) + 16 Nb^3 Nm (rotation) flops, all of it DMMA.
+#include <type_traits>
+
 #include "common.cuh"
 #include "dmma_pipe.cuh"
 
@@ -65,24 +67,41 @@ struct GridFusedParams {
 //   [[re, im], [-im, re]]
 __device__ __forceinline__ double embed(c128 z, int a, int b) { return a == 0 ? (b ? z.y : z.x) : (b ? z.x : -z.y); }
 
+// Fragments of the embedding of U (or conj U) for the lane (g, t): entry (ks, nt) is +-(one component of U[r][c]),
+// r = 2 ks + t/2, c = 4 nt + g/2.  Component and sign depend on the lane only (a = t & 1, b = g & 1):
+//   U:       [[re, im], [-im, re]]   component a ^ b, negative where a = 1, b = 0
+//   conj U:  [[re, -im], [im, re]]   component a ^ b, negative where a = 0, b = 1
+// The loads come first and the sign is applied later (u_frag_sign: an integer XOR on the high word), so that nothing has
+// to wait for the loads before the first pass of an item has been issued.
 template <int NB>
-__device__ __forceinline__ void load_u_frag(const c128 *__restrict__ u, bool conj, int g, int t,
-                                            double (&b)[GF<NB>::KS][GF<NB>::NT]) {
+__device__ __forceinline__ void load_u_frag_raw(const c128 *__restrict__ u, int g, int t,
+                                                double (&b)[GF<NB>::KS][GF<NB>::NT]) {
   typedef GF<NB> C;
-  const int a = t & 1, bb = g & 1;
-  // conj(U): [[re, -im], [im, re]] = the embedding of (re, -im)
-  const int comp = a ^ bb;                                 // which double of the complex entry this lane needs
-  const bool neg = conj ? (a == 0 && bb == 1) : (a == 1 && bb == 0);
-  const double *ud = reinterpret_cast<const double *>(u);
+  const double *ud = reinterpret_cast<const double *>(u) + ((t & 1) ^ (g & 1));
 #pragma unroll
   for (int ks = 0; ks < C::KS; ks++)
 #pragma unroll
     for (int nt = 0; nt < C::NT; nt++) {
       const int r = 2 * ks + (t >> 1), c = 4 * nt + (g >> 1);
-      double v = 0.0;
-      if (r < NB && c < NB) v = ud[(r + NB * c) * 2 + comp];
-      b[ks][nt] = neg ? -v : v;
+      b[ks][nt] = (r < NB && c < NB) ? ud[(r + NB * c) * 2] : 0.0;
     }
+}
+template <int NB>
+__device__ __forceinline__ void u_frag_sign(bool conj, int g, int t, double (&b)[GF<NB>::KS][GF<NB>::NT]) {
+  typedef GF<NB> C;
+  const int a = t & 1, bb = g & 1;
+  const int flip = (conj ? (a == 0 && bb == 1) : (a == 1 && bb == 0)) ? (int)0x80000000 : 0;
+#pragma unroll
+  for (int ks = 0; ks < C::KS; ks++)
+#pragma unroll
+    for (int nt = 0; nt < C::NT; nt++)
+      b[ks][nt] = __hiloint2double(__double2hiint(b[ks][nt]) ^ flip, __double2loint(b[ks][nt]));
+}
+template <int NB>
+__device__ __forceinline__ void load_u_frag(const c128 *__restrict__ u, bool conj, int g, int t,
+                                            double (&b)[GF<NB>::KS][GF<NB>::NT]) {
+  load_u_frag_raw<NB>(u, g, t, b);
+  u_frag_sign<NB>(conj, g, t, b);
 }
 
 // The two rotation products of ONE pair and ONE mode.  sG: this pair's g~ of the mode in the staging buffer [c = n' NB + m'],
@@ -302,14 +321,14 @@ __global__ void __launch_bounds__(GF_WARPS * 32, 1) grid_fused_kernel(const Grid
     if (C::UREG) {
 #pragma unroll
       for (int jj = 0; jj < 4; jj++) {
-        load_u_frag<NB>(ukp[jj], false, g, t, b1[jj % C::UP]);
-        load_u_frag<NB>(ukqp[jj], true, g, t, b2[jj % C::UP]);
+        load_u_frag_raw<NB>(ukp[jj], g, t, b1[jj % C::UP]);
+        load_u_frag_raw<NB>(ukqp[jj], g, t, b2[jj % C::UP]);
       }
     }
     advance_to((int)(tile - tile_lo));
     const c128 *sT2b = sT2 + buf_elems * (held % p.nbuf);
-    for (int nul = 0; nul < nuc; nul++) {
-      // ---- pass: g~_j[c] for the four pairs and the NBB columns c of this mode -> staging buffer [pair][n'][m'] ----
+    // ---- pass: g~_j[c] for the four pairs and the NBB columns c of mode nul -> staging buffer [pair][n'][m'] ----
+    auto pass = [&](int nul, auto exact) {
       const double *tsrc = reinterpret_cast<const double *>(sT2b + (size_t)(t >> 1) * RP + nul * NBB + g) + (t & 1);
 #pragma unroll
       for (int mt0 = 0; mt0 < C::MTP; mt0 += 8) {
@@ -318,7 +337,7 @@ __global__ void __launch_bounds__(GF_WARPS * 32, 1) grid_fused_kernel(const Grid
         for (int i = 0; i < 8; i++) acc[i][0] = acc[i][1] = 0.0;
 #pragma unroll
         for (int ks = 0; ks < KSPMAX; ks++) {
-          if (ks < ksp) {
+          if (decltype(exact)::value || ks < ksp) {
 #pragma unroll
             for (int i = 0; i < 8; i++) {
               if (mt0 + i < C::MTP) {
@@ -336,17 +355,36 @@ __global__ void __launch_bounds__(GF_WARPS * 32, 1) grid_fused_kernel(const Grid
                 make_double2(acc[i][0], acc[i][1]);
         }
       }
-      __syncwarp();
+    };
+    const bool exact = ksp == KSPMAX;   // no k-step to skip: the common case, without the branches
+    if (exact) pass(0, std::true_type());
+    else pass(0, std::false_type());
+    if (C::UREG) {
+      // the first pass is on its way: now wait for the U loads and give the fragments their signs
+#pragma unroll
+      for (int jj = 0; jj < 4; jj++) {
+        u_frag_sign<NB>(false, g, t, b1[jj % C::UP]);
+        u_frag_sign<NB>(true, g, t, b2[jj % C::UP]);
+      }
+    }
+    __syncwarp();
+    for (int nul = 0; nul < nuc; nul++) {
       if (C::UREG) {
-        // ---- product 1 of the four pairs, then product 2 and |.|^2 (no branch inside: eight independent DMMA chains) ----
+        // ---- product 1 of the four pairs (no branch inside: eight independent DMMA chains) ----
 #pragma unroll
         for (int jj = 0; jj < 4; jj++)
           product1<NB>(sG + (size_t)jj * C::PST * 2, sT + (size_t)(jj % C::UP) * C::TROWS * C::SP * 2, g, t, b1[jj % C::UP]);
         __syncwarp();
+        // ---- product 2 and |.|^2 of this mode, and in the same stretch of code the pass of the NEXT mode: the staging
+        //      buffer of g~ is free once product 1 has read it, and the two are independent DMMA chains ----
 #pragma unroll
         for (int jj = 0; jj < 4; jj++)
           product2<NB>(sT + (size_t)(jj % C::UP) * C::TROWS * C::SP * 2, p.g2 + kc[jj] * E + (int64_t)(nu0 + nul) * NBB, g, t,
                        b2[jj % C::UP], live[jj]);
+        if (nul + 1 < nuc) {
+          if (exact) pass(nul + 1, std::true_type());
+          else pass(nul + 1, std::false_type());
+        }
         __syncwarp();
       } else {
         // Nb > 8: the fragments of one U matrix at a time (36 registers at Nb = 11), pair by pair
@@ -362,6 +400,11 @@ __global__ void __launch_bounds__(GF_WARPS * 32, 1) grid_fused_kernel(const Grid
           product2<NB>(sT, p.g2 + k * E + (int64_t)(nu0 + nul) * NBB, g, t, b2[0], true);
           __syncwarp();
         }
+        if (nul + 1 < nuc) {
+          if (exact) pass(nul + 1, std::true_type());
+          else pass(nul + 1, std::false_type());
+        }
+        __syncwarp();
       }
     }
   }

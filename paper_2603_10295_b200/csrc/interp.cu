@@ -700,12 +700,14 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   int64_t slab = 0;          // k-points per i1 plane
   int cs = 0, nchunks = 1;   // i1 planes per k-chunk
   int KB1 = 0, NTc = 0;
-  // grid mode: the last axis pass is fused with S4b (grid_rotate_g2.cu) unless the caller asked for the two-kernel form
-  // measured (bench.py --grid-fused / --grid-unfused, configs[1..3]): with the streaming axis passes and the pipelined
-  // rotation kernel the two-kernel form is as fast as the fused kernel for Nb = 8 (21.27 vs 21.28 ms, 123.0 vs 125.4 ms)
-  // and faster for Nb = 11 (20.9 vs 25.4 ms), so it is the default; the fused kernel stays available by flag
-  const bool want_fused = (h->cfg.flags & EPW_FLAG_GRID_FUSED) != 0;
-  const bool fused = grid && want_fused && grid_fused_supported(nb, nm, h->box_L[0]);
+  // grid mode: the last axis pass, S4b and |g|^2 run as ONE all-DMMA kernel (grid_fused.cu; g~ never reaches HBM) for
+  // Nb <= 8, where the U fragments of four pairs stay in registers: measured (bench.py --grid-fused / --grid-unfused)
+  // 16.7 vs 18.8 ms per 32-q step on configs[1] and 91 vs 110 ms per 13-q step on configs[3].  For 9 <= Nb <= 16 the fused
+  // kernel reloads its U fragments per mode and is no faster than the two-kernel form (21.0 vs 20.7 ms on configs[2]),
+  // which stays the default there.  EPW_FLAG_GRID_FUSED / EPW_FLAG_GRID_UNFUSED force either form.
+  const bool can_fuse = grid && grid_fused_supported(nb, nm, h->box_L[0]);
+  const bool fused = can_fuse && ((h->cfg.flags & EPW_FLAG_GRID_FUSED) != 0 ||
+                                  (nb <= 8 && (h->cfg.flags & EPW_FLAG_GRID_UNFUSED) == 0));
   const int ncolsC = fused ? ncols_h : ncols;   // columns of the [g~ | H(k+q)] buffer that reach HBM
   if (!grid) {
     // k-chunk: one chunk of [g~ | H(k+q)] (16*ncols bytes per k) must stay L2-resident for the eigensolve and the

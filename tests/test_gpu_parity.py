@@ -368,7 +368,7 @@ def run_gpu(epw, w, k_list, q_list, kq_map=None, q_batch=0, host_api=False, path
             return eps_k, eps_kq, om, g2
         if grid is not None:
             out = h.interpolate_grid(grid, dev(q_list), k_shift=shift, kq_map=None if kq_map is None else dev(kq_map))
-            fused = flags == 2
+            fused = flags == 2 or (flags == 0 and w.nbnd <= 8)
             want = "list" if path == 2 or w.nbnd > 16 else ("grid-fused" if fused else "grid")
             assert epw.epw_interp_last_plan(h.h)["k_mode"] == want
         else:
@@ -603,20 +603,59 @@ def test_config1_full_size_sampled(epw):
     print(f"config 1 full size: worst |g|^2 deviation {worst:.3f} x tolerance")
 
 
-@pytest.mark.parametrize("cfg,q_idx", [(1, list(range(0, 28)) + [500, 501, 998, 999]), (2, [0, 1000, 1999]), (3, [0, 255])])
-def test_grid_full_size_sampled(epw, cfg, q_idx):
-    """configs[1..3] at full size through the uniform-grid entry point (what bench.py times by default; configs[1]
-    with the 32 q per call of the default bench step)."""
+# q-points per interpolate call of the default bench.py step of each config (bench.NQ_STEP)
+BENCH_NQ_STEP = {1: 96, 2: 32, 3: 13}
+
+
+@pytest.mark.parametrize("cfg,flags", [(1, 0), (1, 1), (2, 0), (2, 2), (3, 0)])
+def test_grid_full_size_sampled(epw, cfg, flags):
+    """configs[1..3] at full size through the uniform-grid entry point in the launch configuration bench.py times: all k,
+    the bench's number of q-points per call (96 / 32 / 13), default kernel choice (flags 0: one-kernel form for Nb = 8,
+    two-kernel form for Nb = 11) and the other form.  The outputs stay on the device (19 GB for configs[1]); sampled
+    (q, k) pairs -- the S1 batch edges, first / last q, i1-plane and chunk edges in k -- are compared with the oracle."""
+    from parity import g2_pair_close
+
     w = synth.make_config(cfg)
-    k_idx = sample_k(w.nk, 16 if cfg != 1 else 6)
+    nq = BENCH_NQ_STEP[cfg]
+    rng_q = np.random.default_rng(100 + cfg)
+    q_idx = np.sort(rng_q.choice(w.nq, size=nq, replace=False))
+    ql = np.ascontiguousarray(w.q_list[q_idx])
+    check_q = sorted({0, 7, 8, nq // 2, nq - 1}) if cfg == 1 else [0, nq - 1]
+    k_idx = sample_k(w.nk, 12 if cfg != 1 else 6)
     slab = w.k_grid[1] * w.k_grid[2]
     k_idx = sorted(set(k_idx) | {slab - 1, slab, 63 * slab + 5 if 63 * slab + 5 < w.nk else 0,
                                  64 * slab if 64 * slab < w.nk else 0})  # i1-plane and chunk edges
-    worst = check_sampled_pairs(epw, w, q_idx, k_idx, grid=True)
-    print(f"config {cfg} full size (grid): worst |g|^2 deviation {worst:.3f} x tolerance")
-    if cfg == 1:   # and the fused kernel at full size
-        worst = check_sampled_pairs(epw, w, q_idx[:4], k_idx, grid=True, flags=2)
-        print(f"config {cfg} full size (grid, fused kernel): worst |g|^2 deviation {worst:.3f} x tolerance")
+    h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_, flags=flags)
+    try:
+        h.set_operators_from_host(w)
+        eps_k, eps_kq, om, g2 = h.interpolate_grid(w.k_grid, dev(ql))
+        epw.epw_interp_sync(h.h)
+        want = "grid-fused" if (flags == 2 or (flags == 0 and w.nbnd <= 8)) else "grid"
+        assert epw.epw_interp_last_plan(h.h)["k_mode"] == want
+        kt = torch.tensor(k_idx, device="cuda")
+        eps_k_s = eps_k[kt].cpu().numpy()
+        om = om.cpu().numpy()
+        g = w.g_full()
+        worst = 0.0
+        for jq in check_q:
+            eps_kq_s = eps_kq[jq][kt].cpu().numpy()
+            g2_s = g2[jq][kt].cpu().numpy()
+            e_ref, om_ref = oracle.phonon(w.D_R, w.Rp, w.w_p, ql[jq])
+            err, ok = eig_close(om[jq], om_ref)
+            assert ok, f"omega mismatch at q {jq}: {err:.3e}"
+            g1 = oracle.rp_to_q(g, w.Rp, w.w_p, ql[jq])
+            for i, ik in enumerate(k_idx):
+                r_g2, r_ek, r_ekq = oracle.pair(g1, w.H_R, w.Re, w.w_e, e_ref, om_ref, w.k_list[ik], ql[jq])
+                err, ok = eig_close(eps_k_s[i], r_ek)
+                assert ok, f"eps_k mismatch at k {ik}: {err:.3e}"
+                err, ok = eig_close(eps_kq_s[i], r_ekq)
+                assert ok, f"eps_kq mismatch at (q {jq}, k {ik}): {err:.3e}"
+                wst, ok = g2_pair_close(g2_s[i], r_g2, r_ekq, r_ek, om_ref)
+                assert ok, f"|g|^2 mismatch at (q {jq}, k {ik}): {wst:.3f} x tolerance"
+                worst = max(worst, wst)
+    finally:
+        h.close()
+    print(f"config {cfg} full size (grid, flags {flags}, {nq} q per call): worst |g|^2 deviation {worst:.3f} x tolerance")
 
 
 def test_config2_full_size_sampled(epw):
