@@ -695,6 +695,7 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   auto G2 = [&](int64_t q, int64_t k0) { return g2_base + q * g2_qs + k0 * E; };
 
   int64_t kchunk, c_rows;
+  int hbatch = 0;            // grid mode, one-kernel form: q-points whose H(k+q) side is taken in one go (0 = per q)
   // grid mode: extents of the three axis passes (re_to_k_grid.cu)
   const int *L = h->box_L;
   int64_t slab = 0;          // k-points per i1 plane
@@ -735,6 +736,19 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
     if (fit >= grid->N[0]) fit = grid->N[0];
     else if (fit > 64) fit = fit / 64 * 64;
     cs = (int)fit;
+    // One-kernel form with per-pair H(k+q): H(k+q) depends on q and H(Re) only, so its three axis passes and its
+    // eigensolves are taken for QBH q-points of the S1 batch AT ONCE, before the g passes of those q (one eigensolver
+    // launch of QBH*nk matrices instead of QBH launches of nk: 64,000 solves are 3.4 batches per persistent group of the
+    // thread-per-matrix kernel -- a quarter of the GPU idles through the last round of every launch).  Needs the
+    // H(k+q), U_{k+q} (and eps) of QBH q within the workspace cap; otherwise the per-q, chunked form below runs.
+    if (fused && !kq_map) {
+      const size_t per_q = (size_t)nk * (2 * (size_t)nbb * 16 + (size_t)nb * 8);
+      const size_t room = std::min(cap, (size_t)4 << 30);
+      if (per_q <= room && axis_pass_supported(L[0]) && axis_pass_supported(L[1]) && axis_pass_supported(L[2])) {
+        hbatch = (int)std::min<size_t>(room / per_q, (size_t)QB);
+        cs = grid->N[0];
+      }
+    }
     nchunks = (int)ceil_div(grid->N[0], cs);
     kchunk = cs * slab;
     c_rows = nchunks == 1 ? nk : kchunk;
@@ -748,7 +762,8 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
     CU_OR_FAIL(h, h->BpackH.reserve(sizeof(double) * (size_t)NTH * KB * GEMM_CHUNK), "cudaMalloc BpackH");
     CU_OR_FAIL(h, h->Bpack.reserve(sizeof(double) * (size_t)QB * NT * KB * GEMM_CHUNK), "cudaMalloc Bpack");
   } else {
-    const int nc = std::max(ncols, nbb);
+    // columns of the axis-pass buffers: [g~ | H(k+q)] of one q, or (hbatch) g~ of one q and the H(k+q) of hbatch q in turn
+    const int nc = hbatch ? std::max(ncols_g, hbatch * nbb) : std::max(ncols, nbb);
     const int maxN = std::max(std::max(grid->N[0], grid->N[1]), grid->N[2]);
     const int maxL = std::max(std::max(L[0], L[1]), L[2]);
     CU_OR_FAIL(h, h->X.reserve(sizeof(c128) * (size_t)h->box_size * nc), "cudaMalloc X");
@@ -772,9 +787,10 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   CU_OR_FAIL(h, h->Dq.reserve(sizeof(c128) * (size_t)nq * nmm), "cudaMalloc Dq");
   CU_OR_FAIL(h, h->eq.reserve(sizeof(c128) * (size_t)nq * nmm), "cudaMalloc e_q");
   if (!h->ext_g1) CU_OR_FAIL(h, h->g1.reserve(sizeof(c128) * (size_t)QB * h->rows), "cudaMalloc g(Re,q)");
-  if (ncolsC) CU_OR_FAIL(h, h->C.reserve(sizeof(c128) * (size_t)c_rows * ncolsC), "cudaMalloc g~");
-  if (!kq_map) CU_OR_FAIL(h, h->Ukq.reserve(sizeof(c128) * (size_t)c_rows * nbb), "cudaMalloc Ukq");
-  if (!kq_map && !eps_kq) CU_OR_FAIL(h, h->epskq_scratch.reserve(sizeof(double) * (size_t)c_rows * nb), "cudaMalloc eps scratch");
+  const size_t hb = hbatch ? hbatch : 1;
+  if (ncolsC) CU_OR_FAIL(h, h->C.reserve(sizeof(c128) * hb * (size_t)c_rows * ncolsC), "cudaMalloc g~");
+  if (!kq_map) CU_OR_FAIL(h, h->Ukq.reserve(sizeof(c128) * hb * (size_t)c_rows * nbb), "cudaMalloc Ukq");
+  if (!kq_map && !eps_kq) CU_OR_FAIL(h, h->epskq_scratch.reserve(sizeof(double) * hb * (size_t)c_rows * nb), "cudaMalloc eps scratch");
   { const int rc = h->ensure_status(); if (rc != EPW_OK) return rc; }
   if (h->window_on && !h->mask_out) CU_OR_FAIL(h, h->maskbuf.reserve((size_t)nk), "cudaMalloc mask");
   {
@@ -793,23 +809,25 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   // the two leading axis passes of the factorised S2: X [L1][L2][L3][nc] -> T1 [L1][L2][N3][nc] -> T2 [L1][N2][N3][nc]
   // Axis passes: a streaming kernel when the box extent is small (always, for Wigner-Seitz lists), else the in-place
   // tensor-path contraction with the packed phase table.
-  auto grid_pass_ab = [&](int nc) -> cudaError_t {
+  // (nbat > 1: the same passes for nbat operands stored one after the other -- the outermost box index simply runs on)
+  auto grid_pass_ab = [&](int nc, int nbat) -> cudaError_t {
     const int64_t N2 = grid->N[1], N3 = grid->N[2];
+    const int64_t B = (int64_t)nbat * L[0];   // outermost extent of X, T1, T2
     cudaError_t e;
     if (axis_pass_supported(L[2]))
-      e = launch_axis_pass(h->X.as<c128>(), nc, (int64_t)L[2] * nc, nc, (int64_t)L[0] * L[1] * nc, h->P3raw.as<c128>(), L[2],
+      e = launch_axis_pass(h->X.as<c128>(), nc, (int64_t)L[2] * nc, nc, B * L[1] * nc, h->P3raw.as<c128>(), L[2],
                            (int)N3, h->T1.as<c128>(), nc, N3 * nc, nc, h->num_sms, st);
     else
       e = launch_zgemm_strided(h->X.as<c128>(), nc, (int64_t)L[2] * nc, nc, 0, h->P3pack.as<double>(), nullptr, h->T1.p, nc,
-                               N3 * nc, 1, nc, 0, 0, (int64_t)L[0] * L[1] * nc, (int)N3, L[2], 1, h->num_sms, st);
+                               N3 * nc, 1, nc, 0, 0, B * L[1] * nc, (int)N3, L[2], 1, h->num_sms, st);
     if (e != cudaSuccess) return e;
     h->launches++;
     if (axis_pass_supported(L[1]))
-      return launch_axis_pass(h->T1.as<c128>(), N3 * nc, (int64_t)L[1] * N3 * nc, N3 * nc, (int64_t)L[0] * N3 * nc,
+      return launch_axis_pass(h->T1.as<c128>(), N3 * nc, (int64_t)L[1] * N3 * nc, N3 * nc, B * N3 * nc,
                               h->P2raw.as<c128>(), L[1], (int)N2, h->T2.as<c128>(), N3 * nc, N2 * N3 * nc, N3 * nc,
                               h->num_sms, st);
     return launch_zgemm_strided(h->T1.as<c128>(), N3 * nc, (int64_t)L[1] * N3 * nc, N3 * nc, 0, h->P2pack.as<double>(),
-                                nullptr, h->T2.p, N3 * nc, N2 * N3 * nc, 1, N3 * nc, 0, 0, (int64_t)L[0] * N3 * nc,
+                                nullptr, h->T2.p, N3 * nc, N2 * N3 * nc, 1, N3 * nc, 0, 0, B * N3 * nc,
                                 (int)N2, L[1], 1, h->num_sms, st);
   };
   // the last axis pass for the i1 planes of chunk ci: T2 -> out [i1][i2][i3][nc]
@@ -865,7 +883,7 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
     LAUNCH(h, launch_box_scatter(nullptr, nullptr, nullptr, 0.0, h->H.as<c128>(), nullptr, h->we.as<double>(),
                                  h->boxidx.as<int32_t>(), h->box_size, nbb, nm, ne, 0, nbb, h->X.as<c128>(), st),
            "box_scatter(H)");
-    LAUNCH(h, grid_pass_ab(nbb), "grid passes H(k)");
+    LAUNCH(h, grid_pass_ab(nbb, 1), "grid passes H(k)");
     for (int ci = 0; ci < nchunks; ci++)
       LAUNCH(h, grid_pass_c(nbb, ci, h->Hk.as<c128>() + (int64_t)ci * kchunk * nbb), "grid pass H(k)");
   }
@@ -913,17 +931,42 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
     for (int iq = 0; iq < qb; iq++) {
       const int64_t q = q0 + iq;
       const double *Bq = grid ? nullptr : h->Bpack.as<double>() + (int64_t)iq * NT * KB * GEMM_CHUNK;
+      if (hbatch && iq % hbatch == 0) {
+        // ---- S3a + S3b for the next hbatch q-points at once: H(k+q) = sum_Re e^{2 pi i (k+q).Re} H(Re) by the three axis
+        //      passes on Nb^2 columns (operands of the hn q-points one after the other), then ONE eigensolver launch ----
+        const int hn = std::min(hbatch, qb - iq);
+        const int64_t Mh = slab * nbb;
+        sp = h->begin_span(4, st);
+        for (int j = 0; j < hn; j++)
+          LAUNCH(h, launch_box_scatter(nullptr, nullptr, nullptr, 0.0, h->H.as<c128>(), Pqe_b + (int64_t)(iq + j) * ne,
+                                       h->we.as<double>(), h->boxidx.as<int32_t>(), h->box_size, nbb, nm, ne, 0, nbb,
+                                       h->X.as<c128>() + (int64_t)j * h->box_size * nbb, st),
+                 "box_scatter(H e^{iqR})");
+        LAUNCH(h, grid_pass_ab(nbb, hn), "grid passes H(k+q)");
+        LAUNCH(h, launch_axis_pass(h->T2.as<c128>(), Mh, (int64_t)L[0] * Mh, Mh, (int64_t)hn * Mh, h->P1raw.as<c128>(), L[0],
+                                   grid->N[0], h->C.as<c128>(), Mh, (int64_t)grid->N[0] * Mh, Mh, h->num_sms, st),
+               "grid pass H(k+q)");
+        h->end_span(sp, st);
+        sp = h->begin_span(5, st);
+        double *eps_dst = eps_kq ? eps_kq + q * nk * nb : h->epskq_scratch.as<double>();
+        LAUNCH(h, launch_eigh_batched(h->C.as<c128>(), nbb, nb, (int64_t)hn * nk, eps_dst, h->Ukq.as<c128>(), 0,
+                                      h->status.as<int32_t>(), h->eig_scratch.as<c128>(), h->work_slot(1), st),
+               "eigh H(k+q)");
+        h->end_span(sp, st);
+      }
+      const int hslot = hbatch ? iq % hbatch : 0;            // slot of this q in the U_{k+q} / eps scratch of its H batch
+      const int nc_g = hbatch ? ncols_g : ncols;             // columns of the axis-pass buffers of this q
       if (grid) {
         sp = h->begin_span(8, st);
         LAUNCH(h, launch_box_scatter(g1b + (int64_t)iq * h->rows, eq_b + (int64_t)iq * nmm,
                                      omega_q + q * nm, h->cfg.omega_min, h->H.as<c128>(),
-                                     ncols_h ? Pqe_b + (int64_t)iq * ne : nullptr, h->we.as<double>(),
-                                     h->boxidx.as<int32_t>(), h->box_size, nbb, nm, ne, ncols_g, ncols_h,
+                                     (ncols_h && !hbatch) ? Pqe_b + (int64_t)iq * ne : nullptr, h->we.as<double>(),
+                                     h->boxidx.as<int32_t>(), h->box_size, nbb, nm, ne, ncols_g, hbatch ? 0 : ncols_h,
                                      h->X.as<c128>(), st),
                "box_scatter");
         h->end_span(sp, st);
         sp = h->begin_span(4, st);
-        LAUNCH(h, grid_pass_ab(ncols), "grid passes S2");
+        LAUNCH(h, grid_pass_ab(nc_g, 1), "grid passes S2");
         h->end_span(sp, st);
       }
       for (int64_t k0 = 0; k0 < nk; k0 += kchunk) {
@@ -938,7 +981,7 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
                  "zgemm S2");
         } else if (!fused) {
           LAUNCH(h, grid_pass_c(ncols, (int)(k0 / kchunk), Cc), "grid pass S2");
-        } else if (ncols_h) {
+        } else if (ncols_h && !hbatch) {
           // fused form: only the H(k+q) columns of the last axis pass go to HBM (the eigensolver's input)
           const int ci = (int)(k0 / kchunk);
           const int cnt = std::min(cs, grid->N[0] - ci * cs);
@@ -967,6 +1010,8 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
             CU_OR_FAIL(h, cudaGetLastError(), "gather_eps");
             h->end_span(sp, st);
           }
+        } else if (hbatch) {
+          Ukq_ptr = h->Ukq.as<c128>() + (int64_t)hslot * nk * nbb;   // solved with its H batch above
         } else {
           // ---- S3b per pair: eigensolve the H(k+q) block of the contraction output ----
           sp = h->begin_span(5, st);
@@ -983,7 +1028,8 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
         if (h->window_on) {
           uint8_t *m = h->mask_out ? h->mask_out + q * nk + k0 : h->maskbuf.as<uint8_t>();
           const double *ekq = kq_map ? nullptr
-                                     : (eps_kq ? eps_kq + (q * nk + k0) * nb : h->epskq_scratch.as<double>() + crow * nb);
+                                     : (eps_kq ? eps_kq + (q * nk + k0) * nb
+                                               : h->epskq_scratch.as<double>() + ((int64_t)hslot * nk + crow) * nb);
           sp = h->begin_span(5, st);
           LAUNCH(h, launch_window_mask(eps_k + k0 * nb, ekq, eps_k, kq_idx, nb, kn, h->emin, h->emax, m, st), "window mask");
           h->end_span(sp, st);
@@ -998,14 +1044,15 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
         } else {
           const int ci = (int)(k0 / kchunk);
           const int cnt = std::min(cs, grid->N[0] - ci * cs);
-          LAUNCH(h, launch_grid_fused(h->T2.as<c128>(), slab, ncols, L[0], h->P1raw.as<c128>() + (int64_t)ci * L[0] * cs,
+          LAUNCH(h, launch_grid_fused(h->T2.as<c128>(), slab, nc_g, L[0], h->P1raw.as<c128>() + (int64_t)ci * L[0] * cs,
                                           cnt, h->Uk.as<c128>() + k0 * nbb, Ukq_ptr, kq_idx, nb, nm, h->num_sms, mask,
                                           G2(q, k0), st),
                  "grid_fused");
         }
         if (h->cons.on) {
           const double *ekq = kq_map ? nullptr
-                                     : (eps_kq ? eps_kq + (q * nk + k0) * nb : h->epskq_scratch.as<double>() + crow * nb);
+                                     : (eps_kq ? eps_kq + (q * nk + k0) * nb
+                                               : h->epskq_scratch.as<double>() + ((int64_t)hslot * nk + crow) * nb);
           LAUNCH(h, launch_selfenergy_accumulate(G2(q, k0), eps_k + k0 * nb, ekq, eps_k, kq_idx, omega_q + q * nm,
                                                  h->cons.w_q, q, h->cons.mu, h->cons.kT, h->cons.sigma, nb, nm, kn,
                                                  h->cons.out + k0 * nb, st),
