@@ -366,8 +366,9 @@ struct __align__(32) RotB {
 __global__ void __launch_bounds__(EC_THREADS, 1)
     eigh_cluster_kernel(const c128 *__restrict__ Ain, int64_t stride_a, int n, int64_t batch,
                         double *__restrict__ evals, c128 *__restrict__ Vout, int sqrt_mode, int32_t *__restrict__ status,
-                        c128 *__restrict__ scratch, int nr) {
+                        c128 *__restrict__ scratch, int nr, unsigned long long *__restrict__ work) {
   cg::cluster_group cluster = cg::this_cluster();
+  unsigned long long my_rot = 0;   // plane rotations this thread built as the owner of a pair (work counter)
   const int csize = (int)cluster.num_blocks(), crank = (int)cluster.block_rank();
   const int cluster_id = blockIdx.x / csize, num_clusters = gridDim.x / csize;
   extern __shared__ __align__(32) unsigned char smem_raw[];
@@ -469,6 +470,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1)
               if (gr * gr + gi * gi > tol2 * al * be) {
                 const Rot J = make_rot(al, be, cmake(gr, gi));
                 R.c = J.c; R.sr = J.sr; R.si = J.si; R.act = 1.0;
+                my_rot++;
               }
             }
             for (int c2 = 0; c2 < csize; c2++) cluster.map_shared_rank(rot, c2)[s] = R;
@@ -575,6 +577,7 @@ __global__ void __launch_bounds__(EC_THREADS, 1)
     }
     cluster.sync();  // scratch, rot and part are reused by the next matrix
   }
+  if (work != nullptr && my_rot) atomicAdd(work, my_rot);
 }
 
 // cluster size (1, 2, 4, 8) and rows per CTA for an n x n solve, 0 if it does not fit in distributed shared memory
@@ -667,7 +670,7 @@ cudaError_t launch_eigh_batched_algo(const c128 *A, int64_t stride_a, int n, int
         const int64_t cap = std::min<int64_t>(max_clusters, eigh_large_grid(batch));
         cfg.gridDim = dim3((unsigned)(std::min<int64_t>(batch, cap) * cs));
         return cudaLaunchKernelEx(&cfg, eigh_cluster_kernel, A, stride_a, n, batch, evals, V, sqrt_mode, status,
-                                  scratch_large, nr);
+                                  scratch_large, nr, work);
       }
     }
     const int half = (n + (n & 1)) >> 1;

@@ -1029,3 +1029,47 @@ def test_two_handles_from_two_threads_count_their_own_rotations(epw):
     for s, p in zip(serial, par):
         assert s["rot"]["Hkq"] > 0 and s["rot"] == p["rot"]
         assert np.array_equal(s["g2"], p["g2"])
+
+
+def test_large_path_k_side_cache_and_its_invalidation(epw):
+    """Large-Nb family on a uniform grid: the k side (phases, H(k), U_k, eps_k) is kept between calls on the same grid.
+    Second call on the same grid (cache hit: fewer launches, same results), a call with k+q off the grid after one with
+    kq_map (the packed conj U_k is overwritten), a SHIFTED grid (k changes: miss), and new operators (miss) are each
+    checked against the oracle."""
+    w = synth.make_custom("zsnr-c", 20, 12, (2, 0, 0), 1.0, 0.05, 2.0, (10, 1, 1), ("grid", (10, 1, 1)), seed=24)
+    g = w.g_full()
+    h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_)
+    try:
+        h.set_operators_from_host(w)
+
+        def call(q, kq, shift=None):
+            out = h.interpolate_grid(w.k_grid, dev(q), k_shift=shift, kq_map=None if kq is None else dev(kq))
+            epw.epw_interp_sync(h.h)
+            return [t.cpu().numpy() for t in out], epw.epw_interp_last_launch_count(h.h)
+
+        qa, qb = w.q_list[:3], w.q_list[3:6]
+        ref_a = oracle.interpolate(w.H_R, w.D_R, g, w.Re, w.w_e, w.Rp, w.w_p, w.k_list, qa)
+        ref_b = oracle.interpolate(w.H_R, w.D_R, g, w.Re, w.w_e, w.Rp, w.w_p, w.k_list, qb)
+        out1, n1 = call(qa, w.kq_map[:3])
+        assert_path_close(out1, ref_a)
+        out2, n2 = call(qb, w.kq_map[3:6])            # same grid: cache hit
+        assert n2 < n1
+        assert_path_close(out2, ref_b)
+        q_off = qa + 0.013
+        ref_off = oracle.interpolate(w.H_R, w.D_R, g, w.Re, w.w_e, w.Rp, w.w_p, w.k_list, q_off)
+        out3, _ = call(q_off, None)                   # per-pair H(k+q): overwrites the packed conj(U_k)
+        assert_path_close(out3, ref_off)
+        out4, n4 = call(qa, w.kq_map[:3])             # must rebuild it
+        assert_path_close(out4, ref_a)
+        shift = np.array([0.25, 0.0, 0.0])
+        k_sh = w.k_list + shift / np.array(w.k_grid)
+        ref_sh = oracle.interpolate(w.H_R, w.D_R, g, w.Re, w.w_e, w.Rp, w.w_p, k_sh, q_off)
+        out5, n5 = call(q_off, None, shift=shift)     # k changed between calls: miss
+        assert_path_close(out5, ref_sh)
+        w2 = synth.make_custom("zsnr-c2", 20, 12, (2, 0, 0), 1.0, 0.05, 2.0, (10, 1, 1), ("grid", (10, 1, 1)), seed=25)
+        h.set_operators_from_host(w2)                 # new operators, same grid: miss
+        ref_w2 = oracle.interpolate(w2.H_R, w2.D_R, w2.g_full(), w2.Re, w2.w_e, w2.Rp, w2.w_p, k_sh, q_off)
+        out6, _ = call(q_off, None, shift=shift)
+        assert_path_close(out6, ref_w2)
+    finally:
+        h.close()
