@@ -445,7 +445,6 @@ def run_config(args, ctx, cfg_index: int, steps: int, warmup: int, legs: set) ->
         acc_dev = torch.zeros((nk, w.nbnd), dtype=torch.float64, device="cuda")
         # chemical potential in the middle of the bands of the first k-point, room temperature, 20 meV broadening
         epw.epw_interp_set_selfenergy_consumer(h.h, True, 0.0, 0.025, 0.02, None, acc_dev)
-        want_e2e = False
     if args.rp_shard:
         want_e2e = False   # the host-buffer entry point has no Rp-sharded form
     rows = w.slab_elems
@@ -648,7 +647,11 @@ def run_config(args, ctx, cfg_index: int, steps: int, warmup: int, legs: set) ->
         o_eps_k = torch.empty((nk, w.nbnd), dtype=torch.float64).pin_memory()
         o_eps_kq = torch.empty((nq_step, nk, w.nbnd), dtype=torch.float64).pin_memory()
         o_omega = torch.empty((nq_step, w.nmodes), dtype=torch.float64).pin_memory()
-        o_g2 = torch.empty((nq_step, nk, w.nmodes, w.nbnd, w.nbnd), dtype=torch.float64).pin_memory()
+        # with the consumer on nothing of size nk x nq leaves the device: the step returns eps_k, omega_q and Im Sigma_nk
+        o_g2 = None if args.consumer else torch.empty((nq_step, nk, w.nmodes, w.nbnd, w.nbnd), dtype=torch.float64).pin_memory()
+        o_acc = torch.empty((nk, w.nbnd), dtype=torch.float64).pin_memory() if args.consumer else None
+        if args.consumer:
+            o_eps_kq = None
         g2 = None   # the host-buffer entry point stages |g|^2 in the library's own device buffer
         torch.cuda.empty_cache()
 
@@ -661,6 +664,8 @@ def run_config(args, ctx, cfg_index: int, steps: int, warmup: int, legs: set) ->
                 epw.epw_interp_interpolate_host(h.h, k_host, nk, q_host[s], nq_step,
                                                 None if map_host is None else map_host[s], o_eps_k, o_eps_kq, o_omega,
                                                 o_g2)
+            if o_acc is not None:
+                o_acc.copy_(acc_dev, non_blocking=True)   # the step's result: the accumulator, device -> pinned host
 
         n_e2e_warm = min(warmup, 2)
         n_e2e = min(steps, 8)   # PCIe-bound (a third of a second per step on configs[1]): a bounded number of steps
@@ -676,7 +681,7 @@ def run_config(args, ctx, cfg_index: int, steps: int, warmup: int, legs: set) ->
         ms_e2e = e0.elapsed_time(e1)
         ms_e2e = shard.max_over_ranks_ms(ms_e2e, dist, device="cuda")
         h2d = (0 if use_grid else k_host.numel() * 8) + q_host[0].numel() * 8 + (0 if map_host is None else map_host[0].numel() * 4)
-        d2h = (o_eps_k.numel() + o_eps_kq.numel() + o_omega.numel() + o_g2.numel()) * 8
+        d2h = sum(t.numel() for t in (o_eps_k, o_eps_kq, o_omega, o_g2, o_acc) if t is not None) * 8
         e2e = {"value": world * elements_per_step * n_e2e / (ms_e2e * 1e-3), "unit": UNIT,
                "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "ms_per_step": ms_e2e / n_e2e, "steps": n_e2e,
                "api": ("epw_interp_interpolate_grid_host" if use_grid else "epw_interp_interpolate_host")

@@ -163,8 +163,12 @@ int epw_interp_set_energy_window(epw_interp_t h, int enabled, double emin, doubl
  * paper names this consumer without printing it: DESIGN.md reading G18.
  *   w_q      NULL (weight 1) or device f64 [nq of the call]: weight of every q-point of the call
  *   im_sigma device f64 [nk][Nb], ACCUMULATED (+=) by every call: the caller zeroes it and may sum over many calls
- * With the consumer enabled the g2 argument of the interpolate calls may be NULL: the library then keeps |g|^2 of one q
- * at a time in its own scratch (8 Nb^2 Nm nk bytes) and the 8 Nb^2 Nm nk nq byte output never exists.
+ * With the consumer enabled the g2 argument of the interpolate calls (device or host form) may be NULL.  On a uniform grid
+ * with Nb <= 8 (the one-kernel form of the last axis pass + S4b) the reduction happens in the epilogue of that kernel,
+ * straight from the accumulator registers: no |g|^2 is written anywhere and nothing of size nk nq exists.  In the other
+ * kernel routes the library keeps |g|^2 of one q at a time in its own scratch (8 Nb^2 Nm nk bytes) and reduces it with a
+ * second kernel.  The sum over (m, nu) runs in a fixed order (deterministic) unless the modes of a pair are split over
+ * several tiles of the one-kernel form (large Nb^2 Nm L1: atomic adds, the order of the partial sums then varies).
  */
 int epw_interp_set_selfenergy_consumer(epw_interp_t h, int enabled, double mu, double kT, double sigma, const double *w_q,
                                        double *im_sigma);

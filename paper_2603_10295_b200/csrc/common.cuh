@@ -147,9 +147,17 @@ cudaError_t launch_grid_axis_phase(int N, int i0, int cnt, double shift, int lo,
 bool grid_rotate_g2_supported(int nb, int nm, int L1);
 // the same on the FP64 tensor path throughout (grid_fused.cu): pass as a DMMA product over quads of i1, then S4b
 bool grid_fused_supported(int nb, int nm, int L1);
+// fold (may be NULL): the NEXT-4 consumer taken in the epilogue of the kernel (consumer.cu has the formula); with it g2 may be
+// NULL.  out, eps_k, eps_kq relative to the first k of the chunk; eps_kq = eps_k of all k when kq_idx is given.
+struct SelfEnergyFold {
+  double *out;
+  const double *eps_k, *eps_kq, *omega_q, *w_q;
+  int64_t iq;
+  double mu, kT, sigma;
+};
 cudaError_t launch_grid_fused(const c128 *T2, int64_t slab, int ncols, int L1, const c128 *P1c, int cnt, const c128 *Uk,
                               const c128 *Ukq, const int32_t *kq_idx, int nb, int nm, int num_sms, const uint8_t *mask,
-                              double *g2, cudaStream_t st);
+                              double *g2, const SelfEnergyFold *fold, cudaStream_t st);
 cudaError_t launch_grid_rotate_g2(const c128 *T2, int64_t slab, int ncols, int L1, const c128 *P1c, int cnt,
                                   const c128 *Uk, const c128 *Ukq, const int32_t *kq_idx, int nb, int nm, int num_sms,
                                   const uint8_t *mask, double *g2, cudaStream_t st);

@@ -1,0 +1,576 @@
+// grid_fused.cuh -- uniform-grid path, Nb <= 16: the LAST axis pass of S2, S4b and |g|^2 in ONE kernel, all three products
+// on the FP64 tensor path (mma.sync.m8n8k4.f64, SASS DMMA), so that g~(k,q) never goes to HBM.
+//
+//   g~_{m'n' nu}(k,q) = sum_{n1} e^{2 pi i (i1+s1) n1 / N1} T2[n1][(i2,i3)][nu,n',m']      (last axis of the factorised
+//                                                         Re -> k sum, re_to_k_grid.cu; Eq. 10)
+//   g_{mn nu}(k,q)    = sum_{m'n'} conj(U_{k+q}[m',m]) g~_{m'n' nu} U_k[n',n],   out = |g_{mn nu}|^2   (
+//                                                         BASELINE.json north_star stage 4; reading G4)
+// In the two-kernel grid path the last pass writes g~ (16 Nb^2 Nm bytes per pair) and rotate_g2.cu reads it back: 852 of
+// the 1,371 MB moved per q on configs[1].  Here the L1 rows T2[.][cell][mode group] of one (i2,i3) cell of the grid come
+// into shared memory by bulk TMA, and a warp takes a QUAD of four consecutive i1 of that cell:
+//   pass       C[c][(j,re/im)] = sum_{(n1,re/im)} T2[n1][c] (x) p[n1][j]     one DMMA tile = 8 columns c x 4 pairs j:
+//              A' fragments = re/im of T2 straight from shared memory (one LDS.64 per DMMA), B' fragments = the 2x2 real
+//              embedding of the four pairs' phases, held in registers; K = 2 L1 real.  The tile lands as one complex
+//              g~_j[c] per lane and goes to a per-warp staging buffer [pair][c] (the rotation wants all of ONE pair in a
+//              fragment, the pass produces four pairs side by side: the exchange has to cross lanes);
+//   product 1  T[m'][n]  = sum_n' g~[n'][m'] Uk[n'][n]        A' from the staging buffer, B' = embedding of U_k;
+//   product 2  |sum_m' T[m'][n] conj(Ukq[m'][m])|^2           T through a second staging buffer, B'' = conj(U_{k+q});
+// the U fragments of the four pairs stay in registers over all modes when Nb <= 8.
+// HBM traffic per pair: 32 Nb^2 (the two U) + 8 Nb^2 Nm (output) bytes; T2 (16 Nb^2 Nm L1 N2 N3 bytes per q) is L2-resident.
+// FP64 work per pair: 8 L1 Nb^2 Nm (pass) + 16 Nb^3 Nm (rotation) flops, all of it DMMA.
+#pragma once
+#include <type_traits>
+
+#include "common.cuh"
+#include "dmma_pipe.cuh"
+
+namespace epw {
+
+template <int NB>
+struct GF {
+  static constexpr int NBB = NB * NB;
+  static constexpr int KS = (2 * NB + 3) / 4;   // k-steps of 4 real of the two rotation products
+  static constexpr int NT = (2 * NB + 7) / 8;   // column tiles of 8 real
+  static constexpr int MTR = (NB + 7) / 8;      // row tiles of the rotation products per mode
+  static constexpr int MTP = (NBB + 7) / 8;     // row tiles (columns c of g~) of the pass per mode
+  static constexpr int NBP = NB + ((12 - (NB & 7)) & 7);     // row (n') pitch of the g~ staging buffer: = 4 (mod 8) complex
+  static constexpr int PST = NB * NBP + ((10 - ((NB * NBP) & 7)) & 7);   // pair stride of that buffer: = 2 (mod 8) complex
+  static constexpr int SP = NB + ((6 - (NB & 3)) & 3);       // row pitch of the T staging buffer: = 2 (mod 4) complex
+  static constexpr int TROWS = MTR * 8;
+  static constexpr bool UREG = NB <= 8;         // U fragments of the four pairs of a quad resident over all modes
+  static constexpr int UP = UREG ? 4 : 1;
+  static constexpr size_t warp_bytes = sizeof(c128) * (4 * (size_t)PST + (size_t)UP * TROWS * SP);
+  static_assert(2 * KS <= SP, "T pitch must cover the padded K range");
+};
+
+// row pitch of the T2 rows in shared memory: = 4 (mod 8) complex, so that the two rows (n1 = 2 ks, 2 ks + 1) a pass fragment
+// reads fall into different halves of the 32 banks
+__host__ __device__ constexpr int gf_row_pitch(int cols) { return cols + ((12 - (cols & 7)) & 7); }
+
+constexpr int GF_MAX_KSP = 8;   // k-steps of the pass: 2 L1 real <= 32, i.e. L1 <= 16
+constexpr int GF_WARPS = 8;     // warps of the one persistent CTA per SM
+constexpr int GF_MAX_BUF = 4;   // depth of the T2 tile ring
+
+struct GridFusedParams {
+  const c128 *T2;        // [L1][slab][ncols], g columns first
+  int64_t slab;
+  int ncols, L1, cnt;    // cnt: i1 planes of this chunk
+  const c128 *P1c;       // [L1][cnt]
+  int nquads, ngroups, nbuf;   // quads of four i1 in the chunk, mode groups per cell, depth of the T2 tile ring
+  const c128 *Uk, *Ukq;  // relative to the first k of the chunk (k = j*slab + cell)
+  const int32_t *kq_idx;
+  int nm, nug;           // modes, modes per CTA
+  const uint8_t *mask;
+  double *g2;            // NULL allowed when the consumer is on: |g|^2 then never leaves the SM
+  // NEXT-4 consumer folded into the epilogue of product 2 (consumer.cu has the formula, reading G18):
+  //   Im Sigma_nk += pi w_q / (s sqrt(pi)) sum_{m,nu} |g_mn nu|^2 [(n_nu + f_m) e^{-((e_n - e_m + w_nu)/s)^2} + (n_nu + 1 - f_m) e^{-((e_n - e_m - w_nu)/s)^2}]
+  double *cons_out;      // [k][Nb] relative to the chunk, NULL = consumer off
+  const double *eps_k;   // [k][Nb] relative to the chunk
+  const double *eps_kq;  // [k][Nb] relative to the chunk, or (kq_idx given) eps_k of ALL k, indexed through kq_idx
+  const double *omega_q; // [nm] of this q
+  const double *w_q;     // weights of the call's q-points or NULL (= 1)
+  int64_t iq;
+  double mu, kT, sigma;
+};
+
+// per-warp scratch of the consumer, in doubles: e_n, e_m, f_m of the four pairs [4][3][NB], then (omega, bose) of the tile's modes
+template <int NB>
+__host__ __device__ constexpr int gf_cons_doubles(int nug) { return 12 * NB + 2 * nug; }
+
+// embedding entry of a complex number z for fragment coordinates (a = real sub-row, b = real sub-column):
+//   [[re, im], [-im, re]]
+__device__ __forceinline__ double embed(c128 z, int a, int b) { return a == 0 ? (b ? z.y : z.x) : (b ? z.x : -z.y); }
+
+// Fragments of the embedding of U (or conj U) for the lane (g, t): entry (ks, nt) is +-(one component of U[r][c]),
+// r = 2 ks + t/2, c = 4 nt + g/2.  Component and sign depend on the lane only (a = t & 1, b = g & 1):
+//   U:       [[re, im], [-im, re]]   component a ^ b, negative where a = 1, b = 0
+//   conj U:  [[re, -im], [im, re]]   component a ^ b, negative where a = 0, b = 1
+// The loads come first and the sign is applied later (u_frag_sign: an integer XOR on the high word), so that nothing has
+// to wait for the loads before the first pass of an item has been issued.
+template <int NB>
+__device__ __forceinline__ void load_u_frag_raw(const c128 *__restrict__ u, int g, int t,
+                                                double (&b)[GF<NB>::KS][GF<NB>::NT]) {
+  typedef GF<NB> C;
+  const double *ud = reinterpret_cast<const double *>(u) + ((t & 1) ^ (g & 1));
+#pragma unroll
+  for (int ks = 0; ks < C::KS; ks++)
+#pragma unroll
+    for (int nt = 0; nt < C::NT; nt++) {
+      const int r = 2 * ks + (t >> 1), c = 4 * nt + (g >> 1);
+      b[ks][nt] = (r < NB && c < NB) ? ud[(r + NB * c) * 2] : 0.0;
+    }
+}
+template <int NB>
+__device__ __forceinline__ void u_frag_sign(bool conj, int g, int t, double (&b)[GF<NB>::KS][GF<NB>::NT]) {
+  typedef GF<NB> C;
+  const int a = t & 1, bb = g & 1;
+  const int flip = (conj ? (a == 0 && bb == 1) : (a == 1 && bb == 0)) ? (int)0x80000000 : 0;
+#pragma unroll
+  for (int ks = 0; ks < C::KS; ks++)
+#pragma unroll
+    for (int nt = 0; nt < C::NT; nt++)
+      b[ks][nt] = __hiloint2double(__double2hiint(b[ks][nt]) ^ flip, __double2loint(b[ks][nt]));
+}
+template <int NB>
+__device__ __forceinline__ void load_u_frag(const c128 *__restrict__ u, bool conj, int g, int t,
+                                            double (&b)[GF<NB>::KS][GF<NB>::NT]) {
+  load_u_frag_raw<NB>(u, g, t, b);
+  u_frag_sign<NB>(conj, g, t, b);
+}
+
+// e^-y for 0 <= y < 64 without the range checks of the library routine: y = k ln 2 + r (Cody-Waite, |r| <= ln 2 / 2),
+// e^-r by its Taylor polynomial of degree 12 (remainder 2e-16), 2^-k through the exponent field.
+__device__ __forceinline__ double exp_neg(double y) {
+  const double k = rint(y * 1.4426950408889634);
+  double r = fma(-k, 6.93147180369123816490e-01, y);
+  r = -fma(-k, 1.90821492927058770002e-10, r);   // r <- -(y - k ln 2)
+  double p = 1.0 / 479001600.0;
+  p = fma(p, r, 1.0 / 39916800.0);
+  p = fma(p, r, 1.0 / 3628800.0);
+  p = fma(p, r, 1.0 / 362880.0);
+  p = fma(p, r, 1.0 / 40320.0);
+  p = fma(p, r, 1.0 / 5040.0);
+  p = fma(p, r, 1.0 / 720.0);
+  p = fma(p, r, 1.0 / 120.0);
+  p = fma(p, r, 1.0 / 24.0);
+  p = fma(p, r, 1.0 / 6.0);
+  p = fma(p, r, 0.5);
+  p = fma(p, r, 1.0);
+  p = fma(p, r, 1.0);
+  return p * __hiloint2double((1023 - (int)k) << 20, 0);
+}
+
+// The two rotation products of ONE pair and ONE mode.  sG: this pair's g~ of the mode in the staging buffer [c = n' NB + m'],
+// sT: this pair's T buffer [n][m'] (pitch SP, padding rows / columns stay zero).
+template <int NB>
+__device__ __forceinline__ void product1(const double *__restrict__ sG, double *__restrict__ sT, int g, int t,
+                                         const double (&b1)[GF<NB>::KS][GF<NB>::NT]) {
+  typedef GF<NB> C;
+#pragma unroll
+  for (int mtr = 0; mtr < C::MTR; mtr++) {
+    const int mp = 8 * mtr + g;
+    double a[C::KS];
+#pragma unroll
+    for (int ks = 0; ks < C::KS; ks++) {
+      const int np_ = 2 * ks + (t >> 1);
+      a[ks] = (mp < NB && np_ < NB) ? sG[(np_ * C::NBP + mp) * 2 + (t & 1)] : 0.0;
+    }
+    double acc[C::NT][2];
+#pragma unroll
+    for (int nt = 0; nt < C::NT; nt++) acc[nt][0] = acc[nt][1] = 0.0;
+#pragma unroll
+    for (int ks = 0; ks < C::KS; ks++)
+#pragma unroll
+      for (int nt = 0; nt < C::NT; nt++) dmma884(acc[nt][0], acc[nt][1], a[ks], b1[ks][nt]);
+    // lane owns T[m' = mp][n = 4 nt + t]  ->  sT[n][m']
+    if (mp < NB) {
+#pragma unroll
+      for (int nt = 0; nt < C::NT; nt++) {
+        const int n = 4 * nt + t;
+        if (n < NB) *reinterpret_cast<double2 *>(sT + ((size_t)n * C::SP + mp) * 2) = make_double2(acc[nt][0], acc[nt][1]);
+      }
+    }
+  }
+}
+
+// cons (may be NULL): this pair's e_n [NB], e_m [NB], f_m [NB]; wb: (omega, bose) of this mode; the contribution of the
+// pair and mode to Im Sigma_n is reduced over the four lanes that share a row n and added to cdst[n] by one of them
+// (plain read-modify-write: the (pair, n) entries of a tile belong to this warp; atomic when modes are split over tiles)
+template <int NB>
+__device__ __forceinline__ void product2(const double *__restrict__ sT, double *__restrict__ dst, int g, int t,
+                                         const double (&b2)[GF<NB>::KS][GF<NB>::NT], bool store,
+                                         const double *__restrict__ cons = nullptr, const double *__restrict__ wb = nullptr,
+                                         double *__restrict__ cdst = nullptr, double inv_s = 0.0, double pref = 0.0,
+                                         bool atomic = false) {
+  typedef GF<NB> C;
+#pragma unroll
+  for (int mtr = 0; mtr < C::MTR; mtr++) {
+    const int n = 8 * mtr + g;
+    const double *arow = sT + (size_t)n * C::SP * 2 + t;
+    double acc[C::NT][2];
+#pragma unroll
+    for (int nt = 0; nt < C::NT; nt++) acc[nt][0] = acc[nt][1] = 0.0;
+#pragma unroll
+    for (int ks = 0; ks < C::KS; ks++) {
+      const double a = arow[4 * ks];
+#pragma unroll
+      for (int nt = 0; nt < C::NT; nt++) dmma884(acc[nt][0], acc[nt][1], a, b2[ks][nt]);
+    }
+    if (store && dst != nullptr && n < NB) {
+#pragma unroll
+      for (int nt = 0; nt < C::NT; nt++) {
+        const int m = 4 * nt + t;
+        if (m < NB) dst[n * NB + m] = acc[nt][0] * acc[nt][0] + acc[nt][1] * acc[nt][1];
+      }
+    }
+    if (cons != nullptr) {
+      // Every lane has 2 NT candidate terms (absorption and emission peak of each of its elements); a Gaussian below e^-50
+      // of its peak cannot reach the last bit of the sum (same cut as consumer.cu), and few survive.  The exponentials
+      // share the FP64 pipe with the DMMAs, so the warp evaluates them one ROUND at a time -- each lane its next surviving
+      // candidate -- and stops when no lane has one left (1-2 rounds where a fixed order would take 2 NT).
+      const double w = wb[0], bose = wb[1];
+      double y[2 * C::NT], cf[2 * C::NT];
+      unsigned pend = 0;
+#pragma unroll
+      for (int nt = 0; nt < C::NT; nt++) {
+        const int m = 4 * nt + t;
+        const bool on = store && n < NB && m < NB && w > 0.0;
+        const int mm = m < NB ? m : 0, nn = n < NB ? n : 0;
+        const double de_ = cons[nn] - cons[NB + mm], f = cons[2 * NB + mm];
+        const double xa = (de_ + w) * inv_s, xe = (de_ - w) * inv_s;
+        const double v = acc[nt][0] * acc[nt][0] + acc[nt][1] * acc[nt][1];
+        y[2 * nt] = xa * xa;
+        y[2 * nt + 1] = xe * xe;
+        cf[2 * nt] = v * (bose + f);
+        cf[2 * nt + 1] = v * (bose + 1.0 - f);
+        if (on && y[2 * nt] < 50.0) pend |= 1u << (2 * nt);
+        if (on && y[2 * nt + 1] < 50.0) pend |= 1u << (2 * nt + 1);
+      }
+      double sum = 0.0;
+      while (__any_sync(0xffffffffu, pend != 0)) {
+        const int b = __ffs(pend) - 1;   // -1: this lane has nothing left
+        double yy = 0.0, cc = 0.0;
+#pragma unroll
+        for (int i = 0; i < 2 * C::NT; i++)
+          if (b == i) { yy = y[i]; cc = cf[i]; }
+        sum = fma(cc, exp_neg(yy), sum);
+        pend &= pend - 1;
+      }
+      sum += __shfl_xor_sync(0xffffffffu, sum, 1);
+      sum += __shfl_xor_sync(0xffffffffu, sum, 2);
+      if (t == 0 && n < NB && sum != 0.0) {
+        if (atomic) atomicAdd(cdst + n, pref * sum);
+        else cdst[n] += pref * sum;
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// The kernel is PERSISTENT: one CTA of GF_WARPS warps per SM (255 registers per thread: the U fragments of a quad take
+// 128).  Work item = (cell, mode group, quad); the items are numbered with the quad fastest, every CTA takes one
+// contiguous range of them (equal to within one item) and deals it round-robin to its warps.  The T2 rows of a
+// (cell, mode group) tile arrive by bulk TMA in a ring of shared-memory buffers: full[buf] is an mbarrier the copies
+// complete on; a buffer is handed back by the last warp that leaves it (shared-memory counter), and that warp issues the
+// copies of the tile NBUF places further on.  So the T2 loads, the launch and the tail of a cell overlap the DMMAs of
+// the warps that are still at work, which a one-CTA-per-cell grid could not do (half the FP64 pipe idle at ten quads
+// per cell).
+// KSPMAX: k-steps of the pass the phase fragments are sized for (4: L1 <= 8, 8: L1 <= 16)
+// ---------------------------------------------------------------------------------------------------------------
+template <int NB, int KSPMAX, bool CONS>
+__global__ void __launch_bounds__(GF_WARPS * 32, 1) grid_fused_kernel(const GridFusedParams p) {
+  typedef GF<NB> C;
+  constexpr int NBB = C::NBB;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int g = lane >> 2, t = lane & 3;
+  const int L1 = p.L1, ksp = (L1 + 1) >> 1, L1e = 2 * ksp;
+  const int RP = gf_row_pitch(p.nug * NBB);                    // row pitch of a T2 buffer (complex)
+  const size_t buf_elems = (size_t)L1e * RP + 8;                // (+ 8 so that the ragged last pass tile stays inside)
+  const int64_t E = (int64_t)p.nm * NBB;
+  c128 *sT2 = reinterpret_cast<c128 *>(smem_raw);               // [nbuf][L1e][RP]
+  unsigned char *wbase = smem_raw + sizeof(c128) * buf_elems * p.nbuf;
+  const size_t wstride = C::warp_bytes + (CONS ? sizeof(double) * (size_t)((gf_cons_doubles<NB>(p.nug) + 1) & ~1) : 0);
+  double *sG = reinterpret_cast<double *>(wbase + (size_t)warp * wstride);         // [4 pairs][PST] complex
+  double *sT = sG + 4 * C::PST * 2;                                                // [UP pairs][TROWS][SP] complex
+  double *sC = sT + C::UP * C::TROWS * C::SP * 2;                                  // consumer scratch (CONS only)
+  uint64_t *full = reinterpret_cast<uint64_t *>(wbase + (size_t)GF_WARPS * wstride);   // [nbuf]
+  const double c_inv_s = CONS ? 1.0 / p.sigma : 0.0;
+  const double c_pref = CONS ? 3.14159265358979323846 * (p.w_q ? p.w_q[p.iq] : 1.0) * c_inv_s * 0.56418958354775628695 : 0.0;
+  const bool c_atomic = p.ngroups > 1;
+  int *cnt = reinterpret_cast<int *>(full + GF_MAX_BUF);                                      // [nbuf]
+
+  // ---- this CTA's items and tiles ----
+  const int64_t total = p.slab * p.ngroups * p.nquads;
+  const int64_t lo = total * blockIdx.x / gridDim.x, hi = total * (blockIdx.x + 1) / gridDim.x;
+  if (lo >= hi) return;
+  const int64_t tile_lo = lo / p.nquads;
+  const int ntiles = (int)((hi - 1) / p.nquads - tile_lo) + 1;
+
+  auto issue_tile = [&](int tr) {   // one thread: the L1 row copies of tile tile_lo + tr into its ring buffer
+    const int64_t tile = tile_lo + tr;
+    const int64_t cell = tile / p.ngroups;
+    const int nu0 = (int)(tile - cell * p.ngroups) * p.nug;
+    const int nuc = p.nm - nu0 < p.nug ? p.nm - nu0 : p.nug;
+    const int b = tr % p.nbuf;
+    const uint32_t bar = smem_u32(full + b);
+    const uint32_t row_bytes = (uint32_t)(sizeof(c128) * nuc * NBB);
+    mbar_expect_tx(bar, row_bytes * (uint32_t)L1);
+    c128 *dst = sT2 + buf_elems * b;
+    for (int n1 = 0; n1 < L1; n1++)
+      tma_bulk_g2s(smem_u32(dst + (size_t)n1 * RP), p.T2 + ((int64_t)n1 * p.slab + cell) * p.ncols + (int64_t)nu0 * NBB,
+                   row_bytes, bar);
+  };
+
+  if (threadIdx.x == 0) {
+    for (int b = 0; b < p.nbuf; b++) {
+      mbar_init(smem_u32(full + b), 1);
+      cnt[b] = 0;
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  // zero what the copies never write: the padding row n1 = L1 (odd L1) and the tail of every buffer; the T buffers
+  for (int b = 0; b < p.nbuf; b++) {
+    c128 *dst = sT2 + buf_elems * b;
+    for (int i = threadIdx.x; i < RP + 8; i += blockDim.x) {
+      if (L1e > L1 && i < RP) dst[(size_t)L1 * RP + i] = make_double2(0.0, 0.0);
+      if (i >= RP) dst[(size_t)L1e * RP + (i - RP)] = make_double2(0.0, 0.0);
+    }
+  }
+  for (int i = lane; i < C::UP * C::TROWS * C::SP * 2; i += 32) sT[i] = 0.0;
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  __syncthreads();
+  if (threadIdx.x == 0)
+    for (int tr = 0; tr < p.nbuf && tr < ntiles; tr++) issue_tile(tr);
+
+  int held = -1;   // tile (relative) whose buffer this warp is reading
+  auto acquire = [&](int tr) { mbar_wait(smem_u32(full + tr % p.nbuf), (uint32_t)((tr / p.nbuf) & 1)); };
+  auto release = [&](int tr) {
+    __syncwarp();
+    if (lane == 0) {
+      __threadfence_block();
+      const int b = tr % p.nbuf;
+      if (atomicAdd(cnt + b, 1) == GF_WARPS - 1) {   // last warp out: the buffer is free for the tile nbuf places on
+        atomicExch(cnt + b, 0);
+        if (tr + p.nbuf < ntiles) {
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic reads above, async-proxy writes below
+          issue_tile(tr + p.nbuf);
+        }
+      }
+    }
+  };
+  auto advance_to = [&](int tr) {
+    while (held < tr) {
+      if (held >= 0) release(held);
+      held++;
+      acquire(held);
+    }
+  };
+  // pair index of pair jj of an item, and the L2 prefetch of the two U matrices of the four pairs of the NEXT item
+  auto prefetch_u = [&](int64_t item) {
+    const int64_t tile = item / p.nquads;
+    const int quad = (int)(item - tile * p.nquads);
+    const int64_t cell = tile / p.ngroups;
+    const int jj = lane >> 3, line = lane & 7;    // 4 pairs x 8 lines of 128 bytes cover an 8 x 8 matrix; more lines below
+    const int j = 4 * quad + jj;
+    if (j < p.cnt) {
+      const int64_t k = (int64_t)j * p.slab + cell;
+      const char *a = reinterpret_cast<const char *>(p.Uk + k * NBB);
+      const char *b = reinterpret_cast<const char *>(p.Ukq + (p.kq_idx ? (int64_t)p.kq_idx[k] : k) * NBB);
+      for (int off = line * 128; off < (int)(sizeof(c128) * NBB); off += 8 * 128) {
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(a + off));
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(b + off));
+      }
+    }
+  };
+
+  for (int64_t item = lo + warp; item < hi; item += GF_WARPS) {
+    const int64_t tile = item / p.nquads;
+    const int quad = (int)(item - tile * p.nquads);
+    const int64_t cell = tile / p.ngroups;
+    const int nu0 = (int)(tile - cell * p.ngroups) * p.nug;
+    const int nuc = p.nm - nu0 < p.nug ? p.nm - nu0 : p.nug;
+    const int j0 = 4 * quad;
+    if (item + GF_WARPS < hi) prefetch_u(item + GF_WARPS);
+    // ---- per pair of the quad: index, validity, energy-window decision ----
+    int64_t kc[4];
+    bool live[4];
+    bool any = false;
+#pragma unroll
+    for (int jj = 0; jj < 4; jj++) {
+      const bool valid = j0 + jj < p.cnt;
+      kc[jj] = (int64_t)(valid ? j0 + jj : j0) * p.slab + cell;
+      live[jj] = valid && (p.mask == nullptr || p.mask[kc[jj]] != 0);
+      if (valid && !live[jj] && p.g2 != nullptr) {   // a skipped pair reports zeros
+        double *dz = p.g2 + kc[jj] * E + (int64_t)nu0 * NBB;
+        for (int i = lane; i < nuc * NBB; i += 32) dz[i] = 0.0;
+      }
+      any |= live[jj];
+    }
+    if (!any) continue;   // (a quad with some pairs skipped is computed whole; only its stores are predicated)
+    if (CONS) {
+      // e_n(k), e_m(k+q) and the Fermi factor of the final states for the four pairs; (omega, Bose factor) of the modes
+      for (int idx = lane; idx < 4 * NB; idx += 32) {
+        const int jj = idx / NB, i = idx - jj * NB;
+        const int64_t k = (int64_t)(j0 + jj < p.cnt ? j0 + jj : j0) * p.slab + cell;
+        const double e2 = (p.kq_idx ? p.eps_kq + (int64_t)p.kq_idx[k] * NB : p.eps_kq + k * NB)[i];
+        sC[jj * 3 * NB + i] = p.eps_k[k * NB + i];
+        sC[jj * 3 * NB + NB + i] = e2;
+        sC[jj * 3 * NB + 2 * NB + i] = 1.0 / (exp((e2 - p.mu) / p.kT) + 1.0);
+      }
+      for (int nl = lane; nl < nuc; nl += 32) {
+        const double w = p.omega_q[nu0 + nl];
+        sC[12 * NB + 2 * nl] = w;
+        sC[12 * NB + 2 * nl + 1] = w > 0.0 ? 1.0 / expm1(w / p.kT) : 0.0;
+      }
+    }
+    // ---- B' of the pass: 2x2 embedding of the phases p[n1][j] of the four pairs; fragment ks: k-row 4 ks + t, column g ----
+    double bp[KSPMAX];
+#pragma unroll
+    for (int ks = 0; ks < KSPMAX; ks++) {
+      const int n1 = 2 * ks + (t >> 1), j = j0 + (g >> 1);
+      c128 ph = make_double2(0.0, 0.0);
+      if (n1 < L1 && j < p.cnt) ph = p.P1c[(int64_t)n1 * p.cnt + j];
+      bp[ks] = embed(ph, t & 1, g & 1);
+    }
+    // ---- U fragments ----
+    double b1[C::UP][C::KS][C::NT], b2[C::UP][C::KS][C::NT];
+    const c128 *ukp[4], *ukqp[4];
+#pragma unroll
+    for (int jj = 0; jj < 4; jj++) {
+      ukp[jj] = p.Uk + kc[jj] * NBB;
+      ukqp[jj] = p.Ukq + (p.kq_idx ? (int64_t)p.kq_idx[kc[jj]] : kc[jj]) * NBB;
+    }
+    if (C::UREG) {
+#pragma unroll
+      for (int jj = 0; jj < 4; jj++) {
+        load_u_frag_raw<NB>(ukp[jj], g, t, b1[jj % C::UP]);
+        load_u_frag_raw<NB>(ukqp[jj], g, t, b2[jj % C::UP]);
+      }
+    }
+    advance_to((int)(tile - tile_lo));
+    const c128 *sT2b = sT2 + buf_elems * (held % p.nbuf);
+    // ---- pass: g~_j[c] for the four pairs and the NBB columns c of mode nul -> staging buffer [pair][n'][m'] ----
+    auto pass = [&](int nul, auto exact) {
+      const double *tsrc = reinterpret_cast<const double *>(sT2b + (size_t)(t >> 1) * RP + nul * NBB + g) + (t & 1);
+#pragma unroll
+      for (int mt0 = 0; mt0 < C::MTP; mt0 += 8) {
+        double acc[8][2];
+#pragma unroll
+        for (int i = 0; i < 8; i++) acc[i][0] = acc[i][1] = 0.0;
+#pragma unroll
+        for (int ks = 0; ks < KSPMAX; ks++) {
+          if (decltype(exact)::value || ks < ksp) {
+#pragma unroll
+            for (int i = 0; i < 8; i++) {
+              if (mt0 + i < C::MTP) {
+                const double a = tsrc[((size_t)2 * ks * RP + 8 * (mt0 + i)) * 2];
+                dmma884(acc[i][0], acc[i][1], a, bp[ks]);
+              }
+            }
+          }
+        }
+#pragma unroll
+        for (int i = 0; i < 8; i++) {
+          const int cl = 8 * (mt0 + i) + g;
+          if (mt0 + i < C::MTP && cl < NBB)
+            *reinterpret_cast<double2 *>(sG + ((size_t)t * C::PST + (cl / NB) * C::NBP + cl % NB) * 2) =
+                make_double2(acc[i][0], acc[i][1]);
+        }
+      }
+    };
+    const bool exact = ksp == KSPMAX;   // no k-step to skip: the common case, without the branches
+    if (exact) pass(0, std::true_type());
+    else pass(0, std::false_type());
+    if (C::UREG) {
+      // the first pass is on its way: now wait for the U loads and give the fragments their signs
+#pragma unroll
+      for (int jj = 0; jj < 4; jj++) {
+        u_frag_sign<NB>(false, g, t, b1[jj % C::UP]);
+        u_frag_sign<NB>(true, g, t, b2[jj % C::UP]);
+      }
+    }
+    __syncwarp();
+    for (int nul = 0; nul < nuc; nul++) {
+      if (C::UREG) {
+        // ---- product 1 of the four pairs (no branch inside: eight independent DMMA chains) ----
+#pragma unroll
+        for (int jj = 0; jj < 4; jj++)
+          product1<NB>(sG + (size_t)jj * C::PST * 2, sT + (size_t)(jj % C::UP) * C::TROWS * C::SP * 2, g, t, b1[jj % C::UP]);
+        __syncwarp();
+        // ---- product 2 and |.|^2 of this mode, and in the same stretch of code the pass of the NEXT mode: the staging
+        //      buffer of g~ is free once product 1 has read it, and the two are independent DMMA chains ----
+#pragma unroll
+        for (int jj = 0; jj < 4; jj++)
+          product2<NB>(sT + (size_t)(jj % C::UP) * C::TROWS * C::SP * 2,
+                       p.g2 ? p.g2 + kc[jj] * E + (int64_t)(nu0 + nul) * NBB : nullptr, g, t, b2[jj % C::UP], live[jj],
+                       CONS ? sC + jj * 3 * NB : nullptr, sC + 12 * NB + 2 * nul, CONS ? p.cons_out + kc[jj] * NB : nullptr,
+                       c_inv_s, c_pref, c_atomic);
+        if (nul + 1 < nuc) {
+          if (exact) pass(nul + 1, std::true_type());
+          else pass(nul + 1, std::false_type());
+        }
+        __syncwarp();
+      } else {
+        // Nb > 8: the fragments of one U matrix at a time (36 registers at Nb = 11), pair by pair
+#pragma unroll 1
+        for (int jj = 0; jj < 4; jj++) {
+          if (j0 + jj >= p.cnt) break;
+          const int64_t k = (int64_t)(j0 + jj) * p.slab + cell;
+          if (p.mask != nullptr && p.mask[k] == 0) continue;
+          load_u_frag<NB>(p.Uk + k * NBB, false, g, t, b1[0]);
+          product1<NB>(sG + (size_t)jj * C::PST * 2, sT, g, t, b1[0]);
+          __syncwarp();
+          load_u_frag<NB>(p.Ukq + (p.kq_idx ? (int64_t)p.kq_idx[k] : k) * NBB, true, g, t, b2[0]);
+          product2<NB>(sT, p.g2 ? p.g2 + k * E + (int64_t)(nu0 + nul) * NBB : nullptr, g, t, b2[0], true,
+                       CONS ? sC + jj * 3 * NB : nullptr, sC + 12 * NB + 2 * nul, CONS ? p.cons_out + k * NB : nullptr, c_inv_s,
+                       c_pref, c_atomic);
+          __syncwarp();
+        }
+        if (nul + 1 < nuc) {
+          if (exact) pass(nul + 1, std::true_type());
+          else pass(nul + 1, std::false_type());
+        }
+        __syncwarp();
+      }
+    }
+  }
+  // hand back every remaining tile of the CTA (a warp may have had no item in the last ones)
+  advance_to(ntiles - 1);
+  release(held);
+}
+
+// Modes per tile, ring depth and shared memory: all modes in one tile when a ring of two such tiles fits beside the
+// staging buffers (the U fragments are then loaded once per pair), else the largest mode group that does.
+template <int NB>
+static bool gf_plan(int nm, int L1, bool cons, int *nug_out, int *nbuf_out, size_t *smem_out) {
+  typedef GF<NB> C;
+  if (L1 < 1 || L1 > 2 * GF_MAX_KSP || nm < 1) return false;
+  const int L1e = 2 * ((L1 + 1) / 2);
+  const size_t limit = (size_t)225 * 1024;
+  for (int want_buf = 2; want_buf >= 1; want_buf--)
+    for (int n = nm; n >= 1; n--) {
+      const size_t wstride = C::warp_bytes + (cons ? sizeof(double) * (size_t)((gf_cons_doubles<NB>(n) + 1) & ~1) : 0);
+      const size_t fixed = (size_t)GF_WARPS * wstride + GF_MAX_BUF * (sizeof(uint64_t) + sizeof(int)) + 16;
+      const size_t per_buf = sizeof(c128) * ((size_t)L1e * gf_row_pitch(n * C::NBB) + 8);
+      if (fixed + want_buf * per_buf > limit) continue;
+      int nbuf = (int)((limit - fixed) / per_buf);
+      if (nbuf > GF_MAX_BUF) nbuf = GF_MAX_BUF;
+      *nug_out = n;
+      *nbuf_out = nbuf;
+      *smem_out = fixed + nbuf * per_buf;
+      return true;
+    }
+  return false;
+}
+
+template <int NB>
+static cudaError_t launch_gf(const GridFusedParams &p0, int num_sms, cudaStream_t st) {
+  GridFusedParams p = p0;
+  size_t smem = 0;
+  const bool cons = p.cons_out != nullptr;
+  if (!gf_plan<NB>(p.nm, p.L1, cons, &p.nug, &p.nbuf, &smem)) return cudaErrorInvalidConfiguration;
+  p.ngroups = (int)ceil_div(p.nm, p.nug);
+  p.nquads = (p.cnt + 3) / 4;
+  const int64_t total = p.slab * p.ngroups * p.nquads;
+  const int64_t want = ceil_div(total, GF_WARPS);
+  const unsigned grid = (unsigned)(want < num_sms ? want : num_sms);
+#define EPW_GF_LAUNCH(KSP_, CONS_)                                                                                    \
+  do {                                                                                                                \
+    cudaError_t e = cudaFuncSetAttribute(grid_fused_kernel<NB, KSP_, CONS_>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                                         (int)smem);                                                                  \
+    if (e != cudaSuccess) return e;                                                                                   \
+    grid_fused_kernel<NB, KSP_, CONS_><<<grid, GF_WARPS * 32, smem, st>>>(p);                                         \
+  } while (0)
+  if (p.L1 <= 8) {
+    if (cons) EPW_GF_LAUNCH(4, true);
+    else EPW_GF_LAUNCH(4, false);
+  } else {
+    if (cons) EPW_GF_LAUNCH(8, true);
+    else EPW_GF_LAUNCH(8, false);
+  }
+#undef EPW_GF_LAUNCH
+  return cudaGetLastError();
+}
+
+}  // namespace epw

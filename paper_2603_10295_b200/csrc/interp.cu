@@ -755,11 +755,11 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   { const int rc = h->s1_batch(nq, &QB); if (rc != EPW_OK) return rc; }
   const int64_t E = (int64_t)ncols_g;
   const size_t cap = h->cfg.workspace_bytes ? h->cfg.workspace_bytes : ((size_t)6 << 30);
-  // |g|^2 of pair (q, k0..): the caller's buffer, or (consumer on, g2 = NULL) the library's one-q scratch
-  if (!g2) CU_OR_FAIL(h, h->g2_scratch.reserve(sizeof(double) * (size_t)nk * E), "cudaMalloc |g|^2 scratch");
-  double *const g2_base = g2 ? g2 : h->g2_scratch.as<double>();
+  // |g|^2 of pair (q, k0..): the caller's buffer, or (consumer on, g2 = NULL) the library's one-q scratch -- or nothing at
+  // all when the consumer is folded into the one-kernel grid form (see below)
+  double *g2_base = g2;
   const int64_t g2_qs = g2 ? nk * E : 0;
-  auto G2 = [&](int64_t q, int64_t k0) { return g2_base + q * g2_qs + k0 * E; };
+  auto G2 = [&](int64_t q, int64_t k0) { return g2_base ? g2_base + q * g2_qs + k0 * E : nullptr; };
 
   int64_t kchunk, c_rows;
   int hbatch = 0;            // grid mode, one-kernel form: q-points whose H(k+q) side is taken in one go (0 = per q)
@@ -776,6 +776,10 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   const bool can_fuse = grid && grid_fused_supported(nb, nm, h->box_L[0]);
   const bool fused = can_fuse && ((h->cfg.flags & EPW_FLAG_GRID_FUSED) != 0 ||
                                   (nb <= 8 && (h->cfg.flags & EPW_FLAG_GRID_UNFUSED) == 0));
+  if (!g2 && !fused) {
+    CU_OR_FAIL(h, h->g2_scratch.reserve(sizeof(double) * (size_t)nk * E), "cudaMalloc |g|^2 scratch");
+    g2_base = h->g2_scratch.as<double>();
+  }
   const int ncolsC = fused ? ncols_h : ncols;   // columns of the [g~ | H(k+q)] buffer that reach HBM
   if (!grid) {
     // k-chunk: one chunk of [g~ | H(k+q)] (16*ncols bytes per k) must stay L2-resident for the eigensolve and the
@@ -1111,12 +1115,26 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
         } else {
           const int ci = (int)(k0 / kchunk);
           const int cnt = std::min(cs, grid->N[0] - ci * cs);
+          // the consumer, if on, is taken in the epilogue of the same kernel: |g|^2 goes from the accumulator registers into
+          // Im Sigma_nk, and with g2 = NULL nothing else leaves the SM
+          SelfEnergyFold fold;
+          if (h->cons.on) {
+            fold.out = h->cons.out + k0 * nb;
+            fold.eps_k = eps_k + k0 * nb;
+            fold.eps_kq = kq_map ? eps_k
+                                 : (eps_kq ? eps_kq + (q * nk + k0) * nb
+                                           : h->epskq_scratch.as<double>() + ((int64_t)hslot * nk + crow) * nb);
+            fold.omega_q = omega_q + q * nm;
+            fold.w_q = h->cons.w_q;
+            fold.iq = q;
+            fold.mu = h->cons.mu; fold.kT = h->cons.kT; fold.sigma = h->cons.sigma;
+          }
           LAUNCH(h, launch_grid_fused(h->T2.as<c128>(), slab, nc_g, L[0], h->P1raw.as<c128>() + (int64_t)ci * L[0] * cs,
                                           cnt, h->Uk.as<c128>() + k0 * nbb, Ukq_ptr, kq_idx, nb, nm, h->num_sms, mask,
-                                          G2(q, k0), st),
+                                          G2(q, k0), h->cons.on ? &fold : nullptr, st),
                  "grid_fused");
         }
-        if (h->cons.on) {
+        if (h->cons.on && !fused) {
           const double *ekq = kq_map ? nullptr
                                      : (eps_kq ? eps_kq + (q * nk + k0) * nb
                                                : h->epskq_scratch.as<double>() + ((int64_t)hslot * nk + crow) * nb);
@@ -1227,7 +1245,7 @@ static int interpolate_host_impl(epw_interp_t h, const double *k_list, const int
                                  int64_t nk, const double *q_list, int64_t nq, const int32_t *kq_map, double *eps_k,
                                  double *eps_kq, double *omega_q, double *g2, void *cuda_stream) {
   if (!h) return EPW_EINVAL;
-  if ((!k_list && !k_grid) || !q_list || !eps_k || !omega_q || !g2 || nk <= 0 || nq <= 0)
+  if ((!k_list && !k_grid) || !q_list || !eps_k || !omega_q || (!g2 && !h->cons.on) || nk <= 0 || nq <= 0)
     return h->fail(EPW_EINVAL, "epw_interp_interpolate_host: null pointer or non-positive nk/nq");
   CU_OR_FAIL(h, cudaSetDevice(h->cfg.device), "cudaSetDevice");
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
@@ -1238,7 +1256,7 @@ static int interpolate_host_impl(epw_interp_t h, const double *k_list, const int
   CU_OR_FAIL(h, h->hs_epsk.reserve(sizeof(double) * nk * h->nb), "cudaMalloc eps_k staging");
   if (eps_kq) CU_OR_FAIL(h, h->hs_epskq.reserve(sizeof(double) * nk * nq * h->nb), "cudaMalloc eps_kq staging");
   CU_OR_FAIL(h, h->hs_omega.reserve(sizeof(double) * nq * h->nm), "cudaMalloc omega staging");
-  CU_OR_FAIL(h, h->hs_g2.reserve(sizeof(double) * E * nk * nq), "cudaMalloc g2 staging");
+  if (g2) CU_OR_FAIL(h, h->hs_g2.reserve(sizeof(double) * E * nk * nq), "cudaMalloc g2 staging");
   if (k_list)
     CU_OR_FAIL(h, cudaMemcpyAsync(h->hs_k.p, k_list, sizeof(double) * 3 * nk, cudaMemcpyHostToDevice, st), "H2D k");
   CU_OR_FAIL(h, cudaMemcpyAsync(h->hs_q.p, q_list, sizeof(double) * 3 * nq, cudaMemcpyHostToDevice, st), "H2D q");
@@ -1254,10 +1272,10 @@ static int interpolate_host_impl(epw_interp_t h, const double *k_list, const int
   h->sink_ev_used = 0;
   const int rc = k_list ? epw_interp_interpolate(h, h->hs_k.as<double>(), nk, h->hs_q.as<double>(), nq, map_d,
                                                  h->hs_epsk.as<double>(), epskq_d, h->hs_omega.as<double>(),
-                                                 h->hs_g2.as<double>(), cuda_stream)
+                                                 g2 ? h->hs_g2.as<double>() : nullptr, cuda_stream)
                         : epw_interp_interpolate_grid(h, k_grid, k_shift, h->hs_q.as<double>(), nq, map_d,
                                                       h->hs_epsk.as<double>(), epskq_d, h->hs_omega.as<double>(),
-                                                      h->hs_g2.as<double>(), cuda_stream);
+                                                      g2 ? h->hs_g2.as<double>() : nullptr, cuda_stream);
   h->sink.active = false;
   if (rc != EPW_OK) {
     cudaStreamSynchronize(h->copy_stream);
@@ -1265,6 +1283,9 @@ static int interpolate_host_impl(epw_interp_t h, const double *k_list, const int
   }
   CU_OR_FAIL(h, cudaMemcpyAsync(eps_k, h->hs_epsk.p, sizeof(double) * nk * h->nb, cudaMemcpyDeviceToHost, st), "D2H eps_k");
   CU_OR_FAIL(h, cudaMemcpyAsync(omega_q, h->hs_omega.p, sizeof(double) * nq * h->nm, cudaMemcpyDeviceToHost, st), "D2H omega");
+  if (!g2 && eps_kq)   // (with g2 the eps_kq slices left with the |g|^2 of their q)
+    CU_OR_FAIL(h, cudaMemcpyAsync(eps_kq, h->hs_epskq.p, sizeof(double) * nk * nq * h->nb, cudaMemcpyDeviceToHost, st),
+               "D2H eps_kq");
   CU_OR_FAIL(h, cudaStreamSynchronize(h->copy_stream), "cudaStreamSynchronize(copy)");
   return epw_interp_sync(h);
 }

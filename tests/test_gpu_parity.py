@@ -898,9 +898,17 @@ def test_omega_min_cutoff_and_tiny_lists(epw, route):
 # ---------------------------------------------------------------------------------------------------------
 # NEXT-4: a consumer of |g|^2 on the device (Im Sigma_nk accumulator, reading G18)
 # ---------------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("mode", ["grid-fused-nog2", "grid-unfused", "list", "list-kqmap-nog2", "large", "large-nog2"])
+@pytest.mark.parametrize("mode", ["grid-fused-nog2", "grid-fused", "grid-fused-kqmap-nog2", "grid-fused-nb13-nog2",
+                                  "grid-unfused", "list", "list-kqmap-nog2", "large", "large-nog2"])
 def test_selfenergy_consumer(epw, mode):
-    if mode.startswith("large"):
+    """NEXT-4 consumer against oracle.selfenergy_accumulate in every kernel route.  grid-fused*: the reduction runs in the
+    epilogue of the one-kernel grid form (nb13: Nb = 13, Nm = 12, modes split over several tiles -> atomic adds); the other
+    routes reduce a one-q |g|^2 slab with a second kernel.  Tolerance 1e-8 of the largest entry (reading G18:
+    sums of up to Nq Nb Nm products of |g|^2, within 1e-9, and Gaussian weights evaluated in FP64 on both sides)."""
+    if "nb13" in mode:
+        w = synth.make_custom("modes", 13, 12, (3, 1, 0), 1.0, 0.1, 1.0, (10, 3, 1), ("random", 5, 2), seed=15)
+        ql, kq_map = w.q_list, None
+    elif mode.startswith("large"):
         w = synth.make_custom("zsnr-se", 18, 5, (2, 0, 0), 1.0, 0.05, 2.0, (24, 1, 1), ("random", 5, 1), seed=81)
         ql, kq_map = w.q_list, None
     else:
