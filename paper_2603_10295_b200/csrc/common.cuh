@@ -143,9 +143,8 @@ cudaError_t launch_box_scatter(const c128 *g1, const c128 *e, const double *omeg
                                const c128 *phase_qe, const double *w_e, const int32_t *box_idx, int64_t box_size, int nbb,
                                int nm, int ne, int ncols_g, int ncols_h, c128 *X, cudaStream_t st);
 cudaError_t launch_grid_axis_phase(int N, int i0, int cnt, double shift, int lo, int L, c128 *P, cudaStream_t st);
-// last axis pass of the grid form fused with S4b and |g|^2 (grid_rotate_g2.cu)
-bool grid_rotate_g2_supported(int nb, int nm, int L1);
-// the same on the FP64 tensor path throughout (grid_fused.cu): pass as a DMMA product over quads of i1, then S4b
+// last axis pass of the grid form, S4b and |g|^2 as one kernel on the FP64 tensor path (grid_fused.cuh): the pass as a DMMA
+// product over quads of i1, then the two rotation products; g~ never reaches HBM
 bool grid_fused_supported(int nb, int nm, int L1);
 // fold (may be NULL): the NEXT-4 consumer taken in the epilogue of the kernel (consumer.cu has the formula); with it g2 may be
 // NULL.  out, eps_k, eps_kq relative to the first k of the chunk; eps_kq = eps_k of all k when kq_idx is given.
@@ -158,9 +157,9 @@ struct SelfEnergyFold {
 cudaError_t launch_grid_fused(const c128 *T2, int64_t slab, int ncols, int L1, const c128 *P1c, int cnt, const c128 *Uk,
                               const c128 *Ukq, const int32_t *kq_idx, int nb, int nm, int num_sms, const uint8_t *mask,
                               double *g2, const SelfEnergyFold *fold, cudaStream_t st);
-cudaError_t launch_grid_rotate_g2(const c128 *T2, int64_t slab, int ncols, int L1, const c128 *P1c, int cnt,
-                                  const c128 *Uk, const c128 *Ukq, const int32_t *kq_idx, int nb, int nm, int num_sms,
-                                  const uint8_t *mask, double *g2, cudaStream_t st);
+// the last axis pass alone as the DMMA product of that kernel (same conditions as grid_fused_supported)
+cudaError_t launch_grid_pass_dmma(const c128 *T2, int64_t slab, int ncols, int L1, const c128 *P1c, int cnt, int nb, int nm,
+                                  int num_sms, c128 *gt, int64_t gt_stride, cudaStream_t st);
 // one axis pass as a streaming kernel (K = L_d <= 32); P c128 [K][N] row-major (unpacked phases)
 bool axis_pass_supported(int K);
 cudaError_t launch_axis_pass(const c128 *A, int64_t a_rb, int64_t a_bs, int64_t a_ks, int64_t M, const c128 *P, int K, int N,

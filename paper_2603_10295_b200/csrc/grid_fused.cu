@@ -9,13 +9,21 @@ cudaError_t launch_gf_nb5(int nb, const GridFusedParams &p, int num_sms, cudaStr
 cudaError_t launch_gf_nb9(int nb, const GridFusedParams &p, int num_sms, cudaStream_t st);
 cudaError_t launch_gf_nb13(int nb, const GridFusedParams &p, int num_sms, cudaStream_t st);
 
+static cudaError_t gf_dispatch(int nb, const GridFusedParams &p, int num_sms, cudaStream_t st) {
+  if (nb < 1 || nb > 16) return cudaErrorInvalidConfiguration;
+  if (nb <= 4) return launch_gf_nb1(nb, p, num_sms, st);
+  if (nb <= 8) return launch_gf_nb5(nb, p, num_sms, st);
+  if (nb <= 12) return launch_gf_nb9(nb, p, num_sms, st);
+  return launch_gf_nb13(nb, p, num_sms, st);
+}
+
 bool grid_fused_supported(int nb, int nm, int L1) {
   if (nb < 1 || nb > 16 || nm < 1) return false;
   int nug = 0, nbuf = 0;
   size_t smem = 0;
   switch (nb) {
 #define EPW_GF_CASE(NB_) \
-  case NB_: return gf_plan<NB_>(nm, L1, true, &nug, &nbuf, &smem);
+  case NB_: return gf_plan<NB_>(nm, L1, 1, &nug, &nbuf, &smem);
     EPW_GF_CASE(1) EPW_GF_CASE(2) EPW_GF_CASE(3) EPW_GF_CASE(4) EPW_GF_CASE(5) EPW_GF_CASE(6) EPW_GF_CASE(7) EPW_GF_CASE(8)
     EPW_GF_CASE(9) EPW_GF_CASE(10) EPW_GF_CASE(11) EPW_GF_CASE(12) EPW_GF_CASE(13) EPW_GF_CASE(14) EPW_GF_CASE(15)
     EPW_GF_CASE(16)
@@ -38,11 +46,17 @@ cudaError_t launch_grid_fused(const c128 *T2, int64_t slab, int ncols, int L1, c
     p.cons_out = fold->out; p.eps_k = fold->eps_k; p.eps_kq = fold->eps_kq; p.omega_q = fold->omega_q; p.w_q = fold->w_q;
     p.iq = fold->iq; p.mu = fold->mu; p.kT = fold->kT; p.sigma = fold->sigma;
   }
-  if (nb < 1 || nb > 16) return cudaErrorInvalidConfiguration;
-  if (nb <= 4) return launch_gf_nb1(nb, p, num_sms, st);
-  if (nb <= 8) return launch_gf_nb5(nb, p, num_sms, st);
-  if (nb <= 12) return launch_gf_nb9(nb, p, num_sms, st);
-  return launch_gf_nb13(nb, p, num_sms, st);
+  return gf_dispatch(nb, p, num_sms, st);
+}
+
+// The last axis pass ALONE as the same DMMA product: gt c128 [cnt*slab][gt_stride] <- g~ (first Nb^2 Nm columns of each row).
+cudaError_t launch_grid_pass_dmma(const c128 *T2, int64_t slab, int ncols, int L1, const c128 *P1c, int cnt, int nb, int nm,
+                                  int num_sms, c128 *gt, int64_t gt_stride, cudaStream_t st) {
+  if (slab <= 0 || cnt <= 0) return cudaSuccess;
+  if (gt == nullptr) return cudaErrorInvalidValue;
+  GridFusedParams p = {};
+  p.T2 = T2; p.slab = slab; p.ncols = ncols; p.L1 = L1; p.cnt = cnt; p.P1c = P1c; p.nm = nm; p.gt = gt; p.gt_stride = gt_stride;
+  return gf_dispatch(nb, p, num_sms, st);
 }
 
 }  // namespace epw

@@ -62,6 +62,8 @@ struct GridFusedParams {
   int nm, nug;           // modes, modes per CTA
   const uint8_t *mask;
   double *g2;            // NULL allowed when the consumer is on: |g|^2 then never leaves the SM
+  c128 *gt;              // pass-only variant: g~ [k][gt_stride] relative to the chunk (the g columns first)
+  int64_t gt_stride;
   // NEXT-4 consumer folded into the epilogue of product 2 (consumer.cu has the formula, reading G18):
   //   Im Sigma_nk += pi w_q / (s sqrt(pi)) sum_{m,nu} |g_mn nu|^2 [(n_nu + f_m) e^{-((e_n - e_m + w_nu)/s)^2} + (n_nu + 1 - f_m) e^{-((e_n - e_m - w_nu)/s)^2}]
   double *cons_out;      // [k][Nb] relative to the chunk, NULL = consumer off
@@ -257,9 +259,13 @@ __device__ __forceinline__ void product2(const double *__restrict__ sT, double *
 // per cell).
 // KSPMAX: k-steps of the pass the phase fragments are sized for (4: L1 <= 8, 8: L1 <= 16)
 // ---------------------------------------------------------------------------------------------------------------
-template <int NB, int KSPMAX, bool CONS>
+// VAR: 0 = pass + rotation + |g|^2;  1 = the same with the NEXT-4 consumer in the epilogue;  2 = the pass alone, g~ written
+// to global memory for rotate_g2.cu (the two-kernel form of 9 <= Nb <= 16: the streaming axis pass spends 4 L1 DFMA per
+// output element on the plain FP64 pipe and is bound by it at L1 = 13, the DMMA product is not)
+template <int NB, int KSPMAX, int VAR>
 __global__ void __launch_bounds__(GF_WARPS * 32, 1) grid_fused_kernel(const GridFusedParams p) {
   typedef GF<NB> C;
+  constexpr bool CONS = VAR == 1, PASS_ONLY = VAR == 2;
   constexpr int NBB = C::NBB;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -270,7 +276,7 @@ __global__ void __launch_bounds__(GF_WARPS * 32, 1) grid_fused_kernel(const Grid
   const int64_t E = (int64_t)p.nm * NBB;
   c128 *sT2 = reinterpret_cast<c128 *>(smem_raw);               // [nbuf][L1e][RP]
   unsigned char *wbase = smem_raw + sizeof(c128) * buf_elems * p.nbuf;
-  const size_t wstride = C::warp_bytes + (CONS ? sizeof(double) * (size_t)((gf_cons_doubles<NB>(p.nug) + 1) & ~1) : 0);
+  const size_t wstride = PASS_ONLY ? 0 : C::warp_bytes + (CONS ? sizeof(double) * (size_t)((gf_cons_doubles<NB>(p.nug) + 1) & ~1) : 0);
   double *sG = reinterpret_cast<double *>(wbase + (size_t)warp * wstride);         // [4 pairs][PST] complex
   double *sT = sG + 4 * C::PST * 2;                                                // [UP pairs][TROWS][SP] complex
   double *sC = sT + C::UP * C::TROWS * C::SP * 2;                                  // consumer scratch (CONS only)
@@ -317,7 +323,8 @@ __global__ void __launch_bounds__(GF_WARPS * 32, 1) grid_fused_kernel(const Grid
       if (i >= RP) dst[(size_t)L1e * RP + (i - RP)] = make_double2(0.0, 0.0);
     }
   }
-  for (int i = lane; i < C::UP * C::TROWS * C::SP * 2; i += 32) sT[i] = 0.0;
+  if (!PASS_ONLY)
+    for (int i = lane; i < C::UP * C::TROWS * C::SP * 2; i += 32) sT[i] = 0.0;
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   __syncthreads();
   if (threadIdx.x == 0)
@@ -371,7 +378,7 @@ __global__ void __launch_bounds__(GF_WARPS * 32, 1) grid_fused_kernel(const Grid
     const int nu0 = (int)(tile - cell * p.ngroups) * p.nug;
     const int nuc = p.nm - nu0 < p.nug ? p.nm - nu0 : p.nug;
     const int j0 = 4 * quad;
-    if (item + GF_WARPS < hi) prefetch_u(item + GF_WARPS);
+    if (!PASS_ONLY && item + GF_WARPS < hi) prefetch_u(item + GF_WARPS);
     // ---- per pair of the quad: index, validity, energy-window decision ----
     int64_t kc[4];
     bool live[4];
@@ -380,7 +387,7 @@ __global__ void __launch_bounds__(GF_WARPS * 32, 1) grid_fused_kernel(const Grid
     for (int jj = 0; jj < 4; jj++) {
       const bool valid = j0 + jj < p.cnt;
       kc[jj] = (int64_t)(valid ? j0 + jj : j0) * p.slab + cell;
-      live[jj] = valid && (p.mask == nullptr || p.mask[kc[jj]] != 0);
+      live[jj] = valid && (PASS_ONLY || p.mask == nullptr || p.mask[kc[jj]] != 0);
       if (valid && !live[jj] && p.g2 != nullptr) {   // a skipped pair reports zeros
         double *dz = p.g2 + kc[jj] * E + (int64_t)nu0 * NBB;
         for (int i = lane; i < nuc * NBB; i += 32) dz[i] = 0.0;
@@ -421,7 +428,7 @@ __global__ void __launch_bounds__(GF_WARPS * 32, 1) grid_fused_kernel(const Grid
       ukp[jj] = p.Uk + kc[jj] * NBB;
       ukqp[jj] = p.Ukq + (p.kq_idx ? (int64_t)p.kq_idx[kc[jj]] : kc[jj]) * NBB;
     }
-    if (C::UREG) {
+    if (C::UREG && !PASS_ONLY) {
 #pragma unroll
       for (int jj = 0; jj < 4; jj++) {
         load_u_frag_raw<NB>(ukp[jj], g, t, b1[jj % C::UP]);
@@ -453,12 +460,26 @@ __global__ void __launch_bounds__(GF_WARPS * 32, 1) grid_fused_kernel(const Grid
 #pragma unroll
         for (int i = 0; i < 8; i++) {
           const int cl = 8 * (mt0 + i) + g;
-          if (mt0 + i < C::MTP && cl < NBB)
-            *reinterpret_cast<double2 *>(sG + ((size_t)t * C::PST + (cl / NB) * C::NBP + cl % NB) * 2) =
-                make_double2(acc[i][0], acc[i][1]);
+          if (mt0 + i < C::MTP && cl < NBB) {
+            if (PASS_ONLY) {   // lane (g, t): g~ of pair t, column cl -- eight lanes write 128 contiguous bytes
+              if (j0 + t < p.cnt)
+                p.gt[((int64_t)(j0 + t) * p.slab + cell) * p.gt_stride + (int64_t)(nu0 + nul) * NBB + cl] =
+                    make_double2(acc[i][0], acc[i][1]);
+            } else {
+              *reinterpret_cast<double2 *>(sG + ((size_t)t * C::PST + (cl / NB) * C::NBP + cl % NB) * 2) =
+                  make_double2(acc[i][0], acc[i][1]);
+            }
+          }
         }
       }
     };
+    if (PASS_ONLY) {
+      for (int nul = 0; nul < nuc; nul++) {
+        if (ksp == KSPMAX) pass(nul, std::true_type());
+        else pass(nul, std::false_type());
+      }
+      continue;
+    }
     const bool exact = ksp == KSPMAX;   // no k-step to skip: the common case, without the branches
     if (exact) pass(0, std::true_type());
     else pass(0, std::false_type());
@@ -523,14 +544,15 @@ __global__ void __launch_bounds__(GF_WARPS * 32, 1) grid_fused_kernel(const Grid
 // Modes per tile, ring depth and shared memory: all modes in one tile when a ring of two such tiles fits beside the
 // staging buffers (the U fragments are then loaded once per pair), else the largest mode group that does.
 template <int NB>
-static bool gf_plan(int nm, int L1, bool cons, int *nug_out, int *nbuf_out, size_t *smem_out) {
+static bool gf_plan(int nm, int L1, int var, int *nug_out, int *nbuf_out, size_t *smem_out) {
   typedef GF<NB> C;
   if (L1 < 1 || L1 > 2 * GF_MAX_KSP || nm < 1) return false;
   const int L1e = 2 * ((L1 + 1) / 2);
   const size_t limit = (size_t)225 * 1024;
   for (int want_buf = 2; want_buf >= 1; want_buf--)
     for (int n = nm; n >= 1; n--) {
-      const size_t wstride = C::warp_bytes + (cons ? sizeof(double) * (size_t)((gf_cons_doubles<NB>(n) + 1) & ~1) : 0);
+      const size_t wstride =
+          var == 2 ? 0 : C::warp_bytes + (var == 1 ? sizeof(double) * (size_t)((gf_cons_doubles<NB>(n) + 1) & ~1) : 0);
       const size_t fixed = (size_t)GF_WARPS * wstride + GF_MAX_BUF * (sizeof(uint64_t) + sizeof(int)) + 16;
       const size_t per_buf = sizeof(c128) * ((size_t)L1e * gf_row_pitch(n * C::NBB) + 8);
       if (fixed + want_buf * per_buf > limit) continue;
@@ -548,8 +570,8 @@ template <int NB>
 static cudaError_t launch_gf(const GridFusedParams &p0, int num_sms, cudaStream_t st) {
   GridFusedParams p = p0;
   size_t smem = 0;
-  const bool cons = p.cons_out != nullptr;
-  if (!gf_plan<NB>(p.nm, p.L1, cons, &p.nug, &p.nbuf, &smem)) return cudaErrorInvalidConfiguration;
+  const int var = p.gt != nullptr ? 2 : (p.cons_out != nullptr ? 1 : 0);
+  if (!gf_plan<NB>(p.nm, p.L1, var, &p.nug, &p.nbuf, &smem)) return cudaErrorInvalidConfiguration;
   p.ngroups = (int)ceil_div(p.nm, p.nug);
   p.nquads = (p.cnt + 3) / 4;
   const int64_t total = p.slab * p.ngroups * p.nquads;
@@ -563,11 +585,13 @@ static cudaError_t launch_gf(const GridFusedParams &p0, int num_sms, cudaStream_
     grid_fused_kernel<NB, KSP_, CONS_><<<grid, GF_WARPS * 32, smem, st>>>(p);                                         \
   } while (0)
   if (p.L1 <= 8) {
-    if (cons) EPW_GF_LAUNCH(4, true);
-    else EPW_GF_LAUNCH(4, false);
+    if (var == 2) EPW_GF_LAUNCH(4, 2);
+    else if (var == 1) EPW_GF_LAUNCH(4, 1);
+    else EPW_GF_LAUNCH(4, 0);
   } else {
-    if (cons) EPW_GF_LAUNCH(8, true);
-    else EPW_GF_LAUNCH(8, false);
+    if (var == 2) EPW_GF_LAUNCH(8, 2);
+    else if (var == 1) EPW_GF_LAUNCH(8, 1);
+    else EPW_GF_LAUNCH(8, 0);
   }
 #undef EPW_GF_LAUNCH
   return cudaGetLastError();

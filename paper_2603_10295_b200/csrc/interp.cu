@@ -780,7 +780,7 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
     CU_OR_FAIL(h, h->g2_scratch.reserve(sizeof(double) * (size_t)nk * E), "cudaMalloc |g|^2 scratch");
     g2_base = h->g2_scratch.as<double>();
   }
-  const int ncolsC = fused ? ncols_h : ncols;   // columns of the [g~ | H(k+q)] buffer that reach HBM
+  int ncolsC = fused ? ncols_h : ncols;   // columns of the [g~ | H(k+q)] buffer that reach HBM (hbatch: g~ only, see below)
   if (!grid) {
     // k-chunk: one chunk of [g~ | H(k+q)] (16*ncols bytes per k) must stay L2-resident for the eigensolve and the
     // rotation that follow it, and its tile count should fill whole waves of the persistent contraction kernel
@@ -807,17 +807,19 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
     if (fit >= grid->N[0]) fit = grid->N[0];
     else if (fit > 64) fit = fit / 64 * 64;
     cs = (int)fit;
-    // One-kernel form with per-pair H(k+q): H(k+q) depends on q and H(Re) only, so its three axis passes and its
+    // Per-pair H(k+q) on a grid: H(k+q) depends on q and H(Re) only, so its three axis passes and its
     // eigensolves are taken for QBH q-points of the S1 batch AT ONCE, before the g passes of those q (one eigensolver
     // launch of QBH*nk matrices instead of QBH launches of nk: 64,000 solves are 3.4 batches per persistent group of the
     // thread-per-matrix kernel -- a quarter of the GPU idles through the last round of every launch).  Needs the
     // H(k+q), U_{k+q} (and eps) of QBH q within the workspace cap; otherwise the per-q, chunked form below runs.
-    if (fused && !kq_map) {
-      const size_t per_q = (size_t)nk * (2 * (size_t)nbb * 16 + (size_t)nb * 8);
+    if (!kq_map) {
+      // (the two-kernel form also keeps g~ of one q, all k, in the same workspace)
+      const size_t per_q = (size_t)nk * (2 * (size_t)nbb * 16 + (size_t)nb * 8 + (fused ? 0 : (size_t)ncols_g * 16));
       const size_t room = std::min(cap, (size_t)4 << 30);
       if (per_q <= room && axis_pass_supported(L[0]) && axis_pass_supported(L[1]) && axis_pass_supported(L[2])) {
         hbatch = (int)std::min<size_t>(room / per_q, (size_t)QB);
         cs = grid->N[0];
+        ncolsC = fused ? 0 : ncols_g;
       }
     }
     nchunks = (int)ceil_div(grid->N[0], cs);
@@ -859,7 +861,8 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   CU_OR_FAIL(h, h->eq.reserve(sizeof(c128) * (size_t)nq * nmm), "cudaMalloc e_q");
   if (!h->ext_g1) CU_OR_FAIL(h, h->g1.reserve(sizeof(c128) * (size_t)QB * h->rows), "cudaMalloc g(Re,q)");
   const size_t hb = hbatch ? hbatch : 1;
-  if (ncolsC) CU_OR_FAIL(h, h->C.reserve(sizeof(c128) * hb * (size_t)c_rows * ncolsC), "cudaMalloc g~");
+  if (ncolsC) CU_OR_FAIL(h, h->C.reserve(sizeof(c128) * (size_t)c_rows * ncolsC), "cudaMalloc g~");
+  if (hbatch) CU_OR_FAIL(h, h->Hkq.reserve(sizeof(c128) * hb * (size_t)nk * nbb), "cudaMalloc H(k+q)");
   if (!kq_map) CU_OR_FAIL(h, h->Ukq.reserve(sizeof(c128) * hb * (size_t)c_rows * nbb), "cudaMalloc Ukq");
   if (!kq_map && !eps_kq) CU_OR_FAIL(h, h->epskq_scratch.reserve(sizeof(double) * hb * (size_t)c_rows * nb), "cudaMalloc eps scratch");
   { const int rc = h->ensure_status(); if (rc != EPW_OK) return rc; }
@@ -1015,12 +1018,12 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
                  "box_scatter(H e^{iqR})");
         LAUNCH(h, grid_pass_ab(nbb, hn), "grid passes H(k+q)");
         LAUNCH(h, launch_axis_pass(h->T2.as<c128>(), Mh, (int64_t)L[0] * Mh, Mh, (int64_t)hn * Mh, h->P1raw.as<c128>(), L[0],
-                                   grid->N[0], h->C.as<c128>(), Mh, (int64_t)grid->N[0] * Mh, Mh, h->num_sms, st),
+                                   grid->N[0], h->Hkq.as<c128>(), Mh, (int64_t)grid->N[0] * Mh, Mh, h->num_sms, st),
                "grid pass H(k+q)");
         h->end_span(sp, st);
         sp = h->begin_span(5, st);
         double *eps_dst = eps_kq ? eps_kq + q * nk * nb : h->epskq_scratch.as<double>();
-        LAUNCH(h, launch_eigh_batched(h->C.as<c128>(), nbb, nb, (int64_t)hn * nk, eps_dst, h->Ukq.as<c128>(), 0,
+        LAUNCH(h, launch_eigh_batched(h->Hkq.as<c128>(), nbb, nb, (int64_t)hn * nk, eps_dst, h->Ukq.as<c128>(), 0,
                                       h->status.as<int32_t>(), h->eig_scratch.as<c128>(), h->work_slot(1), st),
                "eigh H(k+q)");
         h->end_span(sp, st);
@@ -1051,7 +1054,12 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
                                       KB, ncols, h->num_sms, st),
                  "zgemm S2");
         } else if (!fused) {
-          LAUNCH(h, grid_pass_c(ncols, (int)(k0 / kchunk), Cc), "grid pass S2");
+          if (hbatch && can_fuse)   // g columns only, all i1 planes: the pass as a DMMA product (grid_fused.cuh, pass-only form)
+            LAUNCH(h, launch_grid_pass_dmma(h->T2.as<c128>(), slab, nc_g, L[0], h->P1raw.as<c128>(), grid->N[0], nb, nm,
+                                            h->num_sms, Cc, nc_g, st),
+                   "grid pass S2 (DMMA)");
+          else
+            LAUNCH(h, grid_pass_c(nc_g, (int)(k0 / kchunk), Cc), "grid pass S2");
         } else if (ncols_h && !hbatch) {
           // fused form: only the H(k+q) columns of the last axis pass go to HBM (the eigensolver's input)
           const int ci = (int)(k0 / kchunk);
@@ -1109,7 +1117,7 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
         // ---- S4b: band rotation + |g|^2 ----
         sp = h->begin_span(6, st);
         if (!fused) {
-          LAUNCH(h, launch_rotate_g2(Cc, ncols, h->Uk.as<c128>() + k0 * nbb, Ukq_ptr, kq_idx, nb, nm, kn, mask,
+          LAUNCH(h, launch_rotate_g2(Cc, grid ? nc_g : ncols, h->Uk.as<c128>() + k0 * nbb, Ukq_ptr, kq_idx, nb, nm, kn, mask,
                                      G2(q, k0), st),
                  "rotate_g2");
         } else {
