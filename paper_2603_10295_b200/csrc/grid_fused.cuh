@@ -49,6 +49,7 @@ __host__ __device__ constexpr int gf_row_pitch(int cols) { return cols + ((12 - 
 
 constexpr int GF_MAX_KSP = 8;   // k-steps of the pass: 2 L1 real <= 32, i.e. L1 <= 16
 constexpr int GF_WARPS = 8;     // warps of the one persistent CTA per SM
+constexpr int GF_WARPS_PASS = 16;   // ... of the pass-only variant (no U fragments: 128 registers per thread are plenty)
 constexpr int GF_MAX_BUF = 4;   // depth of the T2 tile ring
 
 struct GridFusedParams {
@@ -263,9 +264,10 @@ __device__ __forceinline__ void product2(const double *__restrict__ sT, double *
 // to global memory for rotate_g2.cu (the two-kernel form of 9 <= Nb <= 16: the streaming axis pass spends 4 L1 DFMA per
 // output element on the plain FP64 pipe and is bound by it at L1 = 13, the DMMA product is not)
 template <int NB, int KSPMAX, int VAR>
-__global__ void __launch_bounds__(GF_WARPS * 32, 1) grid_fused_kernel(const GridFusedParams p) {
+__global__ void __launch_bounds__((VAR == 2 ? GF_WARPS_PASS : GF_WARPS) * 32, 1) grid_fused_kernel(const GridFusedParams p) {
   typedef GF<NB> C;
   constexpr bool CONS = VAR == 1, PASS_ONLY = VAR == 2;
+  constexpr int NW = PASS_ONLY ? GF_WARPS_PASS : GF_WARPS;
   constexpr int NBB = C::NBB;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -280,7 +282,7 @@ __global__ void __launch_bounds__(GF_WARPS * 32, 1) grid_fused_kernel(const Grid
   double *sG = reinterpret_cast<double *>(wbase + (size_t)warp * wstride);         // [4 pairs][PST] complex
   double *sT = sG + 4 * C::PST * 2;                                                // [UP pairs][TROWS][SP] complex
   double *sC = sT + C::UP * C::TROWS * C::SP * 2;                                  // consumer scratch (CONS only)
-  uint64_t *full = reinterpret_cast<uint64_t *>(wbase + (size_t)GF_WARPS * wstride);   // [nbuf]
+  uint64_t *full = reinterpret_cast<uint64_t *>(wbase + (size_t)NW * wstride);   // [nbuf]
   const double c_inv_s = CONS ? 1.0 / p.sigma : 0.0;
   const double c_pref = CONS ? 3.14159265358979323846 * (p.w_q ? p.w_q[p.iq] : 1.0) * c_inv_s * 0.56418958354775628695 : 0.0;
   const bool c_atomic = p.ngroups > 1;
@@ -337,7 +339,7 @@ __global__ void __launch_bounds__(GF_WARPS * 32, 1) grid_fused_kernel(const Grid
     if (lane == 0) {
       __threadfence_block();
       const int b = tr % p.nbuf;
-      if (atomicAdd(cnt + b, 1) == GF_WARPS - 1) {   // last warp out: the buffer is free for the tile nbuf places on
+      if (atomicAdd(cnt + b, 1) == NW - 1) {   // last warp out: the buffer is free for the tile nbuf places on
         atomicExch(cnt + b, 0);
         if (tr + p.nbuf < ntiles) {
           asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic reads above, async-proxy writes below
@@ -371,14 +373,14 @@ __global__ void __launch_bounds__(GF_WARPS * 32, 1) grid_fused_kernel(const Grid
     }
   };
 
-  for (int64_t item = lo + warp; item < hi; item += GF_WARPS) {
+  for (int64_t item = lo + warp; item < hi; item += NW) {
     const int64_t tile = item / p.nquads;
     const int quad = (int)(item - tile * p.nquads);
     const int64_t cell = tile / p.ngroups;
     const int nu0 = (int)(tile - cell * p.ngroups) * p.nug;
     const int nuc = p.nm - nu0 < p.nug ? p.nm - nu0 : p.nug;
     const int j0 = 4 * quad;
-    if (!PASS_ONLY && item + GF_WARPS < hi) prefetch_u(item + GF_WARPS);
+    if (!PASS_ONLY && item + NW < hi) prefetch_u(item + NW);
     // ---- per pair of the quad: index, validity, energy-window decision ----
     int64_t kc[4];
     bool live[4];
@@ -556,11 +558,15 @@ static bool gf_plan(int nm, int L1, int var, int *nug_out, int *nbuf_out, size_t
       const size_t fixed = (size_t)GF_WARPS * wstride + GF_MAX_BUF * (sizeof(uint64_t) + sizeof(int)) + 16;
       const size_t per_buf = sizeof(c128) * ((size_t)L1e * gf_row_pitch(n * C::NBB) + 8);
       if (fixed + want_buf * per_buf > limit) continue;
-      int nbuf = (int)((limit - fixed) / per_buf);
+      // equal mode groups (9 modes that fit four at a time go 3 + 3 + 3, not 4 + 4 + 1: the items are dealt by count)
+      const int groups = (nm + n - 1) / n;
+      n = (nm + groups - 1) / groups;
+      const size_t per_buf2 = sizeof(c128) * ((size_t)L1e * gf_row_pitch(n * C::NBB) + 8);
+      int nbuf = (int)((limit - fixed) / per_buf2);
       if (nbuf > GF_MAX_BUF) nbuf = GF_MAX_BUF;
+      *smem_out = fixed + nbuf * per_buf2;
       *nug_out = n;
       *nbuf_out = nbuf;
-      *smem_out = fixed + nbuf * per_buf;
       return true;
     }
   return false;
@@ -575,14 +581,15 @@ static cudaError_t launch_gf(const GridFusedParams &p0, int num_sms, cudaStream_
   p.ngroups = (int)ceil_div(p.nm, p.nug);
   p.nquads = (p.cnt + 3) / 4;
   const int64_t total = p.slab * p.ngroups * p.nquads;
-  const int64_t want = ceil_div(total, GF_WARPS);
+  const int nw = var == 2 ? GF_WARPS_PASS : GF_WARPS;
+  const int64_t want = ceil_div(total, nw);
   const unsigned grid = (unsigned)(want < num_sms ? want : num_sms);
 #define EPW_GF_LAUNCH(KSP_, CONS_)                                                                                    \
   do {                                                                                                                \
     cudaError_t e = cudaFuncSetAttribute(grid_fused_kernel<NB, KSP_, CONS_>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
                                          (int)smem);                                                                  \
     if (e != cudaSuccess) return e;                                                                                   \
-    grid_fused_kernel<NB, KSP_, CONS_><<<grid, GF_WARPS * 32, smem, st>>>(p);                                         \
+    grid_fused_kernel<NB, KSP_, CONS_><<<grid, nw * 32, smem, st>>>(p);                                         \
   } while (0)
   if (p.L1 <= 8) {
     if (var == 2) EPW_GF_LAUNCH(4, 2);
