@@ -39,7 +39,6 @@ struct GF {
   static constexpr int TROWS = MTR * 8;
   static constexpr bool UREG = NB <= 8;         // U fragments of the four pairs of a quad resident over all modes
   static constexpr int UP = UREG ? 4 : 1;
-  static constexpr size_t warp_bytes = sizeof(c128) * (4 * (size_t)PST + (size_t)UP * TROWS * SP);
   static_assert(2 * KS <= SP, "T pitch must cover the padded K range");
 };
 
@@ -48,7 +47,14 @@ struct GF {
 __host__ __device__ constexpr int gf_row_pitch(int cols) { return cols + ((12 - (cols & 7)) & 7); }
 
 constexpr int GF_MAX_KSP = 8;   // k-steps of the pass: 2 L1 real <= 32, i.e. L1 <= 16
-constexpr int GF_WARPS = 8;     // warps of the one persistent CTA per SM
+constexpr int GF_WARPS = 8;     // warps of the one persistent CTA per SM (one warp per quad)
+// Warps per quad.  With 2, each of two warps takes half of the pass tiles and rotates two of the four pairs: the U
+// fragments of a warp are then those of two pairs (64 registers) and twelve warps fit the register file (152 per thread)
+// where one warp per quad allows eight; the two meet at a named barrier twice per mode.  Measured: no gain -- 18.4 vs
+// 18.3 ms per 96 q on configs[1], 40.6 vs 38.4 ms per 13 q on configs[3], FP64 tensor pipe 70 % busy either way (the
+// short DMMA bursts between the staging steps limit it, not the number of warps) -- so one warp per quad stays.
+constexpr int GF_WPQ = 1;
+constexpr int GF_WARPS_PAIRED = 12;
 constexpr int GF_WARPS_PASS = 16;   // ... of the pass-only variant (no U fragments: 128 registers per thread are plenty)
 constexpr int GF_MAX_BUF = 4;   // depth of the T2 tile ring
 
@@ -76,9 +82,7 @@ struct GridFusedParams {
   double mu, kT, sigma;
 };
 
-// per-warp scratch of the consumer, in doubles: e_n, e_m, f_m of the four pairs [4][3][NB], then (omega, bose) of the tile's modes
-template <int NB>
-__host__ __device__ constexpr int gf_cons_doubles(int nug) { return 12 * NB + 2 * nug; }
+// (per-warp scratch of the consumer: e_n, e_m, f_m of the warp's pairs [pairs][3][NB], then (omega, bose) of the tile's modes)
 
 // embedding entry of a complex number z for fragment coordinates (a = real sub-row, b = real sub-column):
 //   [[re, im], [-im, re]]
@@ -263,11 +267,28 @@ __device__ __forceinline__ void product2(const double *__restrict__ sT, double *
 // VAR: 0 = pass + rotation + |g|^2;  1 = the same with the NEXT-4 consumer in the epilogue;  2 = the pass alone, g~ written
 // to global memory for rotate_g2.cu (the two-kernel form of 9 <= Nb <= 16: the streaming axis pass spends 4 L1 DFMA per
 // output element on the plain FP64 pipe and is bound by it at L1 = 13, the DMMA product is not)
+template <int NB, int VAR>
+struct GFShape {
+  static constexpr bool PASS_ONLY = VAR == 2;
+  static constexpr int WPQ = (GF<NB>::UREG && !PASS_ONLY) ? GF_WPQ : 1;       // warps per quad
+  static constexpr int NW = PASS_ONLY ? GF_WARPS_PASS : (WPQ == 2 ? GF_WARPS_PAIRED : GF_WARPS);
+  static constexpr int PPW = GF<NB>::UREG ? 4 / WPQ : 1;                      // pairs whose U fragments a warp holds
+  static constexpr int CPW = GF<NB>::UREG ? PPW : 4;                          // pairs in a warp's consumer table
+  // shared memory of one quad group (WPQ warps): g~ staging of the four pairs, then per warp its T buffers
+  static constexpr size_t t_bytes = sizeof(c128) * (size_t)PPW * GF<NB>::TROWS * GF<NB>::SP;
+  static constexpr size_t g_bytes = sizeof(c128) * 4 * (size_t)GF<NB>::PST;
+  __host__ __device__ static constexpr size_t cons_bytes(int nug) { return sizeof(double) * (size_t)((3 * CPW * NB + 2 * nug + 1) & ~1); }
+  __host__ __device__ static constexpr size_t group_bytes(int nug) {
+    return PASS_ONLY ? 0 : g_bytes + WPQ * (t_bytes + (VAR == 1 ? cons_bytes(nug) : 0));
+  }
+};
+
 template <int NB, int KSPMAX, int VAR>
-__global__ void __launch_bounds__((VAR == 2 ? GF_WARPS_PASS : GF_WARPS) * 32, 1) grid_fused_kernel(const GridFusedParams p) {
+__global__ void __launch_bounds__(GFShape<NB, VAR>::NW * 32, 1) grid_fused_kernel(const GridFusedParams p) {
   typedef GF<NB> C;
+  typedef GFShape<NB, VAR> S;
   constexpr bool CONS = VAR == 1, PASS_ONLY = VAR == 2;
-  constexpr int NW = PASS_ONLY ? GF_WARPS_PASS : GF_WARPS;
+  constexpr int NW = S::NW, WPQ = S::WPQ, PPW = S::PPW, NQG = NW / WPQ;
   constexpr int NBB = C::NBB;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -278,11 +299,18 @@ __global__ void __launch_bounds__((VAR == 2 ? GF_WARPS_PASS : GF_WARPS) * 32, 1)
   const int64_t E = (int64_t)p.nm * NBB;
   c128 *sT2 = reinterpret_cast<c128 *>(smem_raw);               // [nbuf][L1e][RP]
   unsigned char *wbase = smem_raw + sizeof(c128) * buf_elems * p.nbuf;
-  const size_t wstride = PASS_ONLY ? 0 : C::warp_bytes + (CONS ? sizeof(double) * (size_t)((gf_cons_doubles<NB>(p.nug) + 1) & ~1) : 0);
-  double *sG = reinterpret_cast<double *>(wbase + (size_t)warp * wstride);         // [4 pairs][PST] complex
-  double *sT = sG + 4 * C::PST * 2;                                                // [UP pairs][TROWS][SP] complex
-  double *sC = sT + C::UP * C::TROWS * C::SP * 2;                                  // consumer scratch (CONS only)
-  uint64_t *full = reinterpret_cast<uint64_t *>(wbase + (size_t)NW * wstride);   // [nbuf]
+  const int qgroup = warp / WPQ, half = warp - qgroup * WPQ;   // quad group of this warp, and which of its WPQ warps it is
+  const size_t gstride = S::group_bytes(p.nug);
+  const size_t wpart = S::t_bytes + (CONS ? S::cons_bytes(p.nug) : 0);
+  double *sG = reinterpret_cast<double *>(wbase + (size_t)qgroup * gstride);       // [4 pairs][PST] complex, shared by the group
+  double *sT = reinterpret_cast<double *>(wbase + (size_t)qgroup * gstride + S::g_bytes + (size_t)half * wpart);  // [PPW][TROWS][SP]
+  double *sC = sT + PPW * C::TROWS * C::SP * 2;                                    // consumer scratch (CONS only)
+  uint64_t *full = reinterpret_cast<uint64_t *>(wbase + (size_t)NQG * gstride);   // [nbuf]
+  // the warps of a quad group meet here (a warp alone: __syncwarp)
+  auto group_sync = [&]() {
+    if (WPQ == 1) __syncwarp();
+    else asm volatile("bar.sync %0, %1;" ::"r"(1 + qgroup), "n"(WPQ * 32) : "memory");
+  };
   const double c_inv_s = CONS ? 1.0 / p.sigma : 0.0;
   const double c_pref = CONS ? 3.14159265358979323846 * (p.w_q ? p.w_q[p.iq] : 1.0) * c_inv_s * 0.56418958354775628695 : 0.0;
   const bool c_atomic = p.ngroups > 1;
@@ -326,7 +354,7 @@ __global__ void __launch_bounds__((VAR == 2 ? GF_WARPS_PASS : GF_WARPS) * 32, 1)
     }
   }
   if (!PASS_ONLY)
-    for (int i = lane; i < C::UP * C::TROWS * C::SP * 2; i += 32) sT[i] = 0.0;
+    for (int i = lane; i < PPW * C::TROWS * C::SP * 2; i += 32) sT[i] = 0.0;
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   __syncthreads();
   if (threadIdx.x == 0)
@@ -373,14 +401,14 @@ __global__ void __launch_bounds__((VAR == 2 ? GF_WARPS_PASS : GF_WARPS) * 32, 1)
     }
   };
 
-  for (int64_t item = lo + warp; item < hi; item += NW) {
+  for (int64_t item = lo + qgroup; item < hi; item += NQG) {
     const int64_t tile = item / p.nquads;
     const int quad = (int)(item - tile * p.nquads);
     const int64_t cell = tile / p.ngroups;
     const int nu0 = (int)(tile - cell * p.ngroups) * p.nug;
     const int nuc = p.nm - nu0 < p.nug ? p.nm - nu0 : p.nug;
     const int j0 = 4 * quad;
-    if (!PASS_ONLY && item + NW < hi) prefetch_u(item + NW);
+    if (!PASS_ONLY && half == 0 && item + NQG < hi) prefetch_u(item + NQG);
     // ---- per pair of the quad: index, validity, energy-window decision ----
     int64_t kc[4];
     bool live[4];
@@ -390,27 +418,38 @@ __global__ void __launch_bounds__((VAR == 2 ? GF_WARPS_PASS : GF_WARPS) * 32, 1)
       const bool valid = j0 + jj < p.cnt;
       kc[jj] = (int64_t)(valid ? j0 + jj : j0) * p.slab + cell;
       live[jj] = valid && (PASS_ONLY || p.mask == nullptr || p.mask[kc[jj]] != 0);
-      if (valid && !live[jj] && p.g2 != nullptr) {   // a skipped pair reports zeros
+      if (valid && !live[jj] && p.g2 != nullptr && jj / (4 / WPQ) == half) {   // a skipped pair reports zeros
         double *dz = p.g2 + kc[jj] * E + (int64_t)nu0 * NBB;
         for (int i = lane; i < nuc * NBB; i += 32) dz[i] = 0.0;
       }
       any |= live[jj];
     }
     if (!any) continue;   // (a quad with some pairs skipped is computed whole; only its stores are predicated)
+    // the pairs this warp rotates: jj = half * PPW + jo
+    int64_t kcw[PPW];
+    bool livew[PPW];
+#pragma unroll
+    for (int jo = 0; jo < PPW; jo++) {
+      kcw[jo] = kc[jo];
+      livew[jo] = live[jo];
+#pragma unroll
+      for (int hh = 1; hh < WPQ; hh++)
+        if (half == hh) { kcw[jo] = kc[(hh * PPW + jo) & 3]; livew[jo] = live[(hh * PPW + jo) & 3]; }
+    }
     if (CONS) {
-      // e_n(k), e_m(k+q) and the Fermi factor of the final states for the four pairs; (omega, Bose factor) of the modes
-      for (int idx = lane; idx < 4 * NB; idx += 32) {
-        const int jj = idx / NB, i = idx - jj * NB;
+      // e_n(k), e_m(k+q) and the Fermi factor of the final states for this warp's pairs; (omega, Bose factor) of the modes
+      for (int idx = lane; idx < S::CPW * NB; idx += 32) {
+        const int jo = idx / NB, i = idx - jo * NB, jj = C::UREG ? half * PPW + jo : jo;
         const int64_t k = (int64_t)(j0 + jj < p.cnt ? j0 + jj : j0) * p.slab + cell;
         const double e2 = (p.kq_idx ? p.eps_kq + (int64_t)p.kq_idx[k] * NB : p.eps_kq + k * NB)[i];
-        sC[jj * 3 * NB + i] = p.eps_k[k * NB + i];
-        sC[jj * 3 * NB + NB + i] = e2;
-        sC[jj * 3 * NB + 2 * NB + i] = 1.0 / (exp((e2 - p.mu) / p.kT) + 1.0);
+        sC[jo * 3 * NB + i] = p.eps_k[k * NB + i];
+        sC[jo * 3 * NB + NB + i] = e2;
+        sC[jo * 3 * NB + 2 * NB + i] = 1.0 / (exp((e2 - p.mu) / p.kT) + 1.0);
       }
       for (int nl = lane; nl < nuc; nl += 32) {
         const double w = p.omega_q[nu0 + nl];
-        sC[12 * NB + 2 * nl] = w;
-        sC[12 * NB + 2 * nl + 1] = w > 0.0 ? 1.0 / expm1(w / p.kT) : 0.0;
+        sC[3 * S::CPW * NB + 2 * nl] = w;
+        sC[3 * S::CPW * NB + 2 * nl + 1] = w > 0.0 ? 1.0 / expm1(w / p.kT) : 0.0;
       }
     }
     // ---- B' of the pass: 2x2 embedding of the phases p[n1][j] of the four pairs; fragment ks: k-row 4 ks + t, column g ----
@@ -423,27 +462,25 @@ __global__ void __launch_bounds__((VAR == 2 ? GF_WARPS_PASS : GF_WARPS) * 32, 1)
       bp[ks] = embed(ph, t & 1, g & 1);
     }
     // ---- U fragments ----
-    double b1[C::UP][C::KS][C::NT], b2[C::UP][C::KS][C::NT];
-    const c128 *ukp[4], *ukqp[4];
-#pragma unroll
-    for (int jj = 0; jj < 4; jj++) {
-      ukp[jj] = p.Uk + kc[jj] * NBB;
-      ukqp[jj] = p.Ukq + (p.kq_idx ? (int64_t)p.kq_idx[kc[jj]] : kc[jj]) * NBB;
-    }
+    double b1[PPW][C::KS][C::NT], b2[PPW][C::KS][C::NT];
     if (C::UREG && !PASS_ONLY) {
 #pragma unroll
-      for (int jj = 0; jj < 4; jj++) {
-        load_u_frag_raw<NB>(ukp[jj], g, t, b1[jj % C::UP]);
-        load_u_frag_raw<NB>(ukqp[jj], g, t, b2[jj % C::UP]);
+      for (int jo = 0; jo < PPW; jo++) {
+        load_u_frag_raw<NB>(p.Uk + kcw[jo] * NBB, g, t, b1[jo]);
+        load_u_frag_raw<NB>(p.Ukq + (p.kq_idx ? (int64_t)p.kq_idx[kcw[jo]] : kcw[jo]) * NBB, g, t, b2[jo]);
       }
     }
     advance_to((int)(tile - tile_lo));
     const c128 *sT2b = sT2 + buf_elems * (held % p.nbuf);
     // ---- pass: g~_j[c] for the four pairs and the NBB columns c of mode nul -> staging buffer [pair][n'][m'] ----
+    // (the column tiles of a mode are split between the WPQ warps of the group: warp `half` takes tiles
+    //  half * MTW .. half * MTW + MTW - 1)
+    constexpr int MTW = (C::MTP + WPQ - 1) / WPQ;
     auto pass = [&](int nul, auto exact) {
       const double *tsrc = reinterpret_cast<const double *>(sT2b + (size_t)(t >> 1) * RP + nul * NBB + g) + (t & 1);
 #pragma unroll
-      for (int mt0 = 0; mt0 < C::MTP; mt0 += 8) {
+      for (int mt0 = 0; mt0 < MTW; mt0 += 8) {
+        const int mtb = half * MTW + mt0;   // first tile of this block of (up to) eight
         double acc[8][2];
 #pragma unroll
         for (int i = 0; i < 8; i++) acc[i][0] = acc[i][1] = 0.0;
@@ -452,8 +489,8 @@ __global__ void __launch_bounds__((VAR == 2 ? GF_WARPS_PASS : GF_WARPS) * 32, 1)
           if (decltype(exact)::value || ks < ksp) {
 #pragma unroll
             for (int i = 0; i < 8; i++) {
-              if (mt0 + i < C::MTP) {
-                const double a = tsrc[((size_t)2 * ks * RP + 8 * (mt0 + i)) * 2];
+              if (mt0 + i < MTW && (WPQ == 1 || mtb + i < C::MTP)) {
+                const double a = tsrc[((size_t)2 * ks * RP + 8 * (mtb + i)) * 2];
                 dmma884(acc[i][0], acc[i][1], a, bp[ks]);
               }
             }
@@ -461,8 +498,8 @@ __global__ void __launch_bounds__((VAR == 2 ? GF_WARPS_PASS : GF_WARPS) * 32, 1)
         }
 #pragma unroll
         for (int i = 0; i < 8; i++) {
-          const int cl = 8 * (mt0 + i) + g;
-          if (mt0 + i < C::MTP && cl < NBB) {
+          const int cl = 8 * (mtb + i) + g;
+          if (mt0 + i < MTW && mtb + i < C::MTP && cl < NBB) {
             if (PASS_ONLY) {   // lane (g, t): g~ of pair t, column cl -- eight lanes write 128 contiguous bytes
               if (j0 + t < p.cnt)
                 p.gt[((int64_t)(j0 + t) * p.slab + cell) * p.gt_stride + (int64_t)(nu0 + nul) * NBB + cl] =
@@ -488,32 +525,32 @@ __global__ void __launch_bounds__((VAR == 2 ? GF_WARPS_PASS : GF_WARPS) * 32, 1)
     if (C::UREG) {
       // the first pass is on its way: now wait for the U loads and give the fragments their signs
 #pragma unroll
-      for (int jj = 0; jj < 4; jj++) {
-        u_frag_sign<NB>(false, g, t, b1[jj % C::UP]);
-        u_frag_sign<NB>(true, g, t, b2[jj % C::UP]);
+      for (int jo = 0; jo < PPW; jo++) {
+        u_frag_sign<NB>(false, g, t, b1[jo]);
+        u_frag_sign<NB>(true, g, t, b2[jo]);
       }
     }
-    __syncwarp();
+    group_sync();   // g~ of mode 0 is complete (all tiles, from every warp of the group)
     for (int nul = 0; nul < nuc; nul++) {
       if (C::UREG) {
-        // ---- product 1 of the four pairs (no branch inside: eight independent DMMA chains) ----
+        // ---- product 1 of this warp's pairs (no branch inside: independent DMMA chains) ----
 #pragma unroll
-        for (int jj = 0; jj < 4; jj++)
-          product1<NB>(sG + (size_t)jj * C::PST * 2, sT + (size_t)(jj % C::UP) * C::TROWS * C::SP * 2, g, t, b1[jj % C::UP]);
-        __syncwarp();
+        for (int jo = 0; jo < PPW; jo++)
+          product1<NB>(sG + (size_t)(half * PPW + jo) * C::PST * 2, sT + (size_t)jo * C::TROWS * C::SP * 2, g, t, b1[jo]);
+        group_sync();   // T is written; every warp of the group has read g~ of this mode
         // ---- product 2 and |.|^2 of this mode, and in the same stretch of code the pass of the NEXT mode: the staging
         //      buffer of g~ is free once product 1 has read it, and the two are independent DMMA chains ----
 #pragma unroll
-        for (int jj = 0; jj < 4; jj++)
-          product2<NB>(sT + (size_t)(jj % C::UP) * C::TROWS * C::SP * 2,
-                       p.g2 ? p.g2 + kc[jj] * E + (int64_t)(nu0 + nul) * NBB : nullptr, g, t, b2[jj % C::UP], live[jj],
-                       CONS ? sC + jj * 3 * NB : nullptr, sC + 12 * NB + 2 * nul, CONS ? p.cons_out + kc[jj] * NB : nullptr,
-                       c_inv_s, c_pref, c_atomic);
+        for (int jo = 0; jo < PPW; jo++)
+          product2<NB>(sT + (size_t)jo * C::TROWS * C::SP * 2,
+                       p.g2 ? p.g2 + kcw[jo] * E + (int64_t)(nu0 + nul) * NBB : nullptr, g, t, b2[jo], livew[jo],
+                       CONS ? sC + jo * 3 * NB : nullptr, sC + 3 * S::CPW * NB + 2 * nul,
+                       CONS ? p.cons_out + kcw[jo] * NB : nullptr, c_inv_s, c_pref, c_atomic);
         if (nul + 1 < nuc) {
           if (exact) pass(nul + 1, std::true_type());
           else pass(nul + 1, std::false_type());
         }
-        __syncwarp();
+        group_sync();
       } else {
         // Nb > 8: the fragments of one U matrix at a time (36 registers at Nb = 11), pair by pair
 #pragma unroll 1
@@ -553,9 +590,10 @@ static bool gf_plan(int nm, int L1, int var, int *nug_out, int *nbuf_out, size_t
   const size_t limit = (size_t)225 * 1024;
   for (int want_buf = 2; want_buf >= 1; want_buf--)
     for (int n = nm; n >= 1; n--) {
-      const size_t wstride =
-          var == 2 ? 0 : C::warp_bytes + (var == 1 ? sizeof(double) * (size_t)((gf_cons_doubles<NB>(n) + 1) & ~1) : 0);
-      const size_t fixed = (size_t)GF_WARPS * wstride + GF_MAX_BUF * (sizeof(uint64_t) + sizeof(int)) + 16;
+      const size_t groups_bytes = var == 2 ? 0
+                                  : var == 1 ? (GFShape<NB, 1>::NW / GFShape<NB, 1>::WPQ) * GFShape<NB, 1>::group_bytes(n)
+                                             : (GFShape<NB, 0>::NW / GFShape<NB, 0>::WPQ) * GFShape<NB, 0>::group_bytes(n);
+      const size_t fixed = groups_bytes + GF_MAX_BUF * (sizeof(uint64_t) + sizeof(int)) + 16;
       const size_t per_buf = sizeof(c128) * ((size_t)L1e * gf_row_pitch(n * C::NBB) + 8);
       if (fixed + want_buf * per_buf > limit) continue;
       // equal mode groups (9 modes that fit four at a time go 3 + 3 + 3, not 4 + 4 + 1: the items are dealt by count)
@@ -581,8 +619,8 @@ static cudaError_t launch_gf(const GridFusedParams &p0, int num_sms, cudaStream_
   p.ngroups = (int)ceil_div(p.nm, p.nug);
   p.nquads = (p.cnt + 3) / 4;
   const int64_t total = p.slab * p.ngroups * p.nquads;
-  const int nw = var == 2 ? GF_WARPS_PASS : GF_WARPS;
-  const int64_t want = ceil_div(total, nw);
+  const int nw = var == 2 ? GFShape<NB, 2>::NW : GFShape<NB, 0>::NW;
+  const int64_t want = ceil_div(total, nw / GFShape<NB, 0>::WPQ);
   const unsigned grid = (unsigned)(want < num_sms ? want : num_sms);
 #define EPW_GF_LAUNCH(KSP_, CONS_)                                                                                    \
   do {                                                                                                                \
