@@ -59,6 +59,11 @@ def parse_args():
                     help="NEXT-1 (PAPER.md:L186-188): g(Re,Rp) split by Rp over the ranks; per step every rank contracts "
                          "its slabs for the q-points of ALL ranks, one NCCL reduce-scatter of g(Re,q) hands each rank the "
                          "summed g(Re,q) of its own q-points, and the rest of the path runs unchanged")
+    ap.add_argument("--rp-fused", action="store_true",
+                    help="with --rp-shard: the exchange step fused into the S1 kernel (epw_interp_rp_to_q_scatter_add): every "
+                         "rank adds its partial g(Re,q) straight into the owner's buffer over NVLink peer mappings "
+                         "(torch symmetric memory) instead of a reduce-scatter after the pass.  On one GPU the owner is "
+                         "this GPU; the multi-GPU branch has never run (one GPU per call here)")
     ap.add_argument("--grid-unfused", action="store_true", help="EPW_FLAG_GRID_UNFUSED: keep g~ in HBM between S2 and S4b")
     ap.add_argument("--grid-fused", action="store_true", help="EPW_FLAG_GRID_FUSED: force the fused last-pass + rotation kernel")
     ap.add_argument("--k-mode", default="grid", choices=["grid", "list"],
@@ -454,11 +459,32 @@ def run_config(args, ctx, cfg_index: int, steps: int, warmup: int, legs: set) ->
         q_all_dev = [torch.from_numpy(np.ascontiguousarray(
             w.q_list[np.concatenate([shard.q_block(s, world, r, nq_step, w.nq) for r in range(world)])])).cuda()
             for s in range(total_steps)]
-        g1_part = torch.empty((world * nq_step, rows, 2), dtype=torch.float64, device="cuda")
-        g1_mine = torch.empty((nq_step, rows, 2), dtype=torch.float64, device="cuda")
+        g1_part = None if args.rp_fused else torch.empty((world * nq_step, rows, 2), dtype=torch.float64, device="cuda")
+        symm = None
+        if args.rp_fused and world > 1:
+            # UNEXECUTED branch (no multi-GPU box in this run): the owners' buffers as symmetric memory, so that every rank
+            # holds a peer mapping of every other rank's buffer
+            import torch.distributed._symmetric_memory as symm_mem
+
+            g1_mine = symm_mem.empty((nq_step, rows, 2), dtype=torch.float64, device="cuda")
+            symm = symm_mem.rendezvous(g1_mine, dist.group.WORLD)
+            bases = [int(p_) for p_ in symm.buffer_ptrs]
+        else:
+            g1_mine = torch.empty((nq_step, rows, 2), dtype=torch.float64, device="cuda")
+            bases = [g1_mine.data_ptr()]
+        # q-point j of rank r's block lives in rank r's buffer, row block j
+        dst_ptrs = [bases[r] + j * rows * 16 for r in range(world) for j in range(nq_step)]
 
     def step(s, grid=None):
-        if args.rp_shard:
+        if args.rp_shard and args.rp_fused:
+            g1_mine.zero_()
+            if symm is not None:
+                symm.barrier()    # every owner has zeroed its buffer
+            epw.epw_interp_rp_to_q_scatter_add(h.h, q_all_dev[s], world * nq_step, dst_ptrs)
+            if symm is not None:
+                symm.barrier()    # every rank's additions have landed
+            epw.epw_interp_set_gq(h.h, g1_mine)
+        elif args.rp_shard:
             epw.epw_interp_rp_to_q_partial(h.h, q_all_dev[s], world * nq_step, g1_part)
             if world > 1:
                 dist.reduce_scatter_tensor(g1_mine, g1_part, op=dist.ReduceOp.SUM)   # the one exchange step, on the stream
@@ -706,7 +732,9 @@ def run_config(args, ctx, cfg_index: int, steps: int, warmup: int, legs: set) ->
             "config": {
                 "workload": f"BASELINE.json configs[{w.index}] {w.name}: Nb={w.nbnd} Nm={w.nmodes} Ne={w.ne} Np={w.np_} "
                             f"Nk={nk} ({'x'.join(map(str, w.k_grid))}), {nq_step} q per step per GPU ({w.q_desc})",
-                "global_batch_pairs": world * nk * nq_step, "parallelism": (f"g(Re,Rp) Rp-sharded x{world} + reduce-scatter of g(Re,q) over q" if args.rp_shard
+                "global_batch_pairs": world * nk * nq_step, "parallelism": ((f"g(Re,Rp) Rp-sharded x{world}, partial g(Re,q) added into the owners' buffers inside the S1 kernel (peer memory)"
+                                                                       if args.rp_fused else
+                                                                       f"g(Re,Rp) Rp-sharded x{world} + reduce-scatter of g(Re,q) over q") if args.rp_shard
                                                                       else f"q-sharded x{world}"),
                 "k_mode": ("uniform grid -> epw_interp_interpolate_grid" if use_grid else "k-list -> epw_interp_interpolate"),
                 "l2": "inputs larger than L2: g(Re,Rp) %.0f MB streamed per q-batch, phase table %.0f MB, |g|^2 output %.0f MB "

@@ -191,6 +191,18 @@ int epw_interp_set_selfenergy_consumer(epw_interp_t h, int enabled, double mu, d
  */
 int epw_interp_set_rp_shard(epw_interp_t h, int32_t ip_start, int32_t ip_count);
 int epw_interp_rp_to_q_partial(epw_interp_t h, const double *q_list, int64_t nq, void *g1_partial, void *cuda_stream);
+/*
+ * The same exchange step FUSED into the S1 pass (compute + collective in one kernel): S0 + S1 over the handle's slabs,
+ * with the partial g(Re,q) of q-point iq ADDED (red.global.add.f64, system scope) to dst[iq] instead of being stored.
+ *   dst   HOST array of nq DEVICE pointers, dst[iq] -> c128 [Nb^2 Nm Ne]: the buffer of the rank that owns q-point iq.  It
+ *         may be memory of ANOTHER GPU mapped into this process (NVLink peer access, CUDA IPC or symmetric memory): the
+ *         sums then cross NVLink row tile by row tile while g(Re,Rp) is still being streamed, and no collective follows.
+ * Every rank calls it with the same q_list and its own view of the same buffers; the owners zero their buffers before and
+ * all ranks synchronise after (barrier) before epw_interp_set_gq hands dst[own iq] to the rest of the path.  The order of
+ * the additions varies from run to run: the sum over ranks is reproducible to rounding only (W terms per element).
+ * (The paper: D2H of the partial y, mp_sum on the host.)  Asynchronous on cuda_stream.
+ */
+int epw_interp_rp_to_q_scatter_add(epw_interp_t h, const double *q_list, int64_t nq, void *const *dst, void *cuda_stream);
 int epw_interp_set_gq(epw_interp_t h, const void *g1_reduced);
 
 /* Wait for the handle's last enqueued work and report deferred device-side status (EPW_ENOTCONVERGED, EPW_ECUDA).

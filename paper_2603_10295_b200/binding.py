@@ -36,7 +36,7 @@ EXPORTED_SYMBOLS = [
     "epw_phase_table", "epw_rp_to_q", "epw_interp_operator", "epw_eigh_batched", "epw_eigh_batched_algo", "epw_zgemm", "epw_zgemm_strided",
     "epw_rotate_g2",
     "epw_eq6_unrotate", "epw_wannier_from_bloch",
-    "epw_interp_set_energy_window", "epw_interp_set_selfenergy_consumer", "epw_interp_set_rp_shard", "epw_interp_rp_to_q_partial", "epw_interp_set_gq",
+    "epw_interp_set_energy_window", "epw_interp_set_selfenergy_consumer", "epw_interp_set_rp_shard", "epw_interp_rp_to_q_partial", "epw_interp_rp_to_q_scatter_add", "epw_interp_set_gq",
     "epw_probe_peaks", "epw_version",
 ]
 
@@ -78,6 +78,7 @@ def load_library() -> ctypes.CDLL:
         L.epw_interp_set_selfenergy_consumer.argtypes = [vp, c_int, c_double, c_double, c_double, vp, vp]
         L.epw_interp_set_rp_shard.argtypes = [vp, c_int32, c_int32]
         L.epw_interp_rp_to_q_partial.argtypes = [vp, vp, c_int64, vp, vp]
+        L.epw_interp_rp_to_q_scatter_add.argtypes = [vp, vp, c_int64, vp, vp]
         L.epw_interp_set_gq.argtypes = [vp, vp]
         L.epw_interp_sync.argtypes = [vp]
         L.epw_interp_get_stage_times.argtypes = [vp, POINTER(c_double), c_int]
@@ -211,6 +212,12 @@ def epw_interp_set_rp_shard(h, ip_start, ip_count):
 def epw_interp_rp_to_q_partial(h, q_list, nq, g1_partial, stream=None):
     _check(load_library().epw_interp_rp_to_q_partial(h, _ptr(q_list), nq, _ptr(g1_partial),
                                                      _stream() if stream is None else stream), h)
+
+
+def epw_interp_rp_to_q_scatter_add(h, q_list, nq, dst_ptrs, stream=None):
+    """dst_ptrs: sequence of nq device pointers (ints) or tensors; see include/epw_interp.h."""
+    arr = (c_void_p * nq)(*[(_ptr(d) if not isinstance(d, int) else d) for d in dst_ptrs])
+    _check(load_library().epw_interp_rp_to_q_scatter_add(h, _ptr(q_list), nq, arr, _stream() if stream is None else stream), h)
 
 
 def epw_interp_set_gq(h, g1_reduced):

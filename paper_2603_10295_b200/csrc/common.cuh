@@ -85,6 +85,8 @@ cudaError_t launch_phase_table(const double *x, int64_t nx, const int32_t *R, co
 cudaError_t launch_phase_pack_a(const double *x, int64_t nx, const int32_t *R, const double *w, int nr, double *Apack,
                                 cudaStream_t st);
 cudaError_t launch_rp_to_q(const c128 *g, int64_t rows, int np, const c128 *Pq, int nq, c128 *g1, cudaStream_t st);
+cudaError_t launch_rp_to_q_dst(const c128 *g, int64_t rows, int np, const c128 *Pq, int nq, c128 *g1, c128 *const *dst_tab,
+                               cudaStream_t st);   // dst_tab != NULL: add the sums into dst_tab[iq] (peer memory allowed)
 int rp_to_q_max_nq(int np);   // q-points per pass whose phase table fits shared memory (<= 8; 0 = unsupported Np)
 cudaError_t launch_interp_operator(const c128 *OpR, int n, int nr, const c128 *P, int64_t nx, c128 *out,
                                    cudaStream_t st);

@@ -116,6 +116,7 @@ struct epw_interp {
   // valid for (grid sizes, shift, operators epoch); any k-list call or new operators drop it
   struct KSide { bool valid = false, with_conj = false; int32_t N[3] = {0, 0, 0}; double s[3] = {0, 0, 0}; uint64_t epoch = 0; } kside;
   uint64_t op_epoch = 0;
+  DevBuf dst_tab;     // destination pointers of epw_interp_rp_to_q_scatter_add
   DevBuf epsk_keep;   // eps_k of the cached k side (the caller's buffer is refilled from it)
   int64_t last_eq_slot = 0;  // slot of the last q of the last call inside the e_q buffer (debug getter)
   // host-entry output drain: while a host-buffer call runs, the |g|^2 and eps_kq slices of every finished q are copied
@@ -572,7 +573,7 @@ void epw_interp_destroy(epw_interp_t h) {
   DevBuf *all[] = {&h->g, &h->H, &h->D, &h->Re, &h->Rp, &h->we, &h->wp, &h->ones, &h->Apack, &h->BpackH, &h->Hk,
                    &h->Uk, &h->Pq, &h->Pqe, &h->Dq, &h->eq, &h->g1, &h->Bpack, &h->C, &h->Ukq, &h->epskq_scratch,
                    &h->status, &h->eig_scratch, &h->hs_k, &h->hs_q, &h->hs_map, &h->hs_epsk, &h->hs_epskq,
-                   &h->hs_omega, &h->hs_g2, &h->epsk_keep, &h->Pk, &h->BpackPk, &h->UpackK, &h->UpackKH, &h->BpackE,
+                   &h->hs_omega, &h->hs_g2, &h->epsk_keep, &h->dst_tab, &h->Pk, &h->BpackPk, &h->UpackK, &h->UpackKH, &h->BpackE,
                    &h->ghat, &h->T, &h->Hkq, &h->boxidx, &h->X, &h->T1, &h->T2, &h->Ptmp, &h->P1raw, &h->P2raw, &h->P3raw, &h->P1pack, &h->P2pack,
                    &h->P3pack, &h->klist_gen, &h->workctr, &h->maskbuf, &h->g2_scratch};
   for (DevBuf *b : all) b->release();
@@ -1197,9 +1198,26 @@ int epw_interp_set_rp_shard(epw_interp_t h, int32_t ip_start, int32_t ip_count) 
   return EPW_OK;
 }
 
+static int rp_to_q_partial_impl(epw_interp_t h, const double *q_list, int64_t nq, void *g1_partial, void *const *dst,
+                               void *cuda_stream);
+
 int epw_interp_rp_to_q_partial(epw_interp_t h, const double *q_list, int64_t nq, void *g1_partial, void *cuda_stream) {
   if (!h) return EPW_EINVAL;
-  if (!q_list || !g1_partial || nq <= 0) return h->fail(EPW_EINVAL, "epw_interp_rp_to_q_partial: null pointer or nq <= 0");
+  if (!g1_partial) return h->fail(EPW_EINVAL, "epw_interp_rp_to_q_partial: null output pointer");
+  return rp_to_q_partial_impl(h, q_list, nq, g1_partial, nullptr, cuda_stream);
+}
+
+int epw_interp_rp_to_q_scatter_add(epw_interp_t h, const double *q_list, int64_t nq, void *const *dst, void *cuda_stream) {
+  if (!h) return EPW_EINVAL;
+  if (!dst) return h->fail(EPW_EINVAL, "epw_interp_rp_to_q_scatter_add: null destination table");
+  for (int64_t i = 0; i < nq; i++)
+    if (!dst[i]) return h->fail(EPW_EINVAL, "epw_interp_rp_to_q_scatter_add: null destination pointer");
+  return rp_to_q_partial_impl(h, q_list, nq, nullptr, dst, cuda_stream);
+}
+
+static int rp_to_q_partial_impl(epw_interp_t h, const double *q_list, int64_t nq, void *g1_partial, void *const *dst,
+                               void *cuda_stream) {
+  if (!q_list || nq <= 0) return h->fail(EPW_EINVAL, "epw_interp_rp_to_q_partial: null pointer or nq <= 0");
   if (!h->operators_set) return h->fail(EPW_EINVAL, "epw_interp_rp_to_q_partial: operators not set");
   for (int ip = h->rp_lo; ip < h->rp_lo + h->rp_cnt; ip++)
     if (!h->slab_set[ip]) return h->fail(EPW_EINVAL, "epw_interp_rp_to_q_partial: g(Re,Rp) slab of this shard missing");
@@ -1211,6 +1229,15 @@ int epw_interp_rp_to_q_partial(epw_interp_t h, const double *q_list, int64_t nq,
   { const int rc = h->s1_batch(nq, &QB); if (rc != EPW_OK) return rc; }
   CU_OR_FAIL(h, h->Pq.reserve(sizeof(c128) * (size_t)QB * h->np), "cudaMalloc Pq");
   c128 *out = reinterpret_cast<c128 *>(g1_partial);
+  c128 *const *dst_dev = nullptr;
+  if (dst) {
+    // the destination table on the device (the copy is ordered on the stream; the host array may be reused on return)
+    CU_OR_FAIL(h, h->dst_tab.reserve(sizeof(void *) * (size_t)nq), "cudaMalloc destination table");
+    CU_OR_FAIL(h, cudaMemcpyAsync(h->dst_tab.p, dst, sizeof(void *) * (size_t)nq, cudaMemcpyHostToDevice, st),
+               "cudaMemcpy destination table");
+    CU_OR_FAIL(h, cudaStreamSynchronize(st), "cudaStreamSynchronize");
+    dst_dev = h->dst_tab.as<c128 *>();
+  }
   for (int64_t q0 = 0; q0 < nq; q0 += QB) {
     const int qb = (int)std::min<int64_t>(QB, nq - q0);
     int sp = h->begin_span(0, st);
@@ -1220,7 +1247,8 @@ int epw_interp_rp_to_q_partial(epw_interp_t h, const double *q_list, int64_t nq,
            "phase_table(q,Rp shard)");
     h->end_span(sp, st);
     sp = h->begin_span(1, st);
-    LAUNCH(h, launch_rp_to_q(h->g.as<c128>(), h->rows, h->rp_cnt, h->Pq.as<c128>(), qb, out + q0 * h->rows, st),
+    LAUNCH(h, launch_rp_to_q_dst(h->g.as<c128>(), h->rows, h->rp_cnt, h->Pq.as<c128>(), qb, out ? out + q0 * h->rows : nullptr,
+                                 dst_dev ? dst_dev + q0 : nullptr, st),
            "rp_to_q (partial)");
     h->end_span(sp, st);
   }

@@ -10,9 +10,26 @@
 
 namespace epw {
 
+// Where the sum of a row goes.  Normally g1[iq][row].  With a destination table (the Rp-sharded form, PAPER.md:L186-188,
+// L514-522) the partial sum of this GPU's lattice vectors is ADDED to dst_tab[iq][row] instead -- dst_tab[iq] is the
+// buffer of the rank that owns q-point iq and may be PEER memory (NVLink P2P mapping): the exchange step of the sharded
+// path (a reduce-scatter over q of the partial g(Re,q)) then happens inside the streaming pass, row tile by row tile,
+// as red.global.add.f64 at system scope, instead of as a collective after it.
+__device__ __forceinline__ void emit_row(c128 *__restrict__ g1, c128 *const *__restrict__ dst_tab, int iq, int64_t rows,
+                                         int64_t row, c128 v) {
+  if (dst_tab == nullptr) {
+    g1[(int64_t)iq * rows + row] = v;
+  } else {
+    double *d = reinterpret_cast<double *>(dst_tab[iq] + row);
+    atomicAdd_system(d, v.x);
+    atomicAdd_system(d + 1, v.y);
+  }
+}
+
 template <int NQ>
 __global__ void __launch_bounds__(256) rp_to_q_kernel(const c128 *__restrict__ g, int64_t rows, int np,
-                                                      const c128 *__restrict__ Pq, c128 *__restrict__ g1) {
+                                                      const c128 *__restrict__ Pq, c128 *__restrict__ g1,
+                                                      c128 *const *__restrict__ dst_tab) {
   extern __shared__ double2 sP[];  // [np][NQ]
   for (int e = threadIdx.x; e < np * NQ; e += blockDim.x) {
     const int ip = e / NQ, iq = e - ip * NQ;
@@ -55,7 +72,7 @@ __global__ void __launch_bounds__(256) rp_to_q_kernel(const c128 *__restrict__ g
     for (int iq = 0; iq < NQ; iq++) cfma(acc[iq], v, sP[ip * NQ + iq]);
   }
 #pragma unroll
-  for (int iq = 0; iq < NQ; iq++) g1[(int64_t)iq * rows + row] = acc[iq];
+  for (int iq = 0; iq < NQ; iq++) emit_row(g1, dst_tab, iq, rows, row, acc[iq]);
 }
 
 // NQ >= 5: bulk-TMA staged variant.  With 8 q per pass the arithmetic of one Rp block (32 DFMA per 16 bytes) takes as
@@ -73,7 +90,7 @@ constexpr int RP_THREADS = RP_MAX_RB + 32;
 template <int NQ>
 __global__ void __launch_bounds__(RP_THREADS, 1)
     rp_to_q_tma_kernel(const c128 *__restrict__ g, int64_t rows, int np, const c128 *__restrict__ Pq,
-                       c128 *__restrict__ g1, int RB, int64_t num_tiles) {
+                       c128 *__restrict__ g1, c128 *const *__restrict__ dst_tab, int RB, int64_t num_tiles) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   c128 *ring = reinterpret_cast<c128 *>(smem_raw);                                        // [STAGES][IPS][RB]
   uint64_t *bars = reinterpret_cast<uint64_t *>(smem_raw + sizeof(c128) * (size_t)RP_STAGES * RP_IPS * RB);
@@ -154,16 +171,18 @@ __global__ void __launch_bounds__(RP_THREADS, 1)
     }
     if (valid) {
 #pragma unroll
-      for (int iq = 0; iq < NQ; iq++) g1[(int64_t)iq * rows + row] = acc[iq];
+      for (int iq = 0; iq < NQ; iq++) emit_row(g1, dst_tab, iq, rows, row, acc[iq]);
     }
   }
 }
 
 template <int NQ>
-static cudaError_t launch_nq(const c128 *g, int64_t rows, int np, const c128 *Pq, c128 *g1, cudaStream_t st);
+static cudaError_t launch_nq(const c128 *g, int64_t rows, int np, const c128 *Pq, c128 *g1, c128 *const *dst_tab,
+                             cudaStream_t st);
 
 template <int NQ>
-static cudaError_t launch_nq_tma(const c128 *g, int64_t rows, int np, const c128 *Pq, c128 *g1, cudaStream_t st) {
+static cudaError_t launch_nq_tma(const c128 *g, int64_t rows, int np, const c128 *Pq, c128 *g1, c128 *const *dst_tab,
+                                 cudaStream_t st) {
   const int nsm = device_sm_count();
   // row-tile height: the multiple of 32 in [256, 512] whose tile count fills whole waves best
   int RB = RP_MAX_RB;
@@ -175,23 +194,24 @@ static cudaError_t launch_nq_tma(const c128 *g, int64_t rows, int np, const c128
   }
   const size_t smem = sizeof(c128) * (size_t)RP_STAGES * RP_IPS * RB + 2 * RP_STAGES * sizeof(uint64_t) +
                       sizeof(double2) * (size_t)np * NQ;
-  if (smem > (size_t)225 * 1024 || rows < 4 * (int64_t)nsm * 32) return launch_nq<NQ>(g, rows, np, Pq, g1, st);
+  if (smem > (size_t)225 * 1024 || rows < 4 * (int64_t)nsm * 32) return launch_nq<NQ>(g, rows, np, Pq, g1, dst_tab, st);
   cudaError_t e = cudaFuncSetAttribute(rp_to_q_tma_kernel<NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   const int64_t tiles = ceil_div(rows, RB);
   const int grid = (int)(tiles < nsm ? tiles : nsm);
-  rp_to_q_tma_kernel<NQ><<<grid, RP_THREADS, smem, st>>>(g, rows, np, Pq, g1, RB, tiles);
+  rp_to_q_tma_kernel<NQ><<<grid, RP_THREADS, smem, st>>>(g, rows, np, Pq, g1, dst_tab, RB, tiles);
   return cudaGetLastError();
 }
 
 template <int NQ>
-static cudaError_t launch_nq(const c128 *g, int64_t rows, int np, const c128 *Pq, c128 *g1, cudaStream_t st) {
+static cudaError_t launch_nq(const c128 *g, int64_t rows, int np, const c128 *Pq, c128 *g1, c128 *const *dst_tab,
+                             cudaStream_t st) {
   const size_t smem = sizeof(double2) * (size_t)np * NQ;
   if (smem > 48 * 1024) {
     cudaError_t e = cudaFuncSetAttribute(rp_to_q_kernel<NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
   }
-  rp_to_q_kernel<NQ><<<(unsigned)ceil_div(rows, 256), 256, smem, st>>>(g, rows, np, Pq, g1);
+  rp_to_q_kernel<NQ><<<(unsigned)ceil_div(rows, 256), 256, smem, st>>>(g, rows, np, Pq, g1, dst_tab);
   return cudaGetLastError();
 }
 
@@ -205,16 +225,22 @@ int rp_to_q_max_nq(int np) {
 }
 
 cudaError_t launch_rp_to_q(const c128 *g, int64_t rows, int np, const c128 *Pq, int nq, c128 *g1, cudaStream_t st) {
+  return launch_rp_to_q_dst(g, rows, np, Pq, nq, g1, nullptr, st);
+}
+
+// dst_tab (device array of nq device pointers, may be NULL): see emit_row
+cudaError_t launch_rp_to_q_dst(const c128 *g, int64_t rows, int np, const c128 *Pq, int nq, c128 *g1, c128 *const *dst_tab,
+                               cudaStream_t st) {
   if (nq > rp_to_q_max_nq(np)) return cudaErrorInvalidConfiguration;
   switch (nq) {
-    case 1: return launch_nq<1>(g, rows, np, Pq, g1, st);
-    case 2: return launch_nq<2>(g, rows, np, Pq, g1, st);
-    case 3: return launch_nq<3>(g, rows, np, Pq, g1, st);
-    case 4: return launch_nq<4>(g, rows, np, Pq, g1, st);
-    case 5: return launch_nq_tma<5>(g, rows, np, Pq, g1, st);
-    case 6: return launch_nq_tma<6>(g, rows, np, Pq, g1, st);
-    case 7: return launch_nq_tma<7>(g, rows, np, Pq, g1, st);
-    case 8: return launch_nq_tma<8>(g, rows, np, Pq, g1, st);
+    case 1: return launch_nq<1>(g, rows, np, Pq, g1, dst_tab, st);
+    case 2: return launch_nq<2>(g, rows, np, Pq, g1, dst_tab, st);
+    case 3: return launch_nq<3>(g, rows, np, Pq, g1, dst_tab, st);
+    case 4: return launch_nq<4>(g, rows, np, Pq, g1, dst_tab, st);
+    case 5: return launch_nq_tma<5>(g, rows, np, Pq, g1, dst_tab, st);
+    case 6: return launch_nq_tma<6>(g, rows, np, Pq, g1, dst_tab, st);
+    case 7: return launch_nq_tma<7>(g, rows, np, Pq, g1, dst_tab, st);
+    case 8: return launch_nq_tma<8>(g, rows, np, Pq, g1, dst_tab, st);
     default: return cudaErrorInvalidValue;
   }
 }

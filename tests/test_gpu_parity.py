@@ -765,6 +765,48 @@ def test_rp_sharded_two_handles(epw, large):
             h.close()
 
 
+def test_rp_sharded_fused_scatter_add(epw):
+    """NEXT-1 with the exchange step fused into the S1 kernel (epw_interp_rp_to_q_scatter_add): two Rp-shard handles, each
+    on its own stream at the same time, add their partial g(Re,q) straight into the buffers of the q-points' owners (here
+    both 'owners' live on this GPU; across GPUs the pointers are peer mappings and the adds cross NVLink).  No kernel
+    waits on another.  The summed g(Re,q) against the oracle's Eq. 9, then the rest of the path on it."""
+    from paper_2603_10295_b200 import shard
+
+    # 12 q: two S1 batches of 8 and 4 -> the bulk-TMA kernel (NQ = 8) and the register-staged one (NQ = 4)
+    w = synth.make_custom("si-f", 8, 6, (2, 2, 2), 1.5, 0.1, 1.5, (6, 5, 4), ("random", 12, 3), seed=53)
+    g = w.g_full()
+    rows = w.nbnd * w.nbnd * w.nmodes * w.ne
+    world = 2
+    handles, streams = [], [torch.cuda.Stream() for _ in range(world)]
+    try:
+        for a, b in shard.rp_ranges(w.np_, world):
+            h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_)
+            h.set_operators_from_host(w, rp_range=(a, b))
+            handles.append(h)
+        q_d = dev(w.q_list)
+        # owner of q-point iq = rank iq % 2; every owner zeroes its own buffers
+        own = [torch.zeros((w.nq, rows, 2), dtype=torch.float64, device="cuda") for _ in range(world)]
+        dst = [own[iq % world][iq] for iq in range(w.nq)]
+        torch.cuda.synchronize()
+        for r in range(world):
+            with torch.cuda.stream(streams[r]):
+                epw.epw_interp_rp_to_q_scatter_add(handles[r].h, q_d, w.nq, dst)
+        torch.cuda.synchronize()   # (the barrier between the ranks)
+        total = torch.stack(dst)
+        g1_ref = np.stack([oracle.rp_to_q(g, w.Rp, w.w_p, q) for q in w.q_list]).reshape(w.nq, rows)
+        assert np.abs(znp(total) - g1_ref).max() <= 1e-13 * np.abs(g1_ref).max()
+        # the rest of the path on the summed g(Re,q)
+        ref = oracle.interpolate(w.H_R, w.D_R, g, w.Re, w.w_e, w.Rp, w.w_p, w.k_list, w.q_list)
+        epw.epw_interp_set_gq(handles[0].h, total)
+        out = handles[0].interpolate_grid(w.k_grid, q_d)
+        epw.epw_interp_sync(handles[0].h)
+        epw.epw_interp_set_gq(handles[0].h, None)
+        assert_path_close([t_.cpu().numpy() for t_ in out], ref)
+    finally:
+        for h in handles:
+            h.close()
+
+
 # ---------------------------------------------------------------------------------------------------------
 # NEXT-3: energy-window pre-screening of the pairs (PAPER.md:L241)
 # ---------------------------------------------------------------------------------------------------------
