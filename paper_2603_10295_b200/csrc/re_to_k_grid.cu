@@ -181,7 +181,7 @@ cudaError_t launch_axis_pass_p(const c128 *A, int64_t a_rb, int64_t a_bs, int64_
                                int num_sms, cudaStream_t st) {
   if (M <= 0 || N <= 0 || K <= 0) return cudaSuccess;
   if (K > 32) return cudaErrorInvalidValue;
-  const int R = 1;   // rows per thread (see the kernel comment)   // rows per thread: the K inputs of every row live in registers (96 / ~90 / ~160 per thread)
+  const int R = 1;   // rows per thread (see the kernel comment)
   const int64_t bx = ceil_div(ceil_div(M, R), 256);
   // split the columns while the row blocks alone would not give every SM a few CTAs
   int ny = 1;
