@@ -41,7 +41,7 @@ cudaError_t launch_grid_fused(const c128 *T2, int64_t slab, int ncols, int L1, c
   if (g2 == nullptr && fold == nullptr) return cudaErrorInvalidValue;
   GridFusedParams p = {};
   p.T2 = T2; p.slab = slab; p.ncols = ncols; p.L1 = L1; p.cnt = cnt; p.P1c = P1c;
-  p.Uk = Uk; p.Ukq = Ukq; p.kq_idx = kq_idx; p.nm = nm; p.mask = mask; p.g2 = g2;
+  p.Uk = Uk; p.Ukq = Ukq; p.kq_idx = kq_idx; p.nm = nm; p.mask = mask; p.g2 = g2; p.nbatch = 1;
   if (fold) {
     p.cons_out = fold->out; p.eps_k = fold->eps_k; p.eps_kq = fold->eps_kq; p.omega_q = fold->omega_q; p.w_q = fold->w_q;
     p.iq = fold->iq; p.mu = fold->mu; p.kT = fold->kT; p.sigma = fold->sigma;
@@ -50,12 +50,16 @@ cudaError_t launch_grid_fused(const c128 *T2, int64_t slab, int ncols, int L1, c
 }
 
 // The last axis pass ALONE as the same DMMA product: gt c128 [cnt*slab][gt_stride] <- g~ (first Nb^2 Nm columns of each row).
+// nbatch problems of that shape: input b at T2 + b * in_bstride, output b at gt + b * out_bstride (any axis of the factorised
+// transform is such a batch: the contracted index outermost within a block, the blocks one after the other).
 cudaError_t launch_grid_pass_dmma(const c128 *T2, int64_t slab, int ncols, int L1, const c128 *P1c, int cnt, int nb, int nm,
-                                  int num_sms, c128 *gt, int64_t gt_stride, cudaStream_t st) {
-  if (slab <= 0 || cnt <= 0) return cudaSuccess;
+                                  int num_sms, c128 *gt, int64_t gt_stride, int nbatch, int64_t in_bstride,
+                                  int64_t out_bstride, cudaStream_t st) {
+  if (slab <= 0 || cnt <= 0 || nbatch <= 0) return cudaSuccess;
   if (gt == nullptr) return cudaErrorInvalidValue;
   GridFusedParams p = {};
   p.T2 = T2; p.slab = slab; p.ncols = ncols; p.L1 = L1; p.cnt = cnt; p.P1c = P1c; p.nm = nm; p.gt = gt; p.gt_stride = gt_stride;
+  p.nbatch = nbatch; p.in_bstride = in_bstride; p.out_bstride = out_bstride;
   return gf_dispatch(nb, p, num_sms, st);
 }
 

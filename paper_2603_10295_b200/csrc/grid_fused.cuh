@@ -71,6 +71,10 @@ struct GridFusedParams {
   double *g2;            // NULL allowed when the consumer is on: |g|^2 then never leaves the SM
   c128 *gt;              // pass-only variant: g~ [k][gt_stride] relative to the chunk (the g columns first)
   int64_t gt_stride;
+  // pass-only variant: nbatch independent problems of this shape, input b at T2 + b * in_bstride ([L1][slab][ncols]),
+  // output b at gt + b * out_bstride ([cnt][slab][gt_stride]); "cells" then run over nbatch * slab
+  int nbatch;
+  int64_t in_bstride, out_bstride;
   // NEXT-4 consumer folded into the epilogue of product 2 (consumer.cu has the formula, reading G18):
   //   Im Sigma_nk += pi w_q / (s sqrt(pi)) sum_{m,nu} |g_mn nu|^2 [(n_nu + f_m) e^{-((e_n - e_m + w_nu)/s)^2} + (n_nu + 1 - f_m) e^{-((e_n - e_m - w_nu)/s)^2}]
   double *cons_out;      // [k][Nb] relative to the chunk, NULL = consumer off
@@ -317,7 +321,7 @@ __global__ void __launch_bounds__(GFShape<NB, VAR>::NW * 32, 1) grid_fused_kerne
   int *cnt = reinterpret_cast<int *>(full + GF_MAX_BUF);                                      // [nbuf]
 
   // ---- this CTA's items and tiles ----
-  const int64_t total = p.slab * p.ngroups * p.nquads;
+  const int64_t total = p.slab * p.nbatch * p.ngroups * p.nquads;
   const int64_t lo = total * blockIdx.x / gridDim.x, hi = total * (blockIdx.x + 1) / gridDim.x;
   if (lo >= hi) return;
   const int64_t tile_lo = lo / p.nquads;
@@ -334,7 +338,8 @@ __global__ void __launch_bounds__(GFShape<NB, VAR>::NW * 32, 1) grid_fused_kerne
     mbar_expect_tx(bar, row_bytes * (uint32_t)L1);
     c128 *dst = sT2 + buf_elems * b;
     for (int n1 = 0; n1 < L1; n1++)
-      tma_bulk_g2s(smem_u32(dst + (size_t)n1 * RP), p.T2 + ((int64_t)n1 * p.slab + cell) * p.ncols + (int64_t)nu0 * NBB,
+      tma_bulk_g2s(smem_u32(dst + (size_t)n1 * RP),
+                   p.T2 + (cell / p.slab) * p.in_bstride + ((int64_t)n1 * p.slab + cell % p.slab) * p.ncols + (int64_t)nu0 * NBB,
                    row_bytes, bar);
   };
 
@@ -502,8 +507,8 @@ __global__ void __launch_bounds__(GFShape<NB, VAR>::NW * 32, 1) grid_fused_kerne
           if (mt0 + i < MTW && mtb + i < C::MTP && cl < NBB) {
             if (PASS_ONLY) {   // lane (g, t): g~ of pair t, column cl -- eight lanes write 128 contiguous bytes
               if (j0 + t < p.cnt)
-                p.gt[((int64_t)(j0 + t) * p.slab + cell) * p.gt_stride + (int64_t)(nu0 + nul) * NBB + cl] =
-                    make_double2(acc[i][0], acc[i][1]);
+                p.gt[(cell / p.slab) * p.out_bstride + ((int64_t)(j0 + t) * p.slab + cell % p.slab) * p.gt_stride +
+                     (int64_t)(nu0 + nul) * NBB + cl] = make_double2(acc[i][0], acc[i][1]);
             } else {
               *reinterpret_cast<double2 *>(sG + ((size_t)t * C::PST + (cl / NB) * C::NBP + cl % NB) * 2) =
                   make_double2(acc[i][0], acc[i][1]);
@@ -618,7 +623,7 @@ static cudaError_t launch_gf(const GridFusedParams &p0, int num_sms, cudaStream_
   if (!gf_plan<NB>(p.nm, p.L1, var, &p.nug, &p.nbuf, &smem)) return cudaErrorInvalidConfiguration;
   p.ngroups = (int)ceil_div(p.nm, p.nug);
   p.nquads = (p.cnt + 3) / 4;
-  const int64_t total = p.slab * p.ngroups * p.nquads;
+  const int64_t total = p.slab * p.nbatch * p.ngroups * p.nquads;
   const int nw = var == 2 ? GFShape<NB, 2>::NW : GFShape<NB, 0>::NW;
   const int64_t want = ceil_div(total, nw / GFShape<NB, 0>::WPQ);
   const unsigned grid = (unsigned)(want < num_sms ? want : num_sms);

@@ -885,6 +885,7 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   // Axis passes: a streaming kernel when the box extent is small (always, for Wigner-Seitz lists), else the in-place
   // tensor-path contraction with the packed phase table.
   // (nbat > 1: the same passes for nbat operands stored one after the other -- the outermost box index simply runs on)
+  const bool dmma_axis2 = grid && grid_fused_supported(nb, 1, L[1]);
   auto grid_pass_ab = [&](int nc, int nbat) -> cudaError_t {
     const int64_t N2 = grid->N[1], N3 = grid->N[2];
     const int64_t B = (int64_t)nbat * L[0];   // outermost extent of X, T1, T2
@@ -897,6 +898,13 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
                                N3 * nc, 1, nc, 0, 0, B * L[1] * nc, (int)N3, L[2], 1, h->num_sms, st);
     if (e != cudaSuccess) return e;
     h->launches++;
+    // axis 2 as the DMMA product of grid_fused.cuh (pass-only form): B independent problems [L2][N3][nc] -> [N2][N3][nc].  The
+    // columns are Nb^2 wide "modes" to that kernel: nc / Nb^2 of them.
+    // (worth it for large passes only: 7.1 vs 8.3 ms of S2 per 13 q on configs[3], 3.5e7 outputs per pass; on configs[1], [2]
+    //  -- 4.3e6 and 1.7e6 outputs -- the persistent kernel's start-up costs more than the streaming pass it replaces)
+    if (dmma_axis2 && nc % nbb == 0 && L[1] >= 3 && N2 >= 4 && B * N2 * N3 * nc >= ((int64_t)1 << 24))
+      return launch_grid_pass_dmma(h->T1.as<c128>(), N3, nc, L[1], h->P2raw.as<c128>(), (int)N2, nb, nc / nbb, h->num_sms,
+                                   h->T2.as<c128>(), nc, (int)B, (int64_t)L[1] * N3 * nc, N2 * N3 * nc, st);
     if (axis_pass_supported(L[1]))
       return launch_axis_pass(h->T1.as<c128>(), N3 * nc, (int64_t)L[1] * N3 * nc, N3 * nc, B * N3 * nc,
                               h->P2raw.as<c128>(), L[1], (int)N2, h->T2.as<c128>(), N3 * nc, N2 * N3 * nc, N3 * nc,
@@ -1057,7 +1065,7 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
         } else if (!fused) {
           if (hbatch && can_fuse)   // g columns only, all i1 planes: the pass as a DMMA product (grid_fused.cuh, pass-only form)
             LAUNCH(h, launch_grid_pass_dmma(h->T2.as<c128>(), slab, nc_g, L[0], h->P1raw.as<c128>(), grid->N[0], nb, nm,
-                                            h->num_sms, Cc, nc_g, st),
+                                            h->num_sms, Cc, nc_g, 1, 0, 0, st),
                    "grid pass S2 (DMMA)");
           else
             LAUNCH(h, grid_pass_c(nc_g, (int)(k0 / kchunk), Cc), "grid pass S2");
