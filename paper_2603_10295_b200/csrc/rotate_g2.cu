@@ -36,7 +36,7 @@ __global__ void __launch_bounds__(ROT_THREADS)
   constexpr int SP = rot_pitch(NB);
   constexpr int PPC = ROT_WARPS / WPP;  // pairs in flight per CTA
   static_assert(2 * KS <= SP, "T pitch must cover the padded K range");
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int g = lane >> 2, t = lane & 3;
   const int slot = warp / WPP, sub = warp - slot * WPP;
@@ -160,6 +160,154 @@ __global__ void __launch_bounds__(ROT_THREADS)
   }
 }
 
+
+// ---------------------------------------------------------------------------------------------------------------
+// The same two products with g~ of a pair brought into shared memory by ONE 1-D bulk TMA copy (g~ of a pair is a
+// contiguous run of 16 Nb^2 Nm bytes), two warps per pair, persistent CTAs of 64 threads.  The register-staged kernel
+// above waits for its A' fragments at their point of use (long-scoreboard stalls: 198 us per q on configs[2] for 93 us of
+// DMMA work and 63 us of HBM time); here the copy of the NEXT pair is issued as soon as product 1 has read the buffer, so it
+// flies during product 2, the U loads and the epilogue, and the fragments come from shared memory.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int ROTT_WARPS = 2;
+
+template <int NB>
+__global__ void __launch_bounds__(ROTT_WARPS * 32)
+    rotate_g2_tma_kernel(const c128 *__restrict__ gt, int64_t stride_gt, const c128 *__restrict__ Uk,
+                         const c128 *__restrict__ Ukq, const int32_t *__restrict__ kq_idx, int nm, int64_t nk,
+                         const uint8_t *__restrict__ mask, double *__restrict__ g2) {
+  constexpr int KS = (2 * NB + 3) / 4, NT = (2 * NB + 7) / 8, SP = rot_pitch(NB);
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int g = lane >> 2, t = lane & 3;
+  const int rows = nm * NB, MT = (rows + 7) >> 3;
+  const uint32_t gbytes = (uint32_t)(sizeof(c128) * rows * NB);
+  constexpr uint32_t ubytes = (uint32_t)(sizeof(c128) * NB * NB);
+  double *sGt = reinterpret_cast<double *>(smem_raw);                                   // g~ of the pair [nu][n'][m']
+  double *sU = reinterpret_cast<double *>(smem_raw + ((gbytes + 127) & ~127u));         // U_k, U_{k+q} of the pair
+  double *sT = sU + 2 * NB * NB * 2;                                                    // [MT*8 rows][SP] complex
+  uint64_t *bar = reinterpret_cast<uint64_t *>(sT + (size_t)MT * 8 * SP * 2);
+  const uint32_t bar_a = smem_u32(bar);
+  for (int i = threadIdx.x; i < MT * 8 * SP * 2; i += ROTT_WARPS * 32) sT[i] = 0.0;   // padding must stay finite
+  if (threadIdx.x == 0) {
+    mbar_init(bar_a, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  // the pairs of this CTA: ik = blockIdx.x, + gridDim.x, ...; skipped pairs (energy window) are not loaded
+  auto next_live = [&](int64_t ik) {
+    while (ik < nk && mask != nullptr && mask[ik] == 0) {
+      double *dz = g2 + ik * (int64_t)rows * NB;
+      for (int i = threadIdx.x; i < rows * NB; i += ROTT_WARPS * 32) dz[i] = 0.0;   // a skipped pair reports zeros
+      ik += gridDim.x;
+    }
+    return ik;
+  };
+  auto issue = [&](int64_t ik) {
+    if (threadIdx.x == 0 && ik < nk) {
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      mbar_expect_tx(bar_a, gbytes + 2 * ubytes);
+      tma_bulk_g2s(smem_u32(sGt), gt + ik * stride_gt, gbytes, bar_a);
+      tma_bulk_g2s(smem_u32(sU), Uk + ik * (NB * NB), ubytes, bar_a);
+      tma_bulk_g2s(smem_u32(sU + NB * NB * 2), Ukq + (kq_idx ? (int64_t)kq_idx[ik] : ik) * (NB * NB), ubytes, bar_a);
+    }
+  };
+  int64_t ik = next_live(blockIdx.x);
+  issue(ik);
+  uint32_t phase = 0;
+  while (ik < nk) {
+    mbar_wait(bar_a, phase);
+    phase ^= 1;
+    // ---- B', B'' fragments of this pair, from the two U matrices that came with g~ ----
+    double b1[KS][NT], b2[KS][NT];
+    {
+      const double *uk = sU + ((t & 1) ^ (g & 1));
+      const double *ukq = sU + NB * NB * 2 + ((t & 1) ^ (g & 1));
+      const bool n1 = (t & 1) == 1 && (g & 1) == 0, n2 = (t & 1) == 0 && (g & 1) == 1;   // sign of the embedding entries
+#pragma unroll
+      for (int ks = 0; ks < KS; ks++)
+#pragma unroll
+        for (int nt = 0; nt < NT; nt++) {
+          const int r = 2 * ks + (t >> 1), c = 4 * nt + (g >> 1);
+          const bool ok = r < NB && c < NB;
+          const double x = ok ? uk[(r + NB * c) * 2] : 0.0, y = ok ? ukq[(r + NB * c) * 2] : 0.0;
+          b1[ks][nt] = n1 ? -x : x;
+          b2[ks][nt] = n2 ? -y : y;
+        }
+    }
+    // ---- product 1: T[(nu,m')][n], row tiles dealt to the two warps ----
+    for (int mt = warp; mt < MT; mt += ROTT_WARPS) {
+      const int row = 8 * mt + g;
+      const bool rv = row < rows;
+      const int nu = row / NB, mp = row - nu * NB;
+      double a[KS];
+#pragma unroll
+      for (int ks = 0; ks < KS; ks++) {
+        const int np_ = 2 * ks + (t >> 1);
+        a[ks] = (rv && np_ < NB) ? sGt[(((size_t)nu * NB + np_) * NB + mp) * 2 + (t & 1)] : 0.0;
+      }
+      double acc[NT][2];
+#pragma unroll
+      for (int nt = 0; nt < NT; nt++) acc[nt][0] = acc[nt][1] = 0.0;
+#pragma unroll
+      for (int ks = 0; ks < KS; ks++)
+#pragma unroll
+        for (int nt = 0; nt < NT; nt++) dmma884(acc[nt][0], acc[nt][1], a[ks], b1[ks][nt]);
+      if (rv) {
+#pragma unroll
+        for (int nt = 0; nt < NT; nt++) {
+          const int n = 4 * nt + t;
+          if (n < NB)
+            *reinterpret_cast<double2 *>(sT + ((size_t)(nu * NB + n) * SP + mp) * 2) = make_double2(acc[nt][0], acc[nt][1]);
+        }
+      }
+    }
+    __syncthreads();   // T complete; g~ buffer free: the copy of the next pair flies during product 2
+    const int64_t ik_next = next_live(ik + gridDim.x);
+    issue(ik_next);
+    // ---- product 2: |sum_m' T[(nu,n)][m'] conj(Ukq[m'][m])|^2 ----
+    double *dst = g2 + ik * (int64_t)rows * NB;
+    for (int mt = warp; mt < MT; mt += ROTT_WARPS) {
+      const int row = 8 * mt + g;
+      const double *arow = sT + (size_t)row * SP * 2 + t;
+      double acc[NT][2];
+#pragma unroll
+      for (int nt = 0; nt < NT; nt++) acc[nt][0] = acc[nt][1] = 0.0;
+#pragma unroll
+      for (int ks = 0; ks < KS; ks++) {
+        const double a = arow[4 * ks];
+#pragma unroll
+        for (int nt = 0; nt < NT; nt++) dmma884(acc[nt][0], acc[nt][1], a, b2[ks][nt]);
+      }
+      if (row < rows) {
+#pragma unroll
+        for (int nt = 0; nt < NT; nt++) {
+          const int m = 4 * nt + t;
+          if (m < NB) dst[(int64_t)row * NB + m] = acc[nt][0] * acc[nt][0] + acc[nt][1] * acc[nt][1];
+        }
+      }
+    }
+    __syncthreads();   // T buffer free for the next pair
+    ik = ik_next;
+  }
+}
+
+template <int NB>
+static cudaError_t launch_rot_tma(const c128 *gt, int64_t stride_gt, const c128 *Uk, const c128 *Ukq, const int32_t *kq_idx,
+                                  int nm, int64_t nk, const uint8_t *mask, double *g2, cudaStream_t st) {
+  const int rows = nm * NB, MT = (rows + 7) / 8;
+  const size_t gbytes = sizeof(c128) * (size_t)rows * NB;
+  const size_t smem = ((gbytes + 127) & ~(size_t)127) + 2 * sizeof(c128) * NB * NB + sizeof(c128) * (size_t)MT * 8 * rot_pitch(NB) + 16;
+  cudaError_t e = cudaFuncSetAttribute(rotate_g2_tma_kernel<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  int per_sm = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rotate_g2_tma_kernel<NB>, ROTT_WARPS * 32, smem);
+  if (e != cudaSuccess) return e;
+  if (per_sm < 1) return cudaErrorInvalidConfiguration;
+  const unsigned grid = grid_cap(nk, per_sm);
+  rotate_g2_tma_kernel<NB><<<grid, ROTT_WARPS * 32, smem, st>>>(gt, stride_gt, Uk, Ukq, kq_idx, nm, nk, mask, g2);
+  return cudaGetLastError();
+}
+
 template <int NB, int WPP>
 static cudaError_t launch_rot(const c128 *gt, int64_t stride_gt, const c128 *Uk, const c128 *Ukq, const int32_t *kq_idx,
                               int nm, int64_t nk, const uint8_t *mask, double *g2, size_t smem_per_pair, cudaStream_t st) {
@@ -183,6 +331,11 @@ static cudaError_t launch_rot_nb(const c128 *gt, int64_t stride_gt, const c128 *
   const int MT = (nm * NB + 7) / 8;
   const size_t per_pair = sizeof(c128) * (size_t)MT * 8 * rot_pitch(NB);
   if (per_pair > (size_t)200 * 1024) return cudaErrorInvalidConfiguration;
+  // g~ of a pair through shared memory by bulk TMA when it and the T buffer leave room for at least four CTAs per SM and
+  // there are pairs enough to fill the GPU; the copy needs 16-byte aligned runs (always: complex rows)
+  const size_t tma_smem = sizeof(c128) * ((size_t)nm + 2) * NB * NB + per_pair + 144;
+  if (tma_smem <= (size_t)56 * 1024 && nk >= 1024)
+    return launch_rot_tma<NB>(gt, stride_gt, Uk, Ukq, kq_idx, nm, nk, mask, g2, st);
   // one warp per pair while four staging buffers fit comfortably; otherwise 2 or 4 warps share a pair
   if (per_pair <= (size_t)12 * 1024) return launch_rot<NB, 1>(gt, stride_gt, Uk, Ukq, kq_idx, nm, nk, mask, g2, per_pair, st);
   if (per_pair <= (size_t)24 * 1024) return launch_rot<NB, 2>(gt, stride_gt, Uk, Ukq, kq_idx, nm, nk, mask, g2, per_pair, st);
