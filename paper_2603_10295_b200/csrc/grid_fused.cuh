@@ -38,7 +38,6 @@ struct GF {
   static constexpr int SP = NB + ((6 - (NB & 3)) & 3);       // row pitch of the T staging buffer: = 2 (mod 4) complex
   static constexpr int TROWS = MTR * 8;
   static constexpr bool UREG = NB <= 8;         // U fragments of the four pairs of a quad resident over all modes
-  static constexpr int UP = UREG ? 4 : 1;
   static_assert(2 * KS <= SP, "T pitch must cover the padded K range");
 };
 

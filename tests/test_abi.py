@@ -77,3 +77,22 @@ def test_create_rejects_a_negative_or_nan_omega_min():
             epw.epw_interp_create(8, 6, 27, 27, omega_min=bad)
         assert e.value.code == epw.binding.EPW_EINVAL
         assert "omega_min" in str(e.value)
+
+
+def test_bench_host_logic_without_a_gpu():
+    """bench.py imports on a CPU box, its per-config defaults are the ones the full-size parity tests use, and the record
+    it keeps of an extra config is built from the fields run_config() produces."""
+    import bench
+
+    assert bench.NQ_STEP[1] == 96 and bench.NQ_STEP[2] == 32 and bench.NQ_STEP[3] == 13 and bench.NQ_STEP[4] == 2
+    sub = {"config": {"workload": "w"}, "value": 1.0, "unit": "elements/s", "ms_per_step": 2.0, "steps": 3, "warmup": 1,
+           "gpu_launches": 7, "clocks": {"sm_mhz": 1965.0},
+           "roofline": {"stage": "S4b_rotate_g2", "kernel": "k", "bound": "tensor", "achieved": 1.0, "peak": 2.0,
+                        "unit": "TFLOP/s", "frac": 0.5, "share_of_step": 0.4, "traffic": None,
+                        "stages": {"S1_rp_to_q": {"kernel": "rp_to_q_kernel", "bound": "hbm", "frac": 0.7, "share_of_step": 0.04}}},
+           "klist_path": {"value": 3.0, "ms_per_step": 4.0, "S2_re_to_k": {"kernel": "zgemm_dmma_kernel", "bound": "tensor",
+                                                                          "frac": 0.96, "share_of_step": 0.8}},
+           "parity": {"ok": True}}
+    rec = bench.summarise_config(sub, 1.5)
+    assert rec["dominant"]["frac"] == 0.5 and rec["stages"]["S1_rp_to_q"]["frac"] == 0.7
+    assert rec["klist_path"]["S2_re_to_k"]["frac"] == 0.96 and rec["parity"]["ok"] and rec["wall_s"] == 1.5
