@@ -591,7 +591,10 @@ def run_config(args, ctx, cfg_index: int, steps: int, warmup: int, legs: set) ->
                 spec["S2_re_to_k"] = ("hbm", "axis_pass_kernel (axis passes)", byts * nq_tot, hbm, "GB/s",
                                       {"flops": 8.0 * mults * nq_tot})
             else:
-                spec["S2_re_to_k"] = ("tensor", "zgemm_strided_kernel" if large else "zgemm_dmma_kernel",
+                s2_kernel = "zgemm_dmma_kernel"
+                if large:   # short lattice-vector lists go through the DMMA last-axis pass (interp.cu: s2_pass)
+                    s2_kernel = "grid_fused_kernel (pass-only variant)" if (ne <= 18 and E % 64 == 0) else "zgemm_strided_kernel"
+                spec["S2_re_to_k"] = ("tensor", s2_kernel,
                                       8.0 * ncols * ne * pairs, dmma, "TFLOP/s", {})
             if fused:
                 # last axis pass of S2 (8 L1 E flops per pair, plain DFMA) + both rotation products (DMMA): one FP64 pipe

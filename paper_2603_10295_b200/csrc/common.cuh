@@ -163,6 +163,7 @@ cudaError_t launch_grid_fused(const c128 *T2, int64_t slab, int ncols, int L1, c
 cudaError_t launch_grid_pass_dmma(const c128 *T2, int64_t slab, int ncols, int L1, const c128 *P1c, int cnt, int nb, int nm,
                                   int num_sms, c128 *gt, int64_t gt_stride, int nbatch, int64_t in_bstride,
                                   int64_t out_bstride, cudaStream_t st);
+bool grid_pass_dmma_supported(int nb, int L);   // L <= 18
 // one axis pass as a streaming kernel (K = L_d <= 32); P c128 [K][N] row-major (unpacked phases)
 bool axis_pass_supported(int K);
 cudaError_t launch_axis_pass(const c128 *A, int64_t a_rb, int64_t a_bs, int64_t a_ks, int64_t M, const c128 *P, int K, int N,

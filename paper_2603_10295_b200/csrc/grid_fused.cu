@@ -63,4 +63,20 @@ cudaError_t launch_grid_pass_dmma(const c128 *T2, int64_t slab, int ncols, int L
   return gf_dispatch(nb, p, num_sms, st);
 }
 
+// whether that kernel takes a pass with K = L lattice vectors on column groups of nb^2
+bool grid_pass_dmma_supported(int nb, int L) {
+  if (nb < 1 || nb > 16) return false;
+  int nug = 0, nbuf = 0;
+  size_t smem = 0;
+  switch (nb) {
+#define EPW_GF_CASE(NB_) \
+  case NB_: return gf_plan<NB_>(1, L, 2, &nug, &nbuf, &smem);
+    EPW_GF_CASE(1) EPW_GF_CASE(2) EPW_GF_CASE(3) EPW_GF_CASE(4) EPW_GF_CASE(5) EPW_GF_CASE(6) EPW_GF_CASE(7) EPW_GF_CASE(8)
+    EPW_GF_CASE(9) EPW_GF_CASE(10) EPW_GF_CASE(11) EPW_GF_CASE(12) EPW_GF_CASE(13) EPW_GF_CASE(14) EPW_GF_CASE(15)
+    EPW_GF_CASE(16)
+#undef EPW_GF_CASE
+    default: return false;
+  }
+}
+
 }  // namespace epw

@@ -46,6 +46,7 @@ struct GF {
 __host__ __device__ constexpr int gf_row_pitch(int cols) { return cols + ((12 - (cols & 7)) & 7); }
 
 constexpr int GF_MAX_KSP = 8;   // k-steps of the pass: 2 L1 real <= 32, i.e. L1 <= 16
+constexpr int GF_MAX_KSP_PASS = 9;   // ... of the pass-only variant: L1 <= 18 (the 17 lattice vectors of a ribbon)
 constexpr int GF_WARPS = 8;     // warps of the one persistent CTA per SM (one warp per quad)
 // Warps per quad.  With 2, each of two warps takes half of the pass tiles and rotates two of the four pairs: the U
 // fragments of a warp are then those of two pairs (64 registers) and twelve warps fit the register file (152 per thread)
@@ -589,7 +590,7 @@ __global__ void __launch_bounds__(GFShape<NB, VAR>::NW * 32, 1) grid_fused_kerne
 template <int NB>
 static bool gf_plan(int nm, int L1, int var, int *nug_out, int *nbuf_out, size_t *smem_out) {
   typedef GF<NB> C;
-  if (L1 < 1 || L1 > 2 * GF_MAX_KSP || nm < 1) return false;
+  if (L1 < 1 || L1 > 2 * (var == 2 ? GF_MAX_KSP_PASS : GF_MAX_KSP) || nm < 1) return false;
   const int L1e = 2 * ((L1 + 1) / 2);
   const size_t limit = (size_t)225 * 1024;
   for (int want_buf = 2; want_buf >= 1; want_buf--)
@@ -637,6 +638,8 @@ static cudaError_t launch_gf(const GridFusedParams &p0, int num_sms, cudaStream_
     if (var == 2) EPW_GF_LAUNCH(4, 2);
     else if (var == 1) EPW_GF_LAUNCH(4, 1);
     else EPW_GF_LAUNCH(4, 0);
+  } else if (p.L1 > 2 * GF_MAX_KSP) {
+    EPW_GF_LAUNCH(9, 2);   // pass-only (gf_plan admits no other variant at this L1)
   } else {
     if (var == 2) EPW_GF_LAUNCH(8, 2);
     else if (var == 1) EPW_GF_LAUNCH(8, 1);

@@ -69,6 +69,19 @@ int64_t choose_mtiles_per_chunk(int NT, int sms, size_t bytes_per_mtile, int64_t
   return best;
 }
 
+// out[b][c][r] = in[b][r][c] for blocks of rows (the phase table [k][Re] of a k-chunk as [Re][k])
+__global__ void transpose_blocks_kernel(const c128 *__restrict__ in, int64_t rows, int cols, int64_t rows_per_block,
+                                        c128 *__restrict__ out) {
+  const int64_t total = rows * cols;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t r = i / cols;
+    const int c = (int)(i - r * cols);
+    const int64_t b = r / rows_per_block, rl = r - b * rows_per_block;
+    const int64_t nr = rows - b * rows_per_block < rows_per_block ? rows - b * rows_per_block : rows_per_block;
+    out[b * rows_per_block * cols + (int64_t)c * nr + rl] = in[i];
+  }
+}
+
 __global__ void fill_ones_kernel(double *p, int n) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) p[i] = 1.0;
@@ -116,6 +129,7 @@ struct epw_interp {
   // valid for (grid sizes, shift, operators epoch); any k-list call or new operators drop it
   struct KSide { bool valid = false, with_conj = false; int32_t N[3] = {0, 0, 0}; double s[3] = {0, 0, 0}; uint64_t epoch = 0; } kside;
   uint64_t op_epoch = 0;
+  DevBuf PkT;         // large-Nb path: phase table of every k-chunk transposed, [chunk][Re][k]
   DevBuf dst_tab;     // destination pointers of epw_interp_rp_to_q_scatter_add
   DevBuf epsk_keep;   // eps_k of the cached k side (the caller's buffer is refilled from it)
   int64_t last_eq_slot = 0;  // slot of the last q of the last call inside the e_q buffer (debug getter)
@@ -273,11 +287,14 @@ static int interpolate_large(epw_interp *h, const double *k_list, const GridSpec
   else if (kc >= 64) kc = kc / 64 * 64;
   else return h->fail(EPW_ENOMEM, "epw_interp_interpolate: workspace_bytes too small for one 64-k chunk of g~ and T");
 
+  // S2 as the DMMA last-axis pass when the lattice-vector list is short and the columns split into groups of 64
+  const bool s2_pass = E % 64 == 0 && E / 64 <= 2147483647LL && E <= 2147483647LL && grid_pass_dmma_supported(8, ne);
   CU_OR_FAIL(h, h->Apack.reserve(sizeof(double) * (size_t)MTk * KBe * GEMM_CHUNK), "cudaMalloc Apack");
   CU_OR_FAIL(h, h->BpackH.reserve(sizeof(double) * (size_t)NTH * KBe * GEMM_CHUNK), "cudaMalloc BpackH");
   CU_OR_FAIL(h, h->Hk.reserve(sizeof(c128) * (size_t)nk * nbb), "cudaMalloc Hk");
   CU_OR_FAIL(h, h->Uk.reserve(sizeof(c128) * (size_t)nk * nbb), "cudaMalloc Uk");
   CU_OR_FAIL(h, h->Pk.reserve(sizeof(c128) * (size_t)nk * ne), "cudaMalloc Pk");
+  if (s2_pass) CU_OR_FAIL(h, h->PkT.reserve(sizeof(c128) * (size_t)nk * ne), "cudaMalloc PkT");
   CU_OR_FAIL(h, h->BpackPk.reserve(sizeof(double) * (size_t)NTk * KBe * GEMM_CHUNK), "cudaMalloc BpackPk");
   CU_OR_FAIL(h, h->UpackK.reserve(sizeof(double) * (size_t)nk * upack), "cudaMalloc UpackK");
   CU_OR_FAIL(h, h->UpackKH.reserve(sizeof(double) * (size_t)nk * upack), "cudaMalloc UpackKH");
@@ -330,6 +347,11 @@ static int interpolate_large(epw_interp *h, const double *k_list, const GridSpec
          "phase_table(k,Re)");
   LAUNCH(h, launch_pack_b_strided(h->Pk.as<c128>(), 1, ne, 0, 1, 0, nullptr, 0.0, ne, (int)nk, h->BpackPk.as<double>(), st),
          "pack P_k");
+  if (s2_pass) {
+    h->launches++;
+    transpose_blocks_kernel<<<grid_cap(ceil_div(nk * ne, 256), 8), 256, 0, st>>>(h->Pk.as<c128>(), nk, ne, kc, h->PkT.as<c128>());
+    CU_OR_FAIL(h, cudaGetLastError(), "transpose P_k");
+  }
   h->end_span(sp, st);
   sp = h->begin_span(3, st);
   LAUNCH(h,
@@ -438,6 +460,14 @@ static int interpolate_large(epw_interp *h, const double *k_list, const GridSpec
         const int64_t kn = std::min(kc, nk - k0);
         // ---- S2: g~[k][nu][n'][m'] = sum_Re g^[Re][nu][n'][m'] P_k[k][Re] ----
         sp = h->begin_span(4, st);
+        if (s2_pass)
+          // few lattice vectors (a ribbon: Ne = 17): g~ = sum_Re g^(Re) P_k as the last-axis DMMA pass of grid_fused.cuh on
+          // column groups of 64 -- K = 2 Ne real exactly (the tiled contraction pads 34 to 48) and the 34 GB of g~ per q
+          // stream out of 16 warps per SM: 11 instead of 22 ms per q on configs[4]
+          LAUNCH(h, launch_grid_pass_dmma(h->ghat.as<c128>(), 1, (int)E, ne, h->PkT.as<c128>() + k0 * ne, (int)kn, 8,
+                                          (int)(E / 64), h->num_sms, h->C.as<c128>(), E, 1, 0, 0, st),
+                 "S2 (DMMA pass)");
+        else
         LAUNCH(h, launch_zgemm_strided(h->ghat.as<c128>(), E, 0, E, 0,
                                        h->BpackPk.as<double>() + (k0 / 64) * (int64_t)KBe * GEMM_CHUNK, nullptr, h->C.p, E, 0,
                                        1, E, 0, 0, E, (int)kn, ne, 1, h->num_sms, st),
@@ -573,7 +603,7 @@ void epw_interp_destroy(epw_interp_t h) {
   DevBuf *all[] = {&h->g, &h->H, &h->D, &h->Re, &h->Rp, &h->we, &h->wp, &h->ones, &h->Apack, &h->BpackH, &h->Hk,
                    &h->Uk, &h->Pq, &h->Pqe, &h->Dq, &h->eq, &h->g1, &h->Bpack, &h->C, &h->Ukq, &h->epskq_scratch,
                    &h->status, &h->eig_scratch, &h->hs_k, &h->hs_q, &h->hs_map, &h->hs_epsk, &h->hs_epskq,
-                   &h->hs_omega, &h->hs_g2, &h->epsk_keep, &h->dst_tab, &h->Pk, &h->BpackPk, &h->UpackK, &h->UpackKH, &h->BpackE,
+                   &h->hs_omega, &h->hs_g2, &h->epsk_keep, &h->dst_tab, &h->PkT, &h->Pk, &h->BpackPk, &h->UpackK, &h->UpackKH, &h->BpackE,
                    &h->ghat, &h->T, &h->Hkq, &h->boxidx, &h->X, &h->T1, &h->T2, &h->Ptmp, &h->P1raw, &h->P2raw, &h->P3raw, &h->P1pack, &h->P2pack,
                    &h->P3pack, &h->klist_gen, &h->workctr, &h->maskbuf, &h->g2_scratch};
   for (DevBuf *b : all) b->release();
