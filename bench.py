@@ -588,7 +588,11 @@ def run_config(args, ctx, cfg_index: int, steps: int, warmup: int, legs: set) ->
                 mults = ncols * (L1 * L2 * N3 * L3 + L1 * N2 * N3 * L2) + nc_last * float(nk) * L1     # per q
                 byts = 16.0 * (ncols * ((L1 * L2 * L3 + L1 * L2 * N3) + (L1 * L2 * N3 + L1 * N2 * N3))
                                + nc_last * (L1 * N2 * N3 + nk))
-                spec["S2_re_to_k"] = ("hbm", "axis_pass_kernel (axis passes)", byts * nq_tot, hbm, "GB/s",
+                # (two-kernel form: the last of the three passes is the pass-only variant of grid_fused_kernel; one-kernel
+                #  form: it is inside grid_fused_kernel and counted with S4b)
+                spec["S2_re_to_k"] = ("hbm", "axis_pass_kernel (axis passes)" if fused else
+                                      "axis_pass_kernel (axes 3, 2) + grid_fused_kernel pass-only variant (axis 1)",
+                                      byts * nq_tot, hbm, "GB/s",
                                       {"flops": 8.0 * mults * nq_tot})
             else:
                 s2_kernel = "zgemm_dmma_kernel"
@@ -603,7 +607,11 @@ def run_config(args, ctx, cfg_index: int, steps: int, warmup: int, legs: set) ->
                                          {"hbm_bytes": (32.0 * nb * nb + 8.0 * E) * pairs
                                                        + 16.0 * E * Lbox[0] * w.k_grid[1] * w.k_grid[2] * nq_tot})
             else:
-                spec["S4b_rotate_g2"] = ("tensor", "zgemm_strided_kernel" if large else "rotate_g2_dmma_kernel",
+                # rotate_g2.cu: bulk-TMA staged kernel when g~, the two U and T of a pair fit 56 KB (four CTAs per SM)
+                mt_rows = -(-(nm * nb) // 8) * 8
+                rot_tma = 16 * ((nm + 2) * nb * nb + mt_rows * (nb + ((6 - (nb & 3)) & 3))) + 144 <= 56 * 1024 and nk >= 1024
+                spec["S4b_rotate_g2"] = ("tensor", "zgemm_strided_kernel" if large else
+                                         ("rotate_g2_tma_kernel" if rot_tma else "rotate_g2_dmma_kernel"),
                                          16.0 * nb ** 3 * nm * pairs, dmma, "TFLOP/s",
                                          {"hbm_bytes": (16.0 * (E + 2 * nb * nb) + 8.0 * E) * pairs})
             spec["S4a_mode_rotation"] = ("tensor" if large else "alu",
