@@ -314,6 +314,18 @@ int epw_zgemm_strided(const void *A, int64_t a_rb, int64_t a_bs, int64_t a_ks, i
                       void *C, int64_t c_rb, int64_t c_bs, int64_t c_rs, int64_t c_cs, int64_t c_batch, int abs2,
                       int64_t M, int32_t N, int32_t K, int64_t batch, void *cuda_stream);
 
+/* One axis of the factorised Re -> k sum on a uniform grid (Eq. 10; reading G17) as the FP64
+ * tensor-path (DMMA) product of grid_fused.cuh, for nbatch independent blocks:
+ *     out[b][j][c][col] = sum_{n < L} P[n][j] T[b][n][c][col],    j < cnt, c < slab, col < ncols
+ *   T    c128, block b at T + b*in_bstride, layout [L][slab][ncols];  ncols must be a multiple of nb*nb (the kernel works
+ *        on column groups of nb^2, 1 <= nb <= 16), L <= 18
+ *   P    c128 [L][cnt]: the phases w e^{2 pi i (j+s) n / N} of this axis
+ *   out  c128, block b at out + b*out_bstride, row (j*slab + c) at stride out_stride (>= ncols)
+ * All device pointers; asynchronous on cuda_stream.  EPW_EUNSUPPORTED when the shape does not fit the kernel. */
+int epw_axis_pass_dmma(const void *T, int64_t slab, int32_t ncols, int32_t L, const void *P, int32_t cnt, int32_t nb,
+                       void *out, int64_t out_stride, int32_t nbatch, int64_t in_bstride, int64_t out_bstride,
+                       void *cuda_stream);
+
 /* S4b: g2[ik][nu][n][m] = | sum_{m'n'} conj(Ukq[ik][m',m]) gt[ik][nu][n'][m'] Uk[ik][n',n] |^2.
  * gt c128, pair ik at gt + ik*stride_gt (c128 elements); Uk, Ukq c128 [..][Nb][Nb] column-major;
  * kq_idx NULL (Ukq indexed by ik) or int32 [nk] (Ukq indexed by kq_idx[ik]).

@@ -34,7 +34,7 @@ EXPORTED_SYMBOLS = [
     "epw_interp_interpolate_grid_host", "epw_interp_sync", "epw_interp_get_stage_times",
     "epw_interp_enable_stage_timing", "epw_interp_get_stage_launches", "epw_interp_last_launch_count", "epw_interp_get_eigh_rotations", "epw_interp_last_plan", "epw_interp_debug_get", "epw_interp_last_error",
     "epw_phase_table", "epw_rp_to_q", "epw_interp_operator", "epw_eigh_batched", "epw_eigh_batched_algo", "epw_zgemm", "epw_zgemm_strided",
-    "epw_rotate_g2",
+    "epw_rotate_g2", "epw_axis_pass_dmma",
     "epw_eq6_unrotate", "epw_wannier_from_bloch",
     "epw_interp_set_energy_window", "epw_interp_set_selfenergy_consumer", "epw_interp_set_rp_shard", "epw_interp_rp_to_q_partial", "epw_interp_rp_to_q_scatter_add", "epw_interp_set_gq",
     "epw_probe_peaks", "epw_version",
@@ -102,6 +102,8 @@ def load_library() -> ctypes.CDLL:
                                         c_int64, vp, c_int64, c_int64, c_int64, c_int64, c_int64, c_int, c_int64,
                                         c_int32, c_int32, c_int64, vp]
         L.epw_rotate_g2.argtypes = [vp, c_int64, vp, vp, vp, c_int32, c_int32, c_int64, vp, vp]
+        L.epw_axis_pass_dmma.argtypes = [vp, c_int64, c_int32, c_int32, vp, c_int32, c_int32, vp, c_int64, c_int32, c_int64,
+                                         c_int64, vp]
         L.epw_eq6_unrotate.argtypes = [vp, vp, vp, vp, vp, c_int32, c_int32, c_int64, c_int64, vp, vp]
         L.epw_wannier_from_bloch.argtypes = [vp, vp, c_int64, vp, c_int64, vp, c_int32, vp, c_int32, c_int32, c_int32, vp, vp]
         L.epw_probe_peaks.argtypes = [c_int32, POINTER(c_double)]
@@ -303,6 +305,11 @@ def epw_zgemm_strided(A, a_rb, a_bs, a_ks, a_batch, B, b_sr, b_sn, b_batch, b_co
                                             int(b_conj), _ptr(b_gather), nb_mats, _ptr(C), c_rb, c_bs, c_rs, c_cs,
                                             c_batch, int(abs2), M, N, K, batch,
                                             _stream() if stream is None else stream))
+
+
+def epw_axis_pass_dmma(T, slab, ncols, L, P, cnt, nb, out, out_stride, nbatch=1, in_bstride=0, out_bstride=0, stream=None):
+    _check(load_library().epw_axis_pass_dmma(_ptr(T), slab, ncols, L, _ptr(P), cnt, nb, _ptr(out), out_stride, nbatch,
+                                             in_bstride, out_bstride, _stream() if stream is None else stream))
 
 
 def epw_rotate_g2(gt, stride_gt, Uk, Ukq, kq_idx, nb, nm, nk, g2, stream=None):

@@ -1561,6 +1561,17 @@ int epw_zgemm_strided(const void *A, int64_t a_rb, int64_t a_bs, int64_t a_ks, i
   return rc_of(e);
 }
 
+int epw_axis_pass_dmma(const void *T, int64_t slab, int32_t ncols, int32_t L, const void *P, int32_t cnt, int32_t nb,
+                       void *out, int64_t out_stride, int32_t nbatch, int64_t in_bstride, int64_t out_bstride,
+                       void *cuda_stream) {
+  if (!T || !P || !out || slab <= 0 || ncols <= 0 || L <= 0 || cnt <= 0 || nb <= 0 || nbatch <= 0 || out_stride < ncols)
+    return EPW_EINVAL;
+  if (nb > 16 || ncols % (nb * nb) != 0 || !grid_pass_dmma_supported(nb, L)) return EPW_EUNSUPPORTED;
+  return rc_of(launch_grid_pass_dmma(reinterpret_cast<const c128 *>(T), slab, ncols, L, reinterpret_cast<const c128 *>(P), cnt,
+                                     nb, ncols / (nb * nb), device_sm_count(), reinterpret_cast<c128 *>(out), out_stride,
+                                     nbatch, in_bstride, out_bstride, reinterpret_cast<cudaStream_t>(cuda_stream)));
+}
+
 int epw_rotate_g2(const void *gt, int64_t stride_gt, const void *Uk, const void *Ukq, const int32_t *kq_idx, int32_t nb,
                   int32_t nm, int64_t nk, double *g2, void *cuda_stream) {
   if (!gt || !Uk || !Ukq || !g2 || nb <= 0 || nm <= 0 || nk < 0) return EPW_EINVAL;

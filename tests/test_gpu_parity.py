@@ -342,6 +342,30 @@ def test_rotate_g2_large(epw):
             assert np.abs(got[ik] - ref).max() <= 1e-12 * ref.max()
 
 
+@pytest.mark.parametrize("nb,nmodes,L,cnt,slab,nbatch,extra", [
+    (8, 6, 7, 40, 5, 1, 0),      # configs[1]: K = 14 real exactly 4 k-steps, ten quads
+    (8, 2, 9, 13, 3, 2, 64),     # L = 9 (configs[3]): five of eight k-steps, ragged last quad, two blocks, padded rows
+    (11, 3, 13, 10, 2, 3, 0),    # Nb = 11 (configs[2]): 121 columns per group, ragged column tile
+    (8, 3, 17, 9, 1, 1, 0),      # L = 17 (the ribbon's lattice-vector list): nine k-steps
+    (3, 5, 2, 5, 4, 2, 9),       # tiny shapes
+])
+def test_axis_pass_dmma(epw, nb, nmodes, L, cnt, slab, nbatch, extra):
+    """One axis of the factorised Re -> k sum as the DMMA product (pass-only variant of grid_fused_kernel, batched) against
+    the plain definition out[b][j][c][col] = sum_n P[n][j] T[b][n][c][col]."""
+    ncols = nb * nb * nmodes
+    stride = ncols + extra
+    T = crandn(nbatch, L, slab, ncols)
+    P = crandn(L, cnt)
+    out = torch.zeros((nbatch, cnt, slab, stride, 2), dtype=torch.float64, device="cuda")
+    epw.epw_axis_pass_dmma(zdev(T), slab, ncols, L, zdev(P), cnt, nb, out, stride, nbatch, L * slab * ncols,
+                           cnt * slab * stride)
+    torch.cuda.synchronize()
+    got = znp(out)
+    ref = np.einsum("nj,bncx->bjcx", P, T)
+    assert np.abs(got[..., :ncols] - ref).max() <= 1e-13 * np.abs(ref).max()
+    assert np.abs(got[..., ncols:]).max() == 0.0 if extra else True   # nothing written beyond the columns of a row
+
+
 # ---------------------------------------------------------------------------------------------------------
 # whole path
 # ---------------------------------------------------------------------------------------------------------
