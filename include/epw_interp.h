@@ -133,6 +133,9 @@ int epw_interp_interpolate_host(epw_interp_t h, const double *k_list, int64_t nk
  * (csrc/re_to_k_grid.cu): (L1 L2 N3 L3 + L1 N2 N3 L2 + N1 N2 N3 L1) instead of Nk Ne multiplications per column, with
  * L_d the extents of the bounding box of the Re list -- the same sums re-associated, equal to the list form up to
  * rounding order.  The large-Nb kernel family (one-dimensional grids) expands the grid to a list internally.
+ * The k side of the call (H(k), U_k, eps_k) is kept in the handle and reused by the next grid call with the same sizes and
+ * shift, until the operators change or a k-list call comes in between: a caller looping over batches of q on one fine
+ * k-grid pays for the Nk eigensolves of H(k) once.
  */
 int epw_interp_interpolate_grid(epw_interp_t h, const int32_t *k_grid, const double *k_shift, const double *q_list,
                                 int64_t nq, const int32_t *kq_map, double *eps_k, double *eps_kq, double *omega_q,

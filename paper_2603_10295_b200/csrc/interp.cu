@@ -127,7 +127,7 @@ struct epw_interp {
   int last_kmode = 0;
   // k side of the large-Nb path kept between calls on the SAME uniform grid (phases, H(k), U_k, eps_k, packed operands):
   // valid for (grid sizes, shift, operators epoch); any k-list call or new operators drop it
-  struct KSide { bool valid = false, with_conj = false; int32_t N[3] = {0, 0, 0}; double s[3] = {0, 0, 0}; uint64_t epoch = 0; } kside;
+  struct KSide { bool valid = false, with_conj = false; int path = 0; int32_t N[3] = {0, 0, 0}; double s[3] = {0, 0, 0}; uint64_t epoch = 0; } kside;
   uint64_t op_epoch = 0;
   DevBuf PkT;         // large-Nb path: phase table of every k-chunk transposed, [chunk][Re][k]
   DevBuf dst_tab;     // destination pointers of epw_interp_rp_to_q_scatter_add
@@ -251,8 +251,8 @@ static bool use_large_path(const epw_interp *h) {
 //   S4b  T = g~ U_k ;  |g|^2 = |T conj(U_{k+q})|^2      [Nm Nb x Nb] . [Nb x Nb], batched over the k of the chunk
 // ---------------------------------------------------------------------------------------------------------
 struct GridSpec;
-static bool kside_matches(const epw_interp *h, const GridSpec *grid, bool need_conj);
-static void kside_record(epw_interp *h, const GridSpec *grid, bool with_conj);
+static bool kside_matches(const epw_interp *h, const GridSpec *grid, bool need_conj, int path = EPW_PATH_LARGE);
+static void kside_record(epw_interp *h, const GridSpec *grid, bool with_conj, int path = EPW_PATH_LARGE);
 
 static int interpolate_large(epw_interp *h, const double *k_list, const GridSpec *grid, int64_t nk, const double *q_list,
                              int64_t nq, const int32_t *kq_map, double *eps_k, double *eps_kq, double *omega_q, double *g2,
@@ -516,14 +516,15 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
                              int64_t nq, const int32_t *kq_map, double *eps_k, double *eps_kq, double *omega_q,
                              double *g2, cudaStream_t st);
 
-static bool kside_matches(const epw_interp *h, const GridSpec *grid, bool need_conj) {
-  if (!grid || !h->kside.valid || h->kside.epoch != h->op_epoch) return false;
+static bool kside_matches(const epw_interp *h, const GridSpec *grid, bool need_conj, int path) {
+  if (!grid || !h->kside.valid || h->kside.epoch != h->op_epoch || h->kside.path != path) return false;
   for (int d = 0; d < 3; d++)
     if (h->kside.N[d] != grid->N[d] || h->kside.s[d] != grid->s[d]) return false;
   return h->kside.with_conj || !need_conj;
 }
-static void kside_record(epw_interp *h, const GridSpec *grid, bool with_conj) {
+static void kside_record(epw_interp *h, const GridSpec *grid, bool with_conj, int path) {
   h->kside.valid = true;
+  h->kside.path = path;
   h->kside.with_conj = with_conj;
   h->kside.epoch = h->op_epoch;
   for (int d = 0; d < 3; d++) {
@@ -774,7 +775,10 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
                              int64_t nq, const int32_t *kq_map, double *eps_k, double *eps_kq, double *omega_q,
                              double *g2, cudaStream_t st) {
   const int nb = h->nb, nm = h->nm, ne = h->ne, np = h->np, nbb = h->nbb, nmm = h->nmm;
-  h->kside.valid = false;   // (the small-Nb kernels share the H(k), U_k buffers with the cached k side of the large-Nb path)
+  // (the two kernel families share the H(k), U_k buffers: a cached k side is valid for the family that made it; on a
+  //  uniform grid the small-Nb family keeps U_k and eps_k between calls too -- 10^6 solves per call on configs[3])
+  const bool k_cached = kside_matches(h, grid, false, EPW_PATH_SMALL);
+  if (!k_cached) h->kside.valid = false;
   const int ncols_g = nbb * nm;
   const int ncols_h = kq_map ? 0 : nbb;
   const int ncols = ncols_g + ncols_h;
@@ -984,6 +988,10 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   }
   h->end_span(sp, st);
   sp = h->begin_span(3, st);
+  if (k_cached) {
+    CU_OR_FAIL(h, cudaMemcpyAsync(eps_k, h->epsk_keep.p, sizeof(double) * (size_t)nk * nb, cudaMemcpyDeviceToDevice, st),
+               "copy cached eps_k");
+  } else {
   if (!grid) {
     LAUNCH(h,
            launch_pack_b(nullptr, nullptr, nullptr, 0.0, h->H.as<c128>(), nullptr, nbb, nm, ne, 0, nbb,
@@ -1003,6 +1011,13 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   LAUNCH(h, launch_eigh_batched(h->Hk.as<c128>(), nbb, nb, nk, eps_k, h->Uk.as<c128>(), 0, h->status.as<int32_t>(),
                                 h->eig_scratch.as<c128>(), h->work_slot(0), st),
          "eigh H(k)");
+  if (grid) {
+    CU_OR_FAIL(h, h->epsk_keep.reserve(sizeof(double) * (size_t)nk * nb), "cudaMalloc eps_k cache");
+    CU_OR_FAIL(h, cudaMemcpyAsync(h->epsk_keep.p, eps_k, sizeof(double) * (size_t)nk * nb, cudaMemcpyDeviceToDevice, st),
+               "keep eps_k");
+    kside_record(h, grid, false, EPW_PATH_SMALL);
+  }
+  }
   h->end_span(sp, st);
 
   // ---- q side (once per call): S0 phases of every q, D(q), phonon eigen-systems ----

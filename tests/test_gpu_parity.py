@@ -1147,3 +1147,47 @@ def test_large_path_k_side_cache_and_its_invalidation(epw):
         assert_path_close(out6, ref_w2)
     finally:
         h.close()
+
+
+@pytest.mark.parametrize("flags", [0, 1])
+def test_small_path_k_side_cache_on_a_grid(epw, flags):
+    """Small-Nb family on a uniform grid: U_k and eps_k are kept between calls on the same grid (second call: fewer launches,
+    same results); a shifted grid, a k-list call in between and new operators each invalidate the cache."""
+    w = synth.make_custom("si-k", 8, 6, (1, 1, 1), 1.5, 0.1, 1.5, (6, 5, 4), ("random", 6, 3), seed=61)
+    g = w.g_full()
+    h = epw.EpwInterp(w.nbnd, w.nmodes, w.ne, w.np_, flags=flags)
+    try:
+        h.set_operators_from_host(w)
+
+        def call(q, shift=None):
+            out = h.interpolate_grid(w.k_grid, dev(q), k_shift=shift)
+            epw.epw_interp_sync(h.h)
+            return [t.cpu().numpy() for t in out], epw.epw_interp_last_launch_count(h.h)
+
+        qa, qb = w.q_list[:3], w.q_list[3:]
+        ref_a = oracle.interpolate(w.H_R, w.D_R, g, w.Re, w.w_e, w.Rp, w.w_p, w.k_list, qa)
+        ref_b = oracle.interpolate(w.H_R, w.D_R, g, w.Re, w.w_e, w.Rp, w.w_p, w.k_list, qb)
+        out1, n1 = call(qa)
+        assert_path_close(out1, ref_a)
+        out2, n2 = call(qb)                           # same grid: cache hit
+        assert n2 < n1
+        assert_path_close(out2, ref_b)
+        shift = np.array([0.5, 0.25, 0.0])
+        k_sh = w.k_list + shift / np.array(w.k_grid)
+        ref_sh = oracle.interpolate(w.H_R, w.D_R, g, w.Re, w.w_e, w.Rp, w.w_p, k_sh, qa)
+        out3, n3 = call(qa, shift=shift)              # k changed: miss
+        assert n3 == n1
+        assert_path_close(out3, ref_sh)
+        outl = h.interpolate(dev(w.k_list), dev(qa))  # a k-list call overwrites U_k
+        epw.epw_interp_sync(h.h)
+        assert_path_close([t.cpu().numpy() for t in outl], ref_a)
+        out4, n4 = call(qa, shift=shift)              # ... so the grid call after it recomputes
+        assert n4 == n1
+        assert_path_close(out4, ref_sh)
+        w2 = synth.make_custom("si-k2", 8, 6, (1, 1, 1), 1.5, 0.1, 1.5, (6, 5, 4), ("random", 6, 3), seed=62)
+        h.set_operators_from_host(w2)                 # new operators, same grid: miss
+        ref_w2 = oracle.interpolate(w2.H_R, w2.D_R, w2.g_full(), w2.Re, w2.w_e, w2.Rp, w2.w_p, k_sh, w2.q_list[:3])
+        out5, _ = call(w2.q_list[:3], shift=shift)
+        assert_path_close(out5, ref_w2)
+    finally:
+        h.close()
