@@ -406,6 +406,14 @@ __global__ void __launch_bounds__(GFShape<NB, VAR>::NW * 32, 1) grid_fused_kerne
     }
   };
 
+  // Items have equal length and the two warps that share a scheduler (warp and warp + 4) would walk through them in step:
+  // both in the set-up, the staging steps and the epilogue at the same time, the FP64 pipe idle.  The upper four warps
+  // start half an item late (about half of the DMMA issue time of an item shared by two warps).
+  if (!PASS_ONLY && warp >= 4) {
+    const long long wait = (long long)p.nug * (C::MTP * ksp + 8 * C::MTR * C::KS * C::NT) * 16;
+    const long long t0 = clock64();
+    while (clock64() - t0 < wait) {}
+  }
   for (int64_t item = lo + qgroup; item < hi; item += NQG) {
     const int64_t tile = item / p.nquads;
     const int quad = (int)(item - tile * p.nquads);
