@@ -304,6 +304,41 @@ int epw_eigh_batched_algo(const void *A, int64_t stride_a, int32_t n, int64_t ba
  * (Packs both operands into the DMMA fragment layout, then runs the same TMA + DMMA kernel as S2.) */
 int epw_zgemm(const void *A, const void *B, void *C, int64_t M, int32_t N, int32_t K, int64_t ldc, void *cuda_stream);
 
+/*
+ * epw_zgemm for callers that must not allocate device memory: the same contraction (the K = Ne sum of Eq. 10,
+ * PAPER.md:L112-118, as one FP64 tensor-path product), the same three kernels, the same result bit for bit -- but this
+ * call never reaches cudaMalloc, cudaFree or any other allocating routine, and it does not synchronise.
+ *
+ * Meant for: applications that gave all of HBM to their own pool allocator (a library-side cudaMalloc would fail there,
+ * or fragment the pool), time-critical / in-situ loops where cudaMalloc and cudaFree are banned because each of them
+ * stalls the whole device, and hosts that do not let a loaded library grow the process's device footprint.  epw_zgemm
+ * allocates and frees its two packed operands on every call; here they live in a fixed array of
+ * EPW_ZGEMM_NOALLOC_SCRATCH_BYTES (16 MiB) that is part of the library image: EVERY GPU on which this function has been
+ * called keeps those 16 MiB until the process exits, whether or not the function is called again.
+ *
+ *   A, B, C, M, N, K, ldc, cuda_stream   exactly as epw_zgemm: device pointers owned by the caller, A c128 [M][K],
+ *                                        B c128 [K][N], C c128 [M][ldc] row-major; asynchronous on cuda_stream
+ *   errbuf, errbuf_len                   NULL / 0, or a HOST buffer that receives a one-line message when the call fails
+ *
+ * Limit: ceil(M/128) ceil(K/8) + ceil(N/64) ceil(K/8) <= 1,024 (16 KB per term; e.g. M = 4,096, N = 384, K = 200).
+ * Anything larger returns EPW_EUNSUPPORTED, launches nothing and leaves C untouched: split the product over row blocks
+ * of A, or call epw_zgemm.
+ *
+ * First call on each device: it looks up the device address of the array (and makes the CUDA runtime load the library's
+ * code on that device, which is when the 16 MiB appear).  Make that first call during start-up, in particular before
+ * any stream capture begins; later calls on the device only launch kernels.  The device current at the call must be the
+ * one the pointers and the stream belong to.
+ *
+ * All calls on a device share the one array.  Nothing in it has to be cleared between calls (the packing kernels
+ * rewrite every value the product reads, padding included), and calls on ONE stream are ordered by the stream.  Calls
+ * whose kernels can overlap on the GPU -- issued by one process on different streams of the same device (from one host
+ * thread or several) with no event or synchronise between them -- overwrite each other's packed operands, and the
+ * results are then garbage.  Serialise such calls yourself.  (Each process has its own copy of the array.)
+ */
+#define EPW_ZGEMM_NOALLOC_SCRATCH_BYTES (16u * 1024u * 1024u)
+int epw_zgemm_noalloc(const void *A, const void *B, void *C, int64_t M, int32_t N, int32_t K, int64_t ldc,
+                      void *cuda_stream, char *errbuf, size_t errbuf_len);
+
 /* The contraction kernel of the large-Nb path (zgemm_strided.cu): `batch` problems C_b = A_b B_b on the FP64 tensor
  * path with the big operand A read in place:
  *   A_b[row][r] at A + b*a_batch + (row / a_rb)*a_bs + (row % a_rb) + r*a_ks      (c128 elements; rows contiguous)

@@ -33,7 +33,7 @@ EXPORTED_SYMBOLS = [
     "epw_interp_interpolate", "epw_interp_interpolate_host", "epw_interp_interpolate_grid",
     "epw_interp_interpolate_grid_host", "epw_interp_sync", "epw_interp_get_stage_times",
     "epw_interp_enable_stage_timing", "epw_interp_get_stage_launches", "epw_interp_last_launch_count", "epw_interp_get_eigh_rotations", "epw_interp_last_plan", "epw_interp_debug_get", "epw_interp_last_error",
-    "epw_phase_table", "epw_rp_to_q", "epw_interp_operator", "epw_eigh_batched", "epw_eigh_batched_algo", "epw_zgemm", "epw_zgemm_strided",
+    "epw_phase_table", "epw_rp_to_q", "epw_interp_operator", "epw_eigh_batched", "epw_eigh_batched_algo", "epw_zgemm", "epw_zgemm_noalloc", "epw_zgemm_strided",
     "epw_rotate_g2", "epw_axis_pass_dmma",
     "epw_eq6_unrotate", "epw_wannier_from_bloch",
     "epw_interp_set_energy_window", "epw_interp_set_selfenergy_consumer", "epw_interp_set_rp_shard", "epw_interp_rp_to_q_partial", "epw_interp_rp_to_q_scatter_add", "epw_interp_set_gq",
@@ -98,6 +98,7 @@ def load_library() -> ctypes.CDLL:
         L.epw_eigh_batched.argtypes = [vp, c_int64, c_int32, c_int64, vp, vp, c_int, vp, vp]
         L.epw_eigh_batched_algo.argtypes = [vp, c_int64, c_int32, c_int64, vp, vp, c_int, vp, c_int, vp]
         L.epw_zgemm.argtypes = [vp, vp, vp, c_int64, c_int32, c_int32, c_int64, vp]
+        L.epw_zgemm_noalloc.argtypes = [vp, vp, vp, c_int64, c_int32, c_int32, c_int64, vp, c_char_p, c_size_t]
         L.epw_zgemm_strided.argtypes = [vp, c_int64, c_int64, c_int64, c_int64, vp, c_int64, c_int64, c_int64, c_int, vp,
                                         c_int64, vp, c_int64, c_int64, c_int64, c_int64, c_int64, c_int, c_int64,
                                         c_int32, c_int32, c_int64, vp]
@@ -297,6 +298,22 @@ def epw_eigh_batched_algo(A, stride_a, n, batch, evals, V, sqrt_mode=0, status=N
 
 def epw_zgemm(A, B, C, M, N, K, ldc, stream=None):
     _check(load_library().epw_zgemm(_ptr(A), _ptr(B), _ptr(C), M, N, K, ldc, _stream() if stream is None else stream))
+
+
+EPW_ZGEMM_NOALLOC_SCRATCH_BYTES = 16 * 1024 * 1024
+
+
+def epw_zgemm_noalloc(A, B, C, M, N, K, ldc, stream=None):
+    """epw_zgemm without any device allocation inside the library (packed operands in the library's fixed 16 MiB array).
+    For callers whose device memory belongs to their own pool, or whose loop may not hit the device-wide stall of
+    cudaMalloc / cudaFree.  Asynchronous; raises EpwError(EPW_EUNSUPPORTED) with the library's message when
+    ceil(M/128) ceil(K/8) + ceil(N/64) ceil(K/8) exceeds 1,024.  Calls that can overlap on the GPU share the array and
+    race; the first call on a device does the one-time address look-up and should come before any stream capture."""
+    err = ctypes.create_string_buffer(512)
+    rc = load_library().epw_zgemm_noalloc(_ptr(A), _ptr(B), _ptr(C), M, N, K, ldc, _stream() if stream is None else stream,
+                                          err, len(err))
+    if rc < 0:
+        raise EpwError(rc, err.value.decode())
 
 
 def epw_zgemm_strided(A, a_rb, a_bs, a_ks, a_batch, B, b_sr, b_sn, b_batch, b_conj, b_gather, nb_mats, C, c_rb, c_bs,
