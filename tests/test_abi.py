@@ -85,14 +85,27 @@ def test_bench_host_logic_without_a_gpu():
     import bench
 
     assert bench.NQ_STEP[1] == 96 and bench.NQ_STEP[2] == 32 and bench.NQ_STEP[3] == 13 and bench.NQ_STEP[4] == 2
-    sub = {"config": {"workload": "w"}, "value": 1.0, "unit": "elements/s", "ms_per_step": 2.0, "steps": 3, "warmup": 1,
+    sub = {"config": {"workload": "w", "k_side": "cached after warm-up: H(k) ...", "cold_call_ms": 2.5}, "value": 1.0, "unit": "elements/s", "ms_per_step": 2.0, "steps": 3, "warmup": 1,
            "gpu_launches": 7, "clocks": {"sm_mhz": 1965.0},
            "roofline": {"stage": "S4b_rotate_g2", "kernel": "k", "bound": "tensor", "achieved": 1.0, "peak": 2.0,
                         "unit": "TFLOP/s", "frac": 0.5, "share_of_step": 0.4, "traffic": None,
                         "stages": {"S1_rp_to_q": {"kernel": "rp_to_q_kernel", "bound": "hbm", "frac": 0.7, "share_of_step": 0.04}}},
            "klist_path": {"value": 3.0, "ms_per_step": 4.0, "S2_re_to_k": {"kernel": "zgemm_dmma_kernel", "bound": "tensor",
                                                                           "frac": 0.96, "share_of_step": 0.8}},
-           "parity": {"ok": True}}
+           "parity": {"ok": True, "pairs": 96, "worst_g2_over_tolerance": 0.123456789}}
     rec = bench.summarise_config(sub, 1.5)
+    assert rec["k_side"] == "cached after warm-up" and rec["cold_call_ms"] == 2.5
+    # the compact summary that goes LAST into the JSON line: three configs and the consumer figure within 1,200 characters
+    import json
+
+    sub["value"], sub["ms_per_step"] = 3.123456789e10, 16.123456
+    sub["roofline"]["kernel"] = "rotate_g2_tma_kernel (two-kernel form)"
+    sub["roofline"]["stages"]["S4b_rotate_g2"] = {"kernel": "rotate_g2_tma_kernel", "frac": 0.4812345}
+    sub["clocks"] = {"sm_mhz": 1965.0, "sm_max_mhz": 1965.0, "reasons": ["sw_power_cap"]}
+    recs = {str(i): bench.summarise_config(sub, 1.5) for i in (2, 3, 4)}
+    brief = bench.brief_of(recs, {"value": 4.3e10, "ms": 56.3, "d2h_bytes_per_step": 8000000, "device_ms": 55.0})
+    assert len(json.dumps(brief)) <= 1200, len(json.dumps(brief))
+    assert brief["3"]["kernel"] == "rotate_g2_tma_kernel" and brief["3"]["s4b"] == 0.481 and brief["3"]["parity_ok"] is True
+    assert brief["2"]["worst"] == 0.123 and brief["2"]["cold_ms"] == 2.5 and brief["e2e_consumer"]["ms"] == 56.3
     assert rec["dominant"]["frac"] == 0.5 and rec["stages"]["S1_rp_to_q"]["frac"] == 0.7
     assert rec["klist_path"]["S2_re_to_k"]["frac"] == 0.96 and rec["parity"]["ok"] and rec["wall_s"] == 1.5
