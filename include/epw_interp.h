@@ -25,6 +25,10 @@
  *     epw_interp_set_wannier_operators and owns that copy and its workspace.
  *   - "device" pointers are CUDA device pointers valid on the handle's device; "host" pointers are CPU memory.
  *   - Calls on one handle must not overlap (a handle is not thread-safe); distinct handles are independent.
+ *   - One stream per handle: every call writes the handle's workspace, so the asynchronous calls on a handle are meant to be
+ *     issued on ONE stream, which orders them.  A caller that moves a handle to another stream first orders the new stream
+ *     behind the old one (event, or epw_interp_sync).  The one thing the library orders by itself is its k-side cache: a
+ *     grid call that reuses H(k), U_k, eps_k of an earlier call on a different stream waits on an event recorded behind them.
  *   - There is no CPU fallback: every call fails with EPW_ECUDA if no sm_100 device is usable.
  */
 #ifndef EPW_INTERP_H_
@@ -135,7 +139,8 @@ int epw_interp_interpolate_host(epw_interp_t h, const double *k_list, int64_t nk
  * rounding order.  The large-Nb kernel family (one-dimensional grids) expands the grid to a list internally.
  * The k side of the call (H(k), U_k, eps_k) is kept in the handle and reused by the next grid call with the same sizes and
  * shift, until the operators change or a k-list call comes in between: a caller looping over batches of q on one fine
- * k-grid pays for the Nk eigensolves of H(k) once.
+ * k-grid pays for the Nk eigensolves of H(k) once.  A call that returns an error, and an epw_interp_sync that reports
+ * EPW_ENOTCONVERGED, drop the kept k side: the next grid call computes it again.
  */
 int epw_interp_interpolate_grid(epw_interp_t h, const int32_t *k_grid, const double *k_shift, const double *q_list,
                                 int64_t nq, const int32_t *kq_map, double *eps_k, double *eps_kq, double *omega_q,
@@ -203,7 +208,11 @@ int epw_interp_rp_to_q_partial(epw_interp_t h, const double *q_list, int64_t nq,
  * Every rank calls it with the same q_list and its own view of the same buffers; the owners zero their buffers before and
  * all ranks synchronise after (barrier) before epw_interp_set_gq hands dst[own iq] to the rest of the path.  The order of
  * the additions varies from run to run: the sum over ranks is reproducible to rounding only (W terms per element).
- * (The paper: D2H of the partial y, mp_sum on the host.)  Asynchronous on cuda_stream.
+ * (The paper: D2H of the partial y, mp_sum on the host.)  Asynchronous on cuda_stream: the table is
+ * uploaded on the stream and the host is not made to wait; the dst array may be reused as soon as the call returns.
+ * Adding into another GPU's memory needs native atomics over the link between the two devices
+ * (cudaDevP2PAttrNativeAtomicSupported: NVLink yes, PCIe peer access no); the call checks every destination that the
+ * process knows to be on another device and returns EPW_EUNSUPPORTED if that attribute is 0.
  */
 int epw_interp_rp_to_q_scatter_add(epw_interp_t h, const double *q_list, int64_t nq, void *const *dst, void *cuda_stream);
 int epw_interp_set_gq(epw_interp_t h, const void *g1_reduced);

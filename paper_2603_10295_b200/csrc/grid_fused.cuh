@@ -601,14 +601,33 @@ static bool gf_plan(int nm, int L1, int var, int *nug_out, int *nbuf_out, size_t
   if (L1 < 1 || L1 > 2 * (var == 2 ? GF_MAX_KSP_PASS : GF_MAX_KSP) || nm < 1) return false;
   const int L1e = 2 * ((L1 + 1) / 2);
   const size_t limit = (size_t)225 * 1024;
-  for (int want_buf = 2; want_buf >= 1; want_buf--)
-    for (int n = nm; n >= 1; n--) {
-      const size_t groups_bytes = var == 2 ? 0
-                                  : var == 1 ? (GFShape<NB, 1>::NW / GFShape<NB, 1>::WPQ) * GFShape<NB, 1>::group_bytes(n)
-                                             : (GFShape<NB, 0>::NW / GFShape<NB, 0>::WPQ) * GFShape<NB, 0>::group_bytes(n);
-      const size_t fixed = groups_bytes + GF_MAX_BUF * (sizeof(uint64_t) + sizeof(int)) + 16;
-      const size_t per_buf = sizeof(c128) * ((size_t)L1e * gf_row_pitch(n * C::NBB) + 8);
-      if (fixed + want_buf * per_buf > limit) continue;
+  // bytes of the shared-memory plan with n modes per group: (everything but the T2 ring, one T2 buffer).  Both grow with n
+  // (gf_row_pitch is the next number = 4 mod 8), so the largest n that fits is found by bisection -- nm is E / 64 = 166,000
+  // on configs[4]'s pass-only launches, and this runs on every launch.
+  auto bytes_of = [&](int n, size_t *fixed_out) {
+    const size_t groups_bytes = var == 2 ? 0
+                                : var == 1 ? (GFShape<NB, 1>::NW / GFShape<NB, 1>::WPQ) * GFShape<NB, 1>::group_bytes(n)
+                                           : (GFShape<NB, 0>::NW / GFShape<NB, 0>::WPQ) * GFShape<NB, 0>::group_bytes(n);
+    *fixed_out = groups_bytes + GF_MAX_BUF * (sizeof(uint64_t) + sizeof(int)) + 16;
+    return sizeof(c128) * ((size_t)L1e * gf_row_pitch(n * C::NBB) + 8);
+  };
+  for (int want_buf = 2; want_buf >= 1; want_buf--) {
+    auto fits = [&](int n) {
+      size_t fixed = 0;
+      const size_t per_buf = bytes_of(n, &fixed);
+      return fixed + want_buf * per_buf <= limit;
+    };
+    if (!fits(1)) continue;
+    int lo = 1, hi = nm;   // largest n in [1, nm] that fits
+    while (lo < hi) {
+      const int mid = lo + (hi - lo + 1) / 2;
+      if (fits(mid)) lo = mid;
+      else hi = mid - 1;
+    }
+    {
+      int n = lo;
+      size_t fixed = 0;
+      bytes_of(n, &fixed);
       // equal mode groups (9 modes that fit four at a time go 3 + 3 + 3, not 4 + 4 + 1: the items are dealt by count)
       const int groups = (nm + n - 1) / n;
       n = (nm + groups - 1) / groups;
@@ -620,6 +639,7 @@ static bool gf_plan(int nm, int L1, int var, int *nug_out, int *nbuf_out, size_t
       *nbuf_out = nbuf;
       return true;
     }
+  }
   return false;
 }
 

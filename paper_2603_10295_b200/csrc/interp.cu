@@ -127,10 +127,14 @@ struct epw_interp {
   int last_kmode = 0;
   // k side of the large-Nb path kept between calls on the SAME uniform grid (phases, H(k), U_k, eps_k, packed operands):
   // valid for (grid sizes, shift, operators epoch); any k-list call or new operators drop it
-  struct KSide { bool valid = false, with_conj = false; int path = 0; int32_t N[3] = {0, 0, 0}; double s[3] = {0, 0, 0}; uint64_t epoch = 0; } kside;
+  // `stream` / `ev`: the stream the k side was enqueued on and an event recorded behind it, so that a later call on ANOTHER
+  // stream that hits the cache waits for the cached buffers to be complete (kside_wait)
+  struct KSide { bool valid = false, with_conj = false; int path = 0; int32_t N[3] = {0, 0, 0}; double s[3] = {0, 0, 0}; uint64_t epoch = 0;
+                 cudaStream_t stream = nullptr; cudaEvent_t ev = nullptr; } kside;
   uint64_t op_epoch = 0;
   DevBuf PkT;         // large-Nb path: phase table of every k-chunk transposed, [chunk][Re][k]
   DevBuf dst_tab;     // destination pointers of epw_interp_rp_to_q_scatter_add
+  std::vector<void *> dst_host;   // the library's pageable copy of the caller's table (source of the stream-ordered upload)
   DevBuf epsk_keep;   // eps_k of the cached k side (the caller's buffer is refilled from it)
   int64_t last_eq_slot = 0;  // slot of the last q of the last call inside the e_q buffer (debug getter)
   // host-entry output drain: while a host-buffer call runs, the |g|^2 and eps_kq slices of every finished q are copied
@@ -192,10 +196,13 @@ struct epw_interp {
   }
   // The convergence flag is STICKY: every eigensolve of every enqueued call may set it, only epw_interp_sync reads and
   // clears it, so a caller that enqueues several calls before one sync still learns of a failure in any of them.
-  int ensure_status() {
+  int ensure_status(cudaStream_t st) {
     if (status.p) return EPW_OK;
     cudaError_t e = status.reserve(sizeof(int32_t));
-    if (e == cudaSuccess) e = cudaMemset(status.p, 0, sizeof(int32_t));
+    // cleared ON the caller's stream (a blocking cudaMemset on the legacy stream is not ordered against a
+    // cudaStreamNonBlocking stream) and waited for once, here, at allocation
+    if (e == cudaSuccess) e = cudaMemsetAsync(status.p, 0, sizeof(int32_t), st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     return e == cudaSuccess ? EPW_OK : cuda_fail(e, "cudaMalloc status");
   }
   int cuda_fail(cudaError_t e, const char *where) {
@@ -253,6 +260,7 @@ static bool use_large_path(const epw_interp *h) {
 struct GridSpec;
 static bool kside_matches(const epw_interp *h, const GridSpec *grid, bool need_conj, int path = EPW_PATH_LARGE);
 static void kside_record(epw_interp *h, const GridSpec *grid, bool with_conj, int path = EPW_PATH_LARGE);
+static void kside_wait(epw_interp *h, cudaStream_t st);
 
 static int interpolate_large(epw_interp *h, const double *k_list, const GridSpec *grid, int64_t nk, const double *q_list,
                              int64_t nq, const int32_t *kq_map, double *eps_k, double *eps_kq, double *omega_q, double *g2,
@@ -314,7 +322,7 @@ static int interpolate_large(epw_interp *h, const double *k_list, const GridSpec
     CU_OR_FAIL(h, h->Ukq.reserve(sizeof(c128) * (size_t)nk * nbb), "cudaMalloc Ukq");
     if (!eps_kq) CU_OR_FAIL(h, h->epskq_scratch.reserve(sizeof(double) * (size_t)nk * nb), "cudaMalloc eps scratch");
   }
-  { const int rc = h->ensure_status(); if (rc != EPW_OK) return rc; }
+  { const int rc = h->ensure_status(st); if (rc != EPW_OK) return rc; }
   if (h->window_on && !h->mask_out) CU_OR_FAIL(h, h->maskbuf.reserve((size_t)nk), "cudaMalloc mask");
   {
     const size_t need = std::max(eigh_large_scratch_bytes(nb, nk), eigh_large_scratch_bytes(nm, nq));
@@ -336,6 +344,7 @@ static int interpolate_large(epw_interp *h, const double *k_list, const GridSpec
   int sp;
   const bool k_cached = kside_matches(h, grid, kq_map != nullptr);
   if (k_cached) {
+    kside_wait(h, st);
     CU_OR_FAIL(h, cudaMemcpyAsync(eps_k, h->epsk_keep.p, sizeof(double) * (size_t)nk * nb, cudaMemcpyDeviceToDevice, st),
                "copy cached eps_k");
   } else {
@@ -522,7 +531,19 @@ static bool kside_matches(const epw_interp *h, const GridSpec *grid, bool need_c
     if (h->kside.N[d] != grid->N[d] || h->kside.s[d] != grid->s[d]) return false;
   return h->kside.with_conj || !need_conj;
 }
+// A cache hit on a stream other than the one the k side was computed on: make that stream wait for the cached buffers.
+static void kside_wait(epw_interp *h, cudaStream_t st) {
+  if (h->kside.ev && h->kside.stream != st) cudaStreamWaitEvent(st, h->kside.ev, 0);
+}
 static void kside_record(epw_interp *h, const GridSpec *grid, bool with_conj, int path) {
+  if (!h->kside.ev && cudaEventCreateWithFlags(&h->kside.ev, cudaEventDisableTiming) != cudaSuccess) {
+    h->kside.ev = nullptr;
+    cudaGetLastError();
+    h->kside.valid = false;   // no event, no cache: every call recomputes the k side
+    return;
+  }
+  h->kside.stream = h->last_stream;
+  cudaEventRecord(h->kside.ev, h->last_stream);   // behind the last kernel / copy of the k side
   h->kside.valid = true;
   h->kside.path = path;
   h->kside.with_conj = with_conj;
@@ -614,6 +635,7 @@ void epw_interp_destroy(epw_interp_t h) {
   if (h->aux_stream) cudaStreamDestroy(h->aux_stream);
   if (h->ev_fork) cudaEventDestroy(h->ev_fork);
   if (h->ev_join) cudaEventDestroy(h->ev_join);
+  if (h->kside.ev) cudaEventDestroy(h->kside.ev);
   delete h;
 }
 
@@ -729,9 +751,11 @@ int epw_interp_interpolate(epw_interp_t h, const double *k_list, int64_t nk, con
   h->last_stream = st;
   h->launches = 0;
   h->last_kmode = 0;
-  if (use_large_path(h))
-    return interpolate_large(h, k_list, nullptr, nk, q_list, nq, kq_map, eps_k, eps_kq, omega_q, g2, st);
-  return interpolate_small(h, k_list, nullptr, nk, q_list, nq, kq_map, eps_k, eps_kq, omega_q, g2, st);
+  const int rc2 = use_large_path(h)
+                      ? interpolate_large(h, k_list, nullptr, nk, q_list, nq, kq_map, eps_k, eps_kq, omega_q, g2, st)
+                      : interpolate_small(h, k_list, nullptr, nk, q_list, nq, kq_map, eps_k, eps_kq, omega_q, g2, st);
+  if (rc2 != EPW_OK) h->kside.valid = false;   // a call that failed half-way leaves no cached k side behind
+  return rc2;
 }
 
 int epw_interp_interpolate_grid(epw_interp_t h, const int32_t *k_grid, const double *k_shift, const double *q_list,
@@ -758,10 +782,14 @@ int epw_interp_interpolate_grid(epw_interp_t h, const int32_t *k_grid, const dou
     CU_OR_FAIL(h, h->klist_gen.reserve(sizeof(double) * 3 * (size_t)nk), "cudaMalloc k-list");
     if (!kside_matches(h, &g, kq_map != nullptr))
       LAUNCH(h, launch_grid_klist(g.N, g.s, h->klist_gen.as<double>(), st), "grid k-list");
-    return interpolate_large(h, h->klist_gen.as<double>(), &g, nk, q_list, nq, kq_map, eps_k, eps_kq, omega_q, g2, st);
+    const int rl = interpolate_large(h, h->klist_gen.as<double>(), &g, nk, q_list, nq, kq_map, eps_k, eps_kq, omega_q, g2, st);
+    if (rl != EPW_OK) h->kside.valid = false;
+    return rl;
   }
   h->last_kmode = 1;
-  return interpolate_small(h, nullptr, &g, nk, q_list, nq, kq_map, eps_k, eps_kq, omega_q, g2, st);
+  const int rs = interpolate_small(h, nullptr, &g, nk, q_list, nq, kq_map, eps_k, eps_kq, omega_q, g2, st);
+  if (rs != EPW_OK) h->kside.valid = false;   // a call that failed half-way leaves no cached k side behind
+  return rs;
 }
 
 }  // extern "C"
@@ -778,7 +806,8 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   // (the two kernel families share the H(k), U_k buffers: a cached k side is valid for the family that made it; on a
   //  uniform grid the small-Nb family keeps U_k and eps_k between calls too -- 10^6 solves per call on configs[3])
   const bool k_cached = kside_matches(h, grid, false, EPW_PATH_SMALL);
-  if (!k_cached) h->kside.valid = false;
+  if (k_cached) kside_wait(h, st);
+  else h->kside.valid = false;
   const int ncols_g = nbb * nm;
   const int ncols_h = kq_map ? 0 : nbb;
   const int ncols = ncols_g + ncols_h;
@@ -900,7 +929,7 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   if (hbatch) CU_OR_FAIL(h, h->Hkq.reserve(sizeof(c128) * hb * (size_t)nk * nbb), "cudaMalloc H(k+q)");
   if (!kq_map) CU_OR_FAIL(h, h->Ukq.reserve(sizeof(c128) * hb * (size_t)c_rows * nbb), "cudaMalloc Ukq");
   if (!kq_map && !eps_kq) CU_OR_FAIL(h, h->epskq_scratch.reserve(sizeof(double) * hb * (size_t)c_rows * nb), "cudaMalloc eps scratch");
-  { const int rc = h->ensure_status(); if (rc != EPW_OK) return rc; }
+  { const int rc = h->ensure_status(st); if (rc != EPW_OK) return rc; }
   if (h->window_on && !h->mask_out) CU_OR_FAIL(h, h->maskbuf.reserve((size_t)nk), "cudaMalloc mask");
   {
     const size_t need = std::max(eigh_large_scratch_bytes(nb, nk), eigh_large_scratch_bytes(nm, nq));
@@ -919,7 +948,7 @@ static int interpolate_small(epw_interp *h, const double *k_list, const GridSpec
   // Axis passes: a streaming kernel when the box extent is small (always, for Wigner-Seitz lists), else the in-place
   // tensor-path contraction with the packed phase table.
   // (nbat > 1: the same passes for nbat operands stored one after the other -- the outermost box index simply runs on)
-  const bool dmma_axis2 = grid && grid_fused_supported(nb, 1, L[1]);
+  const bool dmma_axis2 = grid && grid_pass_dmma_supported(nb, L[1]);   // the pass-only variant runs it
   auto grid_pass_ab = [&](int nc, int nbat) -> cudaError_t {
     const int64_t N2 = grid->N[1], N3 = grid->N[2];
     const int64_t B = (int64_t)nbat * L[0];   // outermost extent of X, T1, T2
@@ -1265,6 +1294,29 @@ int epw_interp_rp_to_q_scatter_add(epw_interp_t h, const double *q_list, int64_t
   if (!dst) return h->fail(EPW_EINVAL, "epw_interp_rp_to_q_scatter_add: null destination table");
   for (int64_t i = 0; i < nq; i++)
     if (!dst[i]) return h->fail(EPW_EINVAL, "epw_interp_rp_to_q_scatter_add: null destination pointer");
+  // The kernel adds with red.global.add.f64 at system scope.  Into another GPU's memory that needs native atomics over the
+  // link (NVLink has them, PCIe peer access does not): ask once per peer device and refuse instead of adding wrongly.
+  CU_OR_FAIL(h, cudaSetDevice(h->cfg.device), "cudaSetDevice");
+  int peer_ok[64];
+  for (int &v : peer_ok) v = -1;
+  for (int64_t i = 0; i < nq; i++) {
+    cudaPointerAttributes pa;
+    if (cudaPointerGetAttributes(&pa, dst[i]) != cudaSuccess) { cudaGetLastError(); continue; }   // unknown to this process
+    if (pa.type != cudaMemoryTypeDevice || pa.device == h->cfg.device || pa.device < 0 || pa.device >= 64) continue;
+    if (peer_ok[pa.device] < 0) {
+      int v = 0;
+      if (cudaDeviceGetP2PAttribute(&v, cudaDevP2PAttrNativeAtomicSupported, h->cfg.device, pa.device) != cudaSuccess) {
+        cudaGetLastError();
+        v = 0;
+      }
+      peer_ok[pa.device] = v;
+    }
+    if (!peer_ok[pa.device])
+      return h->fail(EPW_EUNSUPPORTED, "epw_interp_rp_to_q_scatter_add: destination " + std::to_string(i) + " lives on device " +
+                                       std::to_string(pa.device) + ", to which device " + std::to_string(h->cfg.device) +
+                                       " has no native peer atomics (cudaDevP2PAttrNativeAtomicSupported = 0): use "
+                                       "epw_interp_rp_to_q_partial + a reduce-scatter instead");
+  }
   return rp_to_q_partial_impl(h, q_list, nq, nullptr, dst, cuda_stream);
 }
 
@@ -1284,11 +1336,14 @@ static int rp_to_q_partial_impl(epw_interp_t h, const double *q_list, int64_t nq
   c128 *out = reinterpret_cast<c128 *>(g1_partial);
   c128 *const *dst_dev = nullptr;
   if (dst) {
-    // the destination table on the device (the copy is ordered on the stream; the host array may be reused on return)
+    // The destination table on the device, copied ON the stream (so it cannot overtake the previous call's kernels, which
+    // still read the old table) and without waiting for the stream.  The source is the library's own PAGEABLE copy of the
+    // caller's array: a copy from pageable memory is staged by the runtime before cudaMemcpyAsync returns, so both this
+    // copy and the caller's array (pinned or not) are free again on return.
     CU_OR_FAIL(h, h->dst_tab.reserve(sizeof(void *) * (size_t)nq), "cudaMalloc destination table");
-    CU_OR_FAIL(h, cudaMemcpyAsync(h->dst_tab.p, dst, sizeof(void *) * (size_t)nq, cudaMemcpyHostToDevice, st),
+    h->dst_host.assign(dst, dst + nq);
+    CU_OR_FAIL(h, cudaMemcpyAsync(h->dst_tab.p, h->dst_host.data(), sizeof(void *) * (size_t)nq, cudaMemcpyHostToDevice, st),
                "cudaMemcpy destination table");
-    CU_OR_FAIL(h, cudaStreamSynchronize(st), "cudaStreamSynchronize");
     dst_dev = h->dst_tab.as<c128 *>();
   }
   for (int64_t q0 = 0; q0 < nq; q0 += QB) {
@@ -1323,6 +1378,7 @@ int epw_interp_sync(epw_interp_t h) {
     CU_OR_FAIL(h, cudaMemcpy(&s, h->status.p, sizeof(s), cudaMemcpyDeviceToHost), "cudaMemcpy status");
     if (s) {
       CU_OR_FAIL(h, cudaMemset(h->status.p, 0, sizeof(int32_t)), "memset status");   // read once, then cleared
+      h->kside.valid = false;   // the solve that failed may have been one of H(k): the next grid call solves them again
       return h->fail(EPW_ENOTCONVERGED, "a Jacobi eigensolve did not converge within the sweep limit (in this or an "
                                         "earlier call since the last epw_interp_sync)");
     }
