@@ -501,8 +501,10 @@ def run_config(args, ctx, cfg_index: int, steps: int, warmup: int, legs: set) ->
         g1_part = None if args.rp_fused else torch.empty((world * nq_step, rows, 2), dtype=torch.float64, device="cuda")
         symm = None
         if args.rp_fused and world > 1:
-            # UNEXECUTED branch (no multi-GPU box in this run): the owners' buffers as symmetric memory, so that every rank
-            # holds a peer mapping of every other rank's buffer
+            # The owners' buffers as symmetric memory, so that every rank holds a peer mapping of every other rank's buffer.
+            # The pointer-table logic below (own pointers + mapped foreign pointers, zero / barrier / add / barrier) is what
+            # tests/test_gpu_ipc.py runs across two processes with CUDA-IPC mappings on one GPU; the symmetric-memory
+            # rendezvous itself needs a multi-GPU node and has not been executed in this project's runs (one GPU per call).
             import torch.distributed._symmetric_memory as symm_mem
 
             g1_mine = symm_mem.empty((nq_step, rows, 2), dtype=torch.float64, device="cuda")
