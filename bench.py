@@ -696,6 +696,10 @@ def run_config(args, ctx, cfg_index: int, steps: int, warmup: int, legs: set) ->
                     st["hbm_frac"] = extra["hbm_bytes"] / (t_ms * 1e-3) / 1e9 / hbm
                 st.update({k: v for k, v in extra.items() if k != "hbm_bytes"})
                 stages[name] = st
+            if use_grid and mm is m and warmup > 0 and not rot["Hk"] and not args.rp_shard:
+                # no H(k) solve ran inside the timed steps: the k side came from the handle's cache (config.k_side)
+                stages["Hk_eig"] = {"cached": True, "kernel": n_eig, "share_of_step": 0.0,
+                                    "note": "H(k), U_k, eps_k reused from the first call on this grid; see config.cold_call_ms"}
             n_s1 = -(-nq_step // plan["q_batch"])
             s1_bytes = (16.0 * w.slab_elems * w.np_ * n_s1 + 16.0 * w.slab_elems * nq_step) * nsteps
             s1 = {"bound": "hbm", "kernel": "rp_to_q_kernel", "achieved": s1_bytes / (stage_ms["S1_rp_to_q"] * 1e-3) / 1e9,
