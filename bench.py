@@ -696,7 +696,7 @@ def run_config(args, ctx, cfg_index: int, steps: int, warmup: int, legs: set) ->
                     st["hbm_frac"] = extra["hbm_bytes"] / (t_ms * 1e-3) / 1e9 / hbm
                 st.update({k: v for k, v in extra.items() if k != "hbm_bytes"})
                 stages[name] = st
-            if use_grid and mm is m and warmup > 0 and not rot["Hk"] and not args.rp_shard:
+            if use_grid and mm is m and warmup > 0 and not rot["Hk"]:
                 # no H(k) solve ran inside the timed steps: the k side came from the handle's cache (config.k_side)
                 stages["Hk_eig"] = {"cached": True, "kernel": n_eig, "share_of_step": 0.0,
                                     "note": "H(k), U_k, eps_k reused from the first call on this grid; see config.cold_call_ms"}
@@ -815,7 +815,8 @@ def run_config(args, ctx, cfg_index: int, steps: int, warmup: int, legs: set) ->
                 "operator_upload_s": t_upload,
                 "k_side": ("cached after warm-up: H(k), U_k, eps_k of the grid are computed by the first call on the handle and "
                            "reused; the timed steps exclude them, cold_call_ms is one step that recomputes them"
-                           if (use_grid and not args.rp_shard) else "computed inside every timed step"),
+                           + (" (not measured with --rp-shard)" if args.rp_shard else "")
+                           if use_grid else "computed inside every timed step (k-list calls keep no k side)"),
                 "cold_call_ms": cold_ms,
             },
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
